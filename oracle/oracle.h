@@ -1,0 +1,110 @@
+/* oracle/oracle.h — CPU ORACLE (TEST INFRASTRUCTURE ONLY).
+ *
+ * Plain, slow, fp64 restatement of the Valencia GRMHD right-hand-side stage of
+ * arXiv:2409.10384 (PAPER.md, cited as P:line).  It exists to check the CUDA
+ * library; only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * `--impl reference` leg may build, load or call it.  It shares no code, header,
+ * table or helper with paper_2409_10384_b200/csrc (the product).
+ *
+ * Steps follow DESIGN.md §3 (O0..O9) which restates, in the paper's notation,
+ *   Eq. 6 prim->cons, Eq. 7 b^mu, Eq. 8 fluxes,
+ *   Eq. 9 sources, P:133 reconstruction/Riemann/CT choices,
+ *   P:137-139 atmosphere, P:141-157 FOFC(+DMP, Eq. 12), P:161 con2prim.
+ * No blocking, fusion or reordering: loops over blocks, cells, faces, edges.
+ *
+ * Pins (tests/test_oracle_*.py, -m "not gpu"): see DESIGN.md §5.  Policy choices
+ * the paper leaves open (floor order R5, M_max R6, "requires a floor" R8, DMP
+ * variables R13) are "parity unpinned" beyond oracle==GPU and are listed there.
+ *
+ * Data layout (the library boundary's, restated): a MeshBlock has n^3 interior
+ * cells, ng=4 ghosts, nt=n+8 stored cells per direction; i fastest.
+ *   cell field   [nmb][nt][nt][nt]
+ *   x-face field [nmb][nt][nt][px]      px = nt+4 (nt+1 used)
+ *   y-face field [nmb][nt][nt+1][nt]
+ *   z-face field [nmb][nt+1][nt][nt]
+ *   E_x          [nmb][nt+1][nt+1][nt]
+ *   E_y          [nmb][nt+1][nt][px]
+ *   E_z          [nmb][nt][nt+1][px]
+ * Face i of direction x lies between cells i-1 and i.
+ */
+#ifndef GRMHD_ORACLE_H
+#define GRMHD_ORACLE_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct {
+  int nmb, n, ng;
+  double gamma_ad;               /* ideal-gas Gamma                          */
+  double rho_atm, T_atm, f_thr;
+  double mag_max;                /* M_max of P:139 (+inf disables)           */
+  int recon;                     /* 0 donor cell, 1 PPM4, 2 WENO-Z   */
+  int riemann;                   /* 0 LLF, 1 HLLE                    */
+  int fofc, fofc_riemann;
+  double dmp_M;                  /* Eq. 12; <=0 off                          */
+  int c2p_max_iter;
+  double c2p_tol;
+} orc_params;
+
+/* status / flag bits */
+enum { ORC_DFLOOR = 1, ORC_TAUFLOOR = 2, ORC_MAGCAP = 4, ORC_RHOFLOOR = 8,
+       ORC_TFLOOR = 16, ORC_FAIL = 32, ORC_DMP = 64 };
+
+/* ---- point-level steps (unit-test surface) ------------------------------ */
+
+/* O0: det, sqrt(det), inverse of the 3-metric g = {xx,xy,xz,yy,yz,zz}. */
+void orc_metric_inverse(const double g[6], double* det, double* sdet, double ginv[6]);
+
+/* O2 (Eq. 6): prim = {rho,ux,uy,uz,P} with u^i = W v^i, B = undensitised B^i;
+ * cons = {D,Sx,Sy,Sz,tau}, undensitised. */
+void orc_prim2cons(double gamma_ad, const double g[6], const double prim[5],
+                   const double B[3], double cons[5]);
+
+/* O3: Ut = densitised {D,S_i,tau} (rewritten if floored and !check_only),
+ * Btcc = densitised cell-centred B, W out = {rho,ux,uy,uz,P}.
+ * Returns the status byte; *iters = master-function evaluations used. */
+int orc_con2prim_cell(const orc_params* p, const double g[6], double Ut[5],
+                      const double Btcc[3], double W[5], int check_only, int* iters);
+
+/* O3 master function f(mu) exposed for the zero-at-true-root pin.
+ * in: q, r2, bs2 (= B^2/D), rb2 (= (r_i B^i)^2 / D). */
+double orc_c2p_master(double gamma_ad, double q, double r2, double bs2, double rb2, double mu);
+
+/* O4: q[5] = cells i-2..i+2; qm = value at the left face of cell i, qp at the right. */
+void orc_reconstruct(int kind, const double q[5], double* qm, double* qp);
+
+/* O5+O6: one face of direction dir (0,1,2).  gL/gR = cell-centred
+ * {alpha,betax,betay,betaz,gxx,gxy,gxz,gyy,gyz,gzz} of the lower/upper cell.
+ * WL/WR = {rho,ux,uy,uz,P,Bt1,Bt2} (B densitised, t1,t2 cyclic after dir),
+ * Bfd = densitised face-normal B.  apply_floor: face-state floor of P:139.
+ * F[7] = {D,Sx,Sy,Sz,tau,Bt1,Bt2} fluxes.  lam (may be NULL) = {lm_L,lp_L,lm_R,lp_R}. */
+void orc_face_flux(const orc_params* p, int dir, int riemann, const double gL[10],
+                   const double gR[10], const double WL[7], const double WR[7],
+                   double Bfd, int apply_floor, double F[7], double lam[4]);
+
+/* ---- block-level steps --------------------------------------------------- */
+
+/* O3 over all stored cells. U[5], Bf[3], g[6] field pointers; W[8] out
+ * (rho,ux,uy,uz,P,Bccx,Bccy,Bccz); status may be NULL. */
+void orc_con2prim(const orc_params* p, double* const U[5], const double* const Bf[3],
+                  const double* const g[6], double* const W[8], unsigned char* status,
+                  int nthreads);
+
+/* Whole stage O3..O9.  adm[16] = gxx,gxy,gxz,gyy,gyz,gzz,alp,betx,bety,betz,
+ * Kxx,Kxy,Kxz,Kyy,Kyz,Kzz.  dx[nmb][3].  out_dU[5] (interior cells written),
+ * out_E[3] (edges of interior cells written), flag (test cells written; may be NULL),
+ * flux_out[21] may be NULL; else x,y,z face-flux fields (7 each, face layouts above)
+ * receive the post-FOFC fluxes on the computed range.  face_refluxed[3] may be
+ * NULL; else byte per face (face layouts) = 1 where FOFC redid the face. */
+void orc_rhs(const orc_params* p, const double* dx, double* const U[5],
+             const double* const Bf[3], const double* const adm[16], double* const W[8],
+             int w_is_valid, double dt_fofc, double* const out_dU[5],
+             double* const out_E[3], unsigned char* flag, unsigned char* c2p_status,
+             double* const flux_out[21], unsigned char* const face_refluxed[3],
+             int nthreads);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

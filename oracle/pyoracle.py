@@ -1,0 +1,166 @@
+"""ctypes loader for the CPU ORACLE (test infrastructure only — see oracle/oracle.h).
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg
+may import this module.  It never imports the CUDA binding.
+"""
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "liboracle.so")
+_SRC = ["point.cpp", "stage.cpp"]
+
+
+def build(force=False):
+    """g++ -O2 -ffp-contract=off: no FMA contraction, IEEE fp64 in the written order."""
+    srcs = [os.path.join(_HERE, s) for s in _SRC] + [os.path.join(_HERE, "oracle.h")]
+    if not force and os.path.exists(_SO) and all(
+            os.path.getmtime(_SO) >= os.path.getmtime(s) for s in srcs):
+        return _SO
+    cmd = ["g++", "-O2", "-ffp-contract=off", "-fPIC", "-shared", "-std=c++17", "-o", _SO] + \
+          [os.path.join(_HERE, s) for s in _SRC] + ["-lpthread"]
+    subprocess.check_call(cmd)
+    return _SO
+
+
+class OrcParams(C.Structure):
+    _fields_ = [("nmb", C.c_int), ("n", C.c_int), ("ng", C.c_int),
+                ("gamma_ad", C.c_double), ("rho_atm", C.c_double), ("T_atm", C.c_double),
+                ("f_thr", C.c_double), ("mag_max", C.c_double),
+                ("recon", C.c_int), ("riemann", C.c_int), ("fofc", C.c_int),
+                ("fofc_riemann", C.c_int), ("dmp_M", C.c_double),
+                ("c2p_max_iter", C.c_int), ("c2p_tol", C.c_double)]
+
+
+_lib = None
+_dp = C.POINTER(C.c_double)
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        _lib = C.CDLL(_SO)
+        _lib.orc_c2p_master.restype = C.c_double
+        _lib.orc_c2p_master.argtypes = [C.c_double] * 6
+        _lib.orc_con2prim_cell.restype = C.c_int
+    return _lib
+
+
+def make_params(nmb=1, n=4, gamma_ad=2.0, rho_atm=1e-10, T_atm=1e-8, f_thr=1.0,
+                mag_max=float("inf"), recon=1, riemann=1, fofc=1, fofc_riemann=0, dmp_M=0.0,
+                c2p_max_iter=40, c2p_tol=1e-15, **_ignored):
+    return OrcParams(nmb, n, 4, gamma_ad, rho_atm, T_atm, f_thr, mag_max, recon, riemann,
+                     fofc, fofc_riemann, dmp_M, c2p_max_iter, c2p_tol)
+
+
+def _d(a):
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    return a, a.ctypes.data_as(_dp)
+
+
+def _ptrs(arrs, const=True):
+    """array of double* from a list of contiguous float64 arrays (None -> NULL)."""
+    P = (C.c_void_p * len(arrs))()
+    for i, a in enumerate(arrs):
+        if a is None:
+            P[i] = None
+        else:
+            assert a.dtype == np.float64 and a.flags["C_CONTIGUOUS"]
+            P[i] = a.ctypes.data
+    return P
+
+
+# ------------------------------------------------------------------ point level
+def metric_inverse(g):
+    g, gp = _d(g)
+    det, sdet = C.c_double(), C.c_double()
+    gi = np.zeros(6)
+    lib().orc_metric_inverse(gp, C.byref(det), C.byref(sdet), gi.ctypes.data_as(_dp))
+    return det.value, sdet.value, gi
+
+
+def prim2cons(gamma_ad, g, prim, B):
+    g, gp = _d(g); prim, pp = _d(prim); B, bp = _d(B)
+    out = np.zeros(5)
+    lib().orc_prim2cons(C.c_double(gamma_ad), gp, pp, bp, out.ctypes.data_as(_dp))
+    return out
+
+
+def con2prim_cell(par, g, Ut, Btcc, check_only=False):
+    """returns (status, W[5], Ut_after[5], iters)"""
+    g, gp = _d(g); Ut = np.array(Ut, dtype=np.float64); Bt, bp = _d(Btcc)
+    W = np.zeros(5)
+    it = C.c_int(0)
+    st = lib().orc_con2prim_cell(C.byref(par), gp, Ut.ctypes.data_as(_dp), bp,
+                                 W.ctypes.data_as(_dp), int(check_only), C.byref(it))
+    return st, W, Ut, it.value
+
+
+def c2p_master(gamma_ad, q, r2, bs2, rb2, mu):
+    return lib().orc_c2p_master(gamma_ad, q, r2, bs2, rb2, mu)
+
+
+def reconstruct(kind, q5):
+    q5, qp_ = _d(q5)
+    qm, qp = C.c_double(), C.c_double()
+    lib().orc_reconstruct(int(kind), qp_, C.byref(qm), C.byref(qp))
+    return qm.value, qp.value
+
+
+def face_flux(par, d, riemann, gL, gR, WL, WR, Bfd, apply_floor=False, want_lam=False):
+    gL, a = _d(gL); gR, b = _d(gR); WL, c = _d(WL); WR, e = _d(WR)
+    F = np.zeros(7); lam = np.zeros(4)
+    lib().orc_face_flux(C.byref(par), int(d), int(riemann), a, b, c, e, C.c_double(Bfd),
+                        int(apply_floor), F.ctypes.data_as(_dp), lam.ctypes.data_as(_dp))
+    return (F, lam) if want_lam else F
+
+
+# ------------------------------------------------------------------ block level
+def shapes(nmb, n, ng=4):
+    nt = n + 2 * ng
+    px = nt + 4
+    return dict(cell=(nmb, nt, nt, nt), xf=(nmb, nt, nt, px), yf=(nmb, nt, nt + 1, nt),
+                zf=(nmb, nt + 1, nt, nt), ex=(nmb, nt + 1, nt + 1, nt),
+                ey=(nmb, nt + 1, nt, px), ez=(nmb, nt, nt + 1, px))
+
+
+def con2prim(par, U, Bf, g, nthreads=1):
+    """U: list of 5 cell arrays (modified in place), Bf: 3 face arrays, g: 6 cell arrays.
+    returns W (8 arrays), status (u8)."""
+    sh = shapes(par.nmb, par.n)
+    W = [np.zeros(sh["cell"]) for _ in range(8)]
+    st = np.zeros(sh["cell"], dtype=np.uint8)
+    lib().orc_con2prim(C.byref(par), _ptrs(U), _ptrs(Bf), _ptrs(g), _ptrs(W),
+                       st.ctypes.data_as(C.c_void_p), int(nthreads))
+    return W, st
+
+
+def rhs(par, dx, U, Bf, adm, dt_fofc, W=None, nthreads=1, want_flux=False):
+    """One full stage.  U (5, modified in place where floored), Bf (3), adm (16): lists of
+    float64 arrays in the boundary layouts.  Returns dict with W, dU, E, flag, status,
+    and optionally flux (21 arrays) + refl (3 u8 arrays)."""
+    sh = shapes(par.nmb, par.n)
+    dx = np.ascontiguousarray(dx, dtype=np.float64).reshape(par.nmb, 3)
+    w_valid = W is not None
+    if W is None:
+        W = [np.zeros(sh["cell"]) for _ in range(8)]
+    dU = [np.zeros(sh["cell"]) for _ in range(5)]
+    E = [np.zeros(sh["ex"]), np.zeros(sh["ey"]), np.zeros(sh["ez"])]
+    flag = np.zeros(sh["cell"], dtype=np.uint8)
+    status = np.zeros(sh["cell"], dtype=np.uint8)
+    flux = refl = None
+    fp = rp = None
+    if want_flux:
+        flux = [np.zeros(sh[k]) for k in ("xf", "yf", "zf") for _ in range(7)]
+        refl = [np.zeros(sh[k], dtype=np.uint8) for k in ("xf", "yf", "zf")]
+        fp = _ptrs(flux)
+        rp = (C.c_void_p * 3)(*[r.ctypes.data for r in refl])
+    lib().orc_rhs(C.byref(par), dx.ctypes.data_as(_dp), _ptrs(U), _ptrs(Bf), _ptrs(adm),
+                  _ptrs(W), int(w_valid), C.c_double(dt_fofc), _ptrs(dU), _ptrs(E),
+                  flag.ctypes.data_as(C.c_void_p), status.ctypes.data_as(C.c_void_p),
+                  fp, rp, int(nthreads))
+    return dict(W=W, dU=dU, E=E, flag=flag, status=status, flux=flux, refl=refl)
