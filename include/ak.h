@@ -1,0 +1,172 @@
+/* include/ak.h — C-ABI boundary of the B200-native GRMHD right-hand-side stage.
+ *
+ * What the library computes: one finite-volume RHS stage of the 3+1 Valencia GRMHD system
+ * of arXiv:2409.10384 on a frozen ADM snapshot, over a batch of independent MeshBlocks.
+ * Citations "P:n" are line numbers of PAPER.md; "D:§" are sections of DESIGN.md.
+ *
+ *   part (1) conservative -> primitive recovery, ideal gas, floors/atmosphere
+ *   part (2) donor-cell / PPM4 / WENO-Z reconstruction of (rho, W v^i, P, B~)
+ *   part (3) LLF / HLLE fluxes of Eq. 8 with a face-averaged metric
+ *   part (4) first-order flux correction, optional relaxed maximum principle   P:141-157 (Eq. 12)
+ *   part (5) upwind constrained-transport edge EMFs
+ *   part (6) flux divergence + geometric sources of Eq. 9
+ *
+ * Every step runs in hand-written sm_100a CUDA kernels; there is no CPU fallback.  All
+ * arithmetic is IEEE fp64 (the library is built with --fmad=false so that masks are
+ * bit-reproducible against the reference arithmetic stated in D:§3).
+ *
+ * ---- Layout (D:§2).  A MeshBlock has n^3 interior cells and ng = 4 ghost layers per side;
+ * nt = n + 8 stored cells per direction; i (x) is the fastest index, then j, k, then block m.
+ * px = nt + 4 is the padded pitch of every array that has nt+1 points along x (row stride a
+ * multiple of 32 B).  Face i of direction x lies between cells i-1 and i; likewise j, k.
+ *   cell field    [nmb][nt][nt][nt]
+ *   x-face field  [nmb][nt][nt][px]        (nt+1 used)
+ *   y-face field  [nmb][nt][nt+1][nt]
+ *   z-face field  [nmb][nt+1][nt][nt]
+ *   E_x (x-edges) [nmb][nt+1][nt+1][nt]
+ *   E_y (y-edges) [nmb][nt+1][nt][px]
+ *   E_z (z-edges) [nmb][nt][nt+1][px]
+ * A tilde means "densitised", i.e. multiplied by sqrt(det gamma_ij).
+ *
+ * ---- Ownership.  Every field pointer is a DEVICE pointer owned by the caller (8-byte
+ * aligned fp64, or bytes for masks) unless a function says "host".  The context borrows
+ * pointers for the duration of one call (metric: until replaced or ak_destroy) and owns
+ * only its scratch (face fluxes, cell-centred EMFs, FOFC face lists, counters).
+ *
+ * ---- Asynchrony.  ak_con2prim / ak_rhs / ak_emf enqueue on the context's stream and
+ * return; they never synchronise.  ak_get_stats and the *_host entry points synchronise.
+ *
+ * ---- Errors.  Return codes report API misuse and CUDA failures only.  Unphysical cells
+ * are data ("it is flagged"): they are reported through status / flag bytes and the
+ * counters of ak_stats.
+ */
+#ifndef AK_H
+#define AK_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ak_ctx ak_ctx; /* opaque */
+
+enum { AK_OK = 0, AK_EINVAL = -1, AK_ENOMEM = -2, AK_ECUDA = -3, AK_ESTATE = -4 };
+enum { AK_RECON_DC = 0, AK_RECON_PPM4 = 1, AK_RECON_WENOZ = 2 };
+enum { AK_RS_LLF = 0, AK_RS_HLLE = 1 };
+
+/* status / flag bits (D:§2.4).  status = what con2prim did to a cell; fofc_flag = the status
+ * of the FOFC estimate of that cell, plus AK_ST_DMP (Eq. 12). */
+enum {
+  AK_ST_DFLOOR = 1,    /* D < f_thr rho_atm: cell reset to static atmosphere        */
+  AK_ST_TAUFLOOR = 2,  /* tau raised to tau_atm(D,B)                                */
+  AK_ST_MAGCAP = 4,    /* D raised to B^2 / M_max                                   */
+  AK_ST_RHOFLOOR = 8,  /* recovered rho < f_thr rho_atm: reset to atmosphere        */
+  AK_ST_TFLOOR = 16,   /* recovered T < T_atm: T reset, P recomputed                */
+  AK_ST_FAIL = 32,     /* non-finite input, no bracket or no convergence: atmosphere */
+  AK_ST_DMP = 64       /* discrete maximum principle violated (flag byte only)       */
+};
+
+typedef struct {
+  int nmb, n, ng;            /* MeshBlocks, interior cells per edge (even, >= 4), ghosts (== 4) */
+  double gamma_ad;           /* ideal-gas Gamma > 1; P = (Gamma-1) rho eps, T = P/rho (D:R3)     */
+  double rho_atm, T_atm;     /* atmosphere density and temperature                      */
+  double f_thr;              /* threshold factor on rho_atm                             */
+  double mag_max;            /* M_max: cap on B^2/D; +inf disables                      */
+  int recon;                 /* AK_RECON_* of the high-order pass                               */
+  int riemann;               /* AK_RS_*    of the high-order pass                               */
+  int fofc;                  /* 0/1: first-order flux correction                        */
+  int fofc_riemann;          /* AK_RS_* used when a face is redone at first order       */
+  double dmp_M;              /* <= 0: no maximum principle; else M >= 1 of Eq. 12       */
+  int c2p_max_iter;          /* cap on master-function evaluations per root find (e.g. 40)      */
+  double c2p_tol;            /* relative step tolerance on mu (e.g. 1e-15)                      */
+  int device;                /* CUDA device ordinal                                             */
+  void* stream;              /* cudaStream_t (0 = legacy default stream)                        */
+} ak_params;
+
+typedef struct { double *D, *Sx, *Sy, *Sz, *tau; } ak_cons;              /* cell fields, U~   */
+typedef struct { const double *bx, *by, *bz; } ak_faceB;                 /* face fields, B~f  */
+typedef struct { double *rho, *ux, *uy, *uz, *p, *bccx, *bccy, *bccz; } ak_prim;
+                                   /* cell fields: rho, u^i = W v^i, P, cell-centred B~^i     */
+typedef struct {
+  const double *gxx, *gxy, *gxz, *gyy, *gyz, *gzz, *alp, *betx, *bety, *betz,
+               *Kxx, *Kxy, *Kxz, *Kyy, *Kyz, *Kzz;
+} ak_adm;                          /* cell fields: gamma_ij, alpha, beta^i, K_ij (Eq. 5)      */
+typedef struct {
+  double *dD, *dSx, *dSy, *dSz, *dtau; /* cell fields; interior cells written, rest untouched */
+  double *Ex, *Ey, *Ez;                /* edge fields; edges of interior cells written        */
+  unsigned char* fofc_flag;            /* [nmb][nt^3] bytes, fully written (0 outside the     */
+                                       /* tested range); may be NULL                          */
+  unsigned char* c2p_status;           /* [nmb][nt^3] bytes, written when part (1) runs;      */
+                                       /* may be NULL                                         */
+} ak_rhs_out;
+
+typedef struct {
+  long long n_c2p_fail;      /* cells whose con2prim status has AK_ST_FAIL (last part (1))      */
+  long long n_cons_floor;    /* ... any of DFLOOR | TAUFLOOR | MAGCAP                           */
+  long long n_prim_floor;    /* ... any of RHOFLOOR | TFLOOR                                    */
+  long long n_fofc_cells;    /* cells flagged by the last FOFC test                             */
+  long long n_dmp_cells;     /* ... of which carry AK_ST_DMP                                    */
+  long long n_fofc_faces[3]; /* faces redone at first order, per direction                      */
+} ak_stats;
+
+/* Create a context for a batch shape and a parameter set.  dx3 is a HOST array [nmb][3] of
+ * cell widths (dx,dy,dz) per block; it is copied.  Validates everything before touching
+ * CUDA (AK_EINVAL), then allocates scratch (AK_ENOMEM / AK_ECUDA). */
+int ak_create(const ak_params* p, const double* dx3, ak_ctx** out);
+
+/* Borrow the frozen ADM snapshot (16 cell fields).  Must precede the compute calls. */
+int ak_set_metric(ak_ctx*, const ak_adm* adm);
+
+/* Part (1) over all nt^3 stored cells of every block (floors are applied "after ...
+ * the conserved-to-primitive inversion"; ghosts are needed by parts (2)-(4)).
+ * U is in-out: cells with a non-zero status are rewritten from the final primitives
+ * ("a similar policy holds for the conserved variables").  status may be NULL. */
+int ak_con2prim(ak_ctx*, const ak_cons* U, const ak_faceB* Bf, const ak_prim* W,
+                unsigned char* status);
+
+/* Parts (1)-(6).  If w_is_valid != 0 part (1) is skipped and W is read as given.
+ * dt_fofc is the time step of the FOFC estimate U* = U - dt_fofc div F (D:R9). */
+int ak_rhs(ak_ctx*, const ak_cons* U, const ak_faceB* Bf, const ak_prim* W, int w_is_valid,
+           double dt_fofc, const ak_rhs_out* out);
+
+/* Part (5) alone, from the (post-FOFC) fluxes the last ak_rhs left in the context
+ * (AK_ESTATE if there are none) and the primitives W. */
+int ak_emf(ak_ctx*, const ak_prim* W, double* Ex, double* Ey, double* Ez);
+
+/* Copy the device counters to the host.  Synchronises the stream. */
+int ak_get_stats(ak_ctx*, ak_stats* host_out);
+
+/* Read back one post-FOFC face-flux field kept in scratch (dir 0..2, comp 0..6 =
+ * D,Sx,Sy,Sz,tau,B~t1,B~t2 with t1,t2 cyclic after dir) into a caller DEVICE buffer in the
+ * face layout of dir.  For tests and diagnostics.  AK_ESTATE before the first ak_rhs. */
+int ak_get_flux(ak_ctx*, int dir, int comp, double* dst);
+
+/* End-to-end convenience: the same stage with HOST buffers.  All pointers inside U, Bf,
+ * W, out are host pointers (pinned memory recommended); the metric must already be set with
+ * ak_set_metric (device pointers: the snapshot is frozen across stages).  Copies U and Bf
+ * to context-owned device staging, runs parts (1)-(6), copies back U (floored cells), W,
+ * dU, E and the two masks, and synchronises.  Staging is allocated on first use. */
+int ak_rhs_host(ak_ctx*, const ak_cons* U, const ak_faceB* Bf, const ak_prim* W,
+                double dt_fofc, const ak_rhs_out* out);
+
+/* Device-timing hooks for the benchmark: bracket kernel class `which` (0 con2prim, 1-3 flux
+ * sweeps x/y/z, 4 FOFC test, 5 FOFC list+reflux, 6 cell EMF+CT, 7 divergence+sources) with
+ * CUDA events on the context's stream in subsequent calls; ak_kernel_ms synchronises and
+ * returns the accumulated milliseconds and launch count since ak_timing was enabled. */
+int ak_timing(ak_ctx*, int enable);
+int ak_kernel_ms(ak_ctx*, double ms_out[8], long long launches_out[8]);
+
+/* Peak probes used as same-run roofline denominators (D:§7): a fp64 copy kernel over
+ * nbytes (read+write counted) and an independent-DADD/DMUL/DFMA stream.  Results in GB/s and
+ * Gop/s (warp-wide fp64 instructions x 32 lanes / s).  Synchronise. */
+int ak_probe_copy(ak_ctx*, double* dst, const double* src, long long n_doubles, int reps,
+                  double* gbs_out);
+int ak_probe_fp64(ak_ctx*, int use_fma, int reps, double* gops_out);
+
+int ak_destroy(ak_ctx*);
+const char* ak_strerror(int code);
+const char* ak_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AK_H */

@@ -1,0 +1,542 @@
+// ak_api.cu — the C-ABI of include/ak.h: context, validation, launch sequence of one stage.
+// Build: nvcc -gencode arch=compute_100a,code=sm_100a --fmad=false -lineinfo (see build.py).
+#include "../../include/ak.h"
+#include "ak_source.cuh"
+
+#include <cmath>
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+using namespace ak;
+
+namespace {
+
+enum { KC_C2P = 0, KC_FX, KC_FY, KC_FZ, KC_FOFC_TEST, KC_FOFC_FIX, KC_CT, KC_SRC, KC_N };
+
+struct Sizes {
+  long long cell, xf, yf, zf, ex, ey, ez;   // elements per batch
+};
+
+}  // namespace
+
+struct ak_ctx {
+  ak_params hp;
+  Par P;
+  Sizes sz;
+  cudaStream_t stream;
+  bool have_metric, have_flux;
+  const double* adm[16];
+  // scratch
+  double* F[21];
+  double* Ecc[3];
+  unsigned char* flag_own;
+  unsigned int* list[3];
+  unsigned int* count;          // [4]
+  unsigned long long* stats;    // [S_NSTAT]
+  double* dx;
+  // host staging for ak_rhs_host
+  double* stg_U[5]; double* stg_Bf[3]; double* stg_W[8]; double* stg_dU[5]; double* stg_E[3];
+  unsigned char* stg_flag; unsigned char* stg_status;
+  bool have_stg;
+  // timing
+  bool timing;
+  cudaEvent_t ev0, ev1;
+  double ms[KC_N];
+  long long launches[KC_N];
+  struct Pending { int which; cudaEvent_t a, b; };
+  Pending* pend; int npend, cappend;
+};
+
+namespace {
+
+#define CK(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { \
+  last_cuda_error = e_; return e_ == cudaErrorMemoryAllocation ? AK_ENOMEM : AK_ECUDA; } } while (0)
+
+thread_local cudaError_t last_cuda_error = cudaSuccess;
+
+inline bool finite_pos(double x) { return std::isfinite(x) && x > 0.0; }
+
+int validate(const ak_params* p, const double* dx3) {
+  if (!p || !dx3) return AK_EINVAL;
+  if (p->nmb < 1 || p->n < 2 || p->ng != 4) return AK_EINVAL;
+  if (!(std::isfinite(p->gamma_ad) && p->gamma_ad > 1.0)) return AK_EINVAL;
+  if (!finite_pos(p->rho_atm) || !finite_pos(p->T_atm) || !finite_pos(p->f_thr)) return AK_EINVAL;
+  if (!(p->mag_max > 0.0)) return AK_EINVAL;   // +inf allowed, NaN rejected
+  if (p->recon < 0 || p->recon > 2 || p->riemann < 0 || p->riemann > 1) return AK_EINVAL;
+  if (p->fofc < 0 || p->fofc > 1 || p->fofc_riemann < 0 || p->fofc_riemann > 1) return AK_EINVAL;
+  if (std::isnan(p->dmp_M) || (p->dmp_M > 0.0 && p->dmp_M < 1.0)) return AK_EINVAL;
+  if (p->c2p_max_iter < 1 || p->c2p_max_iter > 1000) return AK_EINVAL;
+  if (!(p->c2p_tol > 0.0 && p->c2p_tol < 1.0)) return AK_EINVAL;
+  if (p->device < 0) return AK_EINVAL;
+  const long long nt = p->n + 8;
+  // face-list entries are 32-bit cell indices
+  if ((long long)p->nmb * (nt + 1) * (nt + 1) * (nt + 4) >= (1LL << 31)) return AK_EINVAL;
+  for (long long q = 0; q < 3LL * p->nmb; ++q)
+    if (!finite_pos(dx3[q])) return AK_EINVAL;
+  return AK_OK;
+}
+
+inline unsigned nblk(long long n, int t) { return (unsigned)((n + t - 1) / t); }
+
+struct Timer {
+  ak_ctx* c; int which; cudaEvent_t a, b; bool on;
+  Timer(ak_ctx* c_, int w) : c(c_), which(w), on(c_->timing) {
+    if (on) {
+      cudaEventCreate(&a); cudaEventCreate(&b);
+      cudaEventRecord(a, c->stream);
+    }
+  }
+  ~Timer() {
+    if (!on) return;
+    cudaEventRecord(b, c->stream);
+    if (c->npend == c->cappend) {
+      int nc = c->cappend ? 2 * c->cappend : 256;
+      ak_ctx::Pending* np = (ak_ctx::Pending*)realloc(c->pend, sizeof(ak_ctx::Pending) * nc);
+      if (!np) { cudaEventDestroy(a); cudaEventDestroy(b); return; }
+      c->pend = np; c->cappend = nc;
+    }
+    c->pend[c->npend++] = {which, a, b};
+  }
+};
+
+void fill_fields(ak_ctx* c, Fields& f) {
+  memset(&f, 0, sizeof(f));
+  for (int q = 0; q < 16; ++q) f.adm[q] = c->adm[q];
+  for (int q = 0; q < 21; ++q) f.F[q] = c->F[q];
+  for (int q = 0; q < 3; ++q) { f.Ecc[q] = c->Ecc[q]; f.list[q] = c->list[q]; }
+  f.count = c->count;
+  f.stats = c->stats;
+  f.dx = c->dx;
+  f.flag = c->flag_own;
+}
+
+bool set_cons(Fields& f, const ak_cons* U) {
+  if (!U || !U->D || !U->Sx || !U->Sy || !U->Sz || !U->tau) return false;
+  f.U[0] = U->D; f.U[1] = U->Sx; f.U[2] = U->Sy; f.U[3] = U->Sz; f.U[4] = U->tau;
+  return true;
+}
+bool set_faceB(Fields& f, const ak_faceB* B) {
+  if (!B || !B->bx || !B->by || !B->bz) return false;
+  f.Bf[0] = B->bx; f.Bf[1] = B->by; f.Bf[2] = B->bz;
+  return true;
+}
+bool set_prim(Fields& f, const ak_prim* W) {
+  if (!W || !W->rho || !W->ux || !W->uy || !W->uz || !W->p || !W->bccx || !W->bccy || !W->bccz)
+    return false;
+  f.W[0] = W->rho; f.W[1] = W->ux; f.W[2] = W->uy; f.W[3] = W->uz; f.W[4] = W->p;
+  f.W[5] = W->bccx; f.W[6] = W->bccy; f.W[7] = W->bccz;
+  return true;
+}
+
+int launch_c2p(ak_ctx* c, const Fields& f) {
+  Timer t(c, KC_C2P);
+  CK(cudaMemsetAsync(c->stats, 0, sizeof(unsigned long long) * 3, c->stream));
+  k_con2prim<<<nblk(c->sz.cell, 128), 128, 0, c->stream>>>(c->P, f);
+  c->launches[KC_C2P] += 1;
+  CK(cudaGetLastError());
+  return AK_OK;
+}
+
+template <int DIR>
+int launch_flux(ak_ctx* c, const Fields& f) {
+  Timer t(c, KC_FX + DIR);
+  const long long n = c->P.n;
+  const long long nf = (n + 3) * (n + 2) * (n + 2) * c->P.nmb;
+  const unsigned g = nblk(nf, 128);
+  switch (c->P.recon) {
+    case 0: k_flux<DIR, 0><<<g, 128, 0, c->stream>>>(c->P, f); break;
+    case 1: k_flux<DIR, 1><<<g, 128, 0, c->stream>>>(c->P, f); break;
+    default: k_flux<DIR, 2><<<g, 128, 0, c->stream>>>(c->P, f); break;
+  }
+  CK(cudaGetLastError());
+  c->launches[KC_FX + DIR] += 1;
+  return AK_OK;
+}
+
+int launch_fofc(ak_ctx* c, const Fields& f, double dt) {
+  const long long n = c->P.n;
+  const long long ntest = (n + 2) * (n + 2) * (n + 2) * c->P.nmb;
+  const long long nf = (n + 3) * (n + 2) * (n + 2) * c->P.nmb;
+  {
+    Timer t(c, KC_FOFC_TEST);
+    CK(cudaMemsetAsync(f.flag, 0, (size_t)c->sz.cell, c->stream));
+    CK(cudaMemsetAsync(c->count, 0, sizeof(unsigned) * 4, c->stream));
+    CK(cudaMemsetAsync(c->stats + S_FOFC_CELLS, 0, sizeof(unsigned long long) * 2, c->stream));
+    if (c->P.fofc) {
+      k_fofc_test<<<nblk(ntest, 128), 128, 0, c->stream>>>(c->P, f, dt);
+      c->launches[KC_FOFC_TEST] += 1;
+      CK(cudaGetLastError());
+    }
+  }
+  if (c->P.fofc) {
+    Timer t(c, KC_FOFC_FIX);
+    k_fofc_list<0><<<nblk(nf, 256), 256, 0, c->stream>>>(c->P, f);
+    k_fofc_list<1><<<nblk(nf, 256), 256, 0, c->stream>>>(c->P, f);
+    k_fofc_list<2><<<nblk(nf, 256), 256, 0, c->stream>>>(c->P, f);
+    CK(cudaGetLastError());
+    const unsigned g = (unsigned)(nf < 148LL * 8 * 128 ? nblk(nf, 128) : 148 * 8);
+    k_fofc_reflux<0><<<g, 128, 0, c->stream>>>(c->P, f);
+    k_fofc_reflux<1><<<g, 128, 0, c->stream>>>(c->P, f);
+    k_fofc_reflux<2><<<g, 128, 0, c->stream>>>(c->P, f);
+    CK(cudaGetLastError());
+    c->launches[KC_FOFC_FIX] += 6;
+  }
+  return AK_OK;
+}
+
+int launch_ct(ak_ctx* c, const Fields& f) {
+  Timer t(c, KC_CT);
+  const long long n = c->P.n;
+  const long long ntest = (n + 2) * (n + 2) * (n + 2) * c->P.nmb;
+  const long long ne = n * (n + 1) * (n + 1) * c->P.nmb;
+  k_cell_emf<<<nblk(ntest, 128), 128, 0, c->stream>>>(c->P, f);
+  k_ct<0><<<nblk(ne, 128), 128, 0, c->stream>>>(c->P, f);
+  k_ct<1><<<nblk(ne, 128), 128, 0, c->stream>>>(c->P, f);
+  k_ct<2><<<nblk(ne, 128), 128, 0, c->stream>>>(c->P, f);
+  CK(cudaGetLastError());
+  c->launches[KC_CT] += 4;
+  return AK_OK;
+}
+
+int launch_src(ak_ctx* c, const Fields& f) {
+  Timer t(c, KC_SRC);
+  const long long n = c->P.n;
+  k_div_src<<<nblk(n * n * n * c->P.nmb, 128), 128, 0, c->stream>>>(c->P, f);
+  CK(cudaGetLastError());
+  c->launches[KC_SRC] += 1;
+  return AK_OK;
+}
+
+int drain_timers(ak_ctx* c) {
+  for (int q = 0; q < c->npend; ++q) {
+    float ms = 0.f;
+    cudaError_t e = cudaEventSynchronize(c->pend[q].b);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, c->pend[q].a, c->pend[q].b);
+    cudaEventDestroy(c->pend[q].a); cudaEventDestroy(c->pend[q].b);
+    if (e != cudaSuccess) { c->npend = 0; last_cuda_error = e; return AK_ECUDA; }
+    c->ms[c->pend[q].which] += ms;
+  }
+  c->npend = 0;
+  return AK_OK;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------ probes (roofline denominators)
+namespace {
+__global__ void __launch_bounds__(256) k_probe_copy(double2* __restrict__ dst, const double2* __restrict__ src,
+                                                    long long n2) {
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < n2; q += stride) dst[q] = src[q];
+}
+// 8 independent accumulator chains per thread; FMA = 1 instruction (2 flop), else MUL + ADD.
+template <bool FMA>
+__global__ void __launch_bounds__(256) k_probe_fp64(double* out, int iters, double a, double b) {
+  double x[8];
+#pragma unroll
+  for (int q = 0; q < 8; ++q) x[q] = 1.0 + 1e-3 * (threadIdx.x + q);
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+      if (FMA) x[q] = __fma_rn(x[q], a, b);
+      else x[q] = __dadd_rn(__dmul_rn(x[q], a), b);
+    }
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int q = 0; q < 8; ++q) s += x[q];
+  if (s == 123.456) out[0] = s;   // never true; keeps the chains alive
+}
+}  // namespace
+
+// ------------------------------------------------------------------ C-ABI
+extern "C" {
+
+const char* ak_version(void) { return "ak 0.1 (sm_100a, fp64, --fmad=false)"; }
+
+const char* ak_strerror(int code) {
+  switch (code) {
+    case AK_OK: return "ok";
+    case AK_EINVAL: return "invalid argument";
+    case AK_ENOMEM: return "out of device memory";
+    case AK_ECUDA: return last_cuda_error != cudaSuccess ? cudaGetErrorString(last_cuda_error) : "CUDA error";
+    case AK_ESTATE: return "call out of order (metric or fluxes missing)";
+    default: return "unknown error code";
+  }
+}
+
+int ak_create(const ak_params* p, const double* dx3, ak_ctx** out) {
+  if (!out) return AK_EINVAL;
+  *out = nullptr;
+  const int v = validate(p, dx3);
+  if (v != AK_OK) return v;
+  int ndev = 0;
+  CK(cudaGetDeviceCount(&ndev));
+  if (p->device >= ndev) return AK_EINVAL;
+  CK(cudaSetDevice(p->device));
+  ak_ctx* c = new (std::nothrow) ak_ctx();
+  if (!c) return AK_ENOMEM;
+  memset(c, 0, sizeof(*c));
+  c->hp = *p;
+  c->stream = (cudaStream_t)p->stream;
+  Par& P = c->P;
+  P.nmb = p->nmb; P.n = p->n; P.nt = p->n + 8; P.px = P.nt + 4; P.is = 4; P.ie = p->n + 3;
+  P.Gam = p->gamma_ad; P.gm1 = p->gamma_ad - 1.0; P.gm1r = p->gamma_ad / (p->gamma_ad - 1.0);
+  P.rho_atm = p->rho_atm; P.T_atm = p->T_atm; P.P_atm = p->rho_atm * p->T_atm;
+  P.eps_atm = p->T_atm / P.gm1; P.thr = p->f_thr * p->rho_atm;
+  P.mag_max = p->mag_max;
+  P.dmp_M = p->dmp_M; P.dmp_iM = p->dmp_M > 0.0 ? 1.0 / p->dmp_M : 0.0;
+  P.max_iter = p->c2p_max_iter; P.tol = p->c2p_tol;
+  P.recon = p->recon; P.riemann = p->riemann; P.fofc = p->fofc; P.fofc_riemann = p->fofc_riemann;
+  const long long nt = P.nt, px = P.px, nb = P.nmb;
+  c->sz.cell = nb * nt * nt * nt;
+  c->sz.xf = nb * nt * nt * px; c->sz.yf = nb * nt * (nt + 1) * nt; c->sz.zf = nb * (nt + 1) * nt * nt;
+  c->sz.ex = nb * (nt + 1) * (nt + 1) * nt; c->sz.ey = nb * (nt + 1) * nt * px; c->sz.ez = nb * nt * (nt + 1) * px;
+  const long long fsz[3] = {c->sz.xf, c->sz.yf, c->sz.zf};
+  const long long nfaces = nb * (P.n + 3) * (P.n + 2) * (P.n + 2);
+  cudaError_t e = cudaSuccess;
+  for (int d = 0; d < 3 && e == cudaSuccess; ++d) {
+    for (int q = 0; q < 7 && e == cudaSuccess; ++q) {
+      e = cudaMalloc(&c->F[7 * d + q], sizeof(double) * fsz[d]);
+      // faces outside the computed range are never written: define them once
+      if (e == cudaSuccess) e = cudaMemsetAsync(c->F[7 * d + q], 0, sizeof(double) * fsz[d], c->stream);
+    }
+    if (e == cudaSuccess) e = cudaMalloc(&c->Ecc[d], sizeof(double) * c->sz.cell);
+    if (e == cudaSuccess) e = cudaMemsetAsync(c->Ecc[d], 0, sizeof(double) * c->sz.cell, c->stream);
+    if (e == cudaSuccess) e = cudaMalloc(&c->list[d], sizeof(unsigned) * nfaces);
+  }
+  if (e == cudaSuccess) e = cudaMalloc(&c->flag_own, (size_t)c->sz.cell);
+  if (e == cudaSuccess) e = cudaMalloc(&c->count, sizeof(unsigned) * 4);
+  if (e == cudaSuccess) e = cudaMalloc(&c->stats, sizeof(unsigned long long) * S_NSTAT);
+  if (e == cudaSuccess) e = cudaMemsetAsync(c->count, 0, sizeof(unsigned) * 4, c->stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(c->stats, 0, sizeof(unsigned long long) * S_NSTAT, c->stream);
+  if (e == cudaSuccess) e = cudaMalloc(&c->dx, sizeof(double) * 3 * nb);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(c->dx, dx3, sizeof(double) * 3 * nb, cudaMemcpyHostToDevice, c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);   // dx3 is the caller's: copy must be done
+  if (e != cudaSuccess) {
+    last_cuda_error = e;
+    ak_destroy(c);
+    cudaGetLastError();
+    return e == cudaErrorMemoryAllocation ? AK_ENOMEM : AK_ECUDA;
+  }
+  *out = c;
+  return AK_OK;
+}
+
+int ak_destroy(ak_ctx* c) {
+  if (!c) return AK_EINVAL;
+  cudaSetDevice(c->hp.device);
+  cudaStreamSynchronize(c->stream);
+  for (int q = 0; q < c->npend; ++q) { cudaEventDestroy(c->pend[q].a); cudaEventDestroy(c->pend[q].b); }
+  free(c->pend);
+  for (int q = 0; q < 21; ++q) cudaFree(c->F[q]);
+  for (int q = 0; q < 3; ++q) { cudaFree(c->Ecc[q]); cudaFree(c->list[q]); cudaFree(c->stg_Bf[q]); cudaFree(c->stg_E[q]); }
+  for (int q = 0; q < 5; ++q) { cudaFree(c->stg_U[q]); cudaFree(c->stg_dU[q]); }
+  for (int q = 0; q < 8; ++q) cudaFree(c->stg_W[q]);
+  cudaFree(c->stg_flag); cudaFree(c->stg_status);
+  cudaFree(c->flag_own); cudaFree(c->count); cudaFree(c->stats); cudaFree(c->dx);
+  delete c;
+  return AK_OK;
+}
+
+int ak_set_metric(ak_ctx* c, const ak_adm* a) {
+  if (!c || !a) return AK_EINVAL;
+  const double* p[16] = {a->gxx, a->gxy, a->gxz, a->gyy, a->gyz, a->gzz, a->alp, a->betx, a->bety, a->betz,
+                         a->Kxx, a->Kxy, a->Kxz, a->Kyy, a->Kyz, a->Kzz};
+  for (int q = 0; q < 16; ++q)
+    if (!p[q] || ((uintptr_t)p[q] & 7u)) return AK_EINVAL;
+  for (int q = 0; q < 16; ++q) c->adm[q] = p[q];
+  c->have_metric = true;
+  return AK_OK;
+}
+
+int ak_con2prim(ak_ctx* c, const ak_cons* U, const ak_faceB* Bf, const ak_prim* W, unsigned char* status) {
+  if (!c) return AK_EINVAL;
+  if (!c->have_metric) return AK_ESTATE;
+  Fields f;
+  fill_fields(c, f);
+  if (!set_cons(f, U) || !set_faceB(f, Bf) || !set_prim(f, W)) return AK_EINVAL;
+  f.status = status;
+  CK(cudaSetDevice(c->hp.device));
+  return launch_c2p(c, f);
+}
+
+int ak_rhs(ak_ctx* c, const ak_cons* U, const ak_faceB* Bf, const ak_prim* W, int w_is_valid, double dt_fofc,
+           const ak_rhs_out* out) {
+  if (!c || !out) return AK_EINVAL;
+  if (!c->have_metric) return AK_ESTATE;
+  if (!std::isfinite(dt_fofc)) return AK_EINVAL;
+  Fields f;
+  fill_fields(c, f);
+  if (!set_cons(f, U) || !set_faceB(f, Bf) || !set_prim(f, W)) return AK_EINVAL;
+  if (!out->dD || !out->dSx || !out->dSy || !out->dSz || !out->dtau || !out->Ex || !out->Ey || !out->Ez)
+    return AK_EINVAL;
+  f.dU[0] = out->dD; f.dU[1] = out->dSx; f.dU[2] = out->dSy; f.dU[3] = out->dSz; f.dU[4] = out->dtau;
+  f.E[0] = out->Ex; f.E[1] = out->Ey; f.E[2] = out->Ez;
+  if (out->fofc_flag) f.flag = out->fofc_flag;
+  f.status = out->c2p_status;
+  CK(cudaSetDevice(c->hp.device));
+  int r;
+  if (!w_is_valid && (r = launch_c2p(c, f)) != AK_OK) return r;
+  if ((r = launch_flux<0>(c, f)) != AK_OK) return r;
+  if ((r = launch_flux<1>(c, f)) != AK_OK) return r;
+  if ((r = launch_flux<2>(c, f)) != AK_OK) return r;
+  if ((r = launch_fofc(c, f, dt_fofc)) != AK_OK) return r;
+  c->have_flux = true;
+  if ((r = launch_ct(c, f)) != AK_OK) return r;
+  return launch_src(c, f);
+}
+
+int ak_emf(ak_ctx* c, const ak_prim* W, double* Ex, double* Ey, double* Ez) {
+  if (!c || !Ex || !Ey || !Ez) return AK_EINVAL;
+  if (!c->have_metric || !c->have_flux) return AK_ESTATE;
+  Fields f;
+  fill_fields(c, f);
+  if (!set_prim(f, W)) return AK_EINVAL;
+  f.E[0] = Ex; f.E[1] = Ey; f.E[2] = Ez;
+  CK(cudaSetDevice(c->hp.device));
+  return launch_ct(c, f);
+}
+
+int ak_get_stats(ak_ctx* c, ak_stats* o) {
+  if (!c || !o) return AK_EINVAL;
+  unsigned long long h[S_NSTAT];
+  unsigned cnt[4];
+  CK(cudaSetDevice(c->hp.device));
+  CK(cudaMemcpyAsync(h, c->stats, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaMemcpyAsync(cnt, c->count, sizeof(cnt), cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  o->n_c2p_fail = (long long)h[S_C2P_FAIL];
+  o->n_cons_floor = (long long)h[S_CONS_FLOOR];
+  o->n_prim_floor = (long long)h[S_PRIM_FLOOR];
+  o->n_fofc_cells = (long long)h[S_FOFC_CELLS];
+  o->n_dmp_cells = (long long)h[S_DMP_CELLS];
+  for (int d = 0; d < 3; ++d) o->n_fofc_faces[d] = cnt[d];
+  return AK_OK;
+}
+
+int ak_get_flux(ak_ctx* c, int dir, int comp, double* dst) {
+  if (!c || !dst || dir < 0 || dir > 2 || comp < 0 || comp > 6) return AK_EINVAL;
+  if (!c->have_flux) return AK_ESTATE;
+  const long long fsz[3] = {c->sz.xf, c->sz.yf, c->sz.zf};
+  CK(cudaSetDevice(c->hp.device));
+  CK(cudaMemcpyAsync(dst, c->F[7 * dir + comp], sizeof(double) * fsz[dir], cudaMemcpyDeviceToDevice, c->stream));
+  return AK_OK;
+}
+
+int ak_timing(ak_ctx* c, int enable) {
+  if (!c) return AK_EINVAL;
+  const int r = drain_timers(c);
+  c->timing = enable != 0;
+  for (int q = 0; q < KC_N; ++q) { c->ms[q] = 0.0; c->launches[q] = 0; }
+  return r;
+}
+
+int ak_kernel_ms(ak_ctx* c, double ms_out[8], long long launches_out[8]) {
+  if (!c || !ms_out || !launches_out) return AK_EINVAL;
+  CK(cudaSetDevice(c->hp.device));
+  const int r = drain_timers(c);
+  for (int q = 0; q < KC_N; ++q) { ms_out[q] = c->ms[q]; launches_out[q] = c->launches[q]; }
+  return r;
+}
+
+int ak_rhs_host(ak_ctx* c, const ak_cons* U, const ak_faceB* Bf, const ak_prim* W, double dt_fofc,
+                const ak_rhs_out* out) {
+  if (!c || !U || !Bf || !W || !out) return AK_EINVAL;
+  if (!c->have_metric) return AK_ESTATE;
+  CK(cudaSetDevice(c->hp.device));
+  const size_t cb = sizeof(double) * c->sz.cell;
+  const size_t fb[3] = {sizeof(double) * c->sz.xf, sizeof(double) * c->sz.yf, sizeof(double) * c->sz.zf};
+  const size_t eb[3] = {sizeof(double) * c->sz.ex, sizeof(double) * c->sz.ey, sizeof(double) * c->sz.ez};
+  if (!c->have_stg) {
+    for (int q = 0; q < 5; ++q) { CK(cudaMalloc(&c->stg_U[q], cb)); CK(cudaMalloc(&c->stg_dU[q], cb)); }
+    for (int q = 0; q < 8; ++q) CK(cudaMalloc(&c->stg_W[q], cb));
+    for (int q = 0; q < 3; ++q) { CK(cudaMalloc(&c->stg_Bf[q], fb[q])); CK(cudaMalloc(&c->stg_E[q], eb[q])); }
+    CK(cudaMalloc(&c->stg_flag, (size_t)c->sz.cell));
+    CK(cudaMalloc(&c->stg_status, (size_t)c->sz.cell));
+    for (int q = 0; q < 5; ++q) CK(cudaMemsetAsync(c->stg_dU[q], 0, cb, c->stream));
+    for (int q = 0; q < 3; ++q) CK(cudaMemsetAsync(c->stg_E[q], 0, eb[q], c->stream));
+    c->have_stg = true;
+  }
+  double* hU[5] = {U->D, U->Sx, U->Sy, U->Sz, U->tau};
+  const double* hB[3] = {Bf->bx, Bf->by, Bf->bz};
+  double* hW[8] = {W->rho, W->ux, W->uy, W->uz, W->p, W->bccx, W->bccy, W->bccz};
+  double* hdU[5] = {out->dD, out->dSx, out->dSy, out->dSz, out->dtau};
+  double* hE[3] = {out->Ex, out->Ey, out->Ez};
+  for (int q = 0; q < 5; ++q) if (!hU[q] || !hdU[q]) return AK_EINVAL;
+  for (int q = 0; q < 3; ++q) if (!hB[q] || !hE[q]) return AK_EINVAL;
+  for (int q = 0; q < 8; ++q) if (!hW[q]) return AK_EINVAL;
+  for (int q = 0; q < 5; ++q) CK(cudaMemcpyAsync(c->stg_U[q], hU[q], cb, cudaMemcpyHostToDevice, c->stream));
+  for (int q = 0; q < 3; ++q) CK(cudaMemcpyAsync(c->stg_Bf[q], hB[q], fb[q], cudaMemcpyHostToDevice, c->stream));
+  ak_cons dU_ = {c->stg_U[0], c->stg_U[1], c->stg_U[2], c->stg_U[3], c->stg_U[4]};
+  ak_faceB dB_ = {c->stg_Bf[0], c->stg_Bf[1], c->stg_Bf[2]};
+  ak_prim dW_ = {c->stg_W[0], c->stg_W[1], c->stg_W[2], c->stg_W[3], c->stg_W[4], c->stg_W[5], c->stg_W[6], c->stg_W[7]};
+  ak_rhs_out dO = {c->stg_dU[0], c->stg_dU[1], c->stg_dU[2], c->stg_dU[3], c->stg_dU[4],
+                   c->stg_E[0], c->stg_E[1], c->stg_E[2], c->stg_flag, c->stg_status};
+  const int r = ak_rhs(c, &dU_, &dB_, &dW_, 0, dt_fofc, &dO);
+  if (r != AK_OK) return r;
+  for (int q = 0; q < 5; ++q) {
+    CK(cudaMemcpyAsync(hU[q], c->stg_U[q], cb, cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaMemcpyAsync(hdU[q], c->stg_dU[q], cb, cudaMemcpyDeviceToHost, c->stream));
+  }
+  for (int q = 0; q < 8; ++q) CK(cudaMemcpyAsync(hW[q], c->stg_W[q], cb, cudaMemcpyDeviceToHost, c->stream));
+  for (int q = 0; q < 3; ++q) CK(cudaMemcpyAsync(hE[q], c->stg_E[q], eb[q], cudaMemcpyDeviceToHost, c->stream));
+  if (out->fofc_flag) CK(cudaMemcpyAsync(out->fofc_flag, c->stg_flag, (size_t)c->sz.cell, cudaMemcpyDeviceToHost, c->stream));
+  if (out->c2p_status) CK(cudaMemcpyAsync(out->c2p_status, c->stg_status, (size_t)c->sz.cell, cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  return AK_OK;
+}
+
+int ak_probe_copy(ak_ctx* c, double* dst, const double* src, long long n, int reps, double* gbs) {
+  if (!c || !dst || !src || n < 2 || reps < 1 || !gbs) return AK_EINVAL;
+  if (((uintptr_t)dst | (uintptr_t)src) & 15u) return AK_EINVAL;
+  CK(cudaSetDevice(c->hp.device));
+  cudaEvent_t a, b;
+  CK(cudaEventCreate(&a)); CK(cudaEventCreate(&b));
+  const long long n2 = n / 2;
+  double best = 0.0;
+  for (int r = 0; r < reps + 1; ++r) {
+    CK(cudaEventRecord(a, c->stream));
+    k_probe_copy<<<148 * 16, 256, 0, c->stream>>>((double2*)dst, (const double2*)src, n2);
+    CK(cudaEventRecord(b, c->stream));
+    CK(cudaEventSynchronize(b));
+    float ms = 0.f;
+    CK(cudaEventElapsedTime(&ms, a, b));
+    const double g = 2.0 * 16.0 * (double)n2 / (ms * 1e-3) * 1e-9;
+    if (r > 0 && g > best) best = g;
+  }
+  cudaEventDestroy(a); cudaEventDestroy(b);
+  CK(cudaGetLastError());
+  *gbs = best;
+  return AK_OK;
+}
+
+int ak_probe_fp64(ak_ctx* c, int use_fma, int reps, double* gops) {
+  if (!c || reps < 1 || !gops) return AK_EINVAL;
+  CK(cudaSetDevice(c->hp.device));
+  cudaEvent_t a, b;
+  CK(cudaEventCreate(&a)); CK(cudaEventCreate(&b));
+  const int iters = 4096, grid = 148 * 8, block = 256;
+  double best = 0.0;
+  for (int r = 0; r < reps + 1; ++r) {
+    CK(cudaEventRecord(a, c->stream));
+    if (use_fma) k_probe_fp64<true><<<grid, block, 0, c->stream>>>((double*)c->stats, iters, 1.0000001, 1e-9);
+    else k_probe_fp64<false><<<grid, block, 0, c->stream>>>((double*)c->stats, iters, 1.0000001, 1e-9);
+    CK(cudaEventRecord(b, c->stream));
+    CK(cudaEventSynchronize(b));
+    float ms = 0.f;
+    CK(cudaEventElapsedTime(&ms, a, b));
+    // thread-level fp64 instructions: 8 chains x iters x (1 FMA | MUL+ADD)
+    const double ops = (double)grid * block * 8.0 * iters * (use_fma ? 1.0 : 2.0);
+    const double g = ops / (ms * 1e-3) * 1e-9;
+    if (r > 0 && g > best) best = g;
+  }
+  cudaEventDestroy(a); cudaEventDestroy(b);
+  CK(cudaGetLastError());
+  *gops = best;
+  return AK_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,283 @@
+// ak_dev.cuh — device-side point operators of the GRMHD RHS stage (sm_100a, fp64).
+//
+// Written from DESIGN.md §3 (steps O0..O6, restating PAPER.md Eqs. 6-9; P:133;
+// P:137-139).  Shares nothing with oracle/.  The library is compiled with
+// --fmad=false: every +,-,*,/ and sqrt below is one IEEE fp64 operation evaluated in the
+// order written (C++ left-to-right association), which is what makes the status/flag masks
+// reproducible bit for bit (DESIGN.md §3 "reference arithmetic").
+#pragma once
+#include <cuda_runtime.h>
+#include <math.h>
+
+namespace ak {
+
+// ------------------------------------------------------------------ parameters / fields
+struct Par {
+  int nmb, n, nt, px, is, ie;   // is = 4, ie = n + 3
+  double Gam, gm1, gm1r;        // Gamma, Gamma-1, Gamma/(Gamma-1)
+  double rho_atm, T_atm, P_atm, eps_atm, thr;   // thr = f_thr * rho_atm
+  double mag_max;
+  double dmp_M, dmp_iM;
+  int max_iter;
+  double tol;
+  int recon, riemann, fofc, fofc_riemann;
+};
+
+// All field pointers one stage touches (passed by value as a kernel parameter).
+struct Fields {
+  double* U[5];
+  const double* Bf[3];
+  const double* adm[16];        // gxx gxy gxz gyy gyz gzz alp bx by bz Kxx..Kzz
+  double* W[8];                 // rho ux uy uz P Bccx Bccy Bccz
+  double* F[21];                // face fluxes [dir][7]
+  double* Ecc[3];               // cell-centred EMFs (scratch)
+  double* dU[5];
+  double* E[3];
+  unsigned char* flag;
+  unsigned char* status;
+  const double* dx;             // [nmb][3] device copy
+  unsigned int* list[3];        // FOFC face lists
+  unsigned int* count;          // [3] list lengths
+  unsigned long long* stats;    // device counters (see ak_api.cu)
+};
+
+enum { ST_DFLOOR = 1, ST_TAUFLOOR = 2, ST_MAGCAP = 4, ST_RHOFLOOR = 8, ST_TFLOOR = 16,
+       ST_FAIL = 32, ST_DMP = 64 };
+
+// ------------------------------------------------------------------ O0: 3-metric algebra
+struct Met3 {
+  double xx, xy, xz, yy, yz, zz;
+};
+
+// determinant by cofactors of the first row; inverse = cofactor * (1/det)
+__device__ __forceinline__ void metric_inverse(const Met3& g, double& det, double& sdet, Met3& u) {
+  const double cxx = g.yy * g.zz - g.yz * g.yz;
+  const double cxy = g.xz * g.yz - g.xy * g.zz;
+  const double cxz = g.xy * g.yz - g.xz * g.yy;
+  det = g.xx * cxx + g.xy * cxy + g.xz * cxz;
+  const double id = 1.0 / det;
+  u.xx = cxx * id;
+  u.xy = cxy * id;
+  u.xz = cxz * id;
+  u.yy = (g.xx * g.zz - g.xz * g.xz) * id;
+  u.yz = (g.xy * g.xz - g.xx * g.yz) * id;
+  u.zz = (g.xx * g.yy - g.xy * g.xy) * id;
+  sdet = sqrt(det);
+}
+// determinant and one diagonal element of the inverse only (face geometry, O5)
+template <int DIR>
+__device__ __forceinline__ void metric_det_gdd(const Met3& g, double& sdet, double& gdd) {
+  const double cxx = g.yy * g.zz - g.yz * g.yz;
+  const double cxy = g.xz * g.yz - g.xy * g.zz;
+  const double cxz = g.xy * g.yz - g.xz * g.yy;
+  const double det = g.xx * cxx + g.xy * cxy + g.xz * cxz;
+  const double id = 1.0 / det;
+  if (DIR == 0) gdd = cxx * id;
+  else if (DIR == 1) gdd = (g.xx * g.zz - g.xz * g.xz) * id;
+  else gdd = (g.xx * g.yy - g.xy * g.xy) * id;
+  sdet = sqrt(det);
+}
+
+// a_i = g_ij a^j, accumulated left to right
+__device__ __forceinline__ void lower(const Met3& g, const double a[3], double o[3]) {
+  o[0] = g.xx * a[0] + g.xy * a[1] + g.xz * a[2];
+  o[1] = g.xy * a[0] + g.yy * a[1] + g.yz * a[2];
+  o[2] = g.xz * a[0] + g.yz * a[1] + g.zz * a[2];
+}
+__device__ __forceinline__ double dot3(const double a[3], const double b[3]) {
+  return a[0] * b[0] + a[1] * b[1] + a[2] * b[2];
+}
+
+// ------------------------------------------------------------------ O2: prim -> cons (Eq. 6)
+// prim = rho, u^i = W v^i, P; B undensitised; cons = D, S_i, tau (undensitised).
+// tau in the cancellation-free form of DESIGN.md §3 O2.
+__device__ __forceinline__ void prim2cons(const Par& P, const Met3& g, double rho, const double u[3],
+                                          double pr, const double B[3], double c[5]) {
+  double ul[3], Bl[3];
+  lower(g, u, ul);
+  const double usq = dot3(ul, u);
+  const double W = sqrt(1.0 + usq);
+  const double iW = 1.0 / W;
+  const double vl[3] = {ul[0] * iW, ul[1] * iW, ul[2] * iW};
+  lower(g, B, Bl);
+  const double B2 = dot3(Bl, B);
+  const double Bv = B[0] * vl[0] + B[1] * vl[1] + B[2] * vl[2];
+  const double T = pr / rho;
+  const double hm1 = P.gm1r * T;
+  const double h = 1.0 + hm1;
+  const double D = rho * W;
+  const double wtot = rho * h * W * W + B2;
+  c[0] = D;
+  c[1] = wtot * vl[0] - Bv * Bl[0];
+  c[2] = wtot * vl[1] - Bv * Bl[1];
+  c[3] = wtot * vl[2] - Bv * Bl[2];
+  c[4] = D * (hm1 * W + usq / (1.0 + W)) + B2 - pr - 0.5 * (Bv * Bv + B2 * iW * iW);
+}
+
+// ------------------------------------------------------------------ O3: con2prim
+// Bracketed 1-D solve for mu = 1/(W h) (scheme of Kastaun et al. 2021), h0 = 1.
+struct C2P {
+  double q, r2, bs2, rb2, v0sq, gm1;
+  // quantities at a trial mu
+  double x, rbar2, qbar, vsq, iW, What, eps;
+  __device__ __forceinline__ void aux(double mu) {
+    x = 1.0 / (1.0 + mu * bs2);
+    rbar2 = r2 * x * x + mu * x * (1.0 + x) * rb2;
+    qbar = q - 0.5 * bs2 - 0.5 * mu * mu * x * x * (bs2 * r2 - rb2);
+    vsq = fmin(mu * mu * rbar2, v0sq);
+    iW = sqrt(1.0 - vsq);
+    What = 1.0 / iW;
+    eps = What * (qbar - mu * rbar2) + vsq * What * What / (1.0 + What);
+  }
+  // master function f(mu)
+  __device__ __forceinline__ double f(double mu) {
+    aux(mu);
+    const double e = fmax(eps, 0.0);
+    const double ahat = gm1 * e / (1.0 + e);
+    const double nuA = (1.0 + ahat) * (1.0 + e) * iW;
+    const double nuB = (1.0 + ahat) * (1.0 + qbar - mu * rbar2);
+    return mu - 1.0 / (fmax(nuA, nuB) + mu * rbar2);
+  }
+  // auxiliary function whose root bounds mu from above when r >= h0
+  __device__ __forceinline__ double fa(double mu) const {
+    const double xx = 1.0 / (1.0 + mu * bs2);
+    const double rb = r2 * xx * xx + mu * xx * (1.0 + xx) * rb2;
+    return mu * sqrt(1.0 + rb) - 1.0;
+  }
+};
+
+// Illinois-modified regula falsi on [a,b] with fa_ < 0 <= fb_.  AUX selects fa over f.
+// The iteration cap is uniform (a parameter), so a warp leaves the loop together at the
+// latest after max_iter evaluations.
+template <bool AUX>
+__device__ __forceinline__ bool illinois(C2P& s, double a, double b, double fa_, double fb_,
+                                         int max_iter, double tol, double& root) {
+  int side = 0;
+  double cprev = b;
+  for (int it = 0; it < max_iter; ++it) {
+    const double c = (a * fb_ - b * fa_) / (fb_ - fa_);
+    const double fc = AUX ? s.fa(c) : s.f(c);
+    if (!(fc == fc)) return false;
+    if (fc == 0.0) { root = c; return true; }
+    if (fc > 0.0) {
+      b = c; fb_ = fc;
+      if (side == -1) fa_ = 0.5 * fa_;
+      side = -1;
+    } else {
+      a = c; fa_ = fc;
+      if (side == 1) fb_ = 0.5 * fb_;
+      side = 1;
+    }
+    if (fabs(c - cprev) <= tol * c) { root = c; return true; }
+    cprev = c;
+  }
+  return false;
+}
+
+// One cell.  Ut = densitised D,S_i,tau (rewritten from the final primitives when WRITE_BACK
+// and the status is non-zero); Bt = densitised cell-centred B; W5 = rho,u^x,u^y,u^z,P.
+template <bool WRITE_BACK>
+__device__ __forceinline__ int c2p_cell(const Par& P, const Met3& g, double Ut[5], const double Bt[3],
+                                        double W5[5]) {
+  int status = 0;
+  double det, sdet;
+  Met3 gu;
+  metric_inverse(g, det, sdet, gu);
+  const double isd = 1.0 / sdet;
+  double D = Ut[0] * isd, tau = Ut[4] * isd;
+  const double Sl[3] = {Ut[1] * isd, Ut[2] * isd, Ut[3] * isd};
+  const double B[3] = {Bt[0] * isd, Bt[1] * isd, Bt[2] * isd};
+  double rho = P.rho_atm, ux = 0.0, uy = 0.0, uz = 0.0, pr = P.P_atm;
+  bool solve = true;
+  if (!(isfinite(D) && isfinite(Sl[0]) && isfinite(Sl[1]) && isfinite(Sl[2]) && isfinite(tau) &&
+        isfinite(B[0]) && isfinite(B[1]) && isfinite(B[2]))) {
+    status |= ST_FAIL;
+    solve = false;
+  }
+  double Bl[3];
+  lower(g, B, Bl);
+  const double B2 = dot3(Bl, B);
+  // conserved floors: D floor -> magnetisation cap -> tau floor (reading R5)
+  bool atmo = false;
+  if (solve && D < P.thr) {
+    status |= ST_DFLOOR;
+    D = P.rho_atm;
+    atmo = true;
+  }
+  if (solve && B2 > P.mag_max * D) {
+    D = B2 / P.mag_max;
+    status |= ST_MAGCAP;
+  }
+  if (solve && atmo) {
+    rho = D;
+    pr = D * P.T_atm;
+    solve = false;
+  }
+  if (solve) {
+    const double tau_atm = D * P.eps_atm + 0.5 * B2;
+    if (tau < tau_atm) { tau = tau_atm; status |= ST_TAUFLOOR; }
+    const double iD = 1.0 / D;
+    C2P s;
+    s.q = tau * iD;
+    const double rl[3] = {Sl[0] * iD, Sl[1] * iD, Sl[2] * iD};
+    const double ru[3] = {gu.xx * rl[0] + gu.xy * rl[1] + gu.xz * rl[2],
+                          gu.xy * rl[0] + gu.yy * rl[1] + gu.yz * rl[2],
+                          gu.xz * rl[0] + gu.yz * rl[1] + gu.zz * rl[2]};
+    s.r2 = dot3(rl, ru);
+    s.bs2 = B2 * iD;
+    const double rB = dot3(rl, B);
+    s.rb2 = rB * rB * iD;
+    s.v0sq = s.r2 / (1.0 + s.r2);
+    s.gm1 = P.gm1;
+    bool ok = true;
+    double mu_hi = 1.0;
+    if (!(s.r2 < 1.0)) {
+      ok = illinois<true>(s, 0.0, 1.0, -1.0, s.fa(1.0), P.max_iter, P.tol, mu_hi);
+      mu_hi = mu_hi * (1.0 + 1e-14);
+      if (mu_hi > 1.0) mu_hi = 1.0;
+    }
+    double mu = 0.0;
+    if (ok) {
+      const double f_hi = s.f(mu_hi);
+      const double f_lo = s.f(0.0);
+      if (!(f_hi >= 0.0) || !(f_lo < 0.0)) ok = false;
+      else if (f_hi == 0.0) mu = mu_hi;
+      else ok = illinois<false>(s, 0.0, mu_hi, f_lo, f_hi, P.max_iter, P.tol, mu);
+    }
+    if (!ok) {
+      status |= ST_FAIL;
+    } else {
+      s.aux(mu);
+      rho = D * s.iW;
+      const double T = P.gm1 * s.eps;
+      pr = rho * T;
+      const double c = mu * rB * iD;
+      const double mx = mu * s.x;
+      ux = s.What * (mx * (ru[0] + c * B[0]));
+      uy = s.What * (mx * (ru[1] + c * B[1]));
+      uz = s.What * (mx * (ru[2] + c * B[2]));
+      if (!(isfinite(rho) && isfinite(pr) && isfinite(ux) && isfinite(uy) && isfinite(uz))) {
+        status |= ST_FAIL;
+        rho = P.rho_atm; ux = uy = uz = 0.0; pr = P.P_atm;
+      }
+    }
+  }
+  // primitive floors
+  if (rho < P.thr) {
+    rho = P.rho_atm; ux = uy = uz = 0.0; pr = P.P_atm;
+    status |= ST_RHOFLOOR;
+  } else if (pr < rho * P.T_atm) {
+    pr = rho * P.T_atm;
+    status |= ST_TFLOOR;
+  }
+  W5[0] = rho; W5[1] = ux; W5[2] = uy; W5[3] = uz; W5[4] = pr;
+  if (WRITE_BACK && status != 0) {
+    double c5[5];
+    const double u[3] = {ux, uy, uz};
+    prim2cons(P, g, rho, u, pr, B, c5);
+    for (int v = 0; v < 5; ++v) Ut[v] = sdet * c5[v];
+  }
+  return status;
+}
+
+}  // namespace ak

@@ -1,0 +1,188 @@
+// ak_flux.cuh — reconstruction (O4), face geometry (O5) and Riemann fluxes (O6).
+// DESIGN.md §3; PAPER.md P:133 (donor cell / PPM4 / WENO-Z, LLF / HLLE), Eq. 7-8,
+// face-state floor P:139.  Device code only; shares nothing with oracle/.
+#pragma once
+#include "ak_dev.cuh"
+
+namespace ak {
+
+// ------------------------------------------------------------------ O4: reconstruction
+// Five cell values qmm..qpp centred on cell i  ->  qm at its left face, qp at its right face.
+template <int KIND>
+__device__ __forceinline__ void recon(double qmm, double qm1, double q0, double qp1, double qpp,
+                                      double& qm, double& qp) {
+  if (KIND == 0) {            // donor cell
+    qm = q0; qp = q0;
+  } else if (KIND == 1) {     // PPM4 (Colella & Woodward 1984): 4th-order interface values,
+                              // clamped, then the parabola monotonicity rule
+    const double c12 = 1.0 / 12.0;
+    double ql = (7.0 * (qm1 + q0) - (qmm + qp1)) * c12;
+    double qr = (7.0 * (q0 + qp1) - (qm1 + qpp)) * c12;
+    ql = fmax(fmin(ql, fmax(qm1, q0)), fmin(qm1, q0));
+    qr = fmax(fmin(qr, fmax(q0, qp1)), fmin(q0, qp1));
+    if ((qr - q0) * (q0 - ql) <= 0.0) {
+      ql = q0; qr = q0;
+    } else {
+      const double dq = qr - ql;
+      const double eta = 6.0 * (q0 - 0.5 * (ql + qr));
+      if (dq * eta > dq * dq) ql = 3.0 * q0 - 2.0 * qr;
+      else if (dq * eta < -(dq * dq)) qr = 3.0 * q0 - 2.0 * ql;
+    }
+    qm = ql; qp = qr;
+  } else {                    // WENO-Z (Borges et al. 2008), p = 2, eps = 1e-40
+    const double c6 = 1.0 / 6.0, c1312 = 13.0 / 12.0, eps = 1e-40;
+    const double a0 = qmm - 2.0 * qm1 + q0, a1 = qm1 - 2.0 * q0 + qp1, a2 = q0 - 2.0 * qp1 + qpp;
+    const double e0 = qmm - 4.0 * qm1 + 3.0 * q0, e1 = qm1 - qp1, e2 = 3.0 * q0 - 4.0 * qp1 + qpp;
+    const double b0 = c1312 * (a0 * a0) + 0.25 * (e0 * e0) + eps;
+    const double b1 = c1312 * (a1 * a1) + 0.25 * (e1 * e1) + eps;
+    const double b2 = c1312 * (a2 * a2) + 0.25 * (e2 * e2) + eps;
+    const double tau5 = fabs(b0 - b2);
+    // the three ratios tau5/beta_k through one reciprocal of the product
+    const double ib = 1.0 / (b0 * b1 * b2);
+    const double r0 = tau5 * (b1 * b2) * ib, r1 = tau5 * (b0 * b2) * ib, r2 = tau5 * (b0 * b1) * ib;
+    const double t0 = 1.0 + r0 * r0, t1 = 1.0 + r1 * r1, t2 = 1.0 + r2 * r2;
+    {
+      const double p0 = (2.0 * qmm - 7.0 * qm1 + 11.0 * q0) * c6;
+      const double p1 = (-qm1 + 5.0 * q0 + 2.0 * qp1) * c6;
+      const double p2 = (2.0 * q0 + 5.0 * qp1 - qpp) * c6;
+      const double w0 = 0.1 * t0, w1 = 0.6 * t1, w2 = 0.3 * t2;
+      qp = (w0 * p0 + w1 * p1 + w2 * p2) / (w0 + w1 + w2);
+    }
+    {  // mirror image
+      const double p0 = (2.0 * qpp - 7.0 * qp1 + 11.0 * q0) * c6;
+      const double p1 = (-qp1 + 5.0 * q0 + 2.0 * qm1) * c6;
+      const double p2 = (2.0 * q0 + 5.0 * qm1 - qmm) * c6;
+      const double w0 = 0.1 * t2, w1 = 0.6 * t1, w2 = 0.3 * t0;
+      qm = (w0 * p0 + w1 * p1 + w2 * p2) / (w0 + w1 + w2);
+    }
+  }
+}
+
+// ------------------------------------------------------------------ O5: face geometry
+struct FaceGeo {
+  double alp, ialp, bet[3];
+  Met3 g;
+  double gdd, sdet, isd;
+};
+
+// mL, mR = {alp, betx, bety, betz, gxx, gxy, gxz, gyy, gyz, gzz} of the lower / upper cell
+template <int DIR>
+__device__ __forceinline__ void face_geometry(const double mL[10], const double mR[10], FaceGeo& G) {
+  double m[10];
+#pragma unroll
+  for (int c = 0; c < 10; ++c) m[c] = (mL[c] + mR[c]) * 0.5;
+  G.alp = m[0];
+  G.bet[0] = m[1]; G.bet[1] = m[2]; G.bet[2] = m[3];
+  G.g.xx = m[4]; G.g.xy = m[5]; G.g.xz = m[6]; G.g.yy = m[7]; G.g.yz = m[8]; G.g.zz = m[9];
+  metric_det_gdd<DIR>(G.g, G.sdet, G.gdd);
+  G.isd = 1.0 / G.sdet;
+  G.ialp = 1.0 / G.alp;
+}
+
+// face-state floor ("after reconstruction"); s = rho,ux,uy,uz,P,...
+__device__ __forceinline__ void face_floor(const Par& P, double s[7]) {
+  if (s[0] < P.thr) {
+    s[0] = P.rho_atm; s[1] = 0.0; s[2] = 0.0; s[3] = 0.0;
+    s[4] = P.P_atm;
+  } else if (s[4] < s[0] * P.T_atm) {
+    s[4] = s[0] * P.T_atm;
+  }
+}
+
+// ------------------------------------------------------------------ O6: one side (Eq. 8)
+// s = rho,u^x,u^y,u^z,P,B~t1,B~t2 (transverse B densitised); Bd = undensitised normal B.
+// Out: densitised conserved U[7], densitised fluxes F[7], signal speeds lm, lp.
+template <int DIR>
+__device__ __forceinline__ void side_state(const Par& P, const FaceGeo& G, const double s[7], double Bd,
+                                           double U[7], double F[7], double& lm, double& lp) {
+  constexpr int t1 = (DIR + 1) % 3, t2 = (DIR + 2) % 3;
+  const double rho = s[0], pr = s[4];
+  const double u[3] = {s[1], s[2], s[3]};
+  double B[3];
+  B[DIR] = Bd; B[t1] = s[5] * G.isd; B[t2] = s[6] * G.isd;
+  double ul[3], Bl[3];
+  lower(G.g, u, ul);
+  const double usq = dot3(ul, u);
+  const double W = sqrt(1.0 + usq);
+  const double iW = 1.0 / W;
+  const double v[3] = {u[0] * iW, u[1] * iW, u[2] * iW};
+  const double vl[3] = {ul[0] * iW, ul[1] * iW, ul[2] * iW};
+  lower(G.g, B, Bl);
+  const double B2 = dot3(Bl, B);
+  const double Bv = B[0] * vl[0] + B[1] * vl[1] + B[2] * vl[2];
+  const double b2 = B2 * iW * iW + Bv * Bv;                                   // Eq. 7
+  const double bl[3] = {Bl[0] * iW + Bv * ul[0], Bl[1] * iW + Bv * ul[1], Bl[2] * iW + Bv * ul[2]};
+  const double ab0 = W * Bv;                                                  // alpha b^0
+  const double T = pr / rho;
+  const double hm1 = P.gm1r * T;
+  const double h = 1.0 + hm1;
+  const double Ptot = pr + 0.5 * b2;
+  const double D = rho * W;
+  const double wtot = rho * h * W * W + B2;
+  const double S[3] = {wtot * vl[0] - Bv * Bl[0], wtot * vl[1] - Bv * Bl[1], wtot * vl[2] - Bv * Bl[2]};
+  const double tau = D * (hm1 * W + usq / (1.0 + W)) + B2 - pr - 0.5 * (Bv * Bv + B2 * iW * iW);
+  const double vh[3] = {v[0] - G.bet[0] * G.ialp, v[1] - G.bet[1] * G.ialp, v[2] - G.bet[2] * G.ialp};
+  const double BdW = B[DIR] * iW;
+  const double aP = G.alp * Ptot;
+  U[0] = G.sdet * D;
+  U[1] = G.sdet * S[0]; U[2] = G.sdet * S[1]; U[3] = G.sdet * S[2];
+  U[4] = G.sdet * tau;
+  U[5] = s[5]; U[6] = s[6];
+  F[0] = G.sdet * (G.alp * D * vh[DIR]);
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    double f = G.alp * S[i] * vh[DIR] - G.alp * bl[i] * BdW;
+    if (i == DIR) f = f + aP;
+    F[1 + i] = G.sdet * f;
+  }
+  F[4] = G.sdet * (G.alp * tau * vh[DIR] - G.alp * ab0 * BdW + aP * v[DIR]);
+  F[5] = G.sdet * (G.alp * (B[t1] * vh[DIR] - B[DIR] * vh[t1]));
+  F[6] = G.sdet * (G.alp * (B[t2] * vh[DIR] - B[DIR] * vh[t2]));
+  // fast-magnetosonic bound on the characteristic speeds (DESIGN.md §3 O6, reading R18)
+  const double vsq = v[0] * vl[0] + v[1] * vl[1] + v[2] * vl[2];
+  const double cs2 = P.Gam * T / h;
+  const double rhoh = rho * h;
+  const double va2 = b2 / (rhoh + b2);
+  const double a2 = cs2 + va2 - cs2 * va2;
+  const double om = 1.0 - vsq * a2;
+  const double disc = a2 * (1.0 - vsq) * (G.gdd * om - v[DIR] * v[DIR] * (1.0 - a2));
+  const double root = sqrt(fmax(0.0, disc));
+  const double iom = 1.0 / om;
+  const double vd1 = v[DIR] * (1.0 - a2);
+  lm = G.alp * ((vd1 - root) * iom) - G.bet[DIR];
+  lp = G.alp * ((vd1 + root) * iom) - G.bet[DIR];
+}
+
+// Face flux from left/right states (floored here when FLOOR), the face-normal B~ and the
+// two adjacent cells' metric.  RS: 0 LLF, 1 HLLE.
+template <int DIR, bool FLOOR>
+__device__ __forceinline__ void face_flux(const Par& P, int rs, const double mL[10], const double mR[10],
+                                          double sL[7], double sR[7], double Bfd, double Fo[7]) {
+  FaceGeo G;
+  face_geometry<DIR>(mL, mR, G);
+  const double Bd = Bfd * G.isd;
+  if (FLOOR) { face_floor(P, sL); face_floor(P, sR); }
+  double UL[7], FL[7], UR[7], FR[7], lmL, lpL, lmR, lpR;
+  side_state<DIR>(P, G, sL, Bd, UL, FL, lmL, lpL);
+  side_state<DIR>(P, G, sR, Bd, UR, FR, lmR, lpR);
+  if (rs == 1) {   // HLLE
+    const double lL = fmin(0.0, fmin(lmL, lmR));
+    const double lR = fmax(0.0, fmax(lpL, lpR));
+    const double dl = lR - lL;
+    if (dl == 0.0) {
+#pragma unroll
+      for (int c = 0; c < 7; ++c) Fo[c] = 0.5 * (FL[c] + FR[c]);
+    } else {
+      const double idl = 1.0 / dl;
+      const double lRL = lR * lL;
+#pragma unroll
+      for (int c = 0; c < 7; ++c) Fo[c] = (lR * FL[c] - lL * FR[c] + lRL * (UR[c] - UL[c])) * idl;
+    }
+  } else {         // LLF
+    const double lam = fmax(fmax(fabs(lmL), fabs(lpL)), fmax(fabs(lmR), fabs(lpR)));
+#pragma unroll
+    for (int c = 0; c < 7; ++c) Fo[c] = 0.5 * (FL[c] + FR[c]) - 0.5 * lam * (UR[c] - UL[c]);
+  }
+}
+
+}  // namespace ak

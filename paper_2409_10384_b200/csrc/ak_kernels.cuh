@@ -1,0 +1,333 @@
+// ak_kernels.cuh — the kernels of one RHS stage.
+//   K1  k_con2prim      part (1)  all stored cells
+//   K2  k_flux<DIR>     parts (2)+(3)  one thread per face, direction DIR
+//   K3  k_fofc_test     part (4a) estimate + check-only con2prim (+DMP) -> flag bytes
+//   K3b k_fofc_list     part (4b) warp-ballot compaction of faces with a flagged neighbour
+//   K4  k_fofc_reflux   part (4c) first-order re-solve of the listed faces
+//   K5a k_cell_emf      part (5a) cell-centred EMFs
+//   K5  k_ct<C3>        part (5b) Gardiner-Stone corner EMFs
+//   K6  k_div_src       part (6)  flux divergence + geometric sources (Eq. 9)
+#pragma once
+#include "ak_flux.cuh"
+
+namespace ak {
+
+// stats slots (device counters)
+enum { S_C2P_FAIL = 0, S_CONS_FLOOR, S_PRIM_FLOOR, S_FOFC_CELLS, S_DMP_CELLS, S_NSTAT };
+
+__device__ __forceinline__ void warp_count(unsigned long long* ctr, bool pred) {
+  const unsigned m = __ballot_sync(__activemask(), pred);
+  if (m != 0 && (threadIdx.x & 31) == (__ffs(m) - 1)) atomicAdd(ctr, (unsigned long long)__popc(m));
+}
+
+// ---- index helpers (layouts of include/ak.h) ------------------------------------------
+struct Ix {
+  int nt, px;
+  __device__ __forceinline__ long long cell(int m, int k, int j, int i) const {
+    return (((long long)m * nt + k) * nt + j) * nt + i;
+  }
+  __device__ __forceinline__ long long face(int d, int m, int k, int j, int i) const {
+    if (d == 0) return (((long long)m * nt + k) * nt + j) * px + i;
+    if (d == 1) return (((long long)m * nt + k) * (nt + 1) + j) * nt + i;
+    return (((long long)m * (nt + 1) + k) * nt + j) * nt + i;
+  }
+  __device__ __forceinline__ long long edge(int c, int m, int k, int j, int i) const {
+    if (c == 0) return (((long long)m * (nt + 1) + k) * (nt + 1) + j) * nt + i;
+    if (c == 1) return (((long long)m * (nt + 1) + k) * nt + j) * px + i;
+    return (((long long)m * nt + k) * (nt + 1) + j) * px + i;
+  }
+};
+
+__device__ __forceinline__ void load_met3(const Fields& f, long long c, Met3& g) {
+  g.xx = __ldg(f.adm[0] + c); g.xy = __ldg(f.adm[1] + c); g.xz = __ldg(f.adm[2] + c);
+  g.yy = __ldg(f.adm[3] + c); g.yz = __ldg(f.adm[4] + c); g.zz = __ldg(f.adm[5] + c);
+}
+// {alp, betx, bety, betz, gxx..gzz}
+__device__ __forceinline__ void load_met10(const Fields& f, long long c, double m[10]) {
+  m[0] = __ldg(f.adm[6] + c); m[1] = __ldg(f.adm[7] + c); m[2] = __ldg(f.adm[8] + c);
+  m[3] = __ldg(f.adm[9] + c);
+#pragma unroll
+  for (int q = 0; q < 6; ++q) m[4 + q] = __ldg(f.adm[q] + c);
+}
+
+// ---- K1 ------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) k_con2prim(const __grid_constant__ Par P,
+                                                  const __grid_constant__ Fields f) {
+  const int nt = P.nt;
+  const long long ncell = (long long)P.nmb * nt * nt * nt;
+  const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= ncell) return;
+  const int i = (int)(c % nt);
+  const long long row = c / nt;               // (m*nt + k)*nt + j
+  const int j = (int)(row % nt);
+  const long long mk = row / nt;              // m*nt + k
+  const int k = (int)(mk % nt);
+  const int m = (int)(mk / nt);
+  Met3 g;
+  load_met3(f, c, g);
+  double Ut[5], Bc[3], W5[5];
+#pragma unroll
+  for (int v = 0; v < 5; ++v) Ut[v] = f.U[v][c];
+  const long long fx = row * P.px + i;
+  const long long fy = (mk * (nt + 1) + j) * nt + i;
+  const long long fz = (((long long)m * (nt + 1) + k) * nt + j) * nt + i;
+  Bc[0] = 0.5 * (__ldg(f.Bf[0] + fx) + __ldg(f.Bf[0] + fx + 1));
+  Bc[1] = 0.5 * (__ldg(f.Bf[1] + fy) + __ldg(f.Bf[1] + fy + nt));
+  Bc[2] = 0.5 * (__ldg(f.Bf[2] + fz) + __ldg(f.Bf[2] + fz + (long long)nt * nt));
+  const int st = c2p_cell<true>(P, g, Ut, Bc, W5);
+#pragma unroll
+  for (int v = 0; v < 5; ++v) f.W[v][c] = W5[v];
+#pragma unroll
+  for (int v = 0; v < 3; ++v) f.W[5 + v][c] = Bc[v];
+  if (st != 0) {
+#pragma unroll
+    for (int v = 0; v < 5; ++v) f.U[v][c] = Ut[v];
+  }
+  if (f.status) f.status[c] = (unsigned char)st;
+  warp_count(f.stats + S_C2P_FAIL, (st & ST_FAIL) != 0);
+  warp_count(f.stats + S_CONS_FLOOR, (st & (ST_DFLOOR | ST_TAUFLOOR | ST_MAGCAP)) != 0);
+  warp_count(f.stats + S_PRIM_FLOOR, (st & (ST_RHOFLOOR | ST_TFLOOR)) != 0);
+}
+
+// ---- computed-face range decoding ----------------------------------------------------
+// Faces of direction DIR: DIR-index in [is-1, ie+2] (n+3), transverse in [is-1, ie+1] (n+2).
+template <int DIR>
+__device__ __forceinline__ bool decode_face(const Par& P, long long idx, int& m, int& k, int& j, int& i) {
+  const int ei = P.n + (DIR == 0 ? 3 : 2), ej = P.n + (DIR == 1 ? 3 : 2), ek = P.n + (DIR == 2 ? 3 : 2);
+  const long long per = (long long)ei * ej * ek;
+  if (idx >= per * P.nmb) return false;
+  m = (int)(idx / per);
+  int r = (int)(idx - (long long)m * per);
+  i = r % ei + P.is - 1; r /= ei;
+  j = r % ej + P.is - 1;
+  k = r / ej + P.is - 1;
+  return true;
+}
+
+// ---- K2 (v1: one thread per face; both one-sided reconstructions done by the thread) ----
+template <int DIR, int RECON>
+__global__ void __launch_bounds__(128) k_flux(const __grid_constant__ Par P,
+                                              const __grid_constant__ Fields f) {
+  int m, k, j, i;
+  if (!decode_face<DIR>(P, (long long)blockIdx.x * blockDim.x + threadIdx.x, m, k, j, i)) return;
+  const Ix ix{P.nt, P.px};
+  constexpr int t1 = (DIR + 1) % 3, t2 = (DIR + 2) % 3;
+  const long long stride = DIR == 0 ? 1 : (DIR == 1 ? P.nt : (long long)P.nt * P.nt);
+  const long long cu = ix.cell(m, k, j, i), cl = cu - stride;
+  const int var[7] = {0, 1, 2, 3, 4, 5 + t1, 5 + t2};
+  double sL[7], sR[7];
+#pragma unroll
+  for (int v = 0; v < 7; ++v) {
+    const double* w = f.W[var[v]] + cu;
+    if (RECON == 0) {
+      sL[v] = w[-stride]; sR[v] = w[0];
+    } else {
+      const double q0 = w[-3 * stride], q1 = w[-2 * stride], q2 = w[-stride], q3 = w[0],
+                   q4 = w[stride], q5 = w[2 * stride];
+      double qm, qp;
+      recon<RECON>(q0, q1, q2, q3, q4, qm, qp);
+      sL[v] = qp;                         // right face of the lower cell
+      recon<RECON>(q1, q2, q3, q4, q5, qm, qp);
+      sR[v] = qm;                         // left face of the upper cell
+    }
+  }
+  double mL[10], mR[10], Fo[7];
+  load_met10(f, cl, mL);
+  load_met10(f, cu, mR);
+  const long long fi = ix.face(DIR, m, k, j, i);
+  face_flux<DIR, true>(P, P.riemann, mL, mR, sL, sR, __ldg(f.Bf[DIR] + fi), Fo);
+#pragma unroll
+  for (int v = 0; v < 7; ++v) f.F[7 * DIR + v][fi] = Fo[v];
+}
+
+// ---- test-cell range decoding: cells in [is-1, ie+1]^3 ----------------------------------
+__device__ __forceinline__ bool decode_test(const Par& P, long long idx, int& m, int& k, int& j, int& i) {
+  const int e = P.n + 2;
+  const long long per = (long long)e * e * e;
+  if (idx >= per * P.nmb) return false;
+  m = (int)(idx / per);
+  int r = (int)(idx - (long long)m * per);
+  i = r % e + P.is - 1; r /= e;
+  j = r % e + P.is - 1;
+  k = r / e + P.is - 1;
+  return true;
+}
+
+// flux difference of component v across cell (m,k,j,i), summed x then y then z
+__device__ __forceinline__ double div_flux(const Fields& f, const Ix& ix, int v, int m, int k, int j, int i,
+                                           const double idx[3]) {
+  const long long fx = ix.face(0, m, k, j, i), fy = ix.face(1, m, k, j, i), fz = ix.face(2, m, k, j, i);
+  const long long sy = ix.nt, sz = (long long)ix.nt * ix.nt;
+  return (f.F[v][fx + 1] - f.F[v][fx]) * idx[0] + (f.F[7 + v][fy + sy] - f.F[7 + v][fy]) * idx[1] +
+         (f.F[14 + v][fz + sz] - f.F[14 + v][fz]) * idx[2];
+}
+
+// ---- K3: FOFC estimate and test (DMP Eq. 12) -------------------------------
+__global__ void __launch_bounds__(128) k_fofc_test(const __grid_constant__ Par P,
+                                                   const __grid_constant__ Fields f, double dt) {
+  int m, k, j, i;
+  if (!decode_test(P, (long long)blockIdx.x * blockDim.x + threadIdx.x, m, k, j, i)) return;
+  const Ix ix{P.nt, P.px};
+  const long long c = ix.cell(m, k, j, i);
+  const double idx[3] = {1.0 / f.dx[3 * m + 0], 1.0 / f.dx[3 * m + 1], 1.0 / f.dx[3 * m + 2]};
+  double Us[5], Bc[3], W5[5];
+#pragma unroll
+  for (int v = 0; v < 5; ++v) Us[v] = f.U[v][c] - dt * div_flux(f, ix, v, m, k, j, i, idx);
+  Met3 g;
+  load_met3(f, c, g);
+#pragma unroll
+  for (int v = 0; v < 3; ++v) Bc[v] = f.W[5 + v][c];
+  const double Ds = Us[0], ts = Us[4];
+  int st = c2p_cell<false>(P, g, Us, Bc, W5);
+  if (P.dmp_M > 0.0) {
+    double Dmin = f.U[0][c], Dmax = Dmin, tmin = f.U[4][c], tmax = tmin;
+    const long long sy = P.nt, sz = (long long)P.nt * P.nt;
+#pragma unroll
+    for (int kk = -1; kk <= 1; ++kk)
+#pragma unroll
+      for (int jj = -1; jj <= 1; ++jj)
+#pragma unroll
+        for (int ii = -1; ii <= 1; ++ii) {
+          const long long cn = c + kk * sz + jj * sy + ii;
+          const double d = f.U[0][cn], t = f.U[4][cn];
+          Dmin = fmin(Dmin, d); Dmax = fmax(Dmax, d);
+          tmin = fmin(tmin, t); tmax = fmax(tmax, t);
+        }
+    if (Ds < Dmin * P.dmp_iM || Ds > P.dmp_M * Dmax || ts < tmin * P.dmp_iM || ts > P.dmp_M * tmax)
+      st |= ST_DMP;
+  }
+  f.flag[c] = (unsigned char)st;
+  warp_count(f.stats + S_FOFC_CELLS, st != 0);
+  warp_count(f.stats + S_DMP_CELLS, (st & ST_DMP) != 0);
+}
+
+// ---- K3b: compact the faces that have a flagged neighbour (warp ballots) -------------------
+// A list entry is the linear index of the face's upper cell.  The order of entries depends on
+// the atomics but no output does: each listed face is rewritten exactly once.
+template <int DIR>
+__global__ void __launch_bounds__(256) k_fofc_list(const __grid_constant__ Par P,
+                                                   const __grid_constant__ Fields f) {
+  int m, k, j, i;
+  const bool in = decode_face<DIR>(P, (long long)blockIdx.x * blockDim.x + threadIdx.x, m, k, j, i);
+  bool hit = false;
+  long long cu = 0;
+  if (in) {
+    const Ix ix{P.nt, P.px};
+    const long long stride = DIR == 0 ? 1 : (DIR == 1 ? P.nt : (long long)P.nt * P.nt);
+    cu = ix.cell(m, k, j, i);
+    hit = (f.flag[cu] | f.flag[cu - stride]) != 0;
+  }
+  const unsigned bal = __ballot_sync(0xffffffffu, hit);
+  if (bal == 0) return;
+  const int lane = threadIdx.x & 31;
+  unsigned base = 0;
+  if (lane == 0) base = atomicAdd(f.count + DIR, (unsigned)__popc(bal));
+  base = __shfl_sync(0xffffffffu, base, 0);
+  if (hit) f.list[DIR][base + __popc(bal & ((1u << lane) - 1u))] = (unsigned)cu;
+}
+
+// ---- K4: first-order re-solve of the listed faces ("recalculate the fluxes for all
+// flagged cells but using a first-order scheme") -------------------------------------------
+template <int DIR>
+__global__ void __launch_bounds__(128) k_fofc_reflux(const __grid_constant__ Par P,
+                                                     const __grid_constant__ Fields f) {
+  const unsigned cnt = f.count[DIR];
+  const Ix ix{P.nt, P.px};
+  constexpr int t1 = (DIR + 1) % 3, t2 = (DIR + 2) % 3;
+  const long long stride = DIR == 0 ? 1 : (DIR == 1 ? P.nt : (long long)P.nt * P.nt);
+  const int var[7] = {0, 1, 2, 3, 4, 5 + t1, 5 + t2};
+  for (unsigned e = blockIdx.x * blockDim.x + threadIdx.x; e < cnt; e += gridDim.x * blockDim.x) {
+    const long long cu = f.list[DIR][e], cl = cu - stride;
+    const int nt = P.nt;
+    const int i = (int)(cu % nt);
+    const long long row = cu / nt;
+    const int j = (int)(row % nt);
+    const long long mk = row / nt;
+    const int k = (int)(mk % nt), m = (int)(mk / nt);
+    double sL[7], sR[7], mL[10], mR[10], Fo[7];
+#pragma unroll
+    for (int v = 0; v < 7; ++v) { sL[v] = f.W[var[v]][cl]; sR[v] = f.W[var[v]][cu]; }
+    load_met10(f, cl, mL);
+    load_met10(f, cu, mR);
+    const long long fi = ix.face(DIR, m, k, j, i);
+    face_flux<DIR, true>(P, P.fofc_riemann, mL, mR, sL, sR, __ldg(f.Bf[DIR] + fi), Fo);
+#pragma unroll
+    for (int v = 0; v < 7; ++v) f.F[7 * DIR + v][fi] = Fo[v];
+  }
+}
+
+// ---- K5a: cell-centred EMFs  E_c = -alpha (vhat^a B~^b - vhat^b B~^a) on [is-1,ie+1]^3 --------
+__global__ void __launch_bounds__(128) k_cell_emf(const __grid_constant__ Par P,
+                                                  const __grid_constant__ Fields f) {
+  int m, k, j, i;
+  if (!decode_test(P, (long long)blockIdx.x * blockDim.x + threadIdx.x, m, k, j, i)) return;
+  const Ix ix{P.nt, P.px};
+  const long long c = ix.cell(m, k, j, i);
+  Met3 g;
+  load_met3(f, c, g);
+  const double u[3] = {f.W[1][c], f.W[2][c], f.W[3][c]};
+  double ul[3];
+  lower(g, u, ul);
+  const double usq = dot3(ul, u);
+  const double iW = 1.0 / sqrt(1.0 + usq);
+  const double alp = __ldg(f.adm[6] + c), ialp = 1.0 / alp;
+  const double vh[3] = {u[0] * iW - __ldg(f.adm[7] + c) * ialp, u[1] * iW - __ldg(f.adm[8] + c) * ialp,
+                        u[2] * iW - __ldg(f.adm[9] + c) * ialp};
+  const double Bt[3] = {f.W[5][c], f.W[6][c], f.W[7][c]};
+  f.Ecc[0][c] = -(alp * (vh[1] * Bt[2] - vh[2] * Bt[1]));
+  f.Ecc[1][c] = -(alp * (vh[2] * Bt[0] - vh[0] * Bt[2]));
+  f.Ecc[2][c] = -(alp * (vh[0] * Bt[1] - vh[1] * Bt[0]));
+}
+
+// ---- K5: corner EMFs, component C3 (Gardiner & Stone 2005; DESIGN.md §3 O8) ------------------
+// a, b cyclic after C3.  Edge (ia, ib, ic): ia, ib in [is, ie+1], ic in [is, ie].
+template <int C3>
+__global__ void __launch_bounds__(128) k_ct(const __grid_constant__ Par P,
+                                            const __grid_constant__ Fields f) {
+  constexpr int a = (C3 + 1) % 3, b = (C3 + 2) % 3;
+  const int n = P.n;
+  const int ei = n + (C3 == 0 ? 0 : 1), ej = n + (C3 == 1 ? 0 : 1), ek = n + (C3 == 2 ? 0 : 1);
+  const long long per = (long long)ei * ej * ek;
+  const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= per * P.nmb) return;
+  const int m = (int)(idx / per);
+  int r = (int)(idx - (long long)m * per);
+  int p3[3];
+  p3[0] = r % ei + P.is; r /= ei;
+  p3[1] = r % ej + P.is;
+  p3[2] = r / ej + P.is;
+  const Ix ix{P.nt, P.px};
+  // offsets of one step along a and b, in cells and in the a-face / b-face layouts
+  const long long cst[3] = {1, P.nt, (long long)P.nt * P.nt};
+  const long long c0 = ix.cell(m, p3[2], p3[1], p3[0]);
+  const long long fa0 = ix.face(a, m, p3[2], p3[1], p3[0]);
+  const long long fb0 = ix.face(b, m, p3[2], p3[1], p3[0]);
+  // step of index b inside the a-face layout, and of index a inside the b-face layout
+  int q3[3] = {p3[0], p3[1], p3[2]};
+  q3[b] -= 1;
+  const long long fa_b = ix.face(a, m, q3[2], q3[1], q3[0]) - fa0;   // (ia, ib-1)
+  q3[b] += 1; q3[a] -= 1;
+  const long long fb_a = ix.face(b, m, q3[2], q3[1], q3[0]) - fb0;   // (ia-1, ib)
+  const double* FaB = f.F[7 * a + 5];   // a-face flux of B~^b  -> E_c = -F
+  const double* FbB = f.F[7 * b + 6];   // b-face flux of B~^a  -> E_c = +F
+  const double* FaD = f.F[7 * a];
+  const double* FbD = f.F[7 * b];
+  const double* Ec = f.Ecc[C3];
+  const double Eaf_00 = -FaB[fa0], Eaf_0m = -FaB[fa0 + fa_b];      // (ia,ib), (ia,ib-1)
+  const double Ebf_00 = FbB[fb0], Ebf_m0 = FbB[fb0 + fb_a];        // (ia,ib), (ia-1,ib)
+  const double Ec_00 = Ec[c0], Ec_m0 = Ec[c0 - cst[a]], Ec_0m = Ec[c0 - cst[b]],
+               Ec_mm = Ec[c0 - cst[a] - cst[b]];
+  const double fD_a0 = FaD[fa0], fD_am = FaD[fa0 + fa_b], fD_b0 = FbD[fb0], fD_bm = FbD[fb0 + fb_a];
+  const double w = fD_a0 > 0.0 ? 1.0 : (fD_a0 < 0.0 ? 0.0 : 0.5);
+  const double wp = fD_am > 0.0 ? 1.0 : (fD_am < 0.0 ? 0.0 : 0.5);
+  const double w2 = fD_b0 > 0.0 ? 1.0 : (fD_b0 < 0.0 ? 0.0 : 0.5);
+  const double w2p = fD_bm > 0.0 ? 1.0 : (fD_bm < 0.0 ? 0.0 : 0.5);
+  const double dbm = w * (Ec_m0 - Ebf_m0) + (1.0 - w) * (Ec_00 - Ebf_00);
+  const double dbp = wp * (Ebf_m0 - Ec_mm) + (1.0 - wp) * (Ebf_00 - Ec_0m);
+  const double dam = w2 * (Ec_0m - Eaf_0m) + (1.0 - w2) * (Ec_00 - Eaf_00);
+  const double dap = w2p * (Eaf_0m - Ec_mm) + (1.0 - w2p) * (Eaf_00 - Ec_m0);
+  const double e = 0.25 * (Eaf_00 + Eaf_0m + Ebf_00 + Ebf_m0) + 0.25 * ((dbp - dbm) + (dap - dam));
+  f.E[C3][ix.edge(C3, m, p3[2], p3[1], p3[0])] = e;
+}
+
+}  // namespace ak

@@ -1,0 +1,105 @@
+// ak_source.cuh — K6: flux divergence + geometric source terms (Eq. 9) on the
+// interior cells.  DESIGN.md §3 O9: sources from the cell-centred primitives of the stage
+// input (reading R22), second-order centred metric derivatives (reading R20).
+#pragma once
+#include "ak_kernels.cuh"
+
+namespace ak {
+
+__global__ void __launch_bounds__(128) k_div_src(const __grid_constant__ Par P,
+                                                 const __grid_constant__ Fields f) {
+  const int n = P.n;
+  const long long per = (long long)n * n * n;
+  const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= per * P.nmb) return;
+  const int m = (int)(idx / per);
+  int r = (int)(idx - (long long)m * per);
+  const int i = r % n + P.is; r /= n;
+  const int j = r % n + P.is;
+  const int k = r / n + P.is;
+  const Ix ix{P.nt, P.px};
+  const long long c = ix.cell(m, k, j, i);
+  const double dxm[3] = {f.dx[3 * m + 0], f.dx[3 * m + 1], f.dx[3 * m + 2]};
+  const double idx3[3] = {1.0 / dxm[0], 1.0 / dxm[1], 1.0 / dxm[2]};
+  const double h2[3] = {0.5 / dxm[0], 0.5 / dxm[1], 0.5 / dxm[2]};
+  double du[5];
+#pragma unroll
+  for (int v = 0; v < 5; ++v) du[v] = -div_flux(f, ix, v, m, k, j, i, idx3);
+
+  Met3 g, gu;
+  load_met3(f, c, g);
+  double det, sdet;
+  metric_inverse(g, det, sdet, gu);
+  const double isd = 1.0 / sdet;
+  const double rho = f.W[0][c], pr = f.W[4][c];
+  const double u[3] = {f.W[1][c], f.W[2][c], f.W[3][c]};
+  const double B[3] = {f.W[5][c] * isd, f.W[6][c] * isd, f.W[7][c] * isd};
+  double cons[5];
+  prim2cons(P, g, rho, u, pr, B, cons);
+  double ul[3], Bl[3];
+  lower(g, u, ul);
+  const double usq = dot3(ul, u);
+  const double Wl = sqrt(1.0 + usq), iW = 1.0 / Wl;
+  lower(g, B, Bl);
+  const double B2 = dot3(Bl, B);
+  const double vl[3] = {ul[0] * iW, ul[1] * iW, ul[2] * iW};
+  const double Bv = B[0] * vl[0] + B[1] * vl[1] + B[2] * vl[2];
+  const double b2 = B2 * iW * iW + Bv * Bv;
+  const double bl[3] = {Bl[0] * iW + Bv * ul[0], Bl[1] * iW + Bv * ul[1], Bl[2] * iW + Bv * ul[2]};
+  const double h = 1.0 + P.Gam / (P.Gam - 1.0) * (pr / rho);
+  const double Ptot = pr + 0.5 * b2;
+  const double wt = rho * h + b2;
+  // S_ij = (rho h + b^2) u_i u_j + Ptot gamma_ij - b_i b_j
+  const double gd[6] = {g.xx, g.xy, g.xz, g.yy, g.yz, g.zz};
+  const double gi6[6] = {gu.xx, gu.xy, gu.xz, gu.yy, gu.yz, gu.zz};
+  constexpr int I6[6] = {0, 0, 0, 1, 1, 2}, J6[6] = {0, 1, 2, 1, 2, 2};
+  double Sdd[3][3], gim[3][3];
+#pragma unroll
+  for (int q = 0; q < 6; ++q) {
+    const double s = wt * ul[I6[q]] * ul[J6[q]] + Ptot * gd[q] - bl[I6[q]] * bl[J6[q]];
+    Sdd[I6[q]][J6[q]] = s; Sdd[J6[q]][I6[q]] = s;
+    gim[I6[q]][J6[q]] = gi6[q]; gim[J6[q]][I6[q]] = gi6[q];
+  }
+  // S^{ij} = gamma^{ik} S_kl gamma^{lj}
+  double T[3][3], Suu[6];
+#pragma unroll
+  for (int aa = 0; aa < 3; ++aa)
+#pragma unroll
+    for (int l = 0; l < 3; ++l)
+      T[aa][l] = gim[aa][0] * Sdd[0][l] + gim[aa][1] * Sdd[1][l] + gim[aa][2] * Sdd[2][l];
+#pragma unroll
+  for (int q = 0; q < 6; ++q)
+    Suu[q] = T[I6[q]][0] * gim[0][J6[q]] + T[I6[q]][1] * gim[1][J6[q]] + T[I6[q]][2] * gim[2][J6[q]];
+  const double Sl[3] = {cons[1], cons[2], cons[3]};
+  const double Su[3] = {gu.xx * Sl[0] + gu.xy * Sl[1] + gu.xz * Sl[2],
+                        gu.xy * Sl[0] + gu.yy * Sl[1] + gu.yz * Sl[2],
+                        gu.xz * Sl[0] + gu.yz * Sl[1] + gu.zz * Sl[2]};
+  const double Een = cons[4] + cons[0];
+  const double alp = __ldg(f.adm[6] + c);
+  const long long st3[3] = {1, P.nt, (long long)P.nt * P.nt};
+  double dalp[3];
+#pragma unroll
+  for (int aa = 0; aa < 3; ++aa) {
+    const long long s = st3[aa];
+    dalp[aa] = (__ldg(f.adm[6] + c + s) - __ldg(f.adm[6] + c - s)) * h2[aa];
+    double dg[6], dbeta[3];
+#pragma unroll
+    for (int q = 0; q < 6; ++q) dg[q] = (__ldg(f.adm[q] + c + s) - __ldg(f.adm[q] + c - s)) * h2[aa];
+#pragma unroll
+    for (int bb = 0; bb < 3; ++bb)
+      dbeta[bb] = (__ldg(f.adm[7 + bb] + c + s) - __ldg(f.adm[7 + bb] + c - s)) * h2[aa];
+    const double Sdg = Suu[0] * dg[0] + 2.0 * (Suu[1] * dg[1]) + 2.0 * (Suu[2] * dg[2]) + Suu[3] * dg[3] +
+                       2.0 * (Suu[4] * dg[4]) + Suu[5] * dg[5];
+    const double Sdb = Sl[0] * dbeta[0] + Sl[1] * dbeta[1] + Sl[2] * dbeta[2];
+    du[1 + aa] = du[1 + aa] + sdet * (0.5 * alp * Sdg + Sdb - Een * dalp[aa]);
+  }
+  const double KS = __ldg(f.adm[10] + c) * Suu[0] + 2.0 * (__ldg(f.adm[11] + c) * Suu[1]) +
+                    2.0 * (__ldg(f.adm[12] + c) * Suu[2]) + __ldg(f.adm[13] + c) * Suu[3] +
+                    2.0 * (__ldg(f.adm[14] + c) * Suu[4]) + __ldg(f.adm[15] + c) * Suu[5];
+  const double Sda = Su[0] * dalp[0] + Su[1] * dalp[1] + Su[2] * dalp[2];
+  du[4] = du[4] + sdet * (alp * KS - Sda);
+#pragma unroll
+  for (int v = 0; v < 5; ++v) f.dU[v][c] = du[v];
+}
+
+}  // namespace ak

@@ -1,0 +1,158 @@
+"""GPU parity: the CUDA library (through the C-ABI) against the CPU oracle, element by element,
+on identical seeded inputs.  Bar (BASELINE.json north_star): relative 1e-11 on dU/dt and EMFs
+with an absolute floor 1e-14*max|U|; con2prim status and FOFC flag bytes bit-exact."""
+import copy
+
+import numpy as np
+import pytest
+
+from oracle import pyoracle as orc
+from paper_2409_10384_b200 import workloads as wl
+
+import gpukit
+
+pytestmark = pytest.mark.gpu
+
+
+def run_both(w, want_flux=False, **override):
+    """returns (gpu result, oracle result, report)"""
+    w = copy.deepcopy(w)
+    U_in = [u.copy() for u in w["U"]]
+    with gpukit.GpuStage(w, **override) as g:
+        g.rhs()
+        gres = g.result()
+        gflux = g.flux() if want_flux else None
+        stats = g.stats()
+    p = dict(w["params"]); p.update(override)
+    par = orc.make_params(**p)
+    ores = orc.rhs(par, w["dx"], w["U"], w["Bf"], w["adm"], w["dt_fofc"], nthreads=8, want_flux=want_flux)
+    ores["U"] = w["U"]
+    rep = gpukit.assert_parity(gres, ores, U_in, label=w.get("name", "?"))
+    if want_flux:
+        for q in range(21):
+            assert np.array_equal(gflux[q], ores["flux"][q]) or \
+                gpukit.max_rel_dev(gflux[q], ores["flux"][q], 1e-14 * max(np.max(np.abs(u)) for u in U_in))[0] <= 1.0, \
+                "flux field %d differs" % q
+    # device counters agree with the masks
+    assert stats["n_fofc_cells"] == int(np.count_nonzero(ores["flag"]))
+    assert stats["n_c2p_fail"] == int(np.count_nonzero(ores["status"] & 32))
+    if ores["refl"] is not None:
+        for d in range(3):
+            assert stats["n_fofc_faces"][d] == int(np.count_nonzero(ores["refl"][d]))
+    return gres, ores, rep
+
+
+def test_c0_full():
+    w = wl.make_blocks("C0")
+    g, o, rep = run_both(w, want_flux=True)
+    assert np.count_nonzero(o["flag"]) == 0          # smooth: the empty-list path
+
+
+@pytest.mark.parametrize("recon", [0, 1, 2])
+@pytest.mark.parametrize("riemann", [0, 1])
+def test_c0_variants(recon, riemann):
+    w = wl.make_blocks("C0")
+    run_both(w, want_flux=True, recon=recon, riemann=riemann)
+
+
+@pytest.mark.parametrize("seed", [7, 11])
+@pytest.mark.parametrize("dmp", [0.0, 1.1])
+def test_noise_block_flags(seed, dmp):
+    """C0n: per-cell noise + 1 % low-density cells: floors, FOFC flags and re-fluxed faces."""
+    w = wl.make_test_noise_block(seed=seed, n=8, frac=0.02)
+    g, o, rep = run_both(w, want_flux=True, dmp_M=dmp, recon=2 if dmp else 1)
+    assert np.count_nonzero(o["flag"]) > 0
+
+
+def test_noise_block_ragged_n():
+    """n = 6 and n = 10: block edges that are not multiples of the warp or tile sizes."""
+    for n in (6, 10):
+        w = wl.make_test_noise_block(seed=3, n=n, frac=0.02)
+        run_both(w, want_flux=True, fofc_riemann=1)
+
+
+def test_c1_subset():
+    w = wl.make_blocks("C1", blocks=[0, 7])
+    run_both(w)
+
+
+def test_c2_subset():
+    # blocks that contain the stars' centres and rims (x = +-8) and an atmosphere block
+    w = wl.make_blocks("C2", blocks=[0, 21, 22, 41, 42])
+    g, o, rep = run_both(w, want_flux=True)
+
+
+def test_c3_subset():
+    # the eight innermost blocks around the horizon (level 3) plus torus blocks of level 0/1
+    ids = [192 + 21, 192 + 22, 192 + 25, 192 + 26, 192 + 37, 192 + 38, 64 + 21, 64 + 42, 21, 38]
+    w = wl.make_blocks("C3", blocks=ids)
+    g, o, rep = run_both(w, want_flux=True)
+    assert np.count_nonzero(o["flag"]) > 0
+
+
+def test_c4_subset():
+    spec = wl.config_spec("C4")
+    # one block of every resolution factor near the stars
+    centre = spec["origin"] + 16.0 * spec["delta"][:, None]
+    near = np.argsort(np.abs(centre[:, 0]) - 8.0 + np.abs(centre[:, 1]) + np.abs(centre[:, 2]))[:24]
+    pick = []
+    for fac in (0.5, 1.0, 2.0):
+        pick += [int(b) for b in near if spec["delta"][b] == fac][:2]
+    w = wl.make_blocks("C4", blocks=pick)
+    run_both(w)
+
+
+def test_w_is_valid_and_emf_only():
+    """ak_rhs with w_is_valid=1 after ak_con2prim equals the one-call path; ak_emf reproduces E."""
+    import torch
+    from paper_2409_10384_b200 import ak
+    w = wl.make_test_noise_block(seed=5, n=8, frac=0.02)
+    with gpukit.GpuStage(copy.deepcopy(w)) as a, gpukit.GpuStage(copy.deepcopy(w)) as b:
+        a.rhs()
+        b.con2prim()
+        st = b.status.clone()
+        b.rhs(w_is_valid=True)
+        ra, rb = a.result(), b.result()
+        for k in ("dU", "E", "W"):
+            for x, y in zip(ra[k], rb[k]):
+                assert np.array_equal(x, y)
+        assert np.array_equal(ra["flag"], rb["flag"])
+        assert np.array_equal(ra["status"], st.cpu().numpy())
+        E2 = [torch.zeros_like(e) for e in b.E]
+        ak.ak_emf(b.ctx, b.W, *E2)
+        torch.cuda.synchronize()
+        for x, y in zip(E2, b.E):
+            assert torch.equal(x, y)
+
+
+def test_injected_unphysical_cells():
+    """NaN, negative D, negative tau and huge S: reported as data (status bits), never as errors."""
+    w = wl.make_test_noise_block(seed=9, n=8, frac=0.0)
+    nt = 16
+    w["U"][0][0, 6, 6, 6] = np.nan
+    w["U"][0][0, 7, 9, 5] = -1.0
+    w["U"][4][0, 9, 7, 8] = -5.0
+    w["U"][1][0, 8, 8, 8] = 1e8
+    g, o, rep = run_both(w)
+    assert o["status"][0, 6, 6, 6] & 32
+    assert o["status"][0, 7, 9, 5] & 1
+    assert o["status"][0, 9, 7, 8] & 2
+
+
+def test_host_entry_point_matches_device_path():
+    import torch
+    from paper_2409_10384_b200 import ak
+    w = wl.make_test_noise_block(seed=13, n=8, frac=0.02)
+    with gpukit.GpuStage(copy.deepcopy(w)) as a:
+        a.rhs()
+        ra = a.result()
+        sh = a.sh
+        hU = [u.copy() for u in w["U"]]
+        hW = [np.zeros(sh["cell"]) for _ in range(8)]
+        hdU = [np.zeros(sh["cell"]) for _ in range(5)]
+        hE = [np.zeros(sh[k]) for k in ("ex", "ey", "ez")]
+        hflag = np.zeros(sh["cell"], dtype=np.uint8); hst = np.zeros(sh["cell"], dtype=np.uint8)
+        ak.ak_rhs_host(a.ctx, hU, w["Bf"], hW, w["dt_fofc"], hdU, hE, hflag, hst)
+        for x, y in zip(hdU + hE + hW + hU, ra["dU"] + ra["E"] + ra["W"] + ra["U"]):
+            assert np.array_equal(x, y)
+        assert np.array_equal(hflag, ra["flag"]) and np.array_equal(hst, ra["status"])
