@@ -1,0 +1,420 @@
+#!/usr/bin/env python
+"""bench.py — GRMHD RHS zone-updates/s (fp64) of one ak_rhs stage (parts 1-6) on B200.
+
+    python bench.py --gpus N --steps K --warmup W            (N > 1: launched under torchrun)
+    python bench.py --impl reference ...                     (times the CPU oracle instead)
+
+A step is one pass of the whole hot path (con2prim, x/y/z reconstruct+Riemann, FOFC test and
+re-flux, CT, divergence+sources) over one synthetic MeshBlock batch.  Workload: BASELINE.json
+configs[4] ("C4", 768 x 32^3 blocks + 4 ghosts, WENO-Z/HLLE/FOFC+DMP) — the config the north
+star's bandwidth target is quoted on; it fits one GPU.  Multi-GPU: MeshBlocks are independent
+(DESIGN.md §8), every rank runs its own C4-shaped batch ("weak"), no data-path collective.
+Prints ONE JSON line on rank 0.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2409_10384_b200 import workloads as wl   # noqa: E402  (inputs only; no method arithmetic)
+
+METRIC = "GRMHD RHS zone-updates/sec (fp64)"
+UNIT = "zone-updates/s"
+
+# Algorithmic bytes per processed element of each kernel class:
+# compulsory reads + writes of fp64 fields (8 B each), one pass, no re-reads.
+#   con2prim : 5 U + 3x(nt+1)/nt face B + 6 gamma in, 8 W out (+1 B status)  per stored cell
+#   flux_d   : 8 W-class (7 recon vars) + 10 metric + 1 Bf in, 7 F out       per computed face
+#   fofc_test: 5 U + 15 F(x2 faces shared -> 15) + 6 gamma + 3 Bcc in, 1 B out per test cell
+#   ct       : cell EMF (3 u + 3 Bcc + 10 metric in, 3 out per test cell) + per edge 2 F_B + 2 F_D + 1 Ecc in, 1 out
+#   div_src  : 15 F + 8 W + 16 adm in, 5 out                                 per interior zone
+ALG_BYTES = dict(con2prim=(5 + 3 + 6 + 8) * 8 + 1, flux=(7 + 10 + 1 + 7) * 8, fofc_test=(5 + 15 + 6 + 3) * 8 + 1,
+                 cell_emf=(6 + 10 + 3) * 8, ct_edge=(2 + 2 + 1 + 1) * 8, div_src=(15 + 8 + 16 + 5) * 8)
+
+
+def kernel_units(nmb, n):
+    """elements each kernel class processes per stage."""
+    nt = n + 8
+    return dict(con2prim=nmb * nt ** 3, flux=nmb * (n + 3) * (n + 2) ** 2, fofc_test=nmb * (n + 2) ** 3,
+                cell_emf=nmb * (n + 2) ** 3, ct_edge=3 * nmb * n * (n + 1) ** 2, div_src=nmb * n ** 3)
+
+
+def kernel_alg_bytes(nmb, n):
+    u = kernel_units(nmb, n)
+    b = dict(con2prim=u["con2prim"] * ALG_BYTES["con2prim"], flux_x=u["flux"] * ALG_BYTES["flux"],
+             fofc_test=u["fofc_test"] * ALG_BYTES["fofc_test"],
+             ct=u["cell_emf"] * ALG_BYTES["cell_emf"] + u["ct_edge"] * ALG_BYTES["ct_edge"],
+             div_src=u["div_src"] * ALG_BYTES["div_src"], fofc_fix=0)
+    b["flux_y"] = b["flux_z"] = b["flux_x"]
+    return b
+
+
+def measured_peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            mp = json.load(f)
+        return float(mp["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi sampling of SM clocks and throttle reasons during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.f = None
+        self.p = None
+
+    def start(self):
+        try:
+            self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = dict(sm_mhz=None, sm_max_mhz=None, reasons=[], samples=0)
+        if self.p is None:
+            return out
+        time.sleep(0.15)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for line in self.f:
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 7:
+                continue
+            try:
+                sm.append(float(c[0])); mx.append(float(c[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, c[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        self.f.close()
+        try:
+            os.unlink(self.f.name)
+        except OSError:
+            pass
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), samples=len(sm))
+        out["reasons"] = sorted(reasons)
+        return out
+
+
+def pick_blocks(config, nblocks):
+    nb_all = wl.n_blocks(config)
+    if nblocks is None or nblocks >= nb_all:
+        return None, nb_all
+    # an evenly spread subset keeps the mix of star / atmosphere / refinement-factor blocks
+    ids = np.unique(np.linspace(0, nb_all - 1, nblocks).round().astype(np.int64))
+    return ids, len(ids)
+
+
+def generate(config, ids, chunk=64):
+    """yield workload dicts of at most `chunk` blocks (host memory stays bounded)."""
+    all_ids = np.arange(wl.n_blocks(config)) if ids is None else np.asarray(ids)
+    for s in range(0, len(all_ids), chunk):
+        yield s, wl.make_blocks(config, blocks=all_ids[s:s + chunk])
+
+
+# ------------------------------------------------------------------ CPU oracle arm / baseline
+def oracle_sample(config, target_s=12.0, cores=None):
+    """Time the oracle (as it stands) on a bounded sample of `config`: whole blocks, one thread per
+    block.  Returns zone-updates/s, threads used, a description of the sample and a step closure."""
+    from oracle import pyoracle as orc      # test infrastructure: only this leg may call it
+    cores = cores or os.cpu_count() or 1
+    nb_all = wl.n_blocks(config)
+    spec = wl.config_spec(config)
+    n = spec["params"]["n"]
+    # calibrate on `cores` blocks, then size the sample for ~target_s seconds
+    ids0, _ = pick_blocks(config, min(nb_all, cores))
+    w0 = wl.make_blocks(config, blocks=ids0)
+    par0 = orc.make_params(**w0["params"])
+    t = time.perf_counter()
+    orc.rhs(par0, w0["dx"], [u.copy() for u in w0["U"]], w0["Bf"], w0["adm"], w0["dt_fofc"], nthreads=cores)
+    t0 = time.perf_counter() - t
+    nb0 = w0["params"]["nmb"]
+    nb = int(min(nb_all, max(nb0, round(nb0 * target_s / max(t0, 1e-3)))))
+    nb = max(cores, (nb // cores) * cores) if nb_all >= cores else nb_all
+    nb = min(nb, nb_all)
+    ids, nb = pick_blocks(config, nb)
+    w = wl.make_blocks(config, blocks=ids)
+    par = orc.make_params(**w["params"])
+    zones = nb * n ** 3
+
+    def step():
+        U = [u.copy() for u in w["U"]]
+        t = time.perf_counter()
+        orc.rhs(par, w["dx"], U, w["Bf"], w["adm"], w["dt_fofc"], nthreads=cores)
+        return time.perf_counter() - t
+    sample = "%d of %d %s MeshBlocks (evenly spread), one full oracle stage, %d threads over blocks" % (
+        nb, nb_all, config, min(cores, nb))
+    return zones, min(cores, nb), sample, step
+
+
+def run_reference(args, rank):
+    if rank != 0:
+        return 0
+    # each step is a bounded sample sized so that warm-up + K steps end within ~2 minutes
+    warm = min(args.warmup, 1)
+    steps = max(1, args.steps)
+    zones, cores, sample, step = oracle_sample(
+        args.config, target_s=max(0.5, min(args.cpu_seconds, 120.0 / (steps + warm))))
+    for _ in range(warm):
+        step()
+    ts = [step() for _ in range(steps)]
+    tot = sum(ts)
+    val = zones * steps / tot
+    spec = wl.config_spec(args.config)
+    line = dict(metric=METRIC, value=val, unit=UNIT, n_gpus=args.gpus, steps=steps, warmup=warm,
+                ms_per_step=1e3 * tot / steps, higher_is_better=True, scaling="weak", vs_baseline=None,
+                dtype="f64", data="synthetic", impl="reference",
+                config=dict(workload="%s (BASELINE.json configs[%s]): bounded sample — %s" % (
+                    args.config, args.config[1], sample), n=spec["params"]["n"], ng=4),
+                cpu_baseline=dict(value=val, unit=UNIT, cores=cores, kind="oracle", sample=sample),
+                e2e=dict(value=val, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0),
+                gpu_launches=0)
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------ the CUDA arm
+def run_gpu(args, rank, local_rank, world):
+    import torch
+    import torch.distributed as dist
+    from paper_2409_10384_b200 import ak
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device — the library has no CPU path")
+    dev = torch.device("cuda", local_rank)
+    torch.cuda.set_device(dev)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    config = args.config
+    spec = wl.config_spec(config)
+    ids, nmb = pick_blocks(config, args.blocks)
+    n = spec["params"]["n"]
+    sh = ak.shapes(nmb, n)
+    f64 = torch.float64
+    z = lambda k, dt=f64: torch.zeros(sh[k], dtype=dt, device=dev)
+    # ---- inputs: generated on the host in chunks of blocks, made resident in HBM
+    t_gen = time.perf_counter()
+    U = [z("cell") for _ in range(5)]
+    Bf = [z("xf"), z("yf"), z("zf")]
+    adm = [z("cell") for _ in range(16)]
+    dx = np.zeros((nmb, 3))
+    params_d = None
+    for s0, w in generate(config, ids):
+        nb = w["params"]["nmb"]
+        for dst, src in zip(U + Bf + adm, w["U"] + w["Bf"] + w["adm"]):
+            dst[s0:s0 + nb].copy_(torch.from_numpy(src))
+        dx[s0:s0 + nb] = w["dx"]
+        params_d = dict(w["params"])
+        dt_fofc = w["dt_fofc"]
+    params_d["nmb"] = nmb
+    t_gen = time.perf_counter() - t_gen
+    U0 = [u.clone() for u in U]           # pristine copy: the e2e leg and the parity spot-check use it
+    W = [z("cell") for _ in range(8)]
+    dU = [z("cell") for _ in range(5)]
+    E = [z("ex"), z("ey"), z("ez")]
+    flag = z("cell", torch.uint8)
+    status = z("cell", torch.uint8)
+    stream = torch.cuda.current_stream(dev)
+    par = ak.make_params(device=local_rank, stream=stream.cuda_stream, **params_d)
+    ctx = ak.ak_create(par, dx)
+    ak.ak_set_metric(ctx, adm)
+    zones = nmb * n ** 3
+
+    def step():
+        ak.ak_rhs(ctx, U, Bf, W, 0, dt_fofc, dU, E, flag, status)
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize(dev)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    # ---- timed region: exactly K steps between CUDA events on the launching stream
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    ak.ak_timing(ctx, 1)                  # resets launch counters; per-kernel-class events on the stream
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(stream)
+    for _ in range(args.steps):
+        step()
+    e1.record(stream)
+    barrier()
+    ms_total = e0.elapsed_time(e1)
+    clocks = sampler.stop()
+    kms, klaunch = ak.ak_kernel_ms(ctx)
+    ak.ak_timing(ctx, 0)
+    stats = ak.ak_get_stats(ctx)
+    tmax = torch.tensor([ms_total], dtype=f64, device=dev)
+    if world > 1:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    ms_total = float(tmax.item())
+    ms_step = ms_total / args.steps
+    value = world * zones / (ms_step * 1e-3)
+    return dict(torch=torch, ak=ak, ctx=ctx, dev=dev, stream=stream, U=U, U0=U0, Bf=Bf, W=W, dU=dU, E=E, flag=flag,
+                status=status, sh=sh, nmb=nmb, n=n, ids=ids, zones=zones, dt_fofc=dt_fofc, params_d=params_d,
+                ms_step=ms_step, value=value, clocks=clocks, kms=kms, klaunch=klaunch, stats=stats, t_gen=t_gen,
+                spec=spec, world=world, dx=dx)
+
+
+def run_e2e(R, steps):
+    """Same metric through the C-ABI call with HOST buffers (ak_rhs_host): every step copies the
+    step's inputs U~, B~f from pinned host memory, runs parts 1-6 and reads back U~ (floored cells),
+    W, dU/dt, E and both masks.  The frozen metric snapshot stays resident (ak_set_metric)."""
+    torch, ak = R["torch"], R["ak"]
+    sh = R["sh"]
+    pin = lambda k, dt=torch.float64: torch.zeros(sh[k], dtype=dt).pin_memory()
+    hU = [pin("cell") for _ in range(5)]
+    hB = [pin("xf"), pin("yf"), pin("zf")]
+    for h, d in zip(hU + hB, R["U0"] + R["Bf"]):
+        h.copy_(d)
+    hU0 = [h.clone() for h in hU]
+    hW = [pin("cell") for _ in range(8)]
+    hdU = [pin("cell") for _ in range(5)]
+    hE = [pin("ex"), pin("ey"), pin("ez")]
+    hflag, hst = pin("cell", torch.uint8), pin("cell", torch.uint8)
+    nbytes = lambda ts: int(sum(t.numel() * t.element_size() for t in ts))
+    h2d = nbytes(hU + hB)
+    d2h = nbytes(hU + hW + hdU + hE + [hflag, hst])
+    call = lambda: ak.ak_rhs_host(R["ctx"], hU, hB, hW, R["dt_fofc"], hdU, hE, hflag, hst)
+    call()                                                   # warm-up: allocates staging
+    ts = []
+    for _ in range(steps):
+        for h, h0 in zip(hU, hU0):
+            h.copy_(h0)                                      # outside the timed region
+        torch.cuda.synchronize(R["dev"])
+        t = time.perf_counter()
+        call()                                               # synchronises before returning
+        ts.append(time.perf_counter() - t)
+    tmax = torch.tensor([sum(ts)], dtype=torch.float64, device=R["dev"])
+    if R["world"] > 1:
+        import torch.distributed as dist
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    val = R["world"] * R["zones"] * steps / float(tmax.item())
+    # the host path must give what the device path gave
+    same = all(bool(torch.equal(h, d.cpu())) for h, d in zip(hdU, R["dU"]))
+    return dict(value=val, unit=UNIT, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h, steps=steps,
+                ms_per_step=1e3 * float(tmax.item()) / steps, matches_device_path=same)
+
+
+def roofline(R, hbm_peak, peak_src):
+    """Per-kernel-class table and the roofline object of the dominant class."""
+    torch, ak = R["torch"], R["ak"]
+    algb = kernel_alg_bytes(R["nmb"], R["n"])
+    steps = R["steps"]
+    tot = sum(R["kms"].values())
+    table = {}
+    for k in ak.KERNEL_CLASSES:
+        ms = R["kms"][k] / steps
+        table[k] = dict(ms=round(ms, 4), share=round(R["kms"][k] / tot, 4) if tot > 0 else None,
+                        launches_per_step=R["klaunch"][k] / steps, alg_bytes=algb[k],
+                        alg_gbs=round(algb[k] / (ms * 1e-3) * 1e-9, 1) if ms > 0 else None)
+    dom = max(ak.KERNEL_CLASSES, key=lambda k: R["kms"][k])
+    # same-run denominators: a fp64 copy kernel and independent fp64 instruction streams
+    n_probe = 1 << 28                                         # 2 GiB per buffer, 4 GiB traffic
+    a = torch.empty(n_probe, dtype=torch.float64, device=R["dev"]).normal_()
+    b = torch.empty_like(a)
+    copy_gbs = ak.ak_probe_copy(R["ctx"], b, a, n_probe, 5)
+    del a, b
+    fp64_fma = ak.ak_probe_fp64(R["ctx"], 1, 3)
+    fp64_nofma = ak.ak_probe_fp64(R["ctx"], 0, 3)
+    ach = table[dom]["alg_gbs"]
+    rf = dict(kernel=dom, bound="hbm", achieved=ach, peak=hbm_peak, unit="GB/s",
+              frac=round(ach / hbm_peak, 4) if ach else None, traffic=None, peak_source=peak_src,
+              same_run_copy_gbs=round(copy_gbs, 1), same_run_fp64_ginst=dict(fma=round(fp64_fma, 1),
+                                                                              mul_add=round(fp64_nofma, 1)))
+    stage_bytes = sum(algb.values())
+    stage = dict(alg_bytes_per_zone=round(stage_bytes / R["zones"], 1),
+                 alg_gbs=round(stage_bytes / (R["ms_step"] * 1e-3) * 1e-9, 1))
+    stage["frac_of_hbm_peak"] = round(stage["alg_gbs"] / hbm_peak, 4)
+    return rf, table, stage
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ak", choices=("ak", "reference"))
+    ap.add_argument("--config", default="C4", choices=wl.CONFIG_NAMES)
+    ap.add_argument("--blocks", type=int, default=None, help="use an evenly spread subset of the blocks")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--cpu-seconds", type=float, default=12.0, help="CPU-oracle sample budget per step")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        return run_reference(args, rank)
+    R = run_gpu(args, rank, local_rank, world)
+    R["steps"] = args.steps
+    hbm_peak, peak_src = measured_peaks()
+    rf, table, stage = roofline(R, hbm_peak, peak_src)
+    e2e = None if args.no_e2e else run_e2e(R, max(1, args.e2e_steps))
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        zones, cores, sample, step = oracle_sample(args.config, target_s=args.cpu_seconds)
+        t = step()
+        cpu = dict(value=zones / t, unit=UNIT, cores=cores, kind="oracle", sample=sample, seconds=round(t, 2))
+    if rank == 0:
+        spec = R["spec"]
+        st = R["stats"]
+        ntest = R["nmb"] * (R["n"] + 2) ** 3
+        line = dict(metric=METRIC, value=R["value"], unit=UNIT, n_gpus=world, steps=args.steps,
+                    warmup=max(args.warmup, 3), ms_per_step=R["ms_step"], higher_is_better=True, scaling="weak",
+                    vs_baseline=None, dtype="f64", data="synthetic", impl="ak",
+                    config=dict(workload="%s (BASELINE.json configs[%s]): %d MeshBlocks of %d^3 + 4 ghosts per GPU, "
+                                "%s/%s, FOFC %s, DMP M=%s" % (
+                                    args.config, args.config[1], R["nmb"], R["n"],
+                                    ("donor", "PPM4", "WENO-Z")[spec["params"]["recon"]],
+                                    ("LLF", "HLLE")[spec["params"]["riemann"]],
+                                    "on" if spec["params"]["fofc"] else "off", spec["params"]["dmp_M"]),
+                                interior_zones_per_gpu=R["zones"], parallelism="blocks sharded, no collective",
+                                l2="inputs larger than L2 (working set %.1f GB per GPU)" % (
+                                    64 * 8 * R["nmb"] * (R["n"] + 8) ** 3 * 1e-9),
+                                fofc_flagged_fraction=round(st["n_fofc_cells"] / ntest, 6),
+                                fofc_faces=st["n_fofc_faces"]),
+                    clocks=R["clocks"], e2e=e2e, gpu_launches=int(sum(R["klaunch"].values())),
+                    roofline=rf, kernels=table, stage_hbm=stage, cpu_baseline=cpu,
+                    gen_seconds=round(R["t_gen"], 1))
+        print(json.dumps(line))
+    R["ak"].ak_destroy(R["ctx"])
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

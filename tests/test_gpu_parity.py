@@ -60,15 +60,30 @@ def test_c0_variants(recon, riemann):
 def test_noise_block_flags(seed, dmp):
     """C0n: per-cell noise + 1 % low-density cells: floors, FOFC flags and re-fluxed faces."""
     w = wl.make_test_noise_block(seed=seed, n=8, frac=0.02)
+    if not dmp:
+        w["dt_fofc"] *= 2.0          # without the maximum principle only a larger step raises flags
     g, o, rep = run_both(w, want_flux=True, dmp_M=dmp, recon=2 if dmp else 1)
     assert np.count_nonzero(o["flag"]) > 0
+    assert bool(np.any(o["flag"] & 64)) == bool(dmp)
+
+
+@pytest.mark.parametrize("recon", [1, 2])
+def test_noise_block_floors(recon):
+    """Atmosphere raised above the low-density cells: D floor, rho floor, T floor and tau floor
+    fire in con2prim (status bytes), the face-state floor fires after reconstruction."""
+    w = wl.make_test_noise_block(seed=21, n=8, frac=0.05)
+    w["dt_fofc"] *= 2.0
+    g, o, rep = run_both(w, want_flux=True, recon=recon, rho_atm=3e-6, T_atm=0.6, f_thr=1.0)
+    assert np.any(o["status"] & 1) and np.any(o["status"] & 16)
 
 
 def test_noise_block_ragged_n():
     """n = 6 and n = 10: block edges that are not multiples of the warp or tile sizes."""
     for n in (6, 10):
         w = wl.make_test_noise_block(seed=3, n=n, frac=0.02)
-        run_both(w, want_flux=True, fofc_riemann=1)
+        w["dt_fofc"] *= 2.0
+        g, o, rep = run_both(w, want_flux=True, fofc_riemann=1)
+        assert np.count_nonzero(o["flag"]) > 0
 
 
 def test_c1_subset():
