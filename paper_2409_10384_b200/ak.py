@@ -11,7 +11,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-SO_PATH = os.path.join(_HERE, "libak.so")
+SO_PATH = os.environ.get("AK_LIBRARY") or os.path.join(_HERE, "libak.so")   # AK_LIBRARY: another build of the same library
 
 AK_OK, AK_EINVAL, AK_ENOMEM, AK_ECUDA, AK_ESTATE = 0, -1, -2, -3, -4
 RECON_DC, RECON_PPM4, RECON_WENOZ = 0, 1, 2

@@ -12,6 +12,17 @@
 
 namespace ak {
 
+// occupancy targets (blocks of 128 threads per SM) — tuned with ncu, see profiles/
+#ifndef AK_C2P_MINB
+#define AK_C2P_MINB 6
+#endif
+#ifndef AK_FLUX_MINB
+#define AK_FLUX_MINB 5
+#endif
+#ifndef AK_FOFC_MINB
+#define AK_FOFC_MINB 8
+#endif
+
 // stats slots (device counters)
 enum { S_C2P_FAIL = 0, S_CONS_FLOOR, S_PRIM_FLOOR, S_FOFC_CELLS, S_DMP_CELLS, S_NSTAT };
 
@@ -51,7 +62,7 @@ __device__ __forceinline__ void load_met10(const Fields& f, long long c, double 
 }
 
 // ---- K1 ------------------------------------------------------------------------------
-__global__ void __launch_bounds__(128) k_con2prim(const __grid_constant__ Par P,
+__global__ void __launch_bounds__(128, AK_C2P_MINB) k_con2prim(const __grid_constant__ Par P,
                                                   const __grid_constant__ Fields f) {
   const int nt = P.nt;
   const long long ncell = (long long)P.nmb * nt * nt * nt;
@@ -106,7 +117,7 @@ __device__ __forceinline__ bool decode_face(const Par& P, long long idx, int& m,
 
 // ---- K2 (v1: one thread per face; both one-sided reconstructions done by the thread) ----
 template <int DIR, int RECON>
-__global__ void __launch_bounds__(128) k_flux(const __grid_constant__ Par P,
+__global__ void __launch_bounds__(128, AK_FLUX_MINB) k_flux(const __grid_constant__ Par P,
                                               const __grid_constant__ Fields f) {
   int m, k, j, i;
   if (!decode_face<DIR>(P, (long long)blockIdx.x * blockDim.x + threadIdx.x, m, k, j, i)) return;
@@ -163,7 +174,7 @@ __device__ __forceinline__ double div_flux(const Fields& f, const Ix& ix, int v,
 }
 
 // ---- K3: FOFC estimate and test (DMP Eq. 12) -------------------------------
-__global__ void __launch_bounds__(128) k_fofc_test(const __grid_constant__ Par P,
+__global__ void __launch_bounds__(128, AK_FOFC_MINB) k_fofc_test(const __grid_constant__ Par P,
                                                    const __grid_constant__ Fields f, double dt) {
   int m, k, j, i;
   if (!decode_test(P, (long long)blockIdx.x * blockDim.x + threadIdx.x, m, k, j, i)) return;
