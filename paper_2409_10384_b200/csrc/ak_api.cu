@@ -8,6 +8,10 @@
 #if AK_FLUX_TILE
 #include "ak_flux_tile.cuh"
 #endif
+#ifndef AK_FLUX_TMA
+#define AK_FLUX_TMA 1   // 1: TMA-staged sweeps (ak_flux_tma.cuh) when n is even and a face row fits a block
+#endif
+#include "ak_flux_tma.cuh"
 
 #include <cmath>
 #include <cstdint>
@@ -46,6 +50,7 @@ struct ak_ctx {
   double* stg_U[5]; double* stg_Bf[3]; double* stg_W[8]; double* stg_dU[5]; double* stg_E[3];
   unsigned char* stg_flag; unsigned char* stg_status;
   bool have_stg;
+  bool tma_attr[3];
   // timing
   bool timing;
   cudaEvent_t ev0, ev1;
@@ -145,10 +150,43 @@ int launch_c2p(ak_ctx* c, const Fields& f) {
   return AK_OK;
 }
 
+template <int DIR, int RECON>
+int launch_flux_tma(ak_ctx* c, const Fields& f, int NA, unsigned grid, size_t smem) {
+  if (!c->tma_attr[DIR]) {
+    CK(cudaFuncSetAttribute(k_flux_tma<DIR, RECON>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    c->tma_attr[DIR] = true;
+  }
+  k_flux_tma<DIR, RECON><<<grid, TMA_THREADS, smem, c->stream>>>(c->P, f, NA);
+  return AK_OK;
+}
+
 template <int DIR>
 int launch_flux(ak_ctx* c, const Fields& f) {
   Timer t(c, KC_FX + DIR);
-  const int n = c->P.n;
+  const int n = c->P.n, nt = c->P.nt, e = n + 2;
+  const int nfi = DIR == 0 ? n + 3 : e;            // faces per row of a tile
+  if (AK_FLUX_TMA && n % 2 == 0 && nfi <= TMA_THREADS) {
+    // tile height: as many rows as fit the block, balanced over the extent it tiles
+    const int nfd = DIR == 0 ? e : n + 3;
+    const int namax = TMA_THREADS / nfi;
+    const int tiles = (nfd + namax - 1) / namax;
+    const int NA = (nfd + tiles - 1) / tiles;
+    const int maxW = DIR == 0 ? NA : NA + 5, maxM = DIR == 0 ? NA : NA + 1;
+    const size_t smem = sizeof(double) * (size_t)(7 * maxW + 10 * maxM) * nt;
+    if (smem <= 200 * 1024) {
+      const unsigned grid = (unsigned)((long long)c->P.nmb * e * tiles);
+      int r;
+      switch (c->P.recon) {
+        case 0: r = launch_flux_tma<DIR, 0>(c, f, NA, grid, smem); break;
+        case 1: r = launch_flux_tma<DIR, 1>(c, f, NA, grid, smem); break;
+        default: r = launch_flux_tma<DIR, 2>(c, f, NA, grid, smem); break;
+      }
+      if (r != AK_OK) return r;
+      CK(cudaGetLastError());
+      c->launches[KC_FX + DIR] += 1;
+      return AK_OK;
+    }
+  }
 #if AK_FLUX_TILE
   // tile shape (ak_flux_tile.cuh): x sweeps take whole pencils, y/z sweeps 32 pencils x 8 cells
   int NA, NB;

@@ -46,14 +46,14 @@ __device__ __forceinline__ void recon(double qmm, double qm1, double q0, double 
       const double p1 = (-qm1 + 5.0 * q0 + 2.0 * qp1) * c6;
       const double p2 = (2.0 * q0 + 5.0 * qp1 - qpp) * c6;
       const double w0 = 0.1 * t0, w1 = 0.6 * t1, w2 = 0.3 * t2;
-      qp = (w0 * p0 + w1 * p1 + w2 * p2) / (w0 + w1 + w2);
+      qp = ddiv(w0 * p0 + w1 * p1 + w2 * p2, w0 + w1 + w2);
     }
     {  // mirror image
       const double p0 = (2.0 * qpp - 7.0 * qp1 + 11.0 * q0) * c6;
       const double p1 = (-qp1 + 5.0 * q0 + 2.0 * qm1) * c6;
       const double p2 = (2.0 * q0 + 5.0 * qm1 - qmm) * c6;
       const double w0 = 0.1 * t2, w1 = 0.6 * t1, w2 = 0.3 * t0;
-      qm = (w0 * p0 + w1 * p1 + w2 * p2) / (w0 + w1 + w2);
+      qm = ddiv(w0 * p0 + w1 * p1 + w2 * p2, w0 + w1 + w2);
     }
   }
 }
@@ -120,7 +120,7 @@ __device__ __forceinline__ void side_state(const Par& P, const FaceGeo& G, const
   const double D = rho * W;
   const double wtot = rho * h * W * W + B2;
   const double S[3] = {wtot * vl[0] - Bv * Bl[0], wtot * vl[1] - Bv * Bl[1], wtot * vl[2] - Bv * Bl[2]};
-  const double tau = D * (hm1 * W + usq / (1.0 + W)) + B2 - pr - 0.5 * (Bv * Bv + B2 * iW * iW);
+  const double tau = D * (hm1 * W + ddiv(usq, 1.0 + W)) + B2 - pr - 0.5 * (Bv * Bv + B2 * iW * iW);
   const double vh[3] = {v[0] - G.bet[0] * G.ialp, v[1] - G.bet[1] * G.ialp, v[2] - G.bet[2] * G.ialp};
   const double BdW = B[DIR] * iW;
   const double aP = G.alp * Ptot;
@@ -142,7 +142,7 @@ __device__ __forceinline__ void side_state(const Par& P, const FaceGeo& G, const
   const double vsq = v[0] * vl[0] + v[1] * vl[1] + v[2] * vl[2];
   const double cs2 = P.Gam * T / h;
   const double rhoh = rho * h;
-  const double va2 = b2 / (rhoh + b2);
+  const double va2 = ddiv(b2, rhoh + b2);
   const double a2 = cs2 + va2 - cs2 * va2;
   const double om = 1.0 - vsq * a2;
   const double disc = a2 * (1.0 - vsq) * (G.gdd * om - v[DIR] * v[DIR] * (1.0 - a2));

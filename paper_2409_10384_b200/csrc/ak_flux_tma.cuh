@@ -1,0 +1,135 @@
+// ak_flux_tma.cuh — K2, TMA-staged: the rows of primitives and metric a tile of faces needs are
+// copied global -> shared memory with 1-D bulk TMA copies (cp.async.bulk, SASS UBLKCP) that
+// complete on an mbarrier; the threads then reconstruct and solve one face each out of shared
+// memory.  No thread holds a register for data in flight, stencil re-reads hit shared memory,
+// and the 2-3 blocks resident on an SM overlap one block's copies with the others' arithmetic.
+//
+// Tile (n even, so every row of nt doubles is a multiple of 16 B):
+//   DIR = x : NA rows (consecutive j at fixed k, m); faces i in [is-1, ie+2] of those rows.
+//             shared rows: NA per field (primitives and metric alike).
+//   DIR = y : one k-plane, NA consecutive face rows jf; faces i in [is-1, ie+1].
+//   DIR = z : one j-row,   NA consecutive face planes kf; faces i in [is-1, ie+1].
+//             shared rows: NA+5 per primitive field (cells f-3 .. f+2), NA+1 per metric field.
+// Shared layout: [field][row][nt] doubles; lanes run along i: conflict-free.
+#pragma once
+#include <cstdint>
+#include "ak_kernels.cuh"
+
+namespace ak {
+
+#ifndef AK_TMA_MINB
+#define AK_TMA_MINB 2
+#endif
+constexpr int TMA_THREADS = 256;
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* b, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count) : "memory");
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* b, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_copy_g2s(void* dst, const void* src, unsigned bytes, uint64_t* b) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(b)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* b, unsigned parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "AK_WAIT:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra AK_DONE;\n"
+      "bra AK_WAIT;\n"
+      "AK_DONE:\n"
+      "}\n" ::"r"(smem_u32(b)), "r"(parity) : "memory");
+}
+
+template <int DIR, int RECON>
+__global__ void __launch_bounds__(TMA_THREADS, AK_TMA_MINB)
+k_flux_tma(const __grid_constant__ Par P, const __grid_constant__ Fields f, int NA) {
+  extern __shared__ __align__(128) double sm[];
+  __shared__ uint64_t mbar;
+  const int nt = P.nt, e = P.n + 2, t = threadIdx.x;
+  constexpr int t1 = (DIR + 1) % 3, t2 = (DIR + 2) % 3;
+  const int maxW = DIR == 0 ? NA : NA + 5, maxM = DIR == 0 ? NA : NA + 1;
+  double* sW = sm;                             // [7][maxW][nt]
+  double* sM = sm + 7 * maxW * nt;             // [10][maxM][nt]
+  // ---- which tile
+  const int nfd = DIR == 0 ? e : P.n + 3;      // extent that NA tiles: rows (x) or faces along d (y,z)
+  const int tiles = (nfd + NA - 1) / NA;
+  int bid = blockIdx.x;
+  const int td = bid % tiles; bid /= tiles;
+  const int o = bid % e + P.is - 1;            // the fixed transverse index (k for x,y; j for z)
+  const int m = bid / e;
+  const int d0 = P.is - 1 + td * NA;           // first row (x) / first face along d (y,z)
+  const int na = min(NA, P.is - 1 + nfd - d0); // rows / faces actually present in this tile
+  const int nW = DIR == 0 ? na : na + 5, nM = DIR == 0 ? na : na + 1;
+  const Ix ix{nt, P.px};
+  // first cell of shared row 0 of the primitive slab / of the metric slab, and the row stride
+  long long baseW, baseM, rs;
+  if (DIR == 0) { baseW = baseM = ix.cell(m, o, d0, 0); rs = nt; }
+  else if (DIR == 1) { baseW = ix.cell(m, o, d0 - 3, 0); baseM = ix.cell(m, o, d0 - 1, 0); rs = nt; }
+  else { baseW = ix.cell(m, d0 - 3, o, 0); baseM = ix.cell(m, d0 - 1, o, 0); rs = (long long)nt * nt; }
+  const unsigned rowb = (unsigned)(nt * sizeof(double));
+  if (t == 0) mbar_init(&mbar, 1);
+  __syncthreads();
+  if (t == 0) mbar_arrive_expect_tx(&mbar, (unsigned)(7 * nW + 10 * nM) * rowb);
+  // ---- one bulk copy per (field, row)
+  const int ncW = 7 * nW, nc = ncW + 10 * nM;
+  for (int c = t; c < nc; c += TMA_THREADS) {
+    if (c < ncW) {
+      const int v = c / nW, r = c - v * nW;
+      const int fld = v < 5 ? v : (v == 5 ? 5 + t1 : 5 + t2);
+      bulk_copy_g2s(sW + ((size_t)v * maxW + r) * nt, f.W[fld] + baseW + r * rs, rowb, &mbar);
+    } else {
+      const int cc = c - ncW;
+      const int q = cc / nM, r = cc - q * nM;
+      const int fld = q == 0 ? 6 : (q < 4 ? 6 + q : q - 4);   // alp, betx..betz, gxx..gzz
+      bulk_copy_g2s(sM + ((size_t)q * maxM + r) * nt, f.adm[fld] + baseM + r * rs, rowb, &mbar);
+    }
+  }
+  // ---- this thread's face
+  const int nfi = DIR == 0 ? P.n + 3 : e;      // faces per shared row
+  const int a = t / nfi, ii = t - a * nfi + P.is - 1;   // row within the tile, i index of the face
+  const bool active = a < na;
+  long long fi = 0;
+  double Bfd = 0.0;
+  if (active) {
+    if (DIR == 0) fi = ix.face(0, m, o, d0 + a, ii);
+    else if (DIR == 1) fi = ix.face(1, m, o, d0 + a, ii);
+    else fi = ix.face(2, m, d0 + a, o, ii);
+    Bfd = __ldg(f.Bf[DIR] + fi);
+  }
+  mbar_wait(&mbar, 0);
+  if (!active) return;
+  double sL[7], sR[7], mL[10], mR[10], Fo[7];
+#pragma unroll
+  for (int v = 0; v < 7; ++v) {
+    // six stencil cells f-3 .. f+2: along i in one row (x) or one per shared row (y, z)
+    const double* w = DIR == 0 ? sW + ((size_t)v * maxW + a) * nt + ii - 3 : sW + ((size_t)v * maxW + a) * nt + ii;
+    const int s = DIR == 0 ? 1 : nt;
+    if (RECON == 0) {
+      sL[v] = w[2 * s]; sR[v] = w[3 * s];
+    } else {
+      const double q0 = w[0], q1 = w[s], q2 = w[2 * s], q3 = w[3 * s], q4 = w[4 * s], q5 = w[5 * s];
+      double qm, qp;
+      recon<RECON>(q0, q1, q2, q3, q4, qm, qp);
+      sL[v] = qp;
+      recon<RECON>(q1, q2, q3, q4, q5, qm, qp);
+      sR[v] = qm;
+    }
+  }
+#pragma unroll
+  for (int q = 0; q < 10; ++q) {
+    const double* g = DIR == 0 ? sM + ((size_t)q * maxM + a) * nt + ii - 1 : sM + ((size_t)q * maxM + a) * nt + ii;
+    mL[q] = g[0];
+    mR[q] = g[DIR == 0 ? 1 : nt];
+  }
+  face_flux<DIR, true>(P, P.riemann, mL, mR, sL, sR, Bfd, Fo);
+#pragma unroll
+  for (int v = 0; v < 7; ++v) f.F[7 * DIR + v][fi] = Fo[v];
+}
+
+}  // namespace ak
