@@ -42,7 +42,7 @@ struct ak_ctx {
   double* F[21];
   double* Ecc[3];
   unsigned char* flag_own;
-  unsigned int* list[3];
+  unsigned int* list;
   unsigned int* count;          // [4]
   unsigned long long* stats;    // [S_NSTAT]
   double* dx;
@@ -116,7 +116,8 @@ void fill_fields(ak_ctx* c, Fields& f) {
   memset(&f, 0, sizeof(f));
   for (int q = 0; q < 16; ++q) f.adm[q] = c->adm[q];
   for (int q = 0; q < 21; ++q) f.F[q] = c->F[q];
-  for (int q = 0; q < 3; ++q) { f.Ecc[q] = c->Ecc[q]; f.list[q] = c->list[q]; }
+  for (int q = 0; q < 3; ++q) f.Ecc[q] = c->Ecc[q];
+  f.list = c->list;
   f.count = c->count;
   f.stats = c->stats;
   f.dx = c->dx;
@@ -238,16 +239,12 @@ int launch_fofc(ak_ctx* c, const Fields& f, double dt) {
   }
   if (c->P.fofc) {
     Timer t(c, KC_FOFC_FIX);
-    k_fofc_list<0><<<nblk(nf, 256), 256, 0, c->stream>>>(c->P, f);
-    k_fofc_list<1><<<nblk(nf, 256), 256, 0, c->stream>>>(c->P, f);
-    k_fofc_list<2><<<nblk(nf, 256), 256, 0, c->stream>>>(c->P, f);
-    CK(cudaGetLastError());
     const unsigned g = (unsigned)(nf < 148LL * 8 * 128 ? nblk(nf, 128) : 148 * 8);
     k_fofc_reflux<0><<<g, 128, 0, c->stream>>>(c->P, f);
     k_fofc_reflux<1><<<g, 128, 0, c->stream>>>(c->P, f);
     k_fofc_reflux<2><<<g, 128, 0, c->stream>>>(c->P, f);
     CK(cudaGetLastError());
-    c->launches[KC_FOFC_FIX] += 6;
+    c->launches[KC_FOFC_FIX] += 3;
   }
   return AK_OK;
 }
@@ -361,7 +358,7 @@ int ak_create(const ak_params* p, const double* dx3, ak_ctx** out) {
   c->sz.xf = nb * nt * nt * px; c->sz.yf = nb * nt * (nt + 1) * nt; c->sz.zf = nb * (nt + 1) * nt * nt;
   c->sz.ex = nb * (nt + 1) * (nt + 1) * nt; c->sz.ey = nb * (nt + 1) * nt * px; c->sz.ez = nb * nt * (nt + 1) * px;
   const long long fsz[3] = {c->sz.xf, c->sz.yf, c->sz.zf};
-  const long long nfaces = nb * (P.n + 3) * (P.n + 2) * (P.n + 2);
+  const long long ntest = nb * (P.n + 2) * (P.n + 2) * (P.n + 2);
   cudaError_t e = cudaSuccess;
   for (int d = 0; d < 3 && e == cudaSuccess; ++d) {
     for (int q = 0; q < 7 && e == cudaSuccess; ++q) {
@@ -371,8 +368,8 @@ int ak_create(const ak_params* p, const double* dx3, ak_ctx** out) {
     }
     if (e == cudaSuccess) e = cudaMalloc(&c->Ecc[d], sizeof(double) * c->sz.cell);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->Ecc[d], 0, sizeof(double) * c->sz.cell, c->stream);
-    if (e == cudaSuccess) e = cudaMalloc(&c->list[d], sizeof(unsigned) * nfaces);
   }
+  if (e == cudaSuccess) e = cudaMalloc(&c->list, sizeof(unsigned) * ntest);
   if (e == cudaSuccess) e = cudaMalloc(&c->flag_own, (size_t)c->sz.cell);
   if (e == cudaSuccess) e = cudaMalloc(&c->count, sizeof(unsigned) * 4);
   if (e == cudaSuccess) e = cudaMalloc(&c->stats, sizeof(unsigned long long) * S_NSTAT);
@@ -398,7 +395,8 @@ int ak_destroy(ak_ctx* c) {
   for (int q = 0; q < c->npend; ++q) { cudaEventDestroy(c->pend[q].a); cudaEventDestroy(c->pend[q].b); }
   free(c->pend);
   for (int q = 0; q < 21; ++q) cudaFree(c->F[q]);
-  for (int q = 0; q < 3; ++q) { cudaFree(c->Ecc[q]); cudaFree(c->list[q]); cudaFree(c->stg_Bf[q]); cudaFree(c->stg_E[q]); }
+  for (int q = 0; q < 3; ++q) { cudaFree(c->Ecc[q]); cudaFree(c->stg_Bf[q]); cudaFree(c->stg_E[q]); }
+  cudaFree(c->list);
   for (int q = 0; q < 5; ++q) { cudaFree(c->stg_U[q]); cudaFree(c->stg_dU[q]); }
   for (int q = 0; q < 8; ++q) cudaFree(c->stg_W[q]);
   cudaFree(c->stg_flag); cudaFree(c->stg_status);
@@ -477,7 +475,7 @@ int ak_get_stats(ak_ctx* c, ak_stats* o) {
   o->n_c2p_fail = (long long)h[S_C2P_FAIL];
   o->n_cons_floor = (long long)h[S_CONS_FLOOR];
   o->n_prim_floor = (long long)h[S_PRIM_FLOOR];
-  o->n_fofc_cells = (long long)h[S_FOFC_CELLS];
+  o->n_fofc_cells = (long long)cnt[3];
   o->n_dmp_cells = (long long)h[S_DMP_CELLS];
   for (int d = 0; d < 3; ++d) o->n_fofc_faces[d] = cnt[d];
   return AK_OK;

@@ -37,8 +37,8 @@ struct Fields {
   unsigned char* flag;
   unsigned char* status;
   const double* dx;             // [nmb][3] device copy
-  unsigned int* list[3];        // FOFC face lists
-  unsigned int* count;          // [3] list lengths
+  unsigned int* list;           // FOFC: compacted flagged cells
+  unsigned int* count;          // [0..2] faces redone per direction, [3] length of list
   unsigned long long* stats;    // device counters (see ak_api.cu)
 };
 

@@ -18,7 +18,7 @@
 namespace ak {
 
 #ifndef AK_TMA_MINB
-#define AK_TMA_MINB 2
+#define AK_TMA_MINB 3
 #endif
 constexpr int TMA_THREADS = 256;
 

@@ -1,9 +1,9 @@
 // ak_kernels.cuh — the kernels of one RHS stage.
 //   K1  k_con2prim      part (1)  all stored cells
 //   K2  k_flux<DIR>     parts (2)+(3)  one thread per face, direction DIR
-//   K3  k_fofc_test     part (4a) estimate + check-only con2prim (+DMP) -> flag bytes
-//   K3b k_fofc_list     part (4b) warp-ballot compaction of faces with a flagged neighbour
-//   K4  k_fofc_reflux   part (4c) first-order re-solve of the listed faces
+//   K3  k_fofc_test     part (4a) estimate + check-only con2prim (+DMP) -> flag bytes and the
+//                       warp-ballot-compacted list of flagged cells
+//   K4  k_fofc_reflux   part (4b) first-order re-solve of the faces of the listed cells
 //   K5a k_cell_emf      part (5a) cell-centred EMFs
 //   K5  k_ct<C3>        part (5b) Gardiner-Stone corner EMFs
 //   K6  k_div_src       part (6)  flux divergence + geometric sources (Eq. 9)
@@ -14,7 +14,7 @@ namespace ak {
 
 // occupancy targets (blocks of 128 threads per SM) — tuned with ncu, see profiles/
 #ifndef AK_C2P_MINB
-#define AK_C2P_MINB 6
+#define AK_C2P_MINB 8
 #endif
 #ifndef AK_FLUX_MINB
 #define AK_FLUX_MINB 5
@@ -208,52 +208,44 @@ __global__ void __launch_bounds__(128, AK_FOFC_MINB) k_fofc_test(const __grid_co
       st |= ST_DMP;
   }
   f.flag[c] = (unsigned char)st;
-  warp_count(f.stats + S_FOFC_CELLS, st != 0);
   warp_count(f.stats + S_DMP_CELLS, (st & ST_DMP) != 0);
-}
-
-// ---- K3b: compact the faces that have a flagged neighbour (warp ballots) -------------------
-// A list entry is the linear index of the face's upper cell.  The order of entries depends on
-// the atomics but no output does: each listed face is rewritten exactly once.
-template <int DIR>
-__global__ void __launch_bounds__(256) k_fofc_list(const __grid_constant__ Par P,
-                                                   const __grid_constant__ Fields f) {
-  int m, k, j, i;
-  const bool in = decode_face<DIR>(P, (long long)blockIdx.x * blockDim.x + threadIdx.x, m, k, j, i);
-  bool hit = false;
-  long long cu = 0;
-  if (in) {
-    const Ix ix{P.nt, P.px};
-    const long long stride = DIR == 0 ? 1 : (DIR == 1 ? P.nt : (long long)P.nt * P.nt);
-    cu = ix.cell(m, k, j, i);
-    hit = (f.flag[cu] | f.flag[cu - stride]) != 0;
+  // compact the flagged cells (warp ballot + one atomic per warp); count[3] = list length.
+  // The order of entries depends on the atomics but no output does.
+  const unsigned act = __activemask();
+  const unsigned bal = __ballot_sync(act, st != 0);
+  if (bal != 0) {
+    const int lane = threadIdx.x & 31, leader = __ffs(bal) - 1;
+    unsigned base = 0;
+    if (lane == leader) base = atomicAdd(f.count + 3, (unsigned)__popc(bal));
+    base = __shfl_sync(act, base, leader);
+    if (st != 0) f.list[base + __popc(bal & ((1u << lane) - 1u))] = (unsigned)c;
   }
-  const unsigned bal = __ballot_sync(0xffffffffu, hit);
-  if (bal == 0) return;
-  const int lane = threadIdx.x & 31;
-  unsigned base = 0;
-  if (lane == 0) base = atomicAdd(f.count + DIR, (unsigned)__popc(bal));
-  base = __shfl_sync(0xffffffffu, base, 0);
-  if (hit) f.list[DIR][base + __popc(bal & ((1u << lane) - 1u))] = (unsigned)cu;
 }
 
-// ---- K4: first-order re-solve of the listed faces ("recalculate the fluxes for all
-// flagged cells but using a first-order scheme") -------------------------------------------
+// ---- K4: first-order re-solve of the faces of the flagged cells ("recalculate the fluxes
+// for all flagged cells but using a first-order scheme").  A face between cells A (lower) and B
+// (upper) is redone exactly once: by B's entry if B is flagged, else by A's.  So entry c handles
+// its lower DIR-face always and its upper DIR-face only when the upper neighbour is not flagged.
+// Thread t < 2 * count: which = t / count (0 lower, 1 upper) keeps warps uniform.
 template <int DIR>
 __global__ void __launch_bounds__(128) k_fofc_reflux(const __grid_constant__ Par P,
                                                      const __grid_constant__ Fields f) {
-  const unsigned cnt = f.count[DIR];
+  const unsigned cnt = f.count[3];
   const Ix ix{P.nt, P.px};
   constexpr int t1 = (DIR + 1) % 3, t2 = (DIR + 2) % 3;
-  const long long stride = DIR == 0 ? 1 : (DIR == 1 ? P.nt : (long long)P.nt * P.nt);
+  const unsigned nt = (unsigned)P.nt;
+  const unsigned stride = DIR == 0 ? 1u : (DIR == 1 ? nt : nt * nt);
   const int var[7] = {0, 1, 2, 3, 4, 5 + t1, 5 + t2};
-  for (unsigned e = blockIdx.x * blockDim.x + threadIdx.x; e < cnt; e += gridDim.x * blockDim.x) {
-    const long long cu = f.list[DIR][e], cl = cu - stride;
-    const int nt = P.nt;
+  unsigned nface = 0;
+  for (unsigned e = blockIdx.x * blockDim.x + threadIdx.x; e < 2u * cnt; e += gridDim.x * blockDim.x) {
+    const unsigned which = e >= cnt ? 1u : 0u;
+    const unsigned c = f.list[e - which * cnt];
+    if (which && f.flag[c + stride] != 0) continue;       // the upper neighbour's entry does this face
+    const unsigned cu = c + which * stride, cl = cu - stride;
     const int i = (int)(cu % nt);
-    const long long row = cu / nt;
+    const unsigned row = cu / nt;
     const int j = (int)(row % nt);
-    const long long mk = row / nt;
+    const unsigned mk = row / nt;
     const int k = (int)(mk % nt), m = (int)(mk / nt);
     double sL[7], sR[7], mL[10], mR[10], Fo[7];
 #pragma unroll
@@ -264,7 +256,11 @@ __global__ void __launch_bounds__(128) k_fofc_reflux(const __grid_constant__ Par
     face_flux<DIR, true>(P, P.fofc_riemann, mL, mR, sL, sR, __ldg(f.Bf[DIR] + fi), Fo);
 #pragma unroll
     for (int v = 0; v < 7; ++v) f.F[7 * DIR + v][fi] = Fo[v];
+    ++nface;
   }
+  // faces redone in this direction (reported by ak_get_stats)
+  for (int o = 16; o > 0; o >>= 1) nface += __shfl_xor_sync(0xffffffffu, nface, o);
+  if ((threadIdx.x & 31) == 0 && nface) atomicAdd(f.count + DIR, nface);
 }
 
 // ---- K5a: cell-centred EMFs  E_c = -alpha (vhat^a B~^b - vhat^b B~^a) on [is-1,ie+1]^3 --------
