@@ -41,6 +41,19 @@ ALG_BYTES = dict(con2prim=(5 + 3 + 6 + 8) * 8 + 1, flux=(7 + 10 + 1 + 7) * 8, fo
                  cell_emf=(6 + 10 + 3) * 8, ct_edge=(2 + 2 + 1 + 1) * 8, div_src=(15 + 8 + 16 + 5) * 8)
 
 
+# fp64-pipe instructions one face of a flux sweep needs (recon 0 donor, 1 PPM4, 2 WENO-Z; HLLE/LLF
+# differ by < 1 %): DADD + DMUL + DFMA of the straight-line face path in the SASS of k_flux_tma
+# (cuobjdump), which equals a hand count of DESIGN.md §3 O4-O6 with a division = 8 and a square
+# root = 9 pipe instructions (their correctly rounded Newton sequences).  DESIGN.md §7.
+FLUX_FP64_PER_FACE = {0: 634, 1: 928, 2: 1810}
+# fp64 pipe peak: 148 SMs x 4 sub-partitions x 16 fp64 lanes x 1.965 GHz (one instruction per lane
+# per clock; an FMA counts once).  The same-run probe (ak_probe_fp64) measures 18.4-18.5.
+FP64_PIPE_PEAK_TINST = 148 * 4 * 16 * 1.965e9 * 1e-12
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu capture
+# (profiles/r1_v6_final.md), keyed by (blocks, kernel class); other sizes: null.
+NCU_TRAFFIC_BYTES = {}
+
+
 def kernel_units(nmb, n):
     """elements each kernel class processes per stage."""
     nt = n + 8
@@ -347,11 +360,24 @@ def roofline(R, hbm_peak, peak_src):
     del a, b
     fp64_fma = ak.ak_probe_fp64(R["ctx"], 1, 3)
     fp64_nofma = ak.ak_probe_fp64(R["ctx"], 0, 3)
-    ach = table[dom]["alg_gbs"]
-    rf = dict(kernel=dom, bound="hbm", achieved=ach, peak=hbm_peak, unit="GB/s",
-              frac=round(ach / hbm_peak, 4) if ach else None, traffic=None, peak_source=peak_src,
-              same_run_copy_gbs=round(copy_gbs, 1), same_run_fp64_ginst=dict(fma=round(fp64_fma, 1),
-                                                                              mul_add=round(fp64_nofma, 1)))
+    rf_common = dict(peak_source=peak_src, same_run_copy_gbs=round(copy_gbs, 1),
+                     same_run_fp64_ginst=dict(fma=round(fp64_fma, 1), mul_add=round(fp64_nofma, 1)),
+                     hbm=dict(achieved=table[dom]["alg_gbs"], peak=hbm_peak, unit="GB/s",
+                              frac=round(table[dom]["alg_gbs"] / hbm_peak, 4) if table[dom]["alg_gbs"] else None))
+    if dom.startswith("flux"):
+        # The flux sweeps are bound by the fp64 pipe, not by HBM (ncu: 71 % fp64-pipe active at 1.3 TB/s
+        # of DRAM traffic, profiles/).  achieved = algorithmic fp64 pipe instructions per launch / time.
+        ops = FLUX_FP64_PER_FACE[R["spec"]["params"]["recon"]] * kernel_units(R["nmb"], R["n"])["flux"]
+        ms = table[dom]["ms"]
+        ach = ops / (ms * 1e-3) * 1e-12
+        rf = dict(kernel=dom, bound="alu", achieved=round(ach, 3), peak=FP64_PIPE_PEAK_TINST, unit="Tinst/s (fp64 pipe)",
+                  frac=round(ach / FP64_PIPE_PEAK_TINST, 4), traffic=NCU_TRAFFIC_BYTES.get((R["nmb"], dom)),
+                  alg_ops_per_face=FLUX_FP64_PER_FACE[R["spec"]["params"]["recon"]], **rf_common)
+    else:
+        ach = table[dom]["alg_gbs"]
+        rf = dict(kernel=dom, bound="hbm", achieved=ach, peak=hbm_peak, unit="GB/s",
+                  frac=round(ach / hbm_peak, 4) if ach else None, traffic=NCU_TRAFFIC_BYTES.get((R["nmb"], dom)),
+                  **rf_common)
     stage_bytes = sum(algb.values())
     stage = dict(alg_bytes_per_zone=round(stage_bytes / R["zones"], 1),
                  alg_gbs=round(stage_bytes / (R["ms_step"] * 1e-3) * 1e-9, 1))
