@@ -171,3 +171,72 @@ def test_host_entry_point_matches_device_path():
         for x, y in zip(hdU + hE + hW + hU, ra["dU"] + ra["E"] + ra["W"] + ra["U"]):
             assert np.array_equal(x, y)
         assert np.array_equal(hflag, ra["flag"]) and np.array_equal(hst, ra["status"])
+
+
+# ---------------------------------------------------------------- full-size configurations
+@pytest.mark.parametrize("name", ["C1", "C2", "C3"])
+def test_full_config_every_block(name):
+    """C1-C3 at BASELINE.json's full sizes: every block, every output, against the oracle."""
+    w = wl.make_blocks(name)
+    g, o, rep = run_both(w)
+    if name == "C3":
+        assert np.any(o["status"] & 4), "magnetisation cap never fired in C3"
+        assert np.count_nonzero(o["flag"]) > 0
+
+
+def test_c4_full_size_sampled_blocks():
+    """C4 in the launch configuration bench.py times (768 blocks resident, one ak_rhs): 24 sampled
+    blocks (every resolution factor, star centres and rims, atmosphere corners) are compared with
+    the oracle run on those blocks alone — blocks are independent, so their results must agree
+    element by element; the device counters must equal the sums over the whole batch."""
+    import torch
+    from paper_2409_10384_b200 import ak
+    import bench
+    name = "C4"
+    nmb = wl.n_blocks(name)
+    spec = wl.config_spec(name)
+    n = spec["params"]["n"]
+    sh = ak.shapes(nmb, n)
+    dev = "cuda:0"
+    z = lambda k, dt=torch.float64: torch.zeros(sh[k], dtype=dt, device=dev)
+    U = [z("cell") for _ in range(5)]; Bf = [z("xf"), z("yf"), z("zf")]; adm = [z("cell") for _ in range(16)]
+    dx = np.zeros((nmb, 3))
+    for s0, w in bench.generate(name, None):
+        nb = w["params"]["nmb"]
+        for dst, src in zip(U + Bf + adm, w["U"] + w["Bf"] + w["adm"]):
+            dst[s0:s0 + nb].copy_(torch.from_numpy(src))
+        dx[s0:s0 + nb] = w["dx"]
+        p = dict(w["params"]); dt_fofc = w["dt_fofc"]
+    p["nmb"] = nmb
+    W = [z("cell") for _ in range(8)]; dU = [z("cell") for _ in range(5)]; E = [z("ex"), z("ey"), z("ez")]
+    flag = z("cell", torch.uint8); status = z("cell", torch.uint8)
+    par = ak.make_params(device=0, stream=torch.cuda.current_stream().cuda_stream, **p)
+    ctx = ak.ak_create(par, dx)
+    try:
+        ak.ak_set_metric(ctx, adm)
+        ak.ak_rhs(ctx, U, Bf, W, 0, dt_fofc, dU, E, flag, status)
+        torch.cuda.synchronize()
+        stats = ak.ak_get_stats(ctx)
+        centre = spec["origin"] + 16.0 * spec["delta"][:, None]
+        near = np.argsort(np.abs(np.abs(centre[:, 0]) - 8.0) + np.abs(centre[:, 1]) + np.abs(centre[:, 2]))
+        pick = sorted(set([int(b) for b in near[:16]] + [0, nmb - 1, nmb // 2, 95, 300, 511, 640, 701]))
+        ws = wl.make_blocks(name, blocks=pick)
+        U_in = [u.copy() for u in ws["U"]]
+        ores = orc.rhs(orc.make_params(**ws["params"]), ws["dx"], ws["U"], ws["Bf"], ws["adm"], ws["dt_fofc"],
+                       nthreads=8)
+        ores["U"] = ws["U"]
+        idx = torch.tensor(pick, device=dev)
+        take = lambda ts: [t[idx].cpu().numpy() for t in ts]
+        gres = dict(W=take(W), dU=take(dU), E=take(E), U=take(U), flag=flag[idx].cpu().numpy(),
+                    status=status[idx].cpu().numpy())
+        gpukit.assert_parity(gres, ores, U_in, label="C4 sampled")
+        assert stats["n_fofc_cells"] == int(torch.count_nonzero(flag).item())
+        assert stats["n_c2p_fail"] == int(torch.count_nonzero(status & 32).item())
+        # properties that hold at any size: flags only inside the tested range, outputs finite
+        ng = 4
+        inner = flag[:, ng - 1:ng + n + 1, ng - 1:ng + n + 1, ng - 1:ng + n + 1]
+        assert int(torch.count_nonzero(flag).item()) == int(torch.count_nonzero(inner).item())
+        for t in dU + E:
+            assert bool(torch.isfinite(t).all())
+    finally:
+        ak.ak_destroy(ctx)
