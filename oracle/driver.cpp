@@ -1,0 +1,153 @@
+// oracle/driver.cpp — CPU ORACLE, stage driver (test infrastructure only; see oracle.h).
+// Ghost fill of a self-contained MeshBlock (periodic / outflow), the Shu-Osher register update
+// of SSP-RK2 / SSP-RK3 ("RK2 ... RK3"), the constrained-transport update of the
+// face-centred B~ from the edge EMFs, and the loop that strings them together.
+// DESIGN.md §11.  Straight loops; -ffp-contract=off; every operation in the order written.
+#include "oracle.h"
+#include <cstring>
+#include <vector>
+
+namespace {
+
+struct Lay {
+  int n, ng, nt, px, is, ie;
+  Lay(int n_, int ng_) : n(n_), ng(ng_) { nt = n + 2 * ng; px = nt + 4; is = ng; ie = ng + n - 1; }
+  long c(int m, int k, int j, int i) const { return (((long)m * nt + k) * nt + j) * nt + i; }
+  long f(int d, int m, int k, int j, int i) const {
+    if (d == 0) return (((long)m * nt + k) * nt + j) * px + i;
+    if (d == 1) return (((long)m * nt + k) * (nt + 1) + j) * nt + i;
+    return (((long)m * (nt + 1) + k) * nt + j) * nt + i;
+  }
+  long e(int c3, int m, int k, int j, int i) const {
+    if (c3 == 0) return (((long)m * (nt + 1) + k) * (nt + 1) + j) * nt + i;
+    if (c3 == 1) return (((long)m * (nt + 1) + k) * nt + j) * px + i;
+    return (((long)m * nt + k) * (nt + 1) + j) * px + i;
+  }
+  // source index of a cell-like index q in [0, nt): itself when interior
+  int src_cell(int q, int bc) const {
+    if (q >= is && q <= ie) return q;
+    if (bc == 0) { int r = (q - is) % n; if (r < 0) r += n; return is + r; }
+    return q < is ? is : ie;
+  }
+  // source index of a face-normal index q in [0, nt]: faces is..ie+1 bound the interior;
+  // periodic: face ie+1 is face is
+  int src_face(int q, int bc) const {
+    if (bc == 0) { int r = (q - is) % n; if (r < 0) r += n; return is + r; }
+    if (q < is) return is;
+    if (q > ie + 1) return ie + 1;
+    return q;
+  }
+};
+
+}  // namespace
+
+extern "C" void orc_fill_ghosts(const orc_params* p, const int bc[3], double* const U[5],
+                                double* const Bf[3]) {
+  const Lay L(p->n, p->ng);
+  const int nt = L.nt;
+  for (int m = 0; m < p->nmb; ++m) {
+    for (int k = 0; k < nt; ++k)
+      for (int j = 0; j < nt; ++j)
+        for (int i = 0; i < nt; ++i) {
+          const int ks = L.src_cell(k, bc[2]), js = L.src_cell(j, bc[1]), is_ = L.src_cell(i, bc[0]);
+          if (ks == k && js == j && is_ == i) continue;
+          for (int v = 0; v < 5; ++v) U[v][L.c(m, k, j, i)] = U[v][L.c(m, ks, js, is_)];
+        }
+    // face fields: normal index over nt+1 faces, transverse like cells
+    for (int d = 0; d < 3; ++d) {
+      const int ni = nt + (d == 0), nj = nt + (d == 1), nk = nt + (d == 2);
+      for (int k = 0; k < nk; ++k)
+        for (int j = 0; j < nj; ++j)
+          for (int i = 0; i < ni; ++i) {
+            const int ks = d == 2 ? L.src_face(k, bc[2]) : L.src_cell(k, bc[2]);
+            const int js = d == 1 ? L.src_face(j, bc[1]) : L.src_cell(j, bc[1]);
+            const int is_ = d == 0 ? L.src_face(i, bc[0]) : L.src_cell(i, bc[0]);
+            if (ks == k && js == j && is_ == i) continue;
+            Bf[d][L.f(d, m, k, j, i)] = Bf[d][L.f(d, m, ks, js, is_)];
+          }
+    }
+  }
+}
+
+extern "C" void orc_stage_update(const orc_params* p, const double* dx, double a, double b, double dt,
+                                 const double* const U0[5], const double* const B0[3],
+                                 double* const U[5], double* const Bf[3],
+                                 const double* const dU[5], const double* const E[3]) {
+  const Lay L(p->n, p->ng);
+  const int is = L.is, ie = L.ie;
+  for (int m = 0; m < p->nmb; ++m) {
+    const double idx = 1.0 / dx[3 * m + 0], idy = 1.0 / dx[3 * m + 1], idz = 1.0 / dx[3 * m + 2];
+    for (int k = is; k <= ie; ++k)
+      for (int j = is; j <= ie; ++j)
+        for (int i = is; i <= ie; ++i) {
+          const long c = L.c(m, k, j, i);
+          for (int v = 0; v < 5; ++v) U[v][c] = a * U0[v][c] + b * (U[v][c] + dt * dU[v][c]);
+        }
+    // d_t B~^i = -eps^{ijk} d_j E_k on the faces of interior cells
+    for (int k = is; k <= ie; ++k)
+      for (int j = is; j <= ie; ++j)
+        for (int i = is; i <= ie + 1; ++i) {
+          const double dB = -((E[2][L.e(2, m, k, j + 1, i)] - E[2][L.e(2, m, k, j, i)]) * idy -
+                              (E[1][L.e(1, m, k + 1, j, i)] - E[1][L.e(1, m, k, j, i)]) * idz);
+          const long q = L.f(0, m, k, j, i);
+          Bf[0][q] = a * B0[0][q] + b * (Bf[0][q] + dt * dB);
+        }
+    for (int k = is; k <= ie; ++k)
+      for (int j = is; j <= ie + 1; ++j)
+        for (int i = is; i <= ie; ++i) {
+          const double dB = -((E[0][L.e(0, m, k + 1, j, i)] - E[0][L.e(0, m, k, j, i)]) * idz -
+                              (E[2][L.e(2, m, k, j, i + 1)] - E[2][L.e(2, m, k, j, i)]) * idx);
+          const long q = L.f(1, m, k, j, i);
+          Bf[1][q] = a * B0[1][q] + b * (Bf[1][q] + dt * dB);
+        }
+    for (int k = is; k <= ie + 1; ++k)
+      for (int j = is; j <= ie; ++j)
+        for (int i = is; i <= ie; ++i) {
+          const double dB = -((E[1][L.e(1, m, k, j, i + 1)] - E[1][L.e(1, m, k, j, i)]) * idx -
+                              (E[0][L.e(0, m, k, j + 1, i)] - E[0][L.e(0, m, k, j, i)]) * idy);
+          const long q = L.f(2, m, k, j, i);
+          Bf[2][q] = a * B0[2][q] + b * (Bf[2][q] + dt * dB);
+        }
+  }
+}
+
+extern "C" void orc_advance(const orc_params* p, const double* dx, int integrator, int nsteps,
+                            double dt, const int bc[3], double* const U[5], double* const Bf[3],
+                            const double* const adm[16], double* const W[8],
+                            unsigned char* flag_or, int nthreads) {
+  const Lay L(p->n, p->ng);
+  const long nt = L.nt, px = L.px, nb = p->nmb;
+  const long ncell = nb * nt * nt * nt;
+  const long nface[3] = {nb * nt * nt * px, nb * nt * (nt + 1) * nt, nb * (nt + 1) * nt * nt};
+  const long nedge[3] = {nb * (nt + 1) * (nt + 1) * nt, nb * (nt + 1) * nt * px, nb * nt * (nt + 1) * px};
+  std::vector<double> sU0[5], sB0[3], sdU[5], sE[3];
+  std::vector<unsigned char> flag(ncell, 0);
+  double* dU[5]; double* E[3]; const double* U0[5]; const double* B0[3];
+  for (int v = 0; v < 5; ++v) { sU0[v].assign(ncell, 0.0); sdU[v].assign(ncell, 0.0); dU[v] = sdU[v].data(); U0[v] = sU0[v].data(); }
+  for (int d = 0; d < 3; ++d) { sB0[d].assign(nface[d], 0.0); sE[d].assign(nedge[d], 0.0); E[d] = sE[d].data(); B0[d] = sB0[d].data(); }
+  // Shu-Osher coefficients: U <- a U0 + b (U + dt L(U))
+  const double A[3][3] = {{0.0, 0.0, 0.0}, {0.0, 0.5, 0.0}, {0.0, 0.75, 1.0 / 3.0}};
+  const double B[3][3] = {{1.0, 0.0, 0.0}, {1.0, 0.5, 0.0}, {1.0, 0.25, 2.0 / 3.0}};
+  const int ns = integrator;
+  for (int step = 0; step < nsteps; ++step)
+    for (int s = 0; s < ns; ++s) {
+      const double a = A[ns - 1][s], b = B[ns - 1][s];
+      orc_fill_ghosts(p, bc, U, Bf);
+      orc_rhs_blend(p, dx, U, Bf, adm, W, 0, dt, s == 0 ? nullptr : U0, a, b, dU, E, flag.data(),
+                    nullptr, nthreads);
+      if (flag_or) for (long c = 0; c < ncell; ++c) flag_or[c] |= flag[c];
+      if (s == 0 && ns > 1) {
+        for (int v = 0; v < 5; ++v) std::memcpy(sU0[v].data(), U[v], sizeof(double) * ncell);
+        for (int d = 0; d < 3; ++d) std::memcpy(sB0[d].data(), Bf[d], sizeof(double) * nface[d]);
+      }
+      // for s == 0, a == 0: the register is not read (0 * x would turn inf/nan into nan)
+      if (s == 0) {
+        const double* Uc[5] = {U[0], U[1], U[2], U[3], U[4]};
+        const double* Bc[3] = {Bf[0], Bf[1], Bf[2]};
+        orc_stage_update(p, dx, 0.0, 1.0, dt, Uc, Bc, U, Bf, dU, E);
+      } else {
+        orc_stage_update(p, dx, a, b, dt, U0, B0, U, Bf, dU, E);
+      }
+    }
+  orc_fill_ghosts(p, bc, U, Bf);
+}

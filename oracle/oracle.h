@@ -104,6 +104,33 @@ void orc_rhs(const orc_params* p, const double* dx, double* const U[5],
              double* const flux_out[21], unsigned char* const face_refluxed[3],
              int nthreads);
 
+/* Same stage with the FOFC estimate of a later Runge-Kutta stage (R9):
+ * U* = fa * U0 + fb * (U - dt_fofc div F) when U0 != NULL. */
+void orc_rhs_blend(const orc_params* p, const double* dx, double* const U[5],
+                   const double* const Bf[3], const double* const adm[16], double* const W[8],
+                   int w_is_valid, double dt_fofc, const double* const U0[5], double fa, double fb,
+                   double* const out_dU[5], double* const out_E[3], unsigned char* flag,
+                   unsigned char* c2p_status, int nthreads);
+
+/* ---- stage driver ("RK2 / RK3", method of lines) --------------------
+ * Each MeshBlock is its own domain: ghosts are filled from the block itself.
+ * bc[d]: 0 periodic, 1 outflow (zero-gradient copy), per direction. */
+void orc_fill_ghosts(const orc_params* p, const int bc[3], double* const U[5], double* const Bf[3]);
+
+/* One stage register update on the interior cells and on the faces of interior cells:
+ *   U  <- a U0 + b (U + dt dU),   B~f <- a B0 + b (B~f + dt (-curl E))      (dx[nmb][3]) */
+void orc_stage_update(const orc_params* p, const double* dx, double a, double b, double dt,
+                      const double* const U0[5], const double* const B0[3], double* const U[5],
+                      double* const Bf[3], const double* const dU[5], const double* const E[3]);
+
+/* nsteps steps of SSP-RK1/2/3 (integrator = 1,2,3) with a fixed dt: per stage fill ghosts,
+ * orc_rhs_blend, orc_stage_update.  The step-start register is taken after the first stage's
+ * con2prim (floored state).  W (8) is scratch/out.  flag_or (may be NULL): OR of all FOFC flags. */
+void orc_advance(const orc_params* p, const double* dx, int integrator, int nsteps, double dt,
+                 const int bc[3], double* const U[5], double* const Bf[3],
+                 const double* const adm[16], double* const W[8], unsigned char* flag_or,
+                 int nthreads);
+
 #ifdef __cplusplus
 }
 #endif

@@ -11,7 +11,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_HERE, "liboracle.so")
-_SRC = ["point.cpp", "stage.cpp"]
+_SRC = ["point.cpp", "stage.cpp", "driver.cpp"]
 
 
 def build(force=False):
@@ -164,3 +164,46 @@ def rhs(par, dx, U, Bf, adm, dt_fofc, W=None, nthreads=1, want_flux=False):
                   flag.ctypes.data_as(C.c_void_p), status.ctypes.data_as(C.c_void_p),
                   fp, rp, int(nthreads))
     return dict(W=W, dU=dU, E=E, flag=flag, status=status, flux=flux, refl=refl)
+
+
+# ------------------------------------------------------------------ stage driver
+def _ib(bc):
+    return (C.c_int * 3)(*[int(b) for b in bc])
+
+
+def fill_ghosts(par, bc, U, Bf):
+    """in place.  bc[d]: 0 periodic, 1 outflow."""
+    lib().orc_fill_ghosts(C.byref(par), _ib(bc), _ptrs(U), _ptrs(Bf))
+
+
+def stage_update(par, dx, a, b, dt, U0, B0, U, Bf, dU, E):
+    dx = np.ascontiguousarray(dx, dtype=np.float64).reshape(par.nmb, 3)
+    lib().orc_stage_update(C.byref(par), dx.ctypes.data_as(_dp), C.c_double(a), C.c_double(b), C.c_double(dt),
+                           _ptrs(U0), _ptrs(B0), _ptrs(U), _ptrs(Bf), _ptrs(dU), _ptrs(E))
+
+
+def rhs_blend(par, dx, U, Bf, adm, dt_fofc, U0, fa, fb, nthreads=1):
+    sh = shapes(par.nmb, par.n)
+    dx = np.ascontiguousarray(dx, dtype=np.float64).reshape(par.nmb, 3)
+    W = [np.zeros(sh["cell"]) for _ in range(8)]
+    dU = [np.zeros(sh["cell"]) for _ in range(5)]
+    E = [np.zeros(sh["ex"]), np.zeros(sh["ey"]), np.zeros(sh["ez"])]
+    flag = np.zeros(sh["cell"], dtype=np.uint8)
+    status = np.zeros(sh["cell"], dtype=np.uint8)
+    lib().orc_rhs_blend(C.byref(par), dx.ctypes.data_as(_dp), _ptrs(U), _ptrs(Bf), _ptrs(adm), _ptrs(W), 0,
+                        C.c_double(dt_fofc), _ptrs(U0) if U0 is not None else None, C.c_double(fa),
+                        C.c_double(fb), _ptrs(dU), _ptrs(E), flag.ctypes.data_as(C.c_void_p),
+                        status.ctypes.data_as(C.c_void_p), int(nthreads))
+    return dict(W=W, dU=dU, E=E, flag=flag, status=status)
+
+
+def advance(par, dx, integrator, nsteps, dt, bc, U, Bf, adm, nthreads=1):
+    """nsteps of SSP-RK<integrator>; U, Bf advanced in place.  Returns (W, OR of FOFC flags)."""
+    sh = shapes(par.nmb, par.n)
+    dx = np.ascontiguousarray(dx, dtype=np.float64).reshape(par.nmb, 3)
+    W = [np.zeros(sh["cell"]) for _ in range(8)]
+    flag = np.zeros(sh["cell"], dtype=np.uint8)
+    lib().orc_advance(C.byref(par), dx.ctypes.data_as(_dp), int(integrator), int(nsteps), C.c_double(dt),
+                      _ib(bc), _ptrs(U), _ptrs(Bf), _ptrs(adm), _ptrs(W), flag.ctypes.data_as(C.c_void_p),
+                      int(nthreads))
+    return W, flag

@@ -57,6 +57,10 @@ struct Stage {
   unsigned char* status;
   double* const* flux_out;
   unsigned char* const* refl;
+  // FOFC estimate of a later Runge-Kutta stage ("the next Runge-Kutta step is estimated"):
+  // U* = fa * U0 + fb * (U - dt div F) when U0 is given (reading R9), else U - dt div F
+  const double* const* U0 = nullptr;
+  double fa = 0.0, fb = 1.0;
   Stage(const orc_params* p_) : p(p_), G(p_->n, p_->ng) {}
 
   void cell_metric10(long c, double m[10]) const {
@@ -141,7 +145,8 @@ struct Stage {
               const double div = (Fs[0][v][fl(0, k, j, i + 1)] - Fs[0][v][fl(0, k, j, i)]) * idx[0] +
                                  (Fs[1][v][fl(1, k, j + 1, i)] - Fs[1][v][fl(1, k, j, i)]) * idx[1] +
                                  (Fs[2][v][fl(2, k + 1, j, i)] - Fs[2][v][fl(2, k, j, i)]) * idx[2];
-              Us[v] = U[v][c] - dt * div;
+              if (U0) Us[v] = fa * U0[v][c] + fb * (U[v][c] - dt * div);
+              else Us[v] = U[v][c] - dt * div;
             }
             for (int q = 0; q < 6; ++q) g[q] = adm[q][c];
             for (int v = 0; v < 3; ++v) Bc[v] = W[5 + v][c];
@@ -347,6 +352,20 @@ extern "C" void orc_con2prim(const orc_params* p, double* const U[5], const doub
   Stage S(p);
   S.U = U; S.Bf = Bf; S.adm = g; S.W = W; S.status = status;
   run_blocks(p->nmb, nthreads, [&](int m) { S.con2prim_block(m); });
+}
+
+extern "C" void orc_rhs_blend(const orc_params* p, const double* dx, double* const U[5],
+                              const double* const Bf[3], const double* const adm[16],
+                              double* const W[8], int w_is_valid, double dt_fofc,
+                              const double* const U0[5], double fa, double fb,
+                              double* const out_dU[5], double* const out_E[3], unsigned char* flag,
+                              unsigned char* c2p_status, int nthreads) {
+  Stage S(p);
+  S.dx = dx; S.U = U; S.Bf = Bf; S.adm = adm; S.W = W; S.dt = dt_fofc; S.dU = out_dU;
+  S.E = out_E; S.flag = flag; S.status = c2p_status; S.flux_out = nullptr;
+  S.refl = nullptr; S.W_needs_c2p = !w_is_valid;
+  S.U0 = U0; S.fa = fa; S.fb = fb;
+  run_blocks(p->nmb, nthreads, [&](int m) { S.block(m); });
 }
 
 extern "C" void orc_rhs(const orc_params* p, const double* dx, double* const U[5],
