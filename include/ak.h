@@ -52,6 +52,8 @@ typedef struct ak_ctx ak_ctx; /* opaque */
 enum { AK_OK = 0, AK_EINVAL = -1, AK_ENOMEM = -2, AK_ECUDA = -3, AK_ESTATE = -4 };
 enum { AK_RECON_DC = 0, AK_RECON_PPM4 = 1, AK_RECON_WENOZ = 2 }; /* P:133 */
 enum { AK_RS_LLF = 0, AK_RS_HLLE = 1 };                          /* P:133 */
+enum { AK_BC_PERIODIC = 0, AK_BC_OUTFLOW = 1 };                  /* stage driver, D:§11 */
+enum { AK_RK1 = 1, AK_RK2 = 2, AK_RK3 = 3 };                     /* SSP Runge-Kutta, P:133 */
 
 /* status / flag bits (D:§2.4).  status = what con2prim did to a cell; fofc_flag = the status
  * of the FOFC estimate of that cell (P:141), plus AK_ST_DMP (Eq. 12, P:155). */
@@ -84,6 +86,7 @@ typedef struct {
 
 typedef struct { double *D, *Sx, *Sy, *Sz, *tau; } ak_cons;              /* cell fields, U~   */
 typedef struct { const double *bx, *by, *bz; } ak_faceB;                 /* face fields, B~f  */
+typedef struct { double *bx, *by, *bz; } ak_faceB_rw;                    /* ... written       */
 typedef struct { double *rho, *ux, *uy, *uz, *p, *bccx, *bccy, *bccz; } ak_prim;
                                    /* cell fields: rho, u^i = W v^i, P, cell-centred B~^i     */
 typedef struct {
@@ -147,6 +150,33 @@ int ak_get_flux(ak_ctx*, int dir, int comp, double* dst);
  * dU, E and the two masks, and synchronises.  Staging is allocated on first use. */
 int ak_rhs_host(ak_ctx*, const ak_cons* U, const ak_faceB* Bf, const ak_prim* W,
                 double dt_fofc, const ak_rhs_out* out);
+
+/* ---- stage driver (D:§11; "RK2 ... RK3", method of lines; P:141 FOFC per stage) -------
+ * Every MeshBlock is treated as its own domain: ghosts are filled from the block itself.
+ *
+ * FOFC estimate of a later Runge-Kutta stage ("the next Runge-Kutta step is estimated"):
+ * subsequent ak_rhs calls test U* = a U0 + b (U - dt_fofc div F).  U0 (device, borrowed until
+ * replaced) = the step-start register; U0 == NULL restores U* = U - dt_fofc div F. */
+int ak_set_fofc_blend(ak_ctx*, const ak_cons* U0, double a, double b);
+
+/* Fill the ghost cells of U~ and the ghost faces of B~f in place.  bc[d] = AK_BC_* per direction:
+ * periodic (face ie+1 is made a copy of face is) or outflow (zero-gradient copies). */
+int ak_fill_ghosts(ak_ctx*, const int bc[3], const ak_cons* U, const ak_faceB_rw* Bf);
+
+/* One Shu-Osher register update with the outputs of ak_rhs:
+ *   U~ <- a U0 + b (U~ + dt dU~/dt) on interior cells,
+ *   B~f <- a B0 + b (B~f + dt (-curl E)) on the faces of interior cells (constrained transport).
+ * U0/B0 may alias U/Bf (first stage: a = 0, b = 1). */
+int ak_stage_update(ak_ctx*, double a, double b, double dt, const ak_cons* U0, const ak_faceB* B0,
+                    const ak_cons* U, const ak_faceB_rw* Bf, const ak_rhs_out* rhs);
+
+/* nsteps steps of SSP-RK<integrator> with a fixed dt, all on the device: per stage
+ * ak_fill_ghosts -> ak_rhs (with the stage's FOFC blend) -> ak_stage_update; ghosts filled at the
+ * end.  Registers (U0, B0, dU, E, flags) are context-owned, allocated on first use.  W receives
+ * the last stage's primitives.  flag_or (device bytes [nmb][nt^3], may be NULL) accumulates the OR
+ * of the FOFC flags of every stage (caller zeroes it). */
+int ak_advance(ak_ctx*, int integrator, int nsteps, double dt, const int bc[3], const ak_cons* U,
+               const ak_faceB_rw* Bf, const ak_prim* W, unsigned char* flag_or);
 
 /* Device-timing hooks for the benchmark: bracket kernel class `which` (0 con2prim, 1-3 flux
  * sweeps x/y/z, 4 FOFC test, 5 FOFC list+reflux, 6 cell EMF+CT, 7 divergence+sources) with

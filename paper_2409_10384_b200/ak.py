@@ -20,7 +20,9 @@ ST_DFLOOR, ST_TAUFLOOR, ST_MAGCAP, ST_RHOFLOOR, ST_TFLOOR, ST_FAIL, ST_DMP = 1, 
 KERNEL_CLASSES = ("con2prim", "flux_x", "flux_y", "flux_z", "fofc_test", "fofc_fix", "ct", "div_src")
 EXPORTS = ("ak_create", "ak_set_metric", "ak_con2prim", "ak_rhs", "ak_emf", "ak_get_stats",
            "ak_get_flux", "ak_rhs_host", "ak_timing", "ak_kernel_ms", "ak_probe_copy",
-           "ak_probe_fp64", "ak_destroy", "ak_strerror", "ak_version")
+           "ak_probe_fp64", "ak_destroy", "ak_strerror", "ak_version",
+           "ak_set_fofc_blend", "ak_fill_ghosts", "ak_stage_update", "ak_advance")
+BC_PERIODIC, BC_OUTFLOW = 0, 1
 
 _dp = C.POINTER(C.c_double)
 
@@ -97,6 +99,13 @@ def lib():
         L.ak_probe_copy.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_longlong, C.c_int, _dp]
         L.ak_probe_fp64.argtypes = [C.c_void_p, C.c_int, C.c_int, _dp]
         L.ak_destroy.argtypes = [C.c_void_p]
+        L.ak_set_fofc_blend.argtypes = [C.c_void_p, C.POINTER(AkCons), C.c_double, C.c_double]
+        L.ak_fill_ghosts.argtypes = [C.c_void_p, C.POINTER(C.c_int), C.POINTER(AkCons), C.POINTER(AkFaceB)]
+        L.ak_stage_update.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_double, C.POINTER(AkCons),
+                                      C.POINTER(AkFaceB), C.POINTER(AkCons), C.POINTER(AkFaceB),
+                                      C.POINTER(AkRhsOut)]
+        L.ak_advance.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double, C.POINTER(C.c_int), C.POINTER(AkCons),
+                                 C.POINTER(AkFaceB), C.POINTER(AkPrim), C.c_void_p]
         _lib = L
     return _lib
 
@@ -220,3 +229,34 @@ def ak_probe_fp64(ctx, use_fma, reps=3):
 
 def ak_destroy(ctx):
     _chk(lib().ak_destroy(ctx), "ak_destroy")
+
+
+# ---------------------------------------------------------------- stage driver (same names)
+def _bc(bc):
+    return (C.c_int * 3)(*[int(b) for b in bc])
+
+
+def ak_set_fofc_blend(ctx, U0, a=0.0, b=1.0):
+    if U0 is None:
+        _chk(lib().ak_set_fofc_blend(ctx, None, 0.0, 1.0), "ak_set_fofc_blend")
+    else:
+        u = _struct(AkCons, U0)
+        _chk(lib().ak_set_fofc_blend(ctx, C.byref(u), float(a), float(b)), "ak_set_fofc_blend")
+
+
+def ak_fill_ghosts(ctx, bc, U, Bf):
+    u, b = _struct(AkCons, U), _struct(AkFaceB, Bf)
+    _chk(lib().ak_fill_ghosts(ctx, _bc(bc), C.byref(u), C.byref(b)), "ak_fill_ghosts")
+
+
+def ak_stage_update(ctx, a, b, dt, U0, B0, U, Bf, dU, E):
+    u0, b0, u, bf = _struct(AkCons, U0), _struct(AkFaceB, B0), _struct(AkCons, U), _struct(AkFaceB, Bf)
+    o = _struct(AkRhsOut, list(dU) + list(E) + [None, None])
+    _chk(lib().ak_stage_update(ctx, float(a), float(b), float(dt), C.byref(u0), C.byref(b0), C.byref(u),
+                               C.byref(bf), C.byref(o)), "ak_stage_update")
+
+
+def ak_advance(ctx, integrator, nsteps, dt, bc, U, Bf, W, flag_or=None):
+    u, bf, w = _struct(AkCons, U), _struct(AkFaceB, Bf), _struct(AkPrim, W)
+    _chk(lib().ak_advance(ctx, int(integrator), int(nsteps), float(dt), _bc(bc), C.byref(u), C.byref(bf),
+                          C.byref(w), _ptr(flag_or)), "ak_advance")

@@ -12,6 +12,7 @@
 #define AK_FLUX_TMA 1   // 1: TMA-staged sweeps (ak_flux_tma.cuh) when n is even and a face row fits a block
 #endif
 #include "ak_flux_tma.cuh"
+#include "ak_driver.cuh"
 
 #include <cmath>
 #include <cstdint>
@@ -51,6 +52,11 @@ struct ak_ctx {
   unsigned char* stg_flag; unsigned char* stg_status;
   bool have_stg;
   bool tma_attr[3];
+  // FOFC stage blend (ak_set_fofc_blend)
+  const double* blendU0[5]; double blend_a, blend_b;
+  // stage-driver registers (ak_advance), allocated on first use
+  double* regU0[5]; double* regB0[3]; double* reg_dU[5]; double* regE[3]; unsigned char* reg_flag;
+  bool have_reg;
   // timing
   bool timing;
   cudaEvent_t ev0, ev1;
@@ -122,6 +128,8 @@ void fill_fields(ak_ctx* c, Fields& f) {
   f.stats = c->stats;
   f.dx = c->dx;
   f.flag = c->flag_own;
+  for (int q = 0; q < 5; ++q) f.U0[q] = c->blendU0[q];
+  f.fa = c->blend_a; f.fb = c->blend_b;
 }
 
 bool set_cons(Fields& f, const ak_cons* U) {
@@ -344,6 +352,7 @@ int ak_create(const ak_params* p, const double* dx3, ak_ctx** out) {
   memset(c, 0, sizeof(*c));
   c->hp = *p;
   c->stream = (cudaStream_t)p->stream;
+  c->blend_a = 0.0; c->blend_b = 1.0;
   Par& P = c->P;
   P.nmb = p->nmb; P.n = p->n; P.nt = p->n + 8; P.px = P.nt + 4; P.is = 4; P.ie = p->n + 3;
   P.Gam = p->gamma_ad; P.gm1 = p->gamma_ad - 1.0; P.gm1r = p->gamma_ad / (p->gamma_ad - 1.0);
@@ -400,6 +409,9 @@ int ak_destroy(ak_ctx* c) {
   for (int q = 0; q < 5; ++q) { cudaFree(c->stg_U[q]); cudaFree(c->stg_dU[q]); }
   for (int q = 0; q < 8; ++q) cudaFree(c->stg_W[q]);
   cudaFree(c->stg_flag); cudaFree(c->stg_status);
+  for (int q = 0; q < 5; ++q) { cudaFree(c->regU0[q]); cudaFree(c->reg_dU[q]); }
+  for (int q = 0; q < 3; ++q) { cudaFree(c->regB0[q]); cudaFree(c->regE[q]); }
+  cudaFree(c->reg_flag);
   cudaFree(c->flag_own); cudaFree(c->count); cudaFree(c->stats); cudaFree(c->dx);
   delete c;
   return AK_OK;
@@ -551,6 +563,118 @@ int ak_rhs_host(ak_ctx* c, const ak_cons* U, const ak_faceB* Bf, const ak_prim* 
   if (out->c2p_status) CK(cudaMemcpyAsync(out->c2p_status, c->stg_status, (size_t)c->sz.cell, cudaMemcpyDeviceToHost, c->stream));
   CK(cudaStreamSynchronize(c->stream));
   return AK_OK;
+}
+
+int ak_set_fofc_blend(ak_ctx* c, const ak_cons* U0, double a, double b) {
+  if (!c) return AK_EINVAL;
+  if (!U0) {
+    for (int q = 0; q < 5; ++q) c->blendU0[q] = nullptr;
+    c->blend_a = 0.0; c->blend_b = 1.0;
+    return AK_OK;
+  }
+  if (!U0->D || !U0->Sx || !U0->Sy || !U0->Sz || !U0->tau || !std::isfinite(a) || !std::isfinite(b)) return AK_EINVAL;
+  c->blendU0[0] = U0->D; c->blendU0[1] = U0->Sx; c->blendU0[2] = U0->Sy; c->blendU0[3] = U0->Sz; c->blendU0[4] = U0->tau;
+  c->blend_a = a; c->blend_b = b;
+  return AK_OK;
+}
+
+static bool bc_ok(const int bc[3]) {
+  if (!bc) return false;
+  for (int d = 0; d < 3; ++d) if (bc[d] != AK_BC_PERIODIC && bc[d] != AK_BC_OUTFLOW) return false;
+  return true;
+}
+
+int ak_fill_ghosts(ak_ctx* c, const int bc[3], const ak_cons* U, const ak_faceB_rw* Bf) {
+  if (!c || !bc_ok(bc) || !U || !Bf || !U->D || !U->Sx || !U->Sy || !U->Sz || !U->tau || !Bf->bx || !Bf->by || !Bf->bz)
+    return AK_EINVAL;
+  CK(cudaSetDevice(c->hp.device));
+  DrvFields f;
+  memset(&f, 0, sizeof(f));
+  f.U[0] = U->D; f.U[1] = U->Sx; f.U[2] = U->Sy; f.U[3] = U->Sz; f.U[4] = U->tau;
+  f.Bf[0] = Bf->bx; f.Bf[1] = Bf->by; f.Bf[2] = Bf->bz;
+  const long long nt = c->P.nt, nb = c->P.nmb;
+  k_fill_cells<<<nblk(c->sz.cell, 256), 256, 0, c->stream>>>(c->P, f, bc[0], bc[1], bc[2]);
+  k_fill_faces<0><<<nblk(nb * nt * nt * (nt + 1), 256), 256, 0, c->stream>>>(c->P, f, bc[0], bc[1], bc[2]);
+  k_fill_faces<1><<<nblk(nb * nt * nt * (nt + 1), 256), 256, 0, c->stream>>>(c->P, f, bc[0], bc[1], bc[2]);
+  k_fill_faces<2><<<nblk(nb * nt * nt * (nt + 1), 256), 256, 0, c->stream>>>(c->P, f, bc[0], bc[1], bc[2]);
+  CK(cudaGetLastError());
+  return AK_OK;
+}
+
+int ak_stage_update(ak_ctx* c, double a, double b, double dt, const ak_cons* U0, const ak_faceB* B0,
+                    const ak_cons* U, const ak_faceB_rw* Bf, const ak_rhs_out* rhs) {
+  if (!c || !U0 || !B0 || !U || !Bf || !rhs) return AK_EINVAL;
+  if (!std::isfinite(a) || !std::isfinite(b) || !std::isfinite(dt)) return AK_EINVAL;
+  DrvFields f;
+  memset(&f, 0, sizeof(f));
+  f.U[0] = U->D; f.U[1] = U->Sx; f.U[2] = U->Sy; f.U[3] = U->Sz; f.U[4] = U->tau;
+  f.U0[0] = U0->D; f.U0[1] = U0->Sx; f.U0[2] = U0->Sy; f.U0[3] = U0->Sz; f.U0[4] = U0->tau;
+  f.Bf[0] = Bf->bx; f.Bf[1] = Bf->by; f.Bf[2] = Bf->bz;
+  f.B0[0] = B0->bx; f.B0[1] = B0->by; f.B0[2] = B0->bz;
+  f.dU[0] = rhs->dD; f.dU[1] = rhs->dSx; f.dU[2] = rhs->dSy; f.dU[3] = rhs->dSz; f.dU[4] = rhs->dtau;
+  f.E[0] = rhs->Ex; f.E[1] = rhs->Ey; f.E[2] = rhs->Ez;
+  for (int q = 0; q < 5; ++q) if (!f.U[q] || !f.U0[q] || !f.dU[q]) return AK_EINVAL;
+  for (int q = 0; q < 3; ++q) if (!f.Bf[q] || !f.B0[q] || !f.E[q]) return AK_EINVAL;
+  f.dx = c->dx;
+  CK(cudaSetDevice(c->hp.device));
+  const long long n = c->P.n, nb = c->P.nmb;
+  k_update_cells<<<nblk(nb * n * n * n, 256), 256, 0, c->stream>>>(c->P, f, a, b, dt);
+  k_update_faces<0><<<nblk(nb * n * n * (n + 1), 256), 256, 0, c->stream>>>(c->P, f, a, b, dt);
+  k_update_faces<1><<<nblk(nb * n * n * (n + 1), 256), 256, 0, c->stream>>>(c->P, f, a, b, dt);
+  k_update_faces<2><<<nblk(nb * n * n * (n + 1), 256), 256, 0, c->stream>>>(c->P, f, a, b, dt);
+  CK(cudaGetLastError());
+  return AK_OK;
+}
+
+int ak_advance(ak_ctx* c, int integrator, int nsteps, double dt, const int bc[3], const ak_cons* U,
+               const ak_faceB_rw* Bf, const ak_prim* W, unsigned char* flag_or) {
+  if (!c || integrator < 1 || integrator > 3 || nsteps < 0 || !std::isfinite(dt) || !bc_ok(bc) || !U || !Bf || !W)
+    return AK_EINVAL;
+  if (!c->have_metric) return AK_ESTATE;
+  CK(cudaSetDevice(c->hp.device));
+  const size_t cb = sizeof(double) * c->sz.cell;
+  const size_t fb[3] = {sizeof(double) * c->sz.xf, sizeof(double) * c->sz.yf, sizeof(double) * c->sz.zf};
+  const size_t eb[3] = {sizeof(double) * c->sz.ex, sizeof(double) * c->sz.ey, sizeof(double) * c->sz.ez};
+  if (!c->have_reg) {
+    for (int q = 0; q < 5; ++q) { CK(cudaMalloc(&c->regU0[q], cb)); CK(cudaMalloc(&c->reg_dU[q], cb)); CK(cudaMemsetAsync(c->reg_dU[q], 0, cb, c->stream)); }
+    for (int q = 0; q < 3; ++q) { CK(cudaMalloc(&c->regB0[q], fb[q])); CK(cudaMalloc(&c->regE[q], eb[q])); CK(cudaMemsetAsync(c->regE[q], 0, eb[q], c->stream)); }
+    CK(cudaMalloc(&c->reg_flag, (size_t)c->sz.cell));
+    c->have_reg = true;
+  }
+  // Shu-Osher form: U <- a U0 + b (U + dt L(U))
+  static const double A[3][3] = {{0.0, 0.0, 0.0}, {0.0, 0.5, 0.0}, {0.0, 0.75, 1.0 / 3.0}};
+  static const double B[3][3] = {{1.0, 0.0, 0.0}, {1.0, 0.5, 0.0}, {1.0, 0.25, 2.0 / 3.0}};
+  double* Up[5] = {U->D, U->Sx, U->Sy, U->Sz, U->tau};
+  double* Bp[3] = {Bf->bx, Bf->by, Bf->bz};
+  const ak_cons R0 = {c->regU0[0], c->regU0[1], c->regU0[2], c->regU0[3], c->regU0[4]};
+  const ak_faceB RB0 = {c->regB0[0], c->regB0[1], c->regB0[2]};
+  const ak_faceB Bc = {Bf->bx, Bf->by, Bf->bz};
+  const ak_rhs_out out = {c->reg_dU[0], c->reg_dU[1], c->reg_dU[2], c->reg_dU[3], c->reg_dU[4],
+                          c->regE[0], c->regE[1], c->regE[2], c->reg_flag, nullptr};
+  // the caller's blend setting is restored afterwards
+  const double* sv[5]; for (int q = 0; q < 5; ++q) sv[q] = c->blendU0[q];
+  const double sa = c->blend_a, sb = c->blend_b;
+  int r = AK_OK;
+  for (int step = 0; step < nsteps && r == AK_OK; ++step)
+    for (int s = 0; s < integrator && r == AK_OK; ++s) {
+      const double a = A[integrator - 1][s], b = B[integrator - 1][s];
+      if ((r = ak_fill_ghosts(c, bc, U, Bf)) != AK_OK) break;
+      if (s == 0) r = ak_set_fofc_blend(c, nullptr, 0.0, 1.0); else r = ak_set_fofc_blend(c, &R0, a, b);
+      if (r != AK_OK) break;
+      if ((r = ak_rhs(c, U, &Bc, W, 0, dt, &out)) != AK_OK) break;
+      if (flag_or) k_or_bytes<<<148 * 8, 256, 0, c->stream>>>(flag_or, c->reg_flag, c->sz.cell);
+      if (s == 0 && integrator > 1) {
+        // step-start register: the state after the first stage's con2prim (floored)
+        for (int q = 0; q < 5; ++q) CK(cudaMemcpyAsync(c->regU0[q], Up[q], cb, cudaMemcpyDeviceToDevice, c->stream));
+        for (int q = 0; q < 3; ++q) CK(cudaMemcpyAsync(c->regB0[q], Bp[q], fb[q], cudaMemcpyDeviceToDevice, c->stream));
+      }
+      if (s == 0) r = ak_stage_update(c, 0.0, 1.0, dt, U, &Bc, U, Bf, &out);    // register = the state itself
+      else r = ak_stage_update(c, a, b, dt, &R0, &RB0, U, Bf, &out);
+    }
+  for (int q = 0; q < 5; ++q) c->blendU0[q] = sv[q];
+  c->blend_a = sa; c->blend_b = sb;
+  if (r != AK_OK) return r;
+  return ak_fill_ghosts(c, bc, U, Bf);
 }
 
 int ak_probe_copy(ak_ctx* c, double* dst, const double* src, long long n, int reps, double* gbs) {

@@ -40,6 +40,8 @@ struct Fields {
   unsigned int* list;           // FOFC: compacted flagged cells
   unsigned int* count;          // [0..2] faces redone per direction, [3] length of list
   unsigned long long* stats;    // device counters (see ak_api.cu)
+  const double* U0[5];          // FOFC estimate of a later RK stage: U* = fa U0 + fb (U - dt div F);
+  double fa, fb;                // U0[0] == nullptr: U* = U - dt div F (R9)
 };
 
 enum { ST_DFLOOR = 1, ST_TAUFLOOR = 2, ST_MAGCAP = 4, ST_RHOFLOOR = 8, ST_TFLOOR = 16,

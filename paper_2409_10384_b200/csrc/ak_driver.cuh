@@ -1,0 +1,129 @@
+// ak_driver.cuh — stage driver kernels ("RK2 / RK3", constrained transport):
+//   k_fill_cells / k_fill_faces<D>   ghost fill of self-contained MeshBlocks (periodic / outflow)
+//   k_update_cells / k_update_faces<D>  Shu-Osher register update  U <- a U0 + b (U + dt dU),
+//                                    B~f <- a B0 + b (B~f + dt (-curl E)) on faces of interior cells
+//   k_or_bytes                       OR-accumulation of FOFC flag bytes over stages
+#pragma once
+#include "ak_kernels.cuh"
+
+namespace ak {
+
+struct DrvFields {
+  double* U[5];
+  double* Bf[3];
+  const double* U0[5];
+  const double* B0[3];
+  const double* dU[5];
+  const double* E[3];
+  const double* dx;
+};
+
+// source index of a cell-like index q (itself when interior); bc 0 periodic, 1 outflow
+__device__ __forceinline__ int src_cell(int q, int bc, int is, int ie, int n) {
+  if (q >= is && q <= ie) return q;
+  if (bc == 0) { int r = (q - is) % n; if (r < 0) r += n; return is + r; }
+  return q < is ? is : ie;
+}
+// source index of a face-normal index q in [0, nt]; periodic: face ie+1 is face is
+__device__ __forceinline__ int src_face(int q, int bc, int is, int ie, int n) {
+  if (bc == 0) { int r = (q - is) % n; if (r < 0) r += n; return is + r; }
+  if (q < is) return is;
+  if (q > ie + 1) return ie + 1;
+  return q;
+}
+
+__global__ void __launch_bounds__(256) k_fill_cells(const __grid_constant__ Par P, const __grid_constant__ DrvFields f,
+                                                    int bcx, int bcy, int bcz) {
+  const unsigned nt = (unsigned)P.nt;
+  const unsigned ncell = (unsigned)P.nmb * nt * nt * nt;
+  const unsigned c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= ncell) return;
+  const int i = (int)(c % nt);
+  unsigned r = c / nt;
+  const int j = (int)(r % nt); r /= nt;
+  const int k = (int)(r % nt);
+  const int m = (int)(r / nt);
+  const int is_ = src_cell(i, bcx, P.is, P.ie, P.n), js = src_cell(j, bcy, P.is, P.ie, P.n),
+            ks = src_cell(k, bcz, P.is, P.ie, P.n);
+  if (is_ == i && js == j && ks == k) return;
+  const Ix ix{P.nt, P.px};
+  const long long s = ix.cell(m, ks, js, is_);
+#pragma unroll
+  for (int v = 0; v < 5; ++v) f.U[v][c] = f.U[v][s];
+}
+
+template <int D>
+__global__ void __launch_bounds__(256) k_fill_faces(const __grid_constant__ Par P, const __grid_constant__ DrvFields f,
+                                                    int bcx, int bcy, int bcz) {
+  const unsigned nt = (unsigned)P.nt;
+  const unsigned ni = nt + (D == 0), nj = nt + (D == 1), nk = nt + (D == 2);
+  const unsigned tot = (unsigned)P.nmb * nk * nj * ni;
+  const unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= tot) return;
+  const int i = (int)(t % ni);
+  unsigned r = t / ni;
+  const int j = (int)(r % nj); r /= nj;
+  const int k = (int)(r % nk);
+  const int m = (int)(r / nk);
+  const int is_ = D == 0 ? src_face(i, bcx, P.is, P.ie, P.n) : src_cell(i, bcx, P.is, P.ie, P.n);
+  const int js = D == 1 ? src_face(j, bcy, P.is, P.ie, P.n) : src_cell(j, bcy, P.is, P.ie, P.n);
+  const int ks = D == 2 ? src_face(k, bcz, P.is, P.ie, P.n) : src_cell(k, bcz, P.is, P.ie, P.n);
+  if (is_ == i && js == j && ks == k) return;
+  const Ix ix{P.nt, P.px};
+  f.Bf[D][ix.face(D, m, k, j, i)] = f.Bf[D][ix.face(D, m, ks, js, is_)];
+}
+
+__global__ void __launch_bounds__(256) k_update_cells(const __grid_constant__ Par P, const __grid_constant__ DrvFields f,
+                                                      double a, double b, double dt) {
+  const unsigned n = (unsigned)P.n;
+  const unsigned tot = (unsigned)P.nmb * n * n * n;
+  const unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= tot) return;
+  const int i = (int)(t % n) + P.is;
+  unsigned r = t / n;
+  const int j = (int)(r % n) + P.is; r /= n;
+  const int k = (int)(r % n) + P.is;
+  const int m = (int)(r / n);
+  const Ix ix{P.nt, P.px};
+  const long long c = ix.cell(m, k, j, i);
+#pragma unroll
+  for (int v = 0; v < 5; ++v) f.U[v][c] = a * f.U0[v][c] + b * (f.U[v][c] + dt * f.dU[v][c]);
+}
+
+// D-faces of interior cells: normal index in [is, ie+1], transverse in [is, ie]
+template <int D>
+__global__ void __launch_bounds__(256) k_update_faces(const __grid_constant__ Par P, const __grid_constant__ DrvFields f,
+                                                      double a, double b, double dt) {
+  const unsigned n = (unsigned)P.n;
+  const unsigned ni = n + (D == 0), nj = n + (D == 1), nk = n + (D == 2);
+  const unsigned tot = (unsigned)P.nmb * nk * nj * ni;
+  const unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= tot) return;
+  const int i = (int)(t % ni) + P.is;
+  unsigned r = t / ni;
+  const int j = (int)(r % nj) + P.is; r /= nj;
+  const int k = (int)(r % nk) + P.is;
+  const int m = (int)(r / nk);
+  const Ix ix{P.nt, P.px};
+  const double idx = 1.0 / f.dx[3 * m + 0], idy = 1.0 / f.dx[3 * m + 1], idz = 1.0 / f.dx[3 * m + 2];
+  double dB;
+  if (D == 0)
+    dB = -((f.E[2][ix.edge(2, m, k, j + 1, i)] - f.E[2][ix.edge(2, m, k, j, i)]) * idy -
+           (f.E[1][ix.edge(1, m, k + 1, j, i)] - f.E[1][ix.edge(1, m, k, j, i)]) * idz);
+  else if (D == 1)
+    dB = -((f.E[0][ix.edge(0, m, k + 1, j, i)] - f.E[0][ix.edge(0, m, k, j, i)]) * idz -
+           (f.E[2][ix.edge(2, m, k, j, i + 1)] - f.E[2][ix.edge(2, m, k, j, i)]) * idx);
+  else
+    dB = -((f.E[1][ix.edge(1, m, k, j, i + 1)] - f.E[1][ix.edge(1, m, k, j, i)]) * idx -
+           (f.E[0][ix.edge(0, m, k, j + 1, i)] - f.E[0][ix.edge(0, m, k, j, i)]) * idy);
+  const long long q = ix.face(D, m, k, j, i);
+  f.Bf[D][q] = a * f.B0[D][q] + b * (f.Bf[D][q] + dt * dB);
+}
+
+__global__ void __launch_bounds__(256) k_or_bytes(unsigned char* __restrict__ acc, const unsigned char* __restrict__ src,
+                                                  long long nbytes) {
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < nbytes; q += stride) acc[q] |= src[q];
+}
+
+}  // namespace ak

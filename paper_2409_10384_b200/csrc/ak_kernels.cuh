@@ -183,7 +183,11 @@ __global__ void __launch_bounds__(128, AK_FOFC_MINB) k_fofc_test(const __grid_co
   const double idx[3] = {1.0 / f.dx[3 * m + 0], 1.0 / f.dx[3 * m + 1], 1.0 / f.dx[3 * m + 2]};
   double Us[5], Bc[3], W5[5];
 #pragma unroll
-  for (int v = 0; v < 5; ++v) Us[v] = f.U[v][c] - dt * div_flux(f, ix, v, m, k, j, i, idx);
+  for (int v = 0; v < 5; ++v) {
+    const double div = div_flux(f, ix, v, m, k, j, i, idx);
+    if (f.U0[0]) Us[v] = f.fa * f.U0[v][c] + f.fb * (f.U[v][c] - dt * div);
+    else Us[v] = f.U[v][c] - dt * div;
+  }
   Met3 g;
   load_met3(f, c, g);
 #pragma unroll
