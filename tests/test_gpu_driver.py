@@ -71,6 +71,7 @@ def test_fofc_blend_matches_oracle():
     dt = 2 * w["dt_fofc"]
     rng = np.random.default_rng(1)
     U0 = [u * (1.0 + 0.3 * rng.uniform(-1, 1, u.shape)) for u in w["U"]]
+    U0[4][0, 5, 6, 7] = -40.0; U0[0][0, 6, 6, 6] = 1e-14; U0[1][0, 7, 5, 5] = 500.0   # force flags
     U = [u.copy() for u in w["U"]]
     o = orc.rhs_blend(par, w["dx"], U, w["Bf"], w["adm"], dt, U0, 0.75, 0.25)
     with gpukit.GpuStage(copy.deepcopy(w)) as g:
