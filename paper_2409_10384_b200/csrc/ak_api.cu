@@ -159,13 +159,18 @@ int launch_c2p(ak_ctx* c, const Fields& f) {
   return AK_OK;
 }
 
+#ifndef AK_FLUX_CELL_MASK
+#define AK_FLUX_CELL_MASK 1   // bit d set: direction d uses the reconstruct-once variant k_flux_tma_cell
+#endif
+
 template <int DIR, int RECON>
 int launch_flux_tma(ak_ctx* c, const Fields& f, int NA, unsigned grid, size_t smem) {
+  auto kern = ((AK_FLUX_CELL_MASK >> DIR) & 1) ? k_flux_tma_cell<DIR, RECON> : k_flux_tma<DIR, RECON>;
   if (!c->tma_attr[DIR]) {
-    CK(cudaFuncSetAttribute(k_flux_tma<DIR, RECON>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     c->tma_attr[DIR] = true;
   }
-  k_flux_tma<DIR, RECON><<<grid, TMA_THREADS, smem, c->stream>>>(c->P, f, NA);
+  kern<<<grid, TMA_THREADS, smem, c->stream>>>(c->P, f, NA);
   return AK_OK;
 }
 
@@ -173,15 +178,17 @@ template <int DIR>
 int launch_flux(ak_ctx* c, const Fields& f) {
   Timer t(c, KC_FX + DIR);
   const int n = c->P.n, nt = c->P.nt, e = n + 2;
-  const int nfi = DIR == 0 ? n + 3 : e;            // faces per row of a tile
-  if (AK_FLUX_TMA && n % 2 == 0 && nfi <= TMA_THREADS) {
+  constexpr int AK_FLUX_CELL = (AK_FLUX_CELL_MASK >> DIR) & 1;
+  // threads per row of a tile: faces (k_flux_tma) or cells (k_flux_tma_cell)
+  const int nfi = AK_FLUX_CELL ? (DIR == 0 ? n + 4 : e) : (DIR == 0 ? n + 3 : e);
+  if (AK_FLUX_TMA && n % 2 == 0 && nfi * (AK_FLUX_CELL && DIR != 0 ? 2 : 1) <= TMA_THREADS) {
     // tile height: as many rows as fit the block, balanced over the extent it tiles
     const int nfd = DIR == 0 ? e : n + 3;
-    const int namax = TMA_THREADS / nfi;
+    const int namax = TMA_THREADS / nfi - (AK_FLUX_CELL && DIR != 0 ? 1 : 0);
     const int tiles = (nfd + namax - 1) / namax;
     const int NA = (nfd + tiles - 1) / tiles;
     const int maxW = DIR == 0 ? NA : NA + 5, maxM = DIR == 0 ? NA : NA + 1;
-    const size_t smem = sizeof(double) * (size_t)(7 * maxW + 10 * maxM) * nt;
+    const size_t smem = sizeof(double) * ((size_t)(7 * maxW + 10 * maxM) * nt + (AK_FLUX_CELL ? 7 * TMA_THREADS : 0));
     if (smem <= 200 * 1024) {
       const unsigned grid = (unsigned)((long long)c->P.nmb * e * tiles);
       int r;
