@@ -6,7 +6,10 @@
 
 namespace ak {
 
-__global__ void __launch_bounds__(128) k_div_src(const __grid_constant__ Par P,
+#ifndef AK_SRC_MINB
+#define AK_SRC_MINB 4
+#endif
+__global__ void __launch_bounds__(128, AK_SRC_MINB) k_div_src(const __grid_constant__ Par P,
                                                  const __grid_constant__ Fields f) {
   const int n = P.n;
   const long long per = (long long)n * n * n;
