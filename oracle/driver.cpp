@@ -69,6 +69,68 @@ extern "C" void orc_fill_ghosts(const orc_params* p, const int bc[3], double* co
   }
 }
 
+// ---- same-level ghost exchange between MeshBlocks ("interblock
+// communication") ---------------------------------------------------------------------------
+// nbr[m][27]: block adjacent to m at offset (oz+1)*9 + (oy+1)*3 + (ox+1), ox,oy,oz in {-1,0,1}; -1 = none.
+// Pass 1: a ghost element whose offset block exists is copied from that block's interior (index
+// shifted by n per offset direction; the shared face ie+1 is taken from the upper neighbour's
+// face is).  Pass 2: for the others, every offset direction whose face neighbour is missing is a
+// physical side and gets bc[d] (periodic onto the block itself, or outflow); the source may be a
+// ghost element filled in pass 1.
+namespace {
+inline int region_cell(const Lay& L, int q) { return q < L.is ? -1 : (q > L.ie ? 1 : 0); }
+// faces along their normal: is..ie are owned; ie+1 is the upper neighbour's face is when there is
+// such a neighbour (or the side is periodic onto the block itself), else it is owned too
+inline int region_face(const Lay& L, int q, bool upper_is_image) {
+  if (q < L.is) return -1;
+  if (q > L.ie + 1) return 1;
+  return (q == L.ie + 1 && upper_is_image) ? 1 : 0;
+}
+inline int phys_cell(const Lay& L, int q, int bc) { return L.src_cell(q, bc); }
+inline int phys_face(const Lay& L, int q, int bc) { return L.src_face(q, bc); }
+}  // namespace
+
+extern "C" void orc_exchange_ghosts(const orc_params* p, const int* nbr, const int bc[3],
+                                    double* const U[5], double* const Bf[3]) {
+  const Lay L(p->n, p->ng);
+  const int nt = L.nt, n = L.n;
+  for (int pass = 0; pass < 2; ++pass)
+    for (int m = 0; m < p->nmb; ++m) {
+      const int* nb = nbr + 27 * m;
+      // field 0: cells (5 variables); fields 1..3: faces of direction d = field - 1
+      for (int fld = 0; fld < 4; ++fld) {
+        const int d = fld - 1;
+        const int ni = nt + (d == 0), nj = nt + (d == 1), nk = nt + (d == 2);
+        for (int k = 0; k < nk; ++k)
+          for (int j = 0; j < nj; ++j)
+            for (int i = 0; i < ni; ++i) {
+              const int ox = d == 0 ? region_face(L, i, nb[14] >= 0 || bc[0] == 0) : region_cell(L, i);
+              const int oy = d == 1 ? region_face(L, j, nb[16] >= 0 || bc[1] == 0) : region_cell(L, j);
+              const int oz = d == 2 ? region_face(L, k, nb[22] >= 0 || bc[2] == 0) : region_cell(L, k);
+              if (ox == 0 && oy == 0 && oz == 0) continue;
+              const int mb = nb[(oz + 1) * 9 + (oy + 1) * 3 + (ox + 1)];
+              int ms, is_, js, ks;
+              if (pass == 0) {
+                if (mb < 0) continue;
+                ms = mb; is_ = i - ox * n; js = j - oy * n; ks = k - oz * n;
+              } else {
+                if (mb >= 0) continue;
+                ms = m; is_ = i; js = j; ks = k;
+                if (ox != 0 && nb[13 + ox] < 0) is_ = d == 0 ? phys_face(L, i, bc[0]) : phys_cell(L, i, bc[0]);
+                if (oy != 0 && nb[13 + 3 * oy] < 0) js = d == 1 ? phys_face(L, j, bc[1]) : phys_cell(L, j, bc[1]);
+                if (oz != 0 && nb[13 + 9 * oz] < 0) ks = d == 2 ? phys_face(L, k, bc[2]) : phys_cell(L, k, bc[2]);
+                if (is_ == i && js == j && ks == k) continue;
+              }
+              if (fld == 0) {
+                for (int v = 0; v < 5; ++v) U[v][L.c(m, k, j, i)] = U[v][L.c(ms, ks, js, is_)];
+              } else {
+                Bf[d][L.f(d, m, k, j, i)] = Bf[d][L.f(d, ms, ks, js, is_)];
+              }
+            }
+      }
+    }
+}
+
 extern "C" void orc_stage_update(const orc_params* p, const double* dx, double a, double b, double dt,
                                  const double* const U0[5], const double* const B0[3],
                                  double* const U[5], double* const Bf[3],
@@ -111,10 +173,22 @@ extern "C" void orc_stage_update(const orc_params* p, const double* dx, double a
   }
 }
 
+extern "C" void orc_advance_nbr(const orc_params* p, const double* dx, int integrator, int nsteps,
+                                double dt, const int bc[3], const int* nbr, double* const U[5],
+                                double* const Bf[3], const double* const adm[16], double* const W[8],
+                                unsigned char* flag_or, int nthreads);
+
 extern "C" void orc_advance(const orc_params* p, const double* dx, int integrator, int nsteps,
                             double dt, const int bc[3], double* const U[5], double* const Bf[3],
                             const double* const adm[16], double* const W[8],
                             unsigned char* flag_or, int nthreads) {
+  orc_advance_nbr(p, dx, integrator, nsteps, dt, bc, nullptr, U, Bf, adm, W, flag_or, nthreads);
+}
+
+extern "C" void orc_advance_nbr(const orc_params* p, const double* dx, int integrator, int nsteps,
+                                double dt, const int bc[3], const int* nbr, double* const U[5],
+                                double* const Bf[3], const double* const adm[16], double* const W[8],
+                                unsigned char* flag_or, int nthreads) {
   const Lay L(p->n, p->ng);
   const long nt = L.nt, px = L.px, nb = p->nmb;
   const long ncell = nb * nt * nt * nt;
@@ -132,7 +206,7 @@ extern "C" void orc_advance(const orc_params* p, const double* dx, int integrato
   for (int step = 0; step < nsteps; ++step)
     for (int s = 0; s < ns; ++s) {
       const double a = A[ns - 1][s], b = B[ns - 1][s];
-      orc_fill_ghosts(p, bc, U, Bf);
+      if (nbr) orc_exchange_ghosts(p, nbr, bc, U, Bf); else orc_fill_ghosts(p, bc, U, Bf);
       orc_rhs_blend(p, dx, U, Bf, adm, W, 0, dt, s == 0 ? nullptr : U0, a, b, dU, E, flag.data(),
                     nullptr, nthreads);
       if (flag_or) for (long c = 0; c < ncell; ++c) flag_or[c] |= flag[c];
@@ -149,5 +223,5 @@ extern "C" void orc_advance(const orc_params* p, const double* dx, int integrato
         orc_stage_update(p, dx, a, b, dt, U0, B0, U, Bf, dU, E);
       }
     }
-  orc_fill_ghosts(p, bc, U, Bf);
+  if (nbr) orc_exchange_ghosts(p, nbr, bc, U, Bf); else orc_fill_ghosts(p, bc, U, Bf);
 }

@@ -131,6 +131,15 @@ void orc_advance(const orc_params* p, const double* dx, int integrator, int nste
                  const double* const adm[16], double* const W[8], unsigned char* flag_or,
                  int nthreads);
 
+/* Same-level ghost exchange between MeshBlocks.  nbr[nmb][27]: block at offset
+ * (oz+1)*9+(oy+1)*3+(ox+1), -1 = none; sides without a face neighbour get bc[d]. */
+void orc_exchange_ghosts(const orc_params* p, const int* nbr, const int bc[3], double* const U[5],
+                         double* const Bf[3]);
+void orc_advance_nbr(const orc_params* p, const double* dx, int integrator, int nsteps, double dt,
+                     const int bc[3], const int* nbr, double* const U[5], double* const Bf[3],
+                     const double* const adm[16], double* const W[8], unsigned char* flag_or,
+                     int nthreads);
+
 #ifdef __cplusplus
 }
 #endif

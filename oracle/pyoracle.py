@@ -207,3 +207,25 @@ def advance(par, dx, integrator, nsteps, dt, bc, U, Bf, adm, nthreads=1):
                       _ib(bc), _ptrs(U), _ptrs(Bf), _ptrs(adm), _ptrs(W), flag.ctypes.data_as(C.c_void_p),
                       int(nthreads))
     return W, flag
+
+
+def _nbr(nbr, nmb):
+    a = np.ascontiguousarray(nbr, dtype=np.int32).reshape(nmb, 27)
+    return a, a.ctypes.data_as(C.POINTER(C.c_int))
+
+
+def exchange_ghosts(par, nbr, bc, U, Bf):
+    a, ap = _nbr(nbr, par.nmb)
+    lib().orc_exchange_ghosts(C.byref(par), ap, _ib(bc), _ptrs(U), _ptrs(Bf))
+
+
+def advance_nbr(par, dx, integrator, nsteps, dt, bc, nbr, U, Bf, adm, nthreads=1):
+    sh = shapes(par.nmb, par.n)
+    dx = np.ascontiguousarray(dx, dtype=np.float64).reshape(par.nmb, 3)
+    W = [np.zeros(sh["cell"]) for _ in range(8)]
+    flag = np.zeros(sh["cell"], dtype=np.uint8)
+    a, ap = _nbr(nbr, par.nmb)
+    lib().orc_advance_nbr(C.byref(par), dx.ctypes.data_as(_dp), int(integrator), int(nsteps), C.c_double(dt),
+                          _ib(bc), ap, _ptrs(U), _ptrs(Bf), _ptrs(adm), _ptrs(W),
+                          flag.ctypes.data_as(C.c_void_p), int(nthreads))
+    return W, flag
