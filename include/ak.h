@@ -159,6 +159,14 @@ int ak_rhs_host(ak_ctx*, const ak_cons* U, const ak_faceB* Bf, const ak_prim* W,
  * replaced) = the step-start register; U0 == NULL restores U* = U - dt_fofc div F. */
 int ak_set_fofc_blend(ak_ctx*, const ak_cons* U0, double a, double b);
 
+/* Same-level neighbour table for ak_fill_ghosts / ak_advance (D:§12; "interblock
+ * communication"): nbr = HOST int [nmb][27], entry (oz+1)*9+(oy+1)*3+(ox+1) = index of the block
+ * adjacent at offset (ox,oy,oz) in {-1,0,1}^3, -1 = none (entry 13, the block itself, is ignored).
+ * It is copied.  With a table set, ghosts whose offset block exists are copied from that block's
+ * interior (the shared face ie+1 from the upper neighbour's face is); sides without a face
+ * neighbour are physical and get bc[d].  Needs n >= 6.  nbr == NULL removes the table. */
+int ak_set_neighbors(ak_ctx*, const int* nbr);
+
 /* Fill the ghost cells of U~ and the ghost faces of B~f in place.  bc[d] = AK_BC_* per direction:
  * periodic (face ie+1 is made a copy of face is) or outflow (zero-gradient copies). */
 int ak_fill_ghosts(ak_ctx*, const int bc[3], const ak_cons* U, const ak_faceB_rw* Bf);

@@ -21,7 +21,7 @@ KERNEL_CLASSES = ("con2prim", "flux_x", "flux_y", "flux_z", "fofc_test", "fofc_f
 EXPORTS = ("ak_create", "ak_set_metric", "ak_con2prim", "ak_rhs", "ak_emf", "ak_get_stats",
            "ak_get_flux", "ak_rhs_host", "ak_timing", "ak_kernel_ms", "ak_probe_copy",
            "ak_probe_fp64", "ak_destroy", "ak_strerror", "ak_version",
-           "ak_set_fofc_blend", "ak_fill_ghosts", "ak_stage_update", "ak_advance")
+           "ak_set_fofc_blend", "ak_fill_ghosts", "ak_stage_update", "ak_advance", "ak_set_neighbors")
 BC_PERIODIC, BC_OUTFLOW = 0, 1
 
 _dp = C.POINTER(C.c_double)
@@ -106,6 +106,7 @@ def lib():
                                       C.POINTER(AkRhsOut)]
         L.ak_advance.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double, C.POINTER(C.c_int), C.POINTER(AkCons),
                                  C.POINTER(AkFaceB), C.POINTER(AkPrim), C.c_void_p]
+        L.ak_set_neighbors.argtypes = [C.c_void_p, C.POINTER(C.c_int)]
         _lib = L
     return _lib
 
@@ -260,3 +261,12 @@ def ak_advance(ctx, integrator, nsteps, dt, bc, U, Bf, W, flag_or=None):
     u, bf, w = _struct(AkCons, U), _struct(AkFaceB, Bf), _struct(AkPrim, W)
     _chk(lib().ak_advance(ctx, int(integrator), int(nsteps), float(dt), _bc(bc), C.byref(u), C.byref(bf),
                           C.byref(w), _ptr(flag_or)), "ak_advance")
+
+
+def ak_set_neighbors(ctx, nbr):
+    """nbr: int array [nmb][27] (host) or None."""
+    if nbr is None:
+        _chk(lib().ak_set_neighbors(ctx, None), "ak_set_neighbors")
+        return
+    a = np.ascontiguousarray(nbr, dtype=np.int32)
+    _chk(lib().ak_set_neighbors(ctx, a.ctypes.data_as(C.POINTER(C.c_int))), "ak_set_neighbors")

@@ -57,6 +57,7 @@ struct ak_ctx {
   // stage-driver registers (ak_advance), allocated on first use
   double* regU0[5]; double* regB0[3]; double* reg_dU[5]; double* regE[3]; unsigned char* reg_flag;
   bool have_reg;
+  int* nbr;                     // device copy of the neighbour table (ak_set_neighbors), or NULL
   // timing
   bool timing;
   cudaEvent_t ev0, ev1;
@@ -419,6 +420,7 @@ int ak_destroy(ak_ctx* c) {
   for (int q = 0; q < 5; ++q) { cudaFree(c->regU0[q]); cudaFree(c->reg_dU[q]); }
   for (int q = 0; q < 3; ++q) { cudaFree(c->regB0[q]); cudaFree(c->regE[q]); }
   cudaFree(c->reg_flag);
+  cudaFree(c->nbr);
   cudaFree(c->flag_own); cudaFree(c->count); cudaFree(c->stats); cudaFree(c->dx);
   delete c;
   return AK_OK;
@@ -600,11 +602,40 @@ int ak_fill_ghosts(ak_ctx* c, const int bc[3], const ak_cons* U, const ak_faceB_
   f.U[0] = U->D; f.U[1] = U->Sx; f.U[2] = U->Sy; f.U[3] = U->Sz; f.U[4] = U->tau;
   f.Bf[0] = Bf->bx; f.Bf[1] = Bf->by; f.Bf[2] = Bf->bz;
   const long long nt = c->P.nt, nb = c->P.nmb;
+  if (c->nbr) {
+    const unsigned gf = nblk(nb * nt * nt * (nt + 1), 256);
+    for (int pass = 0; pass < 2; ++pass) {
+      k_exchange<0><<<nblk(c->sz.cell, 256), 256, 0, c->stream>>>(c->P, f, c->nbr, pass, bc[0], bc[1], bc[2]);
+      k_exchange<1><<<gf, 256, 0, c->stream>>>(c->P, f, c->nbr, pass, bc[0], bc[1], bc[2]);
+      k_exchange<2><<<gf, 256, 0, c->stream>>>(c->P, f, c->nbr, pass, bc[0], bc[1], bc[2]);
+      k_exchange<3><<<gf, 256, 0, c->stream>>>(c->P, f, c->nbr, pass, bc[0], bc[1], bc[2]);
+    }
+    CK(cudaGetLastError());
+    return AK_OK;
+  }
   k_fill_cells<<<nblk(c->sz.cell, 256), 256, 0, c->stream>>>(c->P, f, bc[0], bc[1], bc[2]);
   k_fill_faces<0><<<nblk(nb * nt * nt * (nt + 1), 256), 256, 0, c->stream>>>(c->P, f, bc[0], bc[1], bc[2]);
   k_fill_faces<1><<<nblk(nb * nt * nt * (nt + 1), 256), 256, 0, c->stream>>>(c->P, f, bc[0], bc[1], bc[2]);
   k_fill_faces<2><<<nblk(nb * nt * nt * (nt + 1), 256), 256, 0, c->stream>>>(c->P, f, bc[0], bc[1], bc[2]);
   CK(cudaGetLastError());
+  return AK_OK;
+}
+
+int ak_set_neighbors(ak_ctx* c, const int* nbr) {
+  if (!c) return AK_EINVAL;
+  CK(cudaSetDevice(c->hp.device));
+  if (!nbr) {
+    CK(cudaStreamSynchronize(c->stream));
+    cudaFree(c->nbr); c->nbr = nullptr;
+    return AK_OK;
+  }
+  const long long cnt = 27LL * c->P.nmb;
+  if (c->P.n < 6) return AK_EINVAL;             // a ghost layer must come from owned elements only
+  for (long long q = 0; q < cnt; ++q)
+    if (nbr[q] < -1 || nbr[q] >= c->P.nmb) return AK_EINVAL;
+  if (!c->nbr) CK(cudaMalloc(&c->nbr, sizeof(int) * cnt));
+  CK(cudaMemcpyAsync(c->nbr, nbr, sizeof(int) * cnt, cudaMemcpyHostToDevice, c->stream));
+  CK(cudaStreamSynchronize(c->stream));        // nbr is the caller's
   return AK_OK;
 }
 

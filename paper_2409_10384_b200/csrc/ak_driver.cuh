@@ -126,4 +126,58 @@ __global__ void __launch_bounds__(256) k_or_bytes(unsigned char* __restrict__ ac
   for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < nbytes; q += stride) acc[q] |= src[q];
 }
 
+// ---- same-level ghost exchange between MeshBlocks -----------------------------------
+// nbr[m][27]: block at offset (oz+1)*9+(oy+1)*3+(ox+1), -1 = none.  FLD 0: the five cell fields;
+// FLD 1..3: the face field of direction FLD-1.  pass 0 copies from existing offset blocks, pass 1
+// applies bc[d] on the sides that have no face neighbour (sources may be ghosts filled in pass 0).
+__device__ __forceinline__ int region_cell(int q, int is, int ie) { return q < is ? -1 : (q > ie ? 1 : 0); }
+__device__ __forceinline__ int region_face(int q, int is, int ie, bool upper_is_image) {
+  if (q < is) return -1;
+  if (q > ie + 1) return 1;
+  return (q == ie + 1 && upper_is_image) ? 1 : 0;
+}
+
+template <int FLD>
+__global__ void __launch_bounds__(256) k_exchange(const __grid_constant__ Par P, const __grid_constant__ DrvFields f,
+                                                  const int* __restrict__ nbr, int pass, int bcx, int bcy, int bcz) {
+  constexpr int D = FLD - 1;
+  const unsigned nt = (unsigned)P.nt;
+  const unsigned ni = nt + (D == 0), nj = nt + (D == 1), nk = nt + (D == 2);
+  const unsigned tot = (unsigned)P.nmb * nk * nj * ni;
+  const unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= tot) return;
+  const int i = (int)(t % ni);
+  unsigned r = t / ni;
+  const int j = (int)(r % nj); r /= nj;
+  const int k = (int)(r % nk);
+  const int m = (int)(r / nk);
+  const int* nb = nbr + 27 * m;
+  const int is = P.is, ie = P.ie, n = P.n;
+  const int ox = D == 0 ? region_face(i, is, ie, nb[14] >= 0 || bcx == 0) : region_cell(i, is, ie);
+  const int oy = D == 1 ? region_face(j, is, ie, nb[16] >= 0 || bcy == 0) : region_cell(j, is, ie);
+  const int oz = D == 2 ? region_face(k, is, ie, nb[22] >= 0 || bcz == 0) : region_cell(k, is, ie);
+  if (ox == 0 && oy == 0 && oz == 0) return;
+  const int mb = nb[(oz + 1) * 9 + (oy + 1) * 3 + (ox + 1)];
+  int ms, is_, js, ks;
+  if (pass == 0) {
+    if (mb < 0) return;
+    ms = mb; is_ = i - ox * n; js = j - oy * n; ks = k - oz * n;
+  } else {
+    if (mb >= 0) return;
+    ms = m; is_ = i; js = j; ks = k;
+    if (ox != 0 && nb[13 + ox] < 0) is_ = D == 0 ? src_face(i, bcx, is, ie, n) : src_cell(i, bcx, is, ie, n);
+    if (oy != 0 && nb[13 + 3 * oy] < 0) js = D == 1 ? src_face(j, bcy, is, ie, n) : src_cell(j, bcy, is, ie, n);
+    if (oz != 0 && nb[13 + 9 * oz] < 0) ks = D == 2 ? src_face(k, bcz, is, ie, n) : src_cell(k, bcz, is, ie, n);
+    if (is_ == i && js == j && ks == k) return;
+  }
+  const Ix ix{P.nt, P.px};
+  if (FLD == 0) {
+    const long long dst = ix.cell(m, k, j, i), src = ix.cell(ms, ks, js, is_);
+#pragma unroll
+    for (int v = 0; v < 5; ++v) f.U[v][dst] = f.U[v][src];
+  } else {
+    f.Bf[D < 0 ? 0 : D][ix.face(D < 0 ? 0 : D, m, k, j, i)] = f.Bf[D < 0 ? 0 : D][ix.face(D < 0 ? 0 : D, ms, ks, js, is_)];
+  }
+}
+
 }  // namespace ak

@@ -137,3 +137,79 @@ def test_advance_curved_batch():
     """several C2 blocks (curved metric, shift, WENO-Z, FOFC+DMP), each its own periodic domain."""
     w = wl.make_blocks("C2", blocks=[21, 22, 41])
     flag = advance_both(w, dict(w["params"]), 3, 2, 0.05, (0, 0, 0))
+
+
+# ---------------------------------------------------------------- same-level ghost exchange
+@pytest.mark.parametrize("periodic", [(True, True, True), (False, False, False), (True, False, True)])
+def test_exchange_ghosts(periodic):
+    import torch
+    from test_oracle_exchange import lattice_nbr
+    n, nb3, nmb = 6, (2, 2, 2), 8
+    rng = np.random.default_rng(8)
+    sh = orc.shapes(nmb, n)
+    U = [rng.uniform(-1, 1, sh["cell"]) for _ in range(5)]
+    Bf = [rng.uniform(-1, 1, sh[k]) for k in ("xf", "yf", "zf")]
+    nbr = lattice_nbr(nb3, periodic)
+    bc = [0 if p else 1 for p in periodic]
+    par = orc.make_params(nmb=nmb, n=n)
+    U2 = [u.copy() for u in U]; B2 = [b.copy() for b in Bf]
+    orc.exchange_ghosts(par, nbr, bc, U2, B2)
+    ctx = ak.ak_create(ak.make_params(nmb=nmb, n=n, gamma_ad=2.0, rho_atm=1e-10, T_atm=1e-8), np.full((nmb, 3), 0.1))
+    try:
+        ak.ak_set_neighbors(ctx, nbr)
+        dU, dB = _dev(U), _dev(Bf)
+        ak.ak_fill_ghosts(ctx, bc, dU, dB)
+        torch.cuda.synchronize()
+        for a, b in zip(_np(dU) + _np(dB), U2 + B2):
+            assert np.array_equal(a, b)
+        ak.ak_set_neighbors(ctx, None)            # back to self-contained blocks
+        dU, dB = _dev(U), _dev(Bf)
+        ak.ak_fill_ghosts(ctx, bc, dU, dB)
+        torch.cuda.synchronize()
+        U3 = [u.copy() for u in U]; B3 = [b.copy() for b in Bf]
+        orc.fill_ghosts(par, bc, U3, B3)
+        for a, b in zip(_np(dU) + _np(dB), U3 + B3):
+            assert np.array_equal(a, b)
+    finally:
+        ak.ak_destroy(ctx)
+
+
+def test_advance_eight_blocks_with_exchange():
+    """2x2x2 blocks of 6^3 with exchange on the GPU = the oracle's multi-block run = (T27) one block."""
+    import torch
+    from test_oracle_exchange import lattice_nbr
+    N, n = 12, 6
+    d = 1.0 / N
+
+    def prim(x, y, z):
+        rho = 1.0 + 0.3 * np.sin(2 * np.pi * x) * np.cos(2 * np.pi * y) + 0.2 * np.sin(2 * np.pi * z)
+        rho = np.where((abs(x - 0.3) < 0.1) & (abs(y - 0.6) < 0.1) & (abs(z - 0.5) < 0.1), 1e-3 * rho, rho)
+        o = np.ones_like(x)
+        return rho, [0.3 * np.sin(2 * np.pi * y) * o, -0.2 * o, 0.25 * np.cos(2 * np.pi * x) * o], 0.6 * o
+
+    def A(comp, x, y, z):
+        return 0.1 * np.sin(2 * np.pi * (x + 2 * y)) if comp == 2 else 0.05 * np.cos(2 * np.pi * z) * (comp == 0) + 0 * x
+    p = dict(gamma_ad=5.0 / 3.0, rho_atm=1e-10, T_atm=1e-8, recon=2, riemann=1, fofc=1, dmp_M=1.2)
+    blocks = []
+    for bz in range(2):
+        for by in range(2):
+            for bx in range(2):
+                blocks.append(sk.build_block(n, d, (bx * n * d, by * n * d, bz * n * d), sk.flat_metric, prim,
+                                             A_fn=A, gamma_ad=5.0 / 3.0))
+    cat = lambda key, q: np.ascontiguousarray(np.concatenate([b[key][q] for b in blocks], axis=0))
+    U8 = [cat("U", v) for v in range(5)]; B8 = [cat("Bf", c) for c in range(3)]
+    adm8 = [cat("adm", q) for q in range(16)]
+    dx8 = np.full((8, 3), d)
+    p8 = dict(p, nmb=8, n=n)
+    nbr = lattice_nbr((2, 2, 2), (True, True, True))
+    dt = 0.15 * d
+    w = dict(U=[u.copy() for u in U8], Bf=[b.copy() for b in B8], adm=adm8, dx=dx8, params=p8, dt_fofc=dt)
+    Wo, flag_o = orc.advance_nbr(orc.make_params(**p8), dx8, 3, 2, dt, (0, 0, 0), nbr, U8, B8, adm8, nthreads=8)
+    with gpukit.GpuStage(w) as g:
+        ak.ak_set_neighbors(g.ctx, nbr)
+        gflag = torch.zeros_like(g.flag)
+        ak.ak_advance(g.ctx, 3, 2, dt, (0, 0, 0), g.U, g.Bf, g.W, gflag)
+        torch.cuda.synchronize()
+        for k, (a, b) in enumerate(zip(_np(g.U) + _np(g.Bf) + _np(g.W), U8 + B8 + Wo)):
+            assert np.array_equal(a, b), k
+        assert np.array_equal(gflag.cpu().numpy(), flag_o) and np.count_nonzero(flag_o) > 0
