@@ -58,6 +58,14 @@ struct ak_ctx {
   double* regU0[5]; double* regB0[3]; double* reg_dU[5]; double* regE[3]; unsigned char* reg_flag;
   bool have_reg;
   int* nbr;                     // device copy of the neighbour table (ak_set_neighbors), or NULL
+  // pipelined host entry (ak_rhs_host): two lanes, each a child context over `lane_chunk` blocks
+  // with its own stream and device staging; chunks alternate between the lanes
+  double* host_dx;              // [nmb][3] host copy
+  ak_ctx* lane[2]; int lane_chunk;
+  double* lane_buf[2][24];      // staging: U5 Bf3 W8 dU5 E3
+  unsigned char* lane_mask[2][2];
+  unsigned long long* lane_stats_h;   // pinned [nchunks][S_NSTAT + 4]
+  bool stats_from_host; ak_stats host_acc;
   // timing
   bool timing;
   cudaEvent_t ev0, ev1;
@@ -395,6 +403,9 @@ int ak_create(const ak_params* p, const double* dx3, ak_ctx** out) {
   if (e == cudaSuccess) e = cudaMalloc(&c->dx, sizeof(double) * 3 * nb);
   if (e == cudaSuccess) e = cudaMemcpyAsync(c->dx, dx3, sizeof(double) * 3 * nb, cudaMemcpyHostToDevice, c->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);   // dx3 is the caller's: copy must be done
+  c->host_dx = (double*)malloc(sizeof(double) * 3 * nb);
+  if (!c->host_dx && e == cudaSuccess) e = cudaErrorMemoryAllocation;
+  if (c->host_dx) memcpy(c->host_dx, dx3, sizeof(double) * 3 * nb);
   if (e != cudaSuccess) {
     last_cuda_error = e;
     ak_destroy(c);
@@ -421,6 +432,13 @@ int ak_destroy(ak_ctx* c) {
   for (int q = 0; q < 3; ++q) { cudaFree(c->regB0[q]); cudaFree(c->regE[q]); }
   cudaFree(c->reg_flag);
   cudaFree(c->nbr);
+  free(c->host_dx);
+  for (int l = 0; l < 2; ++l) {
+    if (c->lane[l]) { cudaStream_t st = c->lane[l]->stream; ak_destroy(c->lane[l]); cudaStreamDestroy(st); }
+    for (int q = 0; q < 24; ++q) cudaFree(c->lane_buf[l][q]);
+    cudaFree(c->lane_mask[l][0]); cudaFree(c->lane_mask[l][1]);
+  }
+  if (c->lane_stats_h) cudaFreeHost(c->lane_stats_h);
   cudaFree(c->flag_own); cudaFree(c->count); cudaFree(c->stats); cudaFree(c->dx);
   delete c;
   return AK_OK;
@@ -463,6 +481,7 @@ int ak_rhs(ak_ctx* c, const ak_cons* U, const ak_faceB* Bf, const ak_prim* W, in
   if (out->fofc_flag) f.flag = out->fofc_flag;
   f.status = out->c2p_status;
   CK(cudaSetDevice(c->hp.device));
+  c->stats_from_host = false;
   int r;
   if (!w_is_valid && (r = launch_c2p(c, f)) != AK_OK) return r;
   if ((r = launch_flux<0>(c, f)) != AK_OK) return r;
@@ -487,6 +506,7 @@ int ak_emf(ak_ctx* c, const ak_prim* W, double* Ex, double* Ey, double* Ez) {
 
 int ak_get_stats(ak_ctx* c, ak_stats* o) {
   if (!c || !o) return AK_EINVAL;
+  if (c->stats_from_host) { *o = c->host_acc; return AK_OK; }
   unsigned long long h[S_NSTAT];
   unsigned cnt[4];
   CK(cudaSetDevice(c->hp.device));
@@ -527,6 +547,90 @@ int ak_kernel_ms(ak_ctx* c, double ms_out[8], long long launches_out[8]) {
   return r;
 }
 
+// Pipelined host path: the batch is cut into chunks of blocks that alternate between two lanes
+// (child contexts with their own streams), so that the H2D copy of one chunk, the kernels of
+// another and the D2H copy of a third overlap (PCIe is full duplex).
+static int rhs_host_pipelined(ak_ctx* c, int chunk, double* const hU[5], const double* const hB[3], double* const hW[8],
+                              double dt_fofc, double* const hdU[5], double* const hE[3], unsigned char* hflag,
+                              unsigned char* hstatus) {
+  const long long nt = c->P.nt, px = c->P.px;
+  const long long per[7] = {nt * nt * nt, nt * nt * px, nt * (nt + 1) * nt, (nt + 1) * nt * nt,
+                            (nt + 1) * (nt + 1) * nt, (nt + 1) * nt * px, nt * (nt + 1) * px};   // cell xf yf zf ex ey ez
+  const int nchunks = c->P.nmb / chunk;
+  if (c->lane_chunk != chunk) {
+    if (c->lane_chunk != 0) return AK_ESTATE;
+    for (int l = 0; l < 2; ++l) {
+      ak_params hp = c->hp;
+      hp.nmb = chunk;
+      cudaStream_t st;
+      CK(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking));
+      hp.stream = (void*)st;
+      const int r = ak_create(&hp, c->host_dx, &c->lane[l]);
+      if (r != AK_OK) { cudaStreamDestroy(st); return r; }
+      // staging kinds: 0..4 U (cell), 5..7 Bf (xf yf zf), 8..15 W (cell), 16..20 dU (cell), 21..23 E (ex ey ez)
+      for (int q = 0; q < 24; ++q) {
+        const int kind = q < 5 ? 0 : (q < 8 ? 1 + (q - 5) : (q < 21 ? 0 : 4 + (q - 21)));
+        const size_t bytes = sizeof(double) * per[kind] * chunk;
+        CK(cudaMalloc(&c->lane_buf[l][q], bytes));
+        CK(cudaMemsetAsync(c->lane_buf[l][q], 0, bytes, st));
+      }
+      CK(cudaMalloc(&c->lane_mask[l][0], (size_t)per[0] * chunk));
+      CK(cudaMalloc(&c->lane_mask[l][1], (size_t)per[0] * chunk));
+    }
+    CK(cudaMallocHost(&c->lane_stats_h, sizeof(unsigned long long) * (S_NSTAT + 4) * nchunks));
+    c->lane_chunk = chunk;
+  }
+  CK(cudaStreamSynchronize(c->stream));            // the metric and anything queued by the caller
+  for (int ch = 0; ch < nchunks; ++ch) {
+    const int l = ch & 1;
+    ak_ctx* k = c->lane[l];
+    cudaStream_t st = k->stream;
+    const long long m0 = (long long)ch * chunk;
+    double** b = c->lane_buf[l];
+    CK(cudaMemcpyAsync(k->dx, c->host_dx + 3 * m0, sizeof(double) * 3 * chunk, cudaMemcpyHostToDevice, st));
+    for (int q = 0; q < 5; ++q)
+      CK(cudaMemcpyAsync(b[q], hU[q] + m0 * per[0], sizeof(double) * per[0] * chunk, cudaMemcpyHostToDevice, st));
+    for (int q = 0; q < 3; ++q)
+      CK(cudaMemcpyAsync(b[5 + q], hB[q] + m0 * per[1 + q], sizeof(double) * per[1 + q] * chunk, cudaMemcpyHostToDevice, st));
+    for (int q = 0; q < 16; ++q) k->adm[q] = c->adm[q] + m0 * per[0];
+    k->have_metric = true;
+    const ak_cons dU_ = {b[0], b[1], b[2], b[3], b[4]};
+    const ak_faceB dB_ = {b[5], b[6], b[7]};
+    const ak_prim dW_ = {b[8], b[9], b[10], b[11], b[12], b[13], b[14], b[15]};
+    const ak_rhs_out dO = {b[16], b[17], b[18], b[19], b[20], b[21], b[22], b[23], c->lane_mask[l][0], c->lane_mask[l][1]};
+    const int r = ak_rhs(k, &dU_, &dB_, &dW_, 0, dt_fofc, &dO);
+    if (r != AK_OK) return r;
+    for (int q = 0; q < 5; ++q) {
+      CK(cudaMemcpyAsync(hU[q] + m0 * per[0], b[q], sizeof(double) * per[0] * chunk, cudaMemcpyDeviceToHost, st));
+      CK(cudaMemcpyAsync(hdU[q] + m0 * per[0], b[16 + q], sizeof(double) * per[0] * chunk, cudaMemcpyDeviceToHost, st));
+    }
+    for (int q = 0; q < 8; ++q)
+      CK(cudaMemcpyAsync(hW[q] + m0 * per[0], b[8 + q], sizeof(double) * per[0] * chunk, cudaMemcpyDeviceToHost, st));
+    for (int q = 0; q < 3; ++q)
+      CK(cudaMemcpyAsync(hE[q] + m0 * per[4 + q], b[21 + q], sizeof(double) * per[4 + q] * chunk, cudaMemcpyDeviceToHost, st));
+    if (hflag) CK(cudaMemcpyAsync(hflag + m0 * per[0], c->lane_mask[l][0], (size_t)per[0] * chunk, cudaMemcpyDeviceToHost, st));
+    if (hstatus) CK(cudaMemcpyAsync(hstatus + m0 * per[0], c->lane_mask[l][1], (size_t)per[0] * chunk, cudaMemcpyDeviceToHost, st));
+    unsigned long long* hs = c->lane_stats_h + (size_t)(S_NSTAT + 4) * ch;
+    CK(cudaMemcpyAsync(hs, k->stats, sizeof(unsigned long long) * S_NSTAT, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(hs + S_NSTAT, k->count, sizeof(unsigned) * 4, cudaMemcpyDeviceToHost, st));
+  }
+  CK(cudaStreamSynchronize(c->lane[0]->stream));
+  CK(cudaStreamSynchronize(c->lane[1]->stream));
+  ak_stats acc;
+  memset(&acc, 0, sizeof(acc));
+  for (int ch = 0; ch < nchunks; ++ch) {
+    const unsigned long long* hs = c->lane_stats_h + (size_t)(S_NSTAT + 4) * ch;
+    const unsigned* cnt = (const unsigned*)(hs + S_NSTAT);
+    acc.n_c2p_fail += (long long)hs[S_C2P_FAIL]; acc.n_cons_floor += (long long)hs[S_CONS_FLOOR];
+    acc.n_prim_floor += (long long)hs[S_PRIM_FLOOR]; acc.n_dmp_cells += (long long)hs[S_DMP_CELLS];
+    acc.n_fofc_cells += cnt[3];
+    for (int d = 0; d < 3; ++d) acc.n_fofc_faces[d] += cnt[d];
+  }
+  c->host_acc = acc;
+  c->stats_from_host = true;
+  return AK_OK;
+}
+
 int ak_rhs_host(ak_ctx* c, const ak_cons* U, const ak_faceB* Bf, const ak_prim* W, double dt_fofc,
                 const ak_rhs_out* out) {
   if (!c || !U || !Bf || !W || !out) return AK_EINVAL;
@@ -535,6 +639,23 @@ int ak_rhs_host(ak_ctx* c, const ak_cons* U, const ak_faceB* Bf, const ak_prim* 
   const size_t cb = sizeof(double) * c->sz.cell;
   const size_t fb[3] = {sizeof(double) * c->sz.xf, sizeof(double) * c->sz.yf, sizeof(double) * c->sz.zf};
   const size_t eb[3] = {sizeof(double) * c->sz.ex, sizeof(double) * c->sz.ey, sizeof(double) * c->sz.ez};
+  double* hU[5] = {U->D, U->Sx, U->Sy, U->Sz, U->tau};
+  const double* hB[3] = {Bf->bx, Bf->by, Bf->bz};
+  double* hW[8] = {W->rho, W->ux, W->uy, W->uz, W->p, W->bccx, W->bccy, W->bccz};
+  double* hdU[5] = {out->dD, out->dSx, out->dSy, out->dSz, out->dtau};
+  double* hE[3] = {out->Ex, out->Ey, out->Ez};
+  for (int q = 0; q < 5; ++q) if (!hU[q] || !hdU[q]) return AK_EINVAL;
+  for (int q = 0; q < 3; ++q) if (!hB[q] || !hE[q]) return AK_EINVAL;
+  for (int q = 0; q < 8; ++q) if (!hW[q]) return AK_EINVAL;
+  {
+    // chunk = the largest divisor of nmb not above max(8, nmb / 8); small batches go in one piece
+    int chunk = 0;
+    const int cap = c->P.nmb / 8 > 8 ? c->P.nmb / 8 : 8;
+    if (c->P.nmb >= 16 && !c->blendU0[0])
+      for (int q = cap; q >= 4; --q) if (c->P.nmb % q == 0) { chunk = q; break; }
+    if (c->lane_chunk) chunk = c->lane_chunk;
+    if (chunk) return rhs_host_pipelined(c, chunk, hU, hB, hW, dt_fofc, hdU, hE, out->fofc_flag, out->c2p_status);
+  }
   if (!c->have_stg) {
     for (int q = 0; q < 5; ++q) { CK(cudaMalloc(&c->stg_U[q], cb)); CK(cudaMalloc(&c->stg_dU[q], cb)); }
     for (int q = 0; q < 8; ++q) CK(cudaMalloc(&c->stg_W[q], cb));
@@ -545,14 +666,6 @@ int ak_rhs_host(ak_ctx* c, const ak_cons* U, const ak_faceB* Bf, const ak_prim* 
     for (int q = 0; q < 3; ++q) CK(cudaMemsetAsync(c->stg_E[q], 0, eb[q], c->stream));
     c->have_stg = true;
   }
-  double* hU[5] = {U->D, U->Sx, U->Sy, U->Sz, U->tau};
-  const double* hB[3] = {Bf->bx, Bf->by, Bf->bz};
-  double* hW[8] = {W->rho, W->ux, W->uy, W->uz, W->p, W->bccx, W->bccy, W->bccz};
-  double* hdU[5] = {out->dD, out->dSx, out->dSy, out->dSz, out->dtau};
-  double* hE[3] = {out->Ex, out->Ey, out->Ez};
-  for (int q = 0; q < 5; ++q) if (!hU[q] || !hdU[q]) return AK_EINVAL;
-  for (int q = 0; q < 3; ++q) if (!hB[q] || !hE[q]) return AK_EINVAL;
-  for (int q = 0; q < 8; ++q) if (!hW[q]) return AK_EINVAL;
   for (int q = 0; q < 5; ++q) CK(cudaMemcpyAsync(c->stg_U[q], hU[q], cb, cudaMemcpyHostToDevice, c->stream));
   for (int q = 0; q < 3; ++q) CK(cudaMemcpyAsync(c->stg_Bf[q], hB[q], fb[q], cudaMemcpyHostToDevice, c->stream));
   ak_cons dU_ = {c->stg_U[0], c->stg_U[1], c->stg_U[2], c->stg_U[3], c->stg_U[4]};

@@ -240,3 +240,32 @@ def test_c4_full_size_sampled_blocks():
             assert bool(torch.isfinite(t).all())
     finally:
         ak.ak_destroy(ctx)
+
+
+def test_host_entry_point_pipelined_chunks():
+    """ak_rhs_host on a batch large enough for the two-lane pipeline (chunks of blocks on two
+    streams) must equal the device path, and its counters the sums over the chunks."""
+    import torch
+    from paper_2409_10384_b200 import ak
+    w = wl.make_blocks("C3", blocks=list(range(192, 224)))          # 32 blocks of 16^3 -> chunks of 8
+    with gpukit.GpuStage(copy.deepcopy(w)) as a:
+        a.rhs()
+        ra = a.result()
+        sa = a.stats()
+        sh = a.sh
+        pin = lambda arr: torch.from_numpy(np.ascontiguousarray(arr)).pin_memory()
+        hU = [pin(u) for u in w["U"]]
+        hB = [pin(b) for b in w["Bf"]]
+        hW = [pin(np.zeros(sh["cell"])) for _ in range(8)]
+        hdU = [pin(np.zeros(sh["cell"])) for _ in range(5)]
+        hE = [pin(np.zeros(sh[k])) for k in ("ex", "ey", "ez")]
+        hflag = pin(np.zeros(sh["cell"], dtype=np.uint8)); hst = pin(np.zeros(sh["cell"], dtype=np.uint8))
+        for rep in range(2):                                         # second call reuses the lanes
+            for h, u in zip(hU, w["U"]):
+                h.copy_(torch.from_numpy(u))
+            ak.ak_rhs_host(a.ctx, hU, hB, hW, w["dt_fofc"], hdU, hE, hflag, hst)
+            for x, y in zip(hdU + hE + hW + hU, ra["dU"] + ra["E"] + ra["W"] + ra["U"]):
+                assert np.array_equal(x.numpy(), y)
+            assert np.array_equal(hflag.numpy(), ra["flag"]) and np.array_equal(hst.numpy(), ra["status"])
+            assert a.stats() == sa
+        assert np.count_nonzero(ra["flag"]) > 0
