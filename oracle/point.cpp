@@ -270,6 +270,19 @@ extern "C" void orc_reconstruct(int kind, const double q[5], double* qm, double*
     *qm = ql; *qp = qr;
     return;
   }
+  if (kind == 3) {
+    // PLM with the monotonized-central slope limiter ("a van Leer monotonized slope
+    // limiter"; reading R27): slope = minmod(2 dl, 2 dr, (dl + dr)/2)
+    const double dl = q0 - qm1, dr = qp1 - q0;
+    double sl = 0.0;
+    if (dl * dr > 0.0) {
+      const double dc = 0.5 * (dl + dr);
+      sl = std::copysign(std::fmin(std::fmin(2.0 * std::fabs(dl), 2.0 * std::fabs(dr)), std::fabs(dc)), dc);
+    }
+    *qm = q0 - 0.5 * sl;
+    *qp = q0 + 0.5 * sl;
+    return;
+  }
   // WENO-Z, p = 2, eps = 1e-40
   const double c6 = 1.0 / 6.0, c1312 = 13.0 / 12.0, eps = 1e-40;
   const double a0 = qmm - 2.0 * qm1 + q0, a1 = qm1 - 2.0 * q0 + qp1, a2 = q0 - 2.0 * qp1 + qpp;

@@ -29,6 +29,15 @@ __device__ __forceinline__ void recon(double qmm, double qm1, double q0, double 
       else if (dq * eta < -(dq * dq)) qr = 3.0 * q0 - 2.0 * ql;
     }
     qm = ql; qp = qr;
+  } else if (KIND == 3) {     // PLM, monotonized-central limiter: slope = minmod(2 dl, 2 dr, (dl + dr)/2)
+    const double dl = q0 - qm1, dr = qp1 - q0;
+    double sl = 0.0;
+    if (dl * dr > 0.0) {
+      const double dc = 0.5 * (dl + dr);
+      sl = copysign(fmin(fmin(2.0 * fabs(dl), 2.0 * fabs(dr)), fabs(dc)), dc);
+    }
+    qm = q0 - 0.5 * sl;
+    qp = q0 + 0.5 * sl;
   } else {                    // WENO-Z (Borges et al. 2008), p = 2, eps = 1e-40
     const double c6 = 1.0 / 6.0, c1312 = 13.0 / 12.0, eps = 1e-40;
     const double a0 = qmm - 2.0 * qm1 + q0, a1 = qm1 - 2.0 * q0 + qp1, a2 = q0 - 2.0 * qp1 + qpp;

@@ -483,3 +483,36 @@ def test_T17_convergence_order_on_sine(kind, order):
         errs.append(e)
     rate = np.log2(errs[-2] / errs[-1])
     assert rate > order - 0.6, (errs, rate)
+
+
+def test_T17_plm_mc_limiter():
+    """PLM with the monotonized-central limiter (reading R27): exact on linear data, flat at
+    extrema, face values bounded by the neighbouring cells, mirror symmetric, slope never above
+    twice either one-sided difference, second-order on smooth monotone data."""
+    rng = np.random.default_rng(17)
+    for _ in range(200):
+        a, b = rng.uniform(-2, 2, 2)
+        q = a + b * np.arange(-2, 3)
+        qm, qp = po.reconstruct(3, q)
+        assert abs(qm - (a - 0.5 * b)) < 1e-14 and abs(qp - (a + 0.5 * b)) < 1e-14
+    for _ in range(500):
+        q = rng.uniform(-1, 1, 5)
+        qm, qp = po.reconstruct(3, q)
+        dl, dr = q[2] - q[1], q[3] - q[2]
+        if dl * dr <= 0:
+            assert qm == q[2] and qp == q[2]
+        else:
+            s = qp - qm
+            assert abs(s) <= 2 * abs(dl) + 1e-15 and abs(s) <= 2 * abs(dr) + 1e-15
+            assert min(q[1], q[2]) - 1e-15 <= qm <= max(q[1], q[2]) + 1e-15
+            assert min(q[2], q[3]) - 1e-15 <= qp <= max(q[2], q[3]) + 1e-15
+            assert abs(0.5 * (qm + qp) - q[2]) < 1e-15
+        rm, rp = po.reconstruct(3, q[::-1].copy())
+        assert rm == qp and rp == qm
+    errs = []
+    for n in (16, 32):
+        h = 1.0 / n
+        x = 0.3 + (np.arange(-2, 3)) * h
+        qm, qp = po.reconstruct(3, np.exp(x))       # monotone: the limiter leaves the central slope
+        errs.append(abs(qp - np.exp(0.3 + 0.5 * h)))
+    assert 3.5 < errs[0] / errs[1] < 4.5
