@@ -135,6 +135,12 @@ int ak_rhs(ak_ctx*, const ak_cons* U, const ak_faceB* Bf, const ak_prim* W, int 
  * (AK_ESTATE if there are none) and the primitives W. */
 int ak_emf(ak_ctx*, const ak_prim* W, double* Ex, double* Ey, double* Ez);
 
+/* Matter terms a spacetime (Z4c) right-hand side needs from the fluid ("E = tau + D ...
+ * S_ij = T_ij"): E, S_i, S_ij, undensitised, at every stored cell, from the primitives W
+ * and the metric set with ak_set_metric.  Ten caller-owned device cell fields. */
+typedef struct { double *E, *Sx, *Sy, *Sz, *Sxx, *Sxy, *Sxz, *Syy, *Syz, *Szz; } ak_matter;
+int ak_matter_sources(ak_ctx*, const ak_prim* W, const ak_matter* out);
+
 /* Copy the device counters to the host.  Synchronises the stream. */
 int ak_get_stats(ak_ctx*, ak_stats* host_out);
 

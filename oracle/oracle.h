@@ -104,6 +104,11 @@ void orc_rhs(const orc_params* p, const double* dx, double* const U[5],
              double* const flux_out[21], unsigned char* const face_refluxed[3],
              int nthreads);
 
+/* Matter terms for a spacetime solver: out[10] = E = tau + D, S_i, S_ij = T_ij,
+ * undensitised, at every stored cell, from the primitives W and gamma_ij. */
+void orc_matter_sources(const orc_params* p, const double* const W[8], const double* const g6[6],
+                        double* const out[10]);
+
 /* Same stage with the FOFC estimate of a later Runge-Kutta stage (R9):
  * U* = fa * U0 + fb * (U - dt_fofc div F) when U0 != NULL. */
 void orc_rhs_blend(const orc_params* p, const double* dx, double* const U[5],

@@ -229,3 +229,11 @@ def advance_nbr(par, dx, integrator, nsteps, dt, bc, nbr, U, Bf, adm, nthreads=1
                           _ib(bc), ap, _ptrs(U), _ptrs(Bf), _ptrs(adm), _ptrs(W),
                           flag.ctypes.data_as(C.c_void_p), int(nthreads))
     return W, flag
+
+
+def matter_sources(par, W, g6):
+    """E, S_i, S_ij (10 cell arrays, undensitised) from the primitives."""
+    sh = shapes(par.nmb, par.n)
+    out = [np.zeros(sh["cell"]) for _ in range(10)]
+    lib().orc_matter_sources(C.byref(par), _ptrs(W), _ptrs(g6), _ptrs(out))
+    return out

@@ -346,6 +346,45 @@ void run_blocks(int nmb, int nthreads, const std::function<void(int)>& fn) {
 }
 }  // namespace
 
+// Matter terms a spacetime solver needs from the fluid ("E = tau + D ... S_ij = T_ij";
+// P:129 "the matter source terms ... for the Z4c equations"): E, S_i, S_ij (undensitised) at
+// every stored cell from the cell-centred primitives.  out[10] = E, Sx, Sy, Sz, Sxx, Sxy, Sxz, Syy, Syz, Szz.
+extern "C" void orc_matter_sources(const orc_params* p, const double* const W[8],
+                                   const double* const g6[6], double* const out[10]) {
+  const Geo G(p->n, p->ng);
+  const long ncell = (long)p->nmb * G.ncell;
+  for (long c = 0; c < ncell; ++c) {
+    double g[6], det, sdet, gi[6];
+    for (int q = 0; q < 6; ++q) g[q] = g6[q][c];
+    orc_metric_inverse(g, &det, &sdet, gi);
+    const double isd = 1.0 / sdet;
+    const double prim[5] = {W[0][c], W[1][c], W[2][c], W[3][c], W[4][c]};
+    const double B[3] = {W[5][c] * isd, W[6][c] * isd, W[7][c] * isd};
+    double cons[5];
+    orc_prim2cons(p->gamma_ad, g, prim, B, cons);
+    const double rho = prim[0], P = prim[4];
+    const double u[3] = {prim[1], prim[2], prim[3]};
+    const double ul[3] = {g[0] * u[0] + g[1] * u[1] + g[2] * u[2], g[1] * u[0] + g[3] * u[1] + g[4] * u[2],
+                          g[2] * u[0] + g[4] * u[1] + g[5] * u[2]};
+    const double usq = ul[0] * u[0] + ul[1] * u[1] + ul[2] * u[2];
+    const double iW = 1.0 / std::sqrt(1.0 + usq);
+    const double Bl[3] = {g[0] * B[0] + g[1] * B[1] + g[2] * B[2], g[1] * B[0] + g[3] * B[1] + g[4] * B[2],
+                          g[2] * B[0] + g[4] * B[1] + g[5] * B[2]};
+    const double B2 = Bl[0] * B[0] + Bl[1] * B[1] + Bl[2] * B[2];
+    const double vl[3] = {ul[0] * iW, ul[1] * iW, ul[2] * iW};
+    const double Bv = B[0] * vl[0] + B[1] * vl[1] + B[2] * vl[2];
+    const double b2 = B2 * iW * iW + Bv * Bv;
+    const double bl[3] = {Bl[0] * iW + Bv * ul[0], Bl[1] * iW + Bv * ul[1], Bl[2] * iW + Bv * ul[2]};
+    const double h = 1.0 + p->gamma_ad / (p->gamma_ad - 1.0) * (P / rho);
+    const double Ptot = P + 0.5 * b2;
+    const double wt = rho * h + b2;
+    out[0][c] = cons[4] + cons[0];
+    out[1][c] = cons[1]; out[2][c] = cons[2]; out[3][c] = cons[3];
+    const int I[6] = {0, 0, 0, 1, 1, 2}, J[6] = {0, 1, 2, 1, 2, 2};
+    for (int q = 0; q < 6; ++q) out[4 + q][c] = wt * ul[I[q]] * ul[J[q]] + Ptot * g[q] - bl[I[q]] * bl[J[q]];
+  }
+}
+
 extern "C" void orc_con2prim(const orc_params* p, double* const U[5], const double* const Bf[3],
                              const double* const g[6], double* const W[8],
                              unsigned char* status, int nthreads) {

@@ -21,7 +21,7 @@ KERNEL_CLASSES = ("con2prim", "flux_x", "flux_y", "flux_z", "fofc_test", "fofc_f
 EXPORTS = ("ak_create", "ak_set_metric", "ak_con2prim", "ak_rhs", "ak_emf", "ak_get_stats",
            "ak_get_flux", "ak_rhs_host", "ak_timing", "ak_kernel_ms", "ak_probe_copy",
            "ak_probe_fp64", "ak_destroy", "ak_strerror", "ak_version",
-           "ak_set_fofc_blend", "ak_fill_ghosts", "ak_stage_update", "ak_advance", "ak_set_neighbors")
+           "ak_set_fofc_blend", "ak_fill_ghosts", "ak_stage_update", "ak_advance", "ak_set_neighbors", "ak_matter_sources")
 BC_PERIODIC, BC_OUTFLOW = 0, 1
 
 _dp = C.POINTER(C.c_double)
@@ -56,6 +56,10 @@ class AkAdm(C.Structure):
 class AkRhsOut(C.Structure):
     _fields_ = [(k, C.c_void_p) for k in ("dD", "dSx", "dSy", "dSz", "dtau", "Ex", "Ey", "Ez",
                                           "fofc_flag", "c2p_status")]
+
+
+class AkMatter(C.Structure):
+    _fields_ = [(k, C.c_void_p) for k in ("E", "Sx", "Sy", "Sz", "Sxx", "Sxy", "Sxz", "Syy", "Syz", "Szz")]
 
 
 class AkStats(C.Structure):
@@ -106,6 +110,7 @@ def lib():
                                       C.POINTER(AkRhsOut)]
         L.ak_advance.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double, C.POINTER(C.c_int), C.POINTER(AkCons),
                                  C.POINTER(AkFaceB), C.POINTER(AkPrim), C.c_void_p]
+        L.ak_matter_sources.argtypes = [C.c_void_p, C.POINTER(AkPrim), C.POINTER(AkMatter)]
         L.ak_set_neighbors.argtypes = [C.c_void_p, C.POINTER(C.c_int)]
         _lib = L
     return _lib
@@ -266,7 +271,12 @@ def ak_advance(ctx, integrator, nsteps, dt, bc, U, Bf, W, flag_or=None):
 def ak_set_neighbors(ctx, nbr):
     """nbr: int array [nmb][27] (host) or None."""
     if nbr is None:
-        _chk(lib().ak_set_neighbors(ctx, None), "ak_set_neighbors")
+        _chk(lib().ak_set_neighbors(ctx, None), "ak_set_neighbors", "ak_matter_sources")
         return
     a = np.ascontiguousarray(nbr, dtype=np.int32)
-    _chk(lib().ak_set_neighbors(ctx, a.ctypes.data_as(C.POINTER(C.c_int))), "ak_set_neighbors")
+    _chk(lib().ak_set_neighbors(ctx, a.ctypes.data_as(C.POINTER(C.c_int))), "ak_set_neighbors", "ak_matter_sources")
+
+
+def ak_matter_sources(ctx, W, out10):
+    w, o = _struct(AkPrim, W), _struct(AkMatter, out10)
+    _chk(lib().ak_matter_sources(ctx, C.byref(w), C.byref(o)), "ak_matter_sources")

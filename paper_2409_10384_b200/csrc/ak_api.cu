@@ -507,6 +507,20 @@ int ak_emf(ak_ctx* c, const ak_prim* W, double* Ex, double* Ey, double* Ez) {
   return launch_ct(c, f);
 }
 
+int ak_matter_sources(ak_ctx* c, const ak_prim* W, const ak_matter* out) {
+  if (!c || !out) return AK_EINVAL;
+  if (!c->have_metric) return AK_ESTATE;
+  Fields f;
+  fill_fields(c, f);
+  if (!set_prim(f, W)) return AK_EINVAL;
+  MatterOut o = {{out->E, out->Sx, out->Sy, out->Sz, out->Sxx, out->Sxy, out->Sxz, out->Syy, out->Syz, out->Szz}};
+  for (int q = 0; q < 10; ++q) if (!o.q[q]) return AK_EINVAL;
+  CK(cudaSetDevice(c->hp.device));
+  k_matter<<<nblk(c->sz.cell, 128), 128, 0, c->stream>>>(c->P, f, o);
+  CK(cudaGetLastError());
+  return AK_OK;
+}
+
 int ak_get_stats(ak_ctx* c, ak_stats* o) {
   if (!c || !o) return AK_EINVAL;
   if (c->stats_from_host) { *o = c->host_acc; return AK_OK; }

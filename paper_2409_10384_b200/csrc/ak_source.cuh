@@ -105,4 +105,44 @@ __global__ void __launch_bounds__(128, AK_SRC_MINB) k_div_src(const __grid_const
   for (int v = 0; v < 5; ++v) f.dU[v][c] = du[v];
 }
 
+// ---- matter terms for a spacetime solver: E = tau + D, S_i, S_ij = T_ij, undensitised,
+// at every stored cell from the cell-centred primitives ----------------------------------------------
+struct MatterOut { double* q[10]; };   // E, Sx, Sy, Sz, Sxx, Sxy, Sxz, Syy, Syz, Szz
+
+__global__ void __launch_bounds__(128) k_matter(const __grid_constant__ Par P, const __grid_constant__ Fields f,
+                                                const __grid_constant__ MatterOut o) {
+  const long long ncell = (long long)P.nmb * P.nt * P.nt * P.nt;
+  const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= ncell) return;
+  Met3 g, gu;
+  load_met3(f, c, g);
+  double det, sdet;
+  metric_inverse(g, det, sdet, gu);
+  const double isd = 1.0 / sdet;
+  const double rho = f.W[0][c], pr = f.W[4][c];
+  const double u[3] = {f.W[1][c], f.W[2][c], f.W[3][c]};
+  const double B[3] = {f.W[5][c] * isd, f.W[6][c] * isd, f.W[7][c] * isd};
+  double cons[5];
+  prim2cons(P, g, rho, u, pr, B, cons);
+  double ul[3], Bl[3];
+  lower(g, u, ul);
+  const double usq = dot3(ul, u);
+  const double iW = 1.0 / sqrt(1.0 + usq);
+  lower(g, B, Bl);
+  const double B2 = dot3(Bl, B);
+  const double vl[3] = {ul[0] * iW, ul[1] * iW, ul[2] * iW};
+  const double Bv = B[0] * vl[0] + B[1] * vl[1] + B[2] * vl[2];
+  const double b2 = B2 * iW * iW + Bv * Bv;
+  const double bl[3] = {Bl[0] * iW + Bv * ul[0], Bl[1] * iW + Bv * ul[1], Bl[2] * iW + Bv * ul[2]};
+  const double h = 1.0 + P.Gam / (P.Gam - 1.0) * (pr / rho);
+  const double Ptot = pr + 0.5 * b2;
+  const double wt = rho * h + b2;
+  o.q[0][c] = cons[4] + cons[0];
+  o.q[1][c] = cons[1]; o.q[2][c] = cons[2]; o.q[3][c] = cons[3];
+  const double gd[6] = {g.xx, g.xy, g.xz, g.yy, g.yz, g.zz};
+  constexpr int I6[6] = {0, 0, 0, 1, 1, 2}, J6[6] = {0, 1, 2, 1, 2, 2};
+#pragma unroll
+  for (int q = 0; q < 6; ++q) o.q[4 + q][c] = wt * ul[I6[q]] * ul[J6[q]] + Ptot * gd[q] - bl[I6[q]] * bl[J6[q]];
+}
+
 }  // namespace ak

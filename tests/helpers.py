@@ -51,7 +51,7 @@ def tensor_state(alpha, beta_u, g6, rho, v_u, P, B_u, Gamma):
         F[j, 1:4] = alpha * T_ud[1 + j, 1:]
         F[j, 4] = alpha * (alpha * T[0, 1 + j] - rho * u[1 + j])
         F[j, 5:8] = alpha * Fd[1:, 1 + j]
-    return U, sg * F, dict(W=W, h=h, b2=b2, sg=sg)
+    return U, sg * F, dict(W=W, h=h, b2=b2, sg=sg, T=T, g4=g4, alpha=alpha)
 
 
 def slots(d):

@@ -269,3 +269,19 @@ def test_host_entry_point_pipelined_chunks():
             assert np.array_equal(hflag.numpy(), ra["flag"]) and np.array_equal(hst.numpy(), ra["status"])
             assert a.stats() == sa
         assert np.count_nonzero(ra["flag"]) > 0
+
+
+def test_matter_sources():
+    """E, S_i, S_ij for a spacetime solver against the oracle, curved C3 blocks."""
+    import torch
+    from paper_2409_10384_b200 import ak
+    w = wl.make_blocks("C3", blocks=[192 + 21, 64 + 21, 21])
+    with gpukit.GpuStage(copy.deepcopy(w)) as g:
+        g.con2prim()
+        out = [torch.zeros_like(g.W[0]) for _ in range(10)]
+        ak.ak_matter_sources(g.ctx, g.W, out)
+        torch.cuda.synchronize()
+        Wn = [t.cpu().numpy() for t in g.W]
+        exp = orc.matter_sources(orc.make_params(**w["params"]), Wn, w["adm"][:6])
+        for a, b in zip(out, exp):
+            assert np.array_equal(a.cpu().numpy(), b)

@@ -106,3 +106,53 @@ def test_T9_ct_reduces_to_face_emf_in_1d():
     Fx_By = r["flux"][5][0, s, :, :][:, sk.NG - 1:sk.NG + N + 1, s1]   # F^x(B~^y), slot t1
     # E_z on x-faces = -F^x(B~^y); rows j-1 and j are identical for y-uniform data
     assert np.abs(Ez - (-Fx_By[:, 1:, :])).max() <= 1e-15
+
+
+def test_T28_matter_sources_equal_projections_of_the_stress_energy_tensor():
+    """E = n_mu n_nu T^{mu nu}, S_i = -gamma_i^mu n^nu T_{mu nu}, S_ij = T_ij (P:119) with T^{mu nu}
+    built from Eqs. 2, 7 and the full 4-metric (tests/helpers.py), random metrics with shift."""
+    import helpers as H
+    from oracle import pyoracle as po
+    rng = np.random.default_rng(28)
+    n = 2
+    par = po.make_params(nmb=1, n=n, gamma_ad=5.0 / 3.0)
+    sh = po.shapes(1, n)
+    W = [np.zeros(sh["cell"]) for _ in range(8)]
+    g6 = [np.zeros(sh["cell"]) for _ in range(6)]
+    exp = [np.zeros(sh["cell"]) for _ in range(10)]
+    nt = n + 8
+    for k in range(nt):
+        for j in range(nt):
+            for i in range(0, nt, 3):
+                g = H.random_spd(rng)
+                alpha = rng.uniform(0.3, 1.5); beta = rng.uniform(-0.3, 0.3, 3)
+                rho = 10 ** rng.uniform(-6, 0); P = rho * 10 ** rng.uniform(-3, 1)
+                gm = H.sym6_to_mat(g)
+                v = rng.uniform(-1, 1, 3); v *= rng.uniform(0, 0.9) / np.sqrt(v @ gm @ v)
+                B = rng.uniform(-1, 1, 3) * 10 ** rng.uniform(-3, 0)
+                U, F, d = H.tensor_state(alpha, beta, g, rho, v, P, B, 5.0 / 3.0)
+                T, g4 = d["T"], d["g4"]
+                Tdd = g4 @ T @ g4
+                nl = np.array([-alpha, 0, 0, 0]); nu_ = np.concatenate([[1 / alpha], -beta / alpha])
+                E = nl @ T @ nl
+                Si = -(Tdd[1:, :] @ nu_)
+                Sij = Tdd[1:, 1:]
+                Wl = d["W"]
+                vals = [rho, Wl * v[0], Wl * v[1], Wl * v[2], P] + list(d["sg"] * B)
+                for q, a in enumerate(vals):
+                    W[q][0, k, j, i] = a
+                for q in range(6):
+                    g6[q][0, k, j, i] = g[q]
+                e = [E, Si[0], Si[1], Si[2]] + [Sij[a_, b_] for (a_, b_) in H.SYM]
+                for q in range(10):
+                    exp[q][0, k, j, i] = e[q]
+    # unset cells: harmless flat-space fluid at rest
+    for q, a in enumerate((1.0, 0, 0, 0, 1.0, 0, 0, 0)):
+        W[q][W[0] == 0] = a
+    for q, a in enumerate((1.0, 0, 0, 1.0, 0, 1.0)):
+        g6[q][g6[0] == 0] = a
+    out = po.matter_sources(par, W, g6)
+    mask = exp[0] != 0
+    for q in range(10):
+        scale = np.abs(exp[0][mask]) + np.abs(exp[q][mask])
+        assert np.max(np.abs(out[q][mask] - exp[q][mask]) / scale) < 1e-12, q
