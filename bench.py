@@ -45,7 +45,7 @@ ALG_BYTES = dict(con2prim=(5 + 3 + 6 + 8) * 8 + 1, flux=(7 + 10 + 1 + 7) * 8, fo
 # differ by < 1 %): DADD + DMUL + DFMA of the straight-line face path in the SASS of k_flux_tma
 # (cuobjdump), which equals a hand count of DESIGN.md §3 O4-O6 with a division = 8 and a square
 # root = 9 pipe instructions (their correctly rounded Newton sequences).  DESIGN.md §7.
-FLUX_FP64_PER_FACE = {0: 634, 1: 928, 2: 1810, 3: 752}
+FLUX_FP64_PER_FACE = {0: 634, 1: 928, 2: 1810, 3: 752, 4: 1600}   # 4 (PPMX): static count over both limiter branches, an upper bound
 # fp64 pipe peak: 148 SMs x 4 sub-partitions x 16 fp64 lanes x 1.965 GHz (one instruction per lane
 # per clock; an FMA counts once).  The same-run probe (ak_probe_fp64) measures 18.4-18.5.
 FP64_PIPE_PEAK_TINST = 148 * 4 * 16 * 1.965e9 * 1e-12

@@ -50,7 +50,7 @@ extern "C" {
 typedef struct ak_ctx ak_ctx; /* opaque */
 
 enum { AK_OK = 0, AK_EINVAL = -1, AK_ENOMEM = -2, AK_ECUDA = -3, AK_ESTATE = -4 };
-enum { AK_RECON_DC = 0, AK_RECON_PPM4 = 1, AK_RECON_WENOZ = 2, AK_RECON_PLM = 3 };
+enum { AK_RECON_DC = 0, AK_RECON_PPM4 = 1, AK_RECON_WENOZ = 2, AK_RECON_PLM = 3, AK_RECON_PPMX = 4 };
 enum { AK_RS_LLF = 0, AK_RS_HLLE = 1 };
 enum { AK_BC_PERIODIC = 0, AK_BC_OUTFLOW = 1 };                  /* stage driver, D:§11 */
 enum { AK_RK1 = 1, AK_RK2 = 2, AK_RK3 = 3 };                     /* SSP Runge-Kutta */

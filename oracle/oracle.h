@@ -39,7 +39,7 @@ typedef struct {
   double gamma_ad;               /* ideal-gas Gamma                          */
   double rho_atm, T_atm, f_thr;
   double mag_max;                /* M_max of P:139 (+inf disables)           */
-  int recon;                     /* 0 donor cell, 1 PPM4, 2 WENO-Z, 3 PLM */
+  int recon;                     /* 0 donor cell, 1 PPM4, 2 WENO-Z, 3 PLM, 4 PPMX */
   int riemann;                   /* 0 LLF, 1 HLLE                    */
   int fofc, fofc_riemann;
   double dmp_M;                  /* Eq. 12; <=0 off                          */

@@ -14,7 +14,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 SO_PATH = os.environ.get("AK_LIBRARY") or os.path.join(_HERE, "libak.so")   # AK_LIBRARY: another build of the same library
 
 AK_OK, AK_EINVAL, AK_ENOMEM, AK_ECUDA, AK_ESTATE = 0, -1, -2, -3, -4
-RECON_DC, RECON_PPM4, RECON_WENOZ, RECON_PLM = 0, 1, 2, 3
+RECON_DC, RECON_PPM4, RECON_WENOZ, RECON_PLM, RECON_PPMX = 0, 1, 2, 3, 4
 RS_LLF, RS_HLLE = 0, 1
 ST_DFLOOR, ST_TAUFLOOR, ST_MAGCAP, ST_RHOFLOOR, ST_TFLOOR, ST_FAIL, ST_DMP = 1, 2, 4, 8, 16, 32, 64
 KERNEL_CLASSES = ("con2prim", "flux_x", "flux_y", "flux_z", "fofc_test", "fofc_fix", "ct", "div_src")

@@ -90,7 +90,7 @@ int validate(const ak_params* p, const double* dx3) {
   if (!(std::isfinite(p->gamma_ad) && p->gamma_ad > 1.0)) return AK_EINVAL;
   if (!finite_pos(p->rho_atm) || !finite_pos(p->T_atm) || !finite_pos(p->f_thr)) return AK_EINVAL;
   if (!(p->mag_max > 0.0)) return AK_EINVAL;   // +inf allowed, NaN rejected
-  if (p->recon < 0 || p->recon > 3 || p->riemann < 0 || p->riemann > 1) return AK_EINVAL;
+  if (p->recon < 0 || p->recon > 4 || p->riemann < 0 || p->riemann > 1) return AK_EINVAL;
   if (p->fofc < 0 || p->fofc > 1 || p->fofc_riemann < 0 || p->fofc_riemann > 1) return AK_EINVAL;
   if (std::isnan(p->dmp_M) || (p->dmp_M > 0.0 && p->dmp_M < 1.0)) return AK_EINVAL;
   if (p->c2p_max_iter < 1 || p->c2p_max_iter > 1000) return AK_EINVAL;
@@ -205,6 +205,7 @@ int launch_flux(ak_ctx* c, const Fields& f) {
         case 0: r = launch_flux_tma<DIR, 0>(c, f, NA, grid, smem); break;
         case 1: r = launch_flux_tma<DIR, 1>(c, f, NA, grid, smem); break;
         case 3: r = launch_flux_tma<DIR, 3>(c, f, NA, grid, smem); break;
+        case 4: r = launch_flux_tma<DIR, 4>(c, f, NA, grid, smem); break;
         default: r = launch_flux_tma<DIR, 2>(c, f, NA, grid, smem); break;
       }
       if (r != AK_OK) return r;
@@ -232,6 +233,7 @@ int launch_flux(ak_ctx* c, const Fields& f) {
     case 0: k_flux_tile<DIR, 0><<<g, bd, smem, c->stream>>>(c->P, f, NA, NB); break;
     case 1: k_flux_tile<DIR, 1><<<g, bd, smem, c->stream>>>(c->P, f, NA, NB); break;
     case 3: k_flux_tile<DIR, 3><<<g, bd, smem, c->stream>>>(c->P, f, NA, NB); break;
+    case 4: k_flux_tile<DIR, 4><<<g, bd, smem, c->stream>>>(c->P, f, NA, NB); break;
     default: k_flux_tile<DIR, 2><<<g, bd, smem, c->stream>>>(c->P, f, NA, NB); break;
   }
 #else
@@ -241,6 +243,7 @@ int launch_flux(ak_ctx* c, const Fields& f) {
     case 0: k_flux<DIR, 0><<<g, 128, 0, c->stream>>>(c->P, f); break;
     case 1: k_flux<DIR, 1><<<g, 128, 0, c->stream>>>(c->P, f); break;
     case 3: k_flux<DIR, 3><<<g, 128, 0, c->stream>>>(c->P, f); break;
+    case 4: k_flux<DIR, 4><<<g, 128, 0, c->stream>>>(c->P, f); break;
     default: k_flux<DIR, 2><<<g, 128, 0, c->stream>>>(c->P, f); break;
   }
 #endif

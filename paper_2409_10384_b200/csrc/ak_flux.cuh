@@ -38,6 +38,42 @@ __device__ __forceinline__ void recon(double qmm, double qm1, double q0, double 
     }
     qm = q0 - 0.5 * sl;
     qp = q0 + 0.5 * sl;
+  } else if (KIND == 4) {
+    // PPMX: PPM with the extremum-preserving limiter of Colella & Sekora (2008), C = 1.25
+    // ("a newer variant with an extrema-preserving limiter"; reading R28).
+    const double C2 = 1.25, c12 = 1.0 / 12.0;
+    // (1) fourth-order interface values, limited where they leave the range of the two cells
+    double ql = (7.0 * (qm1 + q0) - (qmm + qp1)) * c12;
+    double qr = (7.0 * (q0 + qp1) - (qm1 + qpp)) * c12;
+    const double dL = qmm - 2.0 * qm1 + q0, dC = qm1 - 2.0 * q0 + qp1, dR = q0 - 2.0 * qp1 + qpp;
+    if ((ql - qm1) * (q0 - ql) < 0.0) {
+      const double d2 = 3.0 * (qm1 - 2.0 * ql + q0);
+      double lim = 0.0;
+      if (d2 * dL > 0.0 && d2 * dC > 0.0) lim = copysign(fmin(fmin(C2 * fabs(dL), C2 * fabs(dC)), fabs(d2)), d2);
+      ql = 0.5 * (qm1 + q0) - lim * (1.0 / 6.0);
+    }
+    if ((qr - q0) * (qp1 - qr) < 0.0) {
+      const double d2 = 3.0 * (q0 - 2.0 * qr + qp1);
+      double lim = 0.0;
+      if (d2 * dC > 0.0 && d2 * dR > 0.0) lim = copysign(fmin(fmin(C2 * fabs(dC), C2 * fabs(dR)), fabs(d2)), d2);
+      qr = 0.5 * (q0 + qp1) - lim * (1.0 / 6.0);
+    }
+    // (2) the parabola: at a local extremum scale both deviations by the ratio of limited to
+    // actual second derivative; elsewhere the usual no-overshoot rule
+    const double dm = ql - q0, dp = qr - q0;
+    if (dp * dm >= 0.0 || (qp1 - q0) * (q0 - qm1) <= 0.0) {
+      const double d2 = 6.0 * (ql + qr) - 12.0 * q0;
+      double lim = 0.0;
+      if (d2 * dL > 0.0 && d2 * dC > 0.0 && d2 * dR > 0.0)
+        lim = copysign(fmin(fmin(C2 * fabs(dL), C2 * fabs(dR)), fmin(C2 * fabs(dC), fabs(d2))), d2);
+      const double ratio = d2 != 0.0 ? lim / d2 : 0.0;
+      ql = q0 + dm * ratio;
+      qr = q0 + dp * ratio;
+    } else {
+      if (fabs(dp) >= 2.0 * fabs(dm)) qr = q0 - 2.0 * dm;
+      else if (fabs(dm) >= 2.0 * fabs(dp)) ql = q0 - 2.0 * dp;
+    }
+    qm = ql; qp = qr;
   } else {                    // WENO-Z (Borges et al. 2008), p = 2, eps = 1e-40
     const double c6 = 1.0 / 6.0, c1312 = 13.0 / 12.0, eps = 1e-40;
     const double a0 = qmm - 2.0 * qm1 + q0, a1 = qm1 - 2.0 * q0 + qp1, a2 = q0 - 2.0 * qp1 + qpp;

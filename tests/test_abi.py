@@ -45,7 +45,7 @@ def good_params(**kw):
 
 
 @pytest.mark.parametrize("bad", [dict(n=1), dict(ng=3), dict(gamma_ad=1.0), dict(rho_atm=-1.0), dict(T_atm=0.0),
-                                 dict(f_thr=float("nan")), dict(mag_max=0.0), dict(recon=4), dict(riemann=2),
+                                 dict(f_thr=float("nan")), dict(mag_max=0.0), dict(recon=5), dict(riemann=2),
                                  dict(fofc=2), dict(dmp_M=0.5), dict(c2p_max_iter=0), dict(c2p_tol=0.0),
                                  dict(device=-1), dict(nmb=0), dict(nmb=40000, n=32)])
 def test_create_rejects_bad_params_before_cuda(lib, bad):

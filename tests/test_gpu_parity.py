@@ -48,7 +48,7 @@ def test_c0_full():
     assert np.count_nonzero(o["flag"]) == 0          # smooth: the empty-list path
 
 
-@pytest.mark.parametrize("recon", [0, 1, 2, 3])
+@pytest.mark.parametrize("recon", [0, 1, 2, 3, 4])
 @pytest.mark.parametrize("riemann", [0, 1])
 def test_c0_variants(recon, riemann):
     w = wl.make_blocks("C0")
@@ -67,7 +67,7 @@ def test_noise_block_flags(seed, dmp):
     assert bool(np.any(o["flag"] & 64)) == bool(dmp)
 
 
-@pytest.mark.parametrize("recon", [1, 2, 3])
+@pytest.mark.parametrize("recon", [1, 2, 3, 4])
 def test_noise_block_floors(recon):
     """Atmosphere raised above the low-density cells: D floor, rho floor, T floor and tau floor
     fire in con2prim (status bytes), the face-state floor fires after reconstruction."""

@@ -425,7 +425,12 @@ def test_T17_ppm4_limiter_properties():
         q = rng.normal(size=5)
         qm, qp = po.reconstruct(1, q)
         lo, hi = min(q[1:4]), max(q[1:4])
-        assert lo - 1e-14 <= qm <= hi + 1e-14 and lo - 1e-14 <= qp <= hi + 1e-14
+        if (q[3] - q[2]) * (q[2] - q[1]) > 0:             # monotone cell: faces stay in range
+            assert lo - 1e-14 <= qm <= hi + 1e-14 and lo - 1e-14 <= qp <= hi + 1e-14
+            assert (qp - q[2]) * (q[2] - qm) >= -1e-15    # and the profile in the cell is monotone
+        else:                                             # extremum: overshoot bounded by C |D2 a_C| / 6
+            dC = abs(q[1] - 2 * q[2] + q[3])
+            assert max(abs(qm - q[2]), abs(qp - q[2])) <= max(1.25 * dC / 6.0, hi - lo) + 1e-14
         if (q[3] - q[2]) * (q[2] - q[1]) <= 0:           # local extremum -> flat
             assert qm == q[2] and qp == q[2]
         # mirror symmetry
@@ -516,3 +521,49 @@ def test_T17_plm_mc_limiter():
         qm, qp = po.reconstruct(3, np.exp(x))       # monotone: the limiter leaves the central slope
         errs.append(abs(qp - np.exp(0.3 + 0.5 * h)))
     assert 3.5 < errs[0] / errs[1] < 4.5
+
+
+def test_T17_ppmx_extremum_preserving():
+    """PPMX (Colella & Sekora 2008 limiter; reading R28): exact on monotone cubics, fourth
+    order AT a smooth extremum where PPM4 clips, no new extrema at jumps, mirror symmetric."""
+    rng = np.random.default_rng(41)
+    # cell averages of a monotone cubic: faces exact
+    for _ in range(100):
+        c = rng.uniform(0.5, 1.5, 4)                      # positive coefficients, x in [3, 8]: monotone
+        Pint = lambda x: c[0] * x + c[1] * x ** 2 / 2 + c[2] * x ** 3 / 3 + c[3] * x ** 4 / 4
+        f = lambda x: c[0] + c[1] * x + c[2] * x ** 2 + c[3] * x ** 3
+        x0 = 5.0
+        q = np.array([Pint(x0 + k + 0.5) - Pint(x0 + k - 0.5) for k in range(-2, 3)])
+        qm, qp = po.reconstruct(4, q)
+        assert abs(qm - f(x0 - 0.5)) < 1e-10 * abs(f(x0)) and abs(qp - f(x0 + 0.5)) < 1e-10 * abs(f(x0))
+    # smooth extremum: cell averages of cos(2 pi x) next to its maximum
+    def face_err(kind, n):
+        h = 1.0 / n; x0 = 0.013
+        avg = lambda xc: (np.sin(2 * np.pi * (xc + h / 2)) - np.sin(2 * np.pi * (xc - h / 2))) / (2 * np.pi * h)
+        q = np.array([avg(x0 + k * h) for k in range(-2, 3)])
+        qm, qp = po.reconstruct(kind, q)
+        return max(abs(qp - np.cos(2 * np.pi * (x0 + h / 2))), abs(qm - np.cos(2 * np.pi * (x0 - h / 2))))
+    e16, e32, e64 = (face_err(4, n) for n in (16, 32, 64))
+    assert e16 / e32 > 12 and e32 / e64 > 12
+    assert face_err(1, 16) > 10 * e16                      # the classic limiter flattens the extremum
+    # a single jump: nothing outside the range of the three nearest cells (the second differences
+    # change sign across it, so the limited second derivative vanishes)
+    for _ in range(300):
+        q = np.where(np.arange(5) < rng.integers(1, 5), 1.0, 0.1) * rng.uniform(0.5, 2)
+        if rng.uniform() < 0.5:
+            q = q[::-1].copy()
+        qm, qp = po.reconstruct(4, q)
+        lo, hi = min(q[1:4]), max(q[1:4])
+        assert lo - 1e-14 <= qm <= hi + 1e-14 and lo - 1e-14 <= qp <= hi + 1e-14
+    # noise: Colella-Sekora admit excursions only as large as the limited second derivative allows
+    # (C max|D2 a| / 6 beyond the neighbours' range); mirror symmetry always
+    for _ in range(2000):
+        q = rng.uniform(-1, 1, 5)
+        qm, qp = po.reconstruct(4, q)
+        lo, hi = min(q[1:4]), max(q[1:4])
+        d2 = max(abs(q[0] - 2 * q[1] + q[2]), abs(q[1] - 2 * q[2] + q[3]), abs(q[2] - 2 * q[3] + q[4]))
+        m = 1.25 * d2 / 6.0 + 1e-14
+        assert lo - m <= qm <= hi + m and lo - m <= qp <= hi + m
+        rm, rp = po.reconstruct(4, q[::-1].copy())
+        assert rm == qp and rp == qm
+    assert po.reconstruct(4, np.full(5, 0.7)) == (0.7, 0.7)
