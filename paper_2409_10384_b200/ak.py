@@ -21,7 +21,8 @@ KERNEL_CLASSES = ("con2prim", "flux_x", "flux_y", "flux_z", "fofc_test", "fofc_f
 EXPORTS = ("ak_create", "ak_set_metric", "ak_con2prim", "ak_rhs", "ak_emf", "ak_get_stats",
            "ak_get_flux", "ak_rhs_host", "ak_timing", "ak_kernel_ms", "ak_probe_copy",
            "ak_probe_fp64", "ak_destroy", "ak_strerror", "ak_version",
-           "ak_set_fofc_blend", "ak_fill_ghosts", "ak_stage_update", "ak_advance", "ak_set_neighbors", "ak_matter_sources")
+           "ak_set_fofc_blend", "ak_fill_ghosts", "ak_stage_update", "ak_advance", "ak_set_neighbors",
+           "ak_matter_sources")
 BC_PERIODIC, BC_OUTFLOW = 0, 1
 
 _dp = C.POINTER(C.c_double)
@@ -271,10 +272,10 @@ def ak_advance(ctx, integrator, nsteps, dt, bc, U, Bf, W, flag_or=None):
 def ak_set_neighbors(ctx, nbr):
     """nbr: int array [nmb][27] (host) or None."""
     if nbr is None:
-        _chk(lib().ak_set_neighbors(ctx, None), "ak_set_neighbors", "ak_matter_sources")
+        _chk(lib().ak_set_neighbors(ctx, None), "ak_set_neighbors")
         return
     a = np.ascontiguousarray(nbr, dtype=np.int32)
-    _chk(lib().ak_set_neighbors(ctx, a.ctypes.data_as(C.POINTER(C.c_int))), "ak_set_neighbors", "ak_matter_sources")
+    _chk(lib().ak_set_neighbors(ctx, a.ctypes.data_as(C.POINTER(C.c_int))), "ak_set_neighbors")
 
 
 def ak_matter_sources(ctx, W, out10):

@@ -159,10 +159,11 @@ bool set_prim(Fields& f, const ak_prim* W) {
   return true;
 }
 
-int launch_c2p(ak_ctx* c, const Fields& f) {
+int launch_c2p(ak_ctx* c, const Fields& f, bool with_emf) {
   Timer t(c, KC_C2P);
   CK(cudaMemsetAsync(c->stats, 0, sizeof(unsigned long long) * 3, c->stream));
-  k_con2prim<<<nblk(c->sz.cell, 128), 128, 0, c->stream>>>(c->P, f);
+  if (with_emf) k_con2prim<true><<<nblk(c->sz.cell, 128), 128, 0, c->stream>>>(c->P, f);
+  else k_con2prim<false><<<nblk(c->sz.cell, 128), 128, 0, c->stream>>>(c->P, f);
   c->launches[KC_C2P] += 1;
   CK(cudaGetLastError());
   return AK_OK;
@@ -279,17 +280,17 @@ int launch_fofc(ak_ctx* c, const Fields& f, double dt) {
   return AK_OK;
 }
 
-int launch_ct(ak_ctx* c, const Fields& f) {
+int launch_ct(ak_ctx* c, const Fields& f, bool have_cell_emf) {
   Timer t(c, KC_CT);
   const long long n = c->P.n;
   const long long ntest = (n + 2) * (n + 2) * (n + 2) * c->P.nmb;
   const long long ne = n * (n + 1) * (n + 1) * c->P.nmb;
-  k_cell_emf<<<nblk(ntest, 128), 128, 0, c->stream>>>(c->P, f);
+  if (!have_cell_emf) k_cell_emf<<<nblk(ntest, 128), 128, 0, c->stream>>>(c->P, f);
   k_ct<0><<<nblk(ne, 128), 128, 0, c->stream>>>(c->P, f);
   k_ct<1><<<nblk(ne, 128), 128, 0, c->stream>>>(c->P, f);
   k_ct<2><<<nblk(ne, 128), 128, 0, c->stream>>>(c->P, f);
   CK(cudaGetLastError());
-  c->launches[KC_CT] += 4;
+  c->launches[KC_CT] += have_cell_emf ? 3 : 4;
   return AK_OK;
 }
 
@@ -469,7 +470,7 @@ int ak_con2prim(ak_ctx* c, const ak_cons* U, const ak_faceB* Bf, const ak_prim* 
   if (!set_cons(f, U) || !set_faceB(f, Bf) || !set_prim(f, W)) return AK_EINVAL;
   f.status = status;
   CK(cudaSetDevice(c->hp.device));
-  return launch_c2p(c, f);
+  return launch_c2p(c, f, false);
 }
 
 int ak_rhs(ak_ctx* c, const ak_cons* U, const ak_faceB* Bf, const ak_prim* W, int w_is_valid, double dt_fofc,
@@ -489,13 +490,13 @@ int ak_rhs(ak_ctx* c, const ak_cons* U, const ak_faceB* Bf, const ak_prim* W, in
   CK(cudaSetDevice(c->hp.device));
   c->stats_from_host = false;
   int r;
-  if (!w_is_valid && (r = launch_c2p(c, f)) != AK_OK) return r;
+  if (!w_is_valid && (r = launch_c2p(c, f, true)) != AK_OK) return r;
   if ((r = launch_flux<0>(c, f)) != AK_OK) return r;
   if ((r = launch_flux<1>(c, f)) != AK_OK) return r;
   if ((r = launch_flux<2>(c, f)) != AK_OK) return r;
   if ((r = launch_fofc(c, f, dt_fofc)) != AK_OK) return r;
   c->have_flux = true;
-  if ((r = launch_ct(c, f)) != AK_OK) return r;
+  if ((r = launch_ct(c, f, !w_is_valid)) != AK_OK) return r;
   return launch_src(c, f);
 }
 
@@ -507,7 +508,7 @@ int ak_emf(ak_ctx* c, const ak_prim* W, double* Ex, double* Ey, double* Ez) {
   if (!set_prim(f, W)) return AK_EINVAL;
   f.E[0] = Ex; f.E[1] = Ey; f.E[2] = Ez;
   CK(cudaSetDevice(c->hp.device));
-  return launch_ct(c, f);
+  return launch_ct(c, f, false);
 }
 
 int ak_matter_sources(ak_ctx* c, const ak_prim* W, const ak_matter* out) {

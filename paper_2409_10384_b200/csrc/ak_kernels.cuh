@@ -62,6 +62,9 @@ __device__ __forceinline__ void load_met10(const Fields& f, long long c, double 
 }
 
 // ---- K1 ------------------------------------------------------------------------------
+// EMF: also write the cell-centred EMFs of the final primitives (the arithmetic of k_cell_emf), so
+// that a stage that runs part (1) does not re-read W and the metric for them.
+template <bool EMF>
 __global__ void __launch_bounds__(128, AK_C2P_MINB) k_con2prim(const __grid_constant__ Par P,
                                                   const __grid_constant__ Fields f) {
   const int nt = P.nt;
@@ -95,6 +98,19 @@ __global__ void __launch_bounds__(128, AK_C2P_MINB) k_con2prim(const __grid_cons
     for (int v = 0; v < 5; ++v) f.U[v][c] = Ut[v];
   }
   if (f.status) f.status[c] = (unsigned char)st;
+  if (EMF) {
+    const double u[3] = {W5[1], W5[2], W5[3]};
+    double ul[3];
+    lower(g, u, ul);
+    const double usq = dot3(ul, u);
+    const double iW = 1.0 / sqrt(1.0 + usq);
+    const double alp = __ldg(f.adm[6] + c), ialp = 1.0 / alp;
+    const double vh[3] = {u[0] * iW - __ldg(f.adm[7] + c) * ialp, u[1] * iW - __ldg(f.adm[8] + c) * ialp,
+                          u[2] * iW - __ldg(f.adm[9] + c) * ialp};
+    f.Ecc[0][c] = -(alp * (vh[1] * Bc[2] - vh[2] * Bc[1]));
+    f.Ecc[1][c] = -(alp * (vh[2] * Bc[0] - vh[0] * Bc[2]));
+    f.Ecc[2][c] = -(alp * (vh[0] * Bc[1] - vh[1] * Bc[0]));
+  }
   warp_count(f.stats + S_C2P_FAIL, (st & ST_FAIL) != 0);
   warp_count(f.stats + S_CONS_FLOOR, (st & (ST_DFLOOR | ST_TAUFLOOR | ST_MAGCAP)) != 0);
   warp_count(f.stats + S_PRIM_FLOOR, (st & (ST_RHOFLOOR | ST_TFLOOR)) != 0);
@@ -197,9 +213,13 @@ __global__ void __launch_bounds__(128, AK_FOFC_MINB) k_fofc_test(const __grid_co
   if (P.dmp_M > 0.0) {
     double Dmin = f.U[0][c], Dmax = Dmin, tmin = f.U[4][c], tmax = tmin;
     const long long sy = P.nt, sz = (long long)P.nt * P.nt;
-#pragma unroll
+#ifndef AK_DMP_UNROLL
+#define AK_DMP_UNROLL 1
+#endif
+    constexpr int dmp_unroll = AK_DMP_UNROLL;   // 1: the 27-cell loop stays rolled over k and j (smaller code)
+#pragma unroll dmp_unroll
     for (int kk = -1; kk <= 1; ++kk)
-#pragma unroll
+#pragma unroll dmp_unroll
       for (int jj = -1; jj <= 1; ++jj)
 #pragma unroll
         for (int ii = -1; ii <= 1; ++ii) {
