@@ -285,3 +285,56 @@ def test_matter_sources():
         exp = orc.matter_sources(orc.make_params(**w["params"]), Wn, w["adm"][:6])
         for a, b in zip(out, exp):
             assert np.array_equal(a.cpu().numpy(), b)
+
+
+def test_guard_zones_no_out_of_bounds_access():
+    """Every field the stage touches sits between two NaN-filled guard zones: the guards must still be
+    all-NaN afterwards (no stray write) and the results must equal the oracle (a stray read of a
+    guard would poison them).  Stands in for compute-sanitizer, which is closed on this pool.
+    n = 6 (per-face fallback kernels) and n = 8 with WENO-Z (TMA kernels); RK step included."""
+    import torch
+    from paper_2409_10384_b200 import ak
+    G = 4096
+    for n, recon in ((8, 2), (6, 1), (10, 4)):
+        w = wl.make_test_noise_block(seed=31, n=n, frac=0.03)
+        w["dt_fofc"] *= 2.0
+        p = dict(w["params"]); p.update(recon=recon, dmp_M=1.1)
+        sh = ak.shapes(1, n)
+        bigs = []
+
+        def guarded(arr=None, shape=None, dtype=torch.float64):
+            shape = arr.shape if arr is not None else shape
+            numel = int(np.prod(shape))
+            fill = float("nan") if dtype == torch.float64 else 0xAB
+            big = torch.full((numel + 2 * G,), fill, dtype=dtype, device="cuda:0")
+            v = big[G:G + numel].view(*shape)
+            if arr is not None:
+                v.copy_(torch.from_numpy(np.ascontiguousarray(arr)))
+            else:
+                v.zero_()
+            bigs.append((big, numel, dtype))
+            return v
+        U = [guarded(u) for u in w["U"]]; Bf = [guarded(b) for b in w["Bf"]]; adm = [guarded(a) for a in w["adm"]]
+        W = [guarded(shape=sh["cell"]) for _ in range(8)]; dU = [guarded(shape=sh["cell"]) for _ in range(5)]
+        E = [guarded(shape=sh[k]) for k in ("ex", "ey", "ez")]
+        flag = guarded(shape=sh["cell"], dtype=torch.uint8); status = guarded(shape=sh["cell"], dtype=torch.uint8)
+        ctx = ak.ak_create(ak.make_params(device=0, stream=torch.cuda.current_stream().cuda_stream, **p), w["dx"])
+        try:
+            ak.ak_set_metric(ctx, adm)
+            ak.ak_rhs(ctx, U, Bf, W, 0, w["dt_fofc"], dU, E, flag, status)
+            torch.cuda.synchronize()
+            Uo = [u.copy() for u in w["U"]]
+            o = orc.rhs(orc.make_params(**p), w["dx"], Uo, w["Bf"], w["adm"], w["dt_fofc"])
+            for a, b in zip(dU + E + W, o["dU"] + o["E"] + o["W"]):
+                assert np.array_equal(a.cpu().numpy(), b)
+            assert np.array_equal(flag.cpu().numpy(), o["flag"]) and np.count_nonzero(o["flag"]) > 0
+            ak.ak_advance(ctx, 3, 1, 0.1 / n, (0, 1, 0), U, Bf, W)
+            torch.cuda.synchronize()
+            for big, numel, dtype in bigs:
+                lo, hi = big[:G], big[G + numel:]
+                if dtype == torch.float64:
+                    assert bool(torch.isnan(lo).all()) and bool(torch.isnan(hi).all())
+                else:
+                    assert bool((lo == 0xAB).all()) and bool((hi == 0xAB).all())
+        finally:
+            ak.ak_destroy(ctx)
