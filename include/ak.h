@@ -170,8 +170,12 @@ int ak_set_fofc_blend(ak_ctx*, const ak_cons* U0, double a, double b);
  * adjacent at offset (ox,oy,oz) in {-1,0,1}^3, -1 = none (entry 13, the block itself, is ignored).
  * It is copied.  With a table set, ghosts whose offset block exists are copied from that block's
  * interior (the shared face ie+1 from the upper neighbour's face is); sides without a face
- * neighbour are physical and get bc[d].  Needs n >= 6.  nbr == NULL removes the table. */
-int ak_set_neighbors(ak_ctx*, const int* nbr);
+ * neighbour are physical and get bc[d].  Needs n >= 6.  nbr == NULL removes the table.
+ * nmb_total >= nmb (0 = nmb): the U~ and B~f arrays later passed to ak_fill_ghosts / ak_advance hold
+ * nmb_total blocks, of which only the first nmb are this context's; the others are read-only
+ * mirrors of blocks owned elsewhere (another GPU's shard, refreshed by the caller before each
+ * ghost fill — paper_2409_10384_b200/halo.py) and table entries may point at them. */
+int ak_set_neighbors(ak_ctx*, const int* nbr, int nmb_total);
 
 /* Fill the ghost cells of U~ and the ghost faces of B~f in place.  bc[d] = AK_BC_* per direction:
  * periodic (face ie+1 is made a copy of face is) or outflow (zero-gradient copies). */

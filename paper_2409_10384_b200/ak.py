@@ -112,7 +112,7 @@ def lib():
         L.ak_advance.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double, C.POINTER(C.c_int), C.POINTER(AkCons),
                                  C.POINTER(AkFaceB), C.POINTER(AkPrim), C.c_void_p]
         L.ak_matter_sources.argtypes = [C.c_void_p, C.POINTER(AkPrim), C.POINTER(AkMatter)]
-        L.ak_set_neighbors.argtypes = [C.c_void_p, C.POINTER(C.c_int)]
+        L.ak_set_neighbors.argtypes = [C.c_void_p, C.POINTER(C.c_int), C.c_int]
         _lib = L
     return _lib
 
@@ -269,13 +269,13 @@ def ak_advance(ctx, integrator, nsteps, dt, bc, U, Bf, W, flag_or=None):
                           C.byref(w), _ptr(flag_or)), "ak_advance")
 
 
-def ak_set_neighbors(ctx, nbr):
-    """nbr: int array [nmb][27] (host) or None."""
+def ak_set_neighbors(ctx, nbr, nmb_total=0):
+    """nbr: int array [nmb][27] (host) or None; nmb_total: blocks in the arrays incl. read-only mirrors."""
     if nbr is None:
-        _chk(lib().ak_set_neighbors(ctx, None), "ak_set_neighbors")
+        _chk(lib().ak_set_neighbors(ctx, None, 0), "ak_set_neighbors")
         return
     a = np.ascontiguousarray(nbr, dtype=np.int32)
-    _chk(lib().ak_set_neighbors(ctx, a.ctypes.data_as(C.POINTER(C.c_int))), "ak_set_neighbors")
+    _chk(lib().ak_set_neighbors(ctx, a.ctypes.data_as(C.POINTER(C.c_int)), int(nmb_total)), "ak_set_neighbors")
 
 
 def ak_matter_sources(ctx, W, out10):

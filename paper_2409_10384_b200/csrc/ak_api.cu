@@ -755,7 +755,7 @@ int ak_fill_ghosts(ak_ctx* c, const int bc[3], const ak_cons* U, const ak_faceB_
   return AK_OK;
 }
 
-int ak_set_neighbors(ak_ctx* c, const int* nbr) {
+int ak_set_neighbors(ak_ctx* c, const int* nbr, int nmb_total) {
   if (!c) return AK_EINVAL;
   CK(cudaSetDevice(c->hp.device));
   if (!nbr) {
@@ -766,7 +766,7 @@ int ak_set_neighbors(ak_ctx* c, const int* nbr) {
   const long long cnt = 27LL * c->P.nmb;
   if (c->P.n < 6) return AK_EINVAL;             // a ghost layer must come from owned elements only
   for (long long q = 0; q < cnt; ++q)
-    if (nbr[q] < -1 || nbr[q] >= c->P.nmb) return AK_EINVAL;
+    if (nbr[q] < -1 || nbr[q] >= (nmb_total > c->P.nmb ? nmb_total : c->P.nmb)) return AK_EINVAL;
   if (!c->nbr) CK(cudaMalloc(&c->nbr, sizeof(int) * cnt));
   CK(cudaMemcpyAsync(c->nbr, nbr, sizeof(int) * cnt, cudaMemcpyHostToDevice, c->stream));
   CK(cudaStreamSynchronize(c->stream));        // nbr is the caller's

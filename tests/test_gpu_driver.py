@@ -213,3 +213,93 @@ def test_advance_eight_blocks_with_exchange():
         for k, (a, b) in enumerate(zip(_np(g.U) + _np(g.Bf) + _np(g.W), U8 + B8 + Wo)):
             assert np.array_equal(a, b), k
         assert np.array_equal(gflag.cpu().numpy(), flag_o) and np.count_nonzero(flag_o) > 0
+
+
+# ---------------------------------------------------------------- halo path (paper_2409_10384_b200/halo.py)
+def _eight_blocks():
+    from test_multirank_cpu import _eight_block_domain
+    return _eight_block_domain()
+
+
+def test_halo_advance_single_rank_equals_ak_advance():
+    import torch
+    from paper_2409_10384_b200 import halo
+    from test_oracle_exchange import lattice_nbr
+    dom = _eight_blocks()
+    nbr = lattice_nbr((2, 2, 2), (True, True, True))
+    p8 = dict(dom["p"], nmb=8)
+    w = dict(U=dom["U"], Bf=dom["Bf"], adm=dom["adm"], dx=dom["dx"], params=p8, dt_fofc=dom["dt"])
+    with gpukit.GpuStage(copy.deepcopy(w)) as a, gpukit.GpuStage(copy.deepcopy(w)) as b:
+        ak.ak_set_neighbors(a.ctx, nbr)
+        ak.ak_advance(a.ctx, 3, 2, dom["dt"], (0, 0, 0), a.U, a.Bf, a.W)
+        plan = halo.HaloPlan(nbr, 0, 1)
+        ops = halo.AkOps(b.ctx, plan, (0, 0, 0), b.W, b.dU, b.E)
+        halo.advance(plan, ops, 3, 2, dom["dt"], b.U, b.Bf)
+        torch.cuda.synchronize()
+        for x, y in zip(a.U + a.Bf, b.U + b.Bf):
+            assert torch.equal(x, y)
+
+
+def test_two_shards_with_mirror_blocks_on_one_gpu():
+    """Two shards of the eight-block domain, each with its own context (nmb = 4) and read-only mirror
+    blocks behind its own; the mirror refresh is done here by plain device copies in lock-step (one
+    GPU, no waiting kernels) in place of the NCCL point-to-point operations.  Equals the oracle."""
+    import torch
+    from paper_2409_10384_b200 import halo
+    from test_oracle_exchange import lattice_nbr
+    dom = _eight_blocks()
+    nbr = lattice_nbr((2, 2, 2), (True, True, True))
+    U = [u.copy() for u in dom["U"]]; Bf = [b.copy() for b in dom["Bf"]]
+    orc.advance_nbr(orc.make_params(nmb=8, **dom["p"]), dom["dx"], 3, 2, dom["dt"], (0, 0, 0), nbr, U, Bf,
+                    dom["adm"], nthreads=8)
+    dev = "cuda:0"
+    ranks = []
+    for r in range(2):
+        plan = halo.HaloPlan(nbr, r, 2)
+        lo, hi = plan.lo, plan.hi
+        mk = lambda a: torch.cat([torch.from_numpy(np.ascontiguousarray(a[lo:hi])),
+                                  torch.zeros((plan.n_total - plan.n_own,) + a.shape[1:], dtype=torch.float64)]).to(dev)
+        sh = ak.shapes(plan.n_own, dom["p"]["n"])
+        z = lambda k: torch.zeros(sh[k], dtype=torch.float64, device=dev)
+        st = dict(plan=plan, U=[mk(u) for u in dom["U"]], Bf=[mk(b) for b in dom["Bf"]],
+                  adm=gpukit.to_dev([a[lo:hi] for a in dom["adm"]]), W=[z("cell") for _ in range(8)],
+                  dU=[z("cell") for _ in range(5)], E=[z("ex"), z("ey"), z("ez")])
+        st["ctx"] = ak.ak_create(ak.make_params(nmb=plan.n_own, device=0,
+                                                stream=torch.cuda.current_stream().cuda_stream, **dom["p"]),
+                                 dom["dx"][lo:hi])
+        ak.ak_set_metric(st["ctx"], st["adm"])
+        st["ops"] = halo.AkOps(st["ctx"], plan, (0, 0, 0), st["W"], st["dU"], st["E"])
+        ranks.append(st)
+
+    def refresh():
+        for me in ranks:
+            other = ranks[1 - me["plan"].rank]
+            for q, g in enumerate(me["plan"].mirrors):
+                src = g - other["plan"].lo
+                for t_me, t_ot in zip(me["U"] + me["Bf"], other["U"] + other["Bf"]):
+                    t_me[me["plan"].n_own + q].copy_(t_ot[src])
+    try:
+        dt = dom["dt"]
+        for _ in range(2):
+            for s in range(3):
+                a, b = halo.RK_A[3][s], halo.RK_B[3][s]
+                refresh()
+                for st in ranks:
+                    st["ops"].fill(st["U"], st["Bf"])
+                    st["rhs"] = st["ops"].rhs(st["U"], st["Bf"], None if s == 0 else st["U0"], a, b, dt)
+                    if s == 0:
+                        st["U0"], st["B0"] = st["ops"].snapshot(st["U"], st["Bf"])
+                        st["ops"].update(0.0, 1.0, dt, st["U"], st["Bf"], st["U"], st["Bf"], *st["rhs"])
+                    else:
+                        st["ops"].update(a, b, dt, st["U0"], st["B0"], st["U"], st["Bf"], *st["rhs"])
+        refresh()
+        for st in ranks:
+            st["ops"].fill(st["U"], st["Bf"])
+        torch.cuda.synchronize()
+        for st in ranks:
+            lo, hi, no = st["plan"].lo, st["plan"].hi, st["plan"].n_own
+            for g, o in zip(st["U"] + st["Bf"], U + Bf):
+                assert np.array_equal(g[:no].cpu().numpy(), o[lo:hi])
+    finally:
+        for st in ranks:
+            ak.ak_destroy(st["ctx"])

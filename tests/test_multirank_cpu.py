@@ -6,6 +6,8 @@ import socket
 
 import numpy as np
 import pytest
+import sys
+sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
 import torch
 import torch.distributed as dist
 import torch.multiprocessing as mp
@@ -87,3 +89,133 @@ def test_sharded_stage_equals_single_process():
             assert np.array_equal(part["Ez"][local], ref["E"][2][g])
             assert np.array_equal(part["flag"][local], ref["flag"][g])
     assert sorted(seen) == sorted(ids.tolist())
+
+
+# ---------------------------------------------------------------- halo exchange across ranks
+def _eight_block_domain():
+    """the periodic 12^3 domain of T27 as 2x2x2 blocks of 6^3 (identical in every process)."""
+    import stagekit as sk
+    from oracle import pyoracle as orc
+    N, n, NG = 12, 6, 4
+    d = 1.0 / N
+
+    def prim(x, y, z):
+        rho = 1.0 + 0.3 * np.sin(2 * np.pi * x) * np.cos(2 * np.pi * y) + 0.2 * np.sin(2 * np.pi * z)
+        rho = np.where((abs(x - 0.3) < 0.1) & (abs(y - 0.6) < 0.1) & (abs(z - 0.5) < 0.1), 1e-3 * rho, rho)
+        o = np.ones_like(x)
+        return rho, [0.3 * np.sin(2 * np.pi * y) * o, -0.2 * o, 0.25 * np.cos(2 * np.pi * x) * o], 0.6 * o
+
+    def A(comp, x, y, z):
+        return 0.1 * np.sin(2 * np.pi * (x + 2 * y)) if comp == 2 else 0.05 * np.cos(2 * np.pi * z) * (comp == 0) + 0 * x
+    blocks = []
+    for bz in range(2):
+        for by in range(2):
+            for bx in range(2):
+                blocks.append(sk.build_block(n, d, (bx * n * d, by * n * d, bz * n * d), sk.flat_metric, prim,
+                                             A_fn=A, gamma_ad=5.0 / 3.0))
+    cat = lambda key, q: np.ascontiguousarray(np.concatenate([b[key][q] for b in blocks], axis=0))
+    p = dict(n=n, gamma_ad=5.0 / 3.0, rho_atm=1e-10, T_atm=1e-8, recon=2, riemann=1, fofc=1, dmp_M=1.2)
+    return dict(U=[cat("U", v) for v in range(5)], Bf=[cat("Bf", c) for c in range(3)],
+                adm=[cat("adm", q) for q in range(16)], dx=np.full((8, 3), d), p=p, dt=0.15 * d)
+
+
+class _OracleOps:
+    """halo.advance `ops` backed by the CPU oracle (numpy views of the CPU tensors)."""
+
+    def __init__(self, par, plan, dx, adm, bc):
+        from oracle import pyoracle as orc
+        self.orc, self.par, self.plan, self.dx, self.adm, self.bc = orc, par, plan, dx, adm, bc
+
+    def fill(self, U, Bf):
+        self.orc.exchange_ghosts(self.par, self.plan.local_nbr, self.bc, [u.numpy() for u in U], [b.numpy() for b in Bf])
+
+    def rhs(self, U, Bf, U0, a, b, dt):
+        r = self.orc.rhs_blend(self.par, self.dx, [u.numpy() for u in U], [x.numpy() for x in Bf], self.adm, dt,
+                               None if U0 is None else [u.numpy() for u in U0], a, b)
+        return r["dU"], r["E"]
+
+    def snapshot(self, U, Bf):
+        return [u.clone() for u in U], [b.clone() for b in Bf]
+
+    def update(self, a, b, dt, U0, B0, U, Bf, dU, E):
+        self.orc.stage_update(self.par, self.dx, a, b, dt, [u.numpy() for u in U0], [x.numpy() for x in B0],
+                              [u.numpy() for u in U], [x.numpy() for x in Bf], dU, E)
+
+
+def _halo_worker(rank, world, port, out):
+    from oracle import pyoracle as orc
+    from paper_2409_10384_b200 import halo
+    from test_oracle_exchange import lattice_nbr
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        dom = _eight_block_domain()
+        nbr = lattice_nbr((2, 2, 2), (True, True, True))
+        plan = halo.HaloPlan(nbr, rank, world)
+        lo, hi = plan.lo, plan.hi
+
+        def with_mirrors(a):
+            t = torch.zeros((plan.n_total,) + a.shape[1:], dtype=torch.float64)
+            t[:plan.n_own] = torch.from_numpy(a[lo:hi])
+            return t
+        U = [with_mirrors(u) for u in dom["U"]]; Bf = [with_mirrors(b) for b in dom["Bf"]]
+        par = orc.make_params(nmb=plan.n_own, **dom["p"])
+        ops = _OracleOps(par, plan, dom["dx"][lo:hi], [np.ascontiguousarray(a[lo:hi]) for a in dom["adm"]], (0, 0, 0))
+        halo.advance(plan, ops, 3, 2, dom["dt"], U, Bf)
+        payload = dict(lo=lo, hi=hi, U=[u[:plan.n_own].numpy().copy() for u in U],
+                       Bf=[b[:plan.n_own].numpy().copy() for b in Bf], mirrors=plan.mirrors)
+        gathered = [None] * world if rank == 0 else None
+        dist.gather_object(payload, gathered, dst=0)
+        if rank == 0:
+            out.put(gathered)
+    finally:
+        dist.destroy_process_group()
+
+
+def test_halo_plan_tables():
+    from paper_2409_10384_b200 import halo
+    from test_oracle_exchange import lattice_nbr
+    nbr = lattice_nbr((2, 2, 2), (True, True, True))
+    plans = [halo.HaloPlan(nbr, r, 2) for r in range(2)]
+    for r, pl in enumerate(plans):
+        other = plans[1 - r]
+        assert pl.n_own == 4 and pl.mirrors == list(range(other.lo, other.hi))     # 2x2x2 periodic: all remote
+        assert sorted(pl.send[1 - r]) == [g - pl.lo for g in other.mirrors]
+        assert len(pl.recv[1 - r]) == len(other.send[r])
+        # every table entry resolves to the right global block
+        glob = list(range(pl.lo, pl.hi)) + pl.mirrors
+        for m in range(pl.n_own):
+            for o in range(27):
+                if o != 13:
+                    assert glob[pl.local_nbr[m, o]] == nbr[pl.lo + m, o]
+    one = halo.HaloPlan(nbr, 0, 1)
+    assert one.n_total == 8 and not one.send and not one.recv and np.array_equal(one.local_nbr, nbr)
+
+
+def test_two_ranks_with_halo_exchange_equal_one_process():
+    from oracle import pyoracle as orc
+    from test_oracle_exchange import lattice_nbr
+    orc.build()
+    world = 2
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_halo_worker, args=(r, world, port, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    gathered = q.get(timeout=300)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    dom = _eight_block_domain()
+    nbr = lattice_nbr((2, 2, 2), (True, True, True))
+    par = orc.make_params(nmb=8, **dom["p"])
+    U = [u.copy() for u in dom["U"]]; Bf = [b.copy() for b in dom["Bf"]]
+    orc.advance_nbr(par, dom["dx"], 3, 2, dom["dt"], (0, 0, 0), nbr, U, Bf, dom["adm"], nthreads=4)
+    for part in gathered:
+        lo, hi = part["lo"], part["hi"]
+        for v in range(5):
+            assert np.array_equal(part["U"][v], U[v][lo:hi]), (lo, v)
+        for c in range(3):
+            assert np.array_equal(part["Bf"][c], Bf[c][lo:hi]), (lo, c)
