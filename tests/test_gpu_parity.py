@@ -78,8 +78,9 @@ def test_noise_block_floors(recon):
 
 
 def test_noise_block_ragged_n():
-    """n = 6 and n = 10: block edges that are not multiples of the warp or tile sizes."""
-    for n in (6, 10):
+    """n = 6 and n = 10: block edges that are not multiples of the warp or tile sizes; n = 5, 7: odd
+    sizes, whose rows are not multiples of 16 B, take the one-thread-per-face fallback sweeps."""
+    for n in (6, 10, 5, 7):
         w = wl.make_test_noise_block(seed=3, n=n, frac=0.02)
         w["dt_fofc"] *= 2.0
         g, o, rep = run_both(w, want_flux=True, fofc_riemann=1)
