@@ -192,6 +192,27 @@ __device__ __forceinline__ bool illinois(C2P& s, double a, double b, double fa_,
   return false;
 }
 
+// Rare paths: the upper
+// bracket when r >= h0 (ultra-relativistic momentum) and the write-back of floored cells (optionally out of line).
+#ifndef AK_C2P_RARE_NOINLINE
+#define AK_C2P_RARE_NOINLINE 0   // measured: out-of-line costs 17 % (call ABI, stack frame); kept inline
+#endif
+#if AK_C2P_RARE_NOINLINE
+#define AK_RARE __noinline__
+#else
+#define AK_RARE __forceinline__
+#endif
+__device__ AK_RARE bool c2p_upper_bracket(C2P& s, int max_iter, double tol, double& mu_hi) {
+  return illinois<true>(s, 0.0, 1.0, -1.0, s.fa(1.0), max_iter, tol, mu_hi);
+}
+__device__ AK_RARE void c2p_write_back(const Par& P, const Met3& g, double sdet, double rho, double ux, double uy,
+                                       double uz, double pr, const double B[3], double Ut[5]) {
+  double c5[5];
+  const double u[3] = {ux, uy, uz};
+  prim2cons(P, g, rho, u, pr, B, c5);
+  for (int v = 0; v < 5; ++v) Ut[v] = sdet * c5[v];
+}
+
 // One cell.  Ut = densitised D,S_i,tau (rewritten from the final primitives when WRITE_BACK
 // and the status is non-zero); Bt = densitised cell-centred B; W5 = rho,u^x,u^y,u^z,P.
 template <bool WRITE_BACK>
@@ -250,7 +271,7 @@ __device__ __forceinline__ int c2p_cell(const Par& P, const Met3& g, double Ut[5
     bool ok = true;
     double mu_hi = 1.0;
     if (!(s.r2 < 1.0)) {
-      ok = illinois<true>(s, 0.0, 1.0, -1.0, s.fa(1.0), P.max_iter, P.tol, mu_hi);
+      ok = c2p_upper_bracket(s, P.max_iter, P.tol, mu_hi);
       mu_hi = mu_hi * (1.0 + 1e-14);
       if (mu_hi > 1.0) mu_hi = 1.0;
     }
@@ -289,12 +310,7 @@ __device__ __forceinline__ int c2p_cell(const Par& P, const Met3& g, double Ut[5
     status |= ST_TFLOOR;
   }
   W5[0] = rho; W5[1] = ux; W5[2] = uy; W5[3] = uz; W5[4] = pr;
-  if (WRITE_BACK && status != 0) {
-    double c5[5];
-    const double u[3] = {ux, uy, uz};
-    prim2cons(P, g, rho, u, pr, B, c5);
-    for (int v = 0; v < 5; ++v) Ut[v] = sdet * c5[v];
-  }
+  if (WRITE_BACK && status != 0) c2p_write_back(P, g, sdet, rho, ux, uy, uz, pr, B, Ut);
   return status;
 }
 
