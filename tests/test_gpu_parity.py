@@ -339,3 +339,12 @@ def test_guard_zones_no_out_of_bounds_access():
                     assert bool((lo == 0xAB).all()) and bool((hi == 0xAB).all())
         finally:
             ak.ak_destroy(ctx)
+
+
+def test_large_block_64():
+    """one 64^3 MeshBlock (the paper's TOV scaling runs use 64^3 blocks): tiles of the TMA sweeps
+    shrink to three rows, everything else scales; against the oracle."""
+    w = wl.make_test_noise_block(seed=64, n=64, frac=0.002)
+    w["dt_fofc"] *= 2.0
+    g, o, rep = run_both(w, recon=2, dmp_M=1.1)
+    assert np.count_nonzero(o["flag"]) > 0
