@@ -174,13 +174,13 @@ int launch_c2p(ak_ctx* c, const Fields& f, bool with_emf) {
 #endif
 
 template <int DIR, int RECON>
-int launch_flux_tma(ak_ctx* c, const Fields& f, int NA, unsigned grid, size_t smem) {
+int launch_flux_tma(ak_ctx* c, const Fields& f, int NA, unsigned grid, int bd, size_t smem) {
   auto kern = ((AK_FLUX_CELL_MASK >> DIR) & 1) ? k_flux_tma_cell<DIR, RECON> : k_flux_tma<DIR, RECON>;
   if (!c->tma_attr[DIR]) {
     CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     c->tma_attr[DIR] = true;
   }
-  kern<<<grid, TMA_THREADS, smem, c->stream>>>(c->P, f, NA);
+  kern<<<grid, bd, smem, c->stream>>>(c->P, f, NA);
   return AK_OK;
 }
 
@@ -201,13 +201,16 @@ int launch_flux(ak_ctx* c, const Fields& f) {
     const size_t smem = sizeof(double) * ((size_t)(7 * maxW + 10 * maxM) * nt + (AK_FLUX_CELL ? 7 * TMA_THREADS : 0));
     if (smem <= 200 * 1024) {
       const unsigned grid = (unsigned)((long long)c->P.nmb * e * tiles);
+      // threads: one per face (or cell) of the tile, rounded up to whole warps
+      const int rows = NA + ((AK_FLUX_CELL && DIR != 0) ? 1 : 0);
+      const int bd = ((rows * nfi + 31) / 32) * 32;
       int r;
       switch (c->P.recon) {
-        case 0: r = launch_flux_tma<DIR, 0>(c, f, NA, grid, smem); break;
-        case 1: r = launch_flux_tma<DIR, 1>(c, f, NA, grid, smem); break;
-        case 3: r = launch_flux_tma<DIR, 3>(c, f, NA, grid, smem); break;
-        case 4: r = launch_flux_tma<DIR, 4>(c, f, NA, grid, smem); break;
-        default: r = launch_flux_tma<DIR, 2>(c, f, NA, grid, smem); break;
+        case 0: r = launch_flux_tma<DIR, 0>(c, f, NA, grid, bd, smem); break;
+        case 1: r = launch_flux_tma<DIR, 1>(c, f, NA, grid, bd, smem); break;
+        case 3: r = launch_flux_tma<DIR, 3>(c, f, NA, grid, bd, smem); break;
+        case 4: r = launch_flux_tma<DIR, 4>(c, f, NA, grid, bd, smem); break;
+        default: r = launch_flux_tma<DIR, 2>(c, f, NA, grid, bd, smem); break;
       }
       if (r != AK_OK) return r;
       CK(cudaGetLastError());

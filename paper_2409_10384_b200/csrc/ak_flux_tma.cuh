@@ -78,7 +78,7 @@ k_flux_tma(const __grid_constant__ Par P, const __grid_constant__ Fields f, int 
   if (t == 0) mbar_arrive_expect_tx(&mbar, (unsigned)(7 * nW + 10 * nM) * rowb);
   // ---- one bulk copy per (field, row)
   const int ncW = 7 * nW, nc = ncW + 10 * nM;
-  for (int c = t; c < nc; c += TMA_THREADS) {
+  for (int c = t; c < nc; c += (int)blockDim.x) {
     if (c < ncW) {
       const int v = c / nW, r = c - v * nW;
       const int fld = v < 5 ? v : (v == 5 ? 5 + t1 : 5 + t2);
@@ -176,7 +176,7 @@ k_flux_tma_cell(const __grid_constant__ Par P, const __grid_constant__ Fields f,
   __syncthreads();
   if (t == 0) mbar_arrive_expect_tx(&mbar, (unsigned)(7 * nW + 10 * nM) * rowb);
   const int ncW = 7 * nW, nc = ncW + 10 * nM;
-  for (int c = t; c < nc; c += TMA_THREADS) {
+  for (int c = t; c < nc; c += (int)blockDim.x) {
     if (c < ncW) {
       const int v = c / nW, r = c - v * nW;
       const int fld = v < 5 ? v : (v == 5 ? 5 + t1 : 5 + t2);
