@@ -373,3 +373,12 @@ def test_side_stream_is_honoured():
         for x, y in zip(ra[k], rb[k]):
             assert np.array_equal(x, y)
     assert np.array_equal(ra["flag"], rb["flag"]) and np.array_equal(ra["status"], rb["status"])
+
+
+@pytest.mark.parametrize("recon,riemann,fofc_riemann", [(3, 0, 1), (4, 1, 0), (4, 0, 1), (0, 1, 1)])
+def test_curved_blocks_all_reconstructions(recon, riemann, fofc_riemann):
+    """Kerr-Schild blocks near the horizon and in the torus (C3) with the other reconstructions and
+    Riemann-solver pairings (PLM/PPMX/donor; LLF/HLLE; HLLE as the FOFC solver)."""
+    w = wl.make_blocks("C3", blocks=[192 + 21, 192 + 38, 64 + 21, 38])
+    g, o, rep = run_both(w, want_flux=True, recon=recon, riemann=riemann, fofc_riemann=fofc_riemann)
+    assert np.count_nonzero(o["flag"]) > 0
