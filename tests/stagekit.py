@@ -73,3 +73,41 @@ def curlE_div(E, n, d):
     div = ((dBx[..., 1:] - dBx[..., :-1]) + (dBy[:, :, 1:, :] - dBy[:, :, :-1, :]) +
            (dBz[:, 1:] - dBz[:, :-1])) / d
     return dBx, dBy, dBz, div
+
+
+def loop_block(n):
+    """Magnetic loop advection (Eq. 13): A_z = A0 max(R - r, 0), A0 = 1e-3, R = 0.3,
+    rho = 1, P = 3, v = (1/1.2, 1/2.4, 0) on the periodic unit square, here one n^3 block (uniform
+    in z).  The paper does not print Gamma for this test; 5/3 is used.  Returns (w, params, d)."""
+    d = 1.0 / n
+    v = np.array([1 / 1.2, 1 / 2.4, 0.0])
+    lor = 1.0 / np.sqrt(1.0 - v @ v)
+
+    def prim(x, y, z):
+        o = np.ones_like(x)
+        return o, [lor * v[0] * o, lor * v[1] * o, 0 * o], 3.0 * o
+
+    def A(comp, x, y, z):
+        if comp != 2:
+            return 0 * x
+        return 1e-3 * np.maximum(0.3 - np.sqrt(x * x + y * y), 0.0)
+    w = build_block(n, d, (-0.5, -0.5, -0.5), flat_metric, prim, A_fn=A, gamma_ad=5.0 / 3.0)
+    p = dict(nmb=1, n=n, gamma_ad=5.0 / 3.0, rho_atm=1e-10, T_atm=1e-8, recon=2, riemann=1, fofc=1)
+    return w, p, d
+
+
+def divB_rel(Bf, n, d, bmax):
+    """max |div B~| dx / max|B~| over interior cells (the quantity of the paper's Figure 6, bottom)."""
+    s = slice(NG, NG + n); s1 = slice(NG + 1, NG + n + 1)
+    div = ((Bf[0][:, s, s, s1] - Bf[0][:, s, s, s]) + (Bf[1][:, s, s1, s] - Bf[1][:, s, s, s]) +
+           (Bf[2][:, s1, s, s] - Bf[2][:, s, s, s]))
+    return np.abs(div).max() / bmax
+
+
+def loop_metrics(Bf, B0, n, shift_y):
+    """correlation of the interior B~x with the initial loop displaced by shift_y cells in y, with the
+    undisplaced one, and the ratio of sum B~x^2 to its initial value."""
+    s = slice(NG, NG + n)
+    bx = Bf[0][0, s, s, NG:NG + n]; b0 = B0[0][0, s, s, NG:NG + n]
+    cor = lambda a, b: np.sum(a * b) / np.sqrt(np.sum(a * a) * np.sum(b * b))
+    return cor(bx, np.roll(b0, shift_y, axis=1)), cor(bx, b0), np.sum(bx * bx) / np.sum(b0 * b0)

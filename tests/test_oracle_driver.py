@@ -265,3 +265,26 @@ def test_T25_shock_tube_stays_one_dimensional_and_physical():
     assert abs(np.sum(sk.interior(U[0], n)) - m0) < 1e-8 * m0      # only diffusive tails reach the x boundaries
     rho = W[0][0, NG, NG, NG:NG + n]
     assert rho.max() <= 1.0 + 1e-3 and rho.min() >= 0.125 - 1e-3 and np.any((rho < 0.99) & (rho > 0.13))
+
+
+def test_T29_magnetic_loop_is_advected_at_the_right_speed():
+    """Loop advection: with RK3, HLLE+FOFC, WENO-Z at CFL 0.25 the loop moves with
+    v = (1/1.2, 1/2.4, 0).  After t = 1.2 it has crossed the periodic box once in x and half of it
+    in y, so B~x must match the initial loop displaced by n/2 cells in y (and not the undisplaced one);
+    div B~ stays at round-off (paper: 7e-14 -> 3e-12 relative to max|B| at 240^2), mass is conserved,
+    no B~z appears and no cell is flagged by the FOFC."""
+    n = 16
+    w, p, d = sk.loop_block(n)
+    par = orc.make_params(**p)
+    U = [u.copy() for u in w["U"]]; Bf = [b.copy() for b in w["Bf"]]
+    bmax = max(np.abs(b).max() for b in Bf)
+    assert abs(bmax - 1e-3) < 1e-15 and sk.divB_rel(Bf, n, d, bmax) < 1e-14
+    m0 = np.sum(sk.interior(U[0], n))
+    nsteps = int(np.ceil(1.2 / (0.25 * d)))
+    W, flag = orc.advance(par, w["dx"], 3, nsteps, 1.2 / nsteps, (0, 0, 0), U, Bf, w["adm"], nthreads=4)
+    c_moved, c_same, e_ratio = sk.loop_metrics(Bf, w["Bf"], n, n // 2)
+    assert c_moved > 0.93 and c_same < 0.0
+    assert 0.6 < e_ratio <= 1.0                       # diffusion only removes magnetic energy
+    assert sk.divB_rel(Bf, n, d, bmax) < 1e-13
+    assert abs(np.sum(sk.interior(U[0], n)) / m0 - 1.0) < 1e-13
+    assert np.abs(Bf[2]).max() < 1e-15 and np.count_nonzero(flag) == 0
