@@ -1,0 +1,218 @@
+"""The paper's flat-space tests run end to end on the GPU through ak_advance with the
+same-level ghost exchange: properties the paper states (first-order convergence of the shock tubes,
+P:196-198; the blast wave stays physical with FOFC), not element-wise parity - the
+element-wise parity of ak_advance is in test_gpu_driver.py.  Exact Riemann solutions are not
+available here, so convergence is measured between successive resolutions."""
+import os
+
+import numpy as np
+import pytest
+
+from paper_2409_10384_b200 import ak, workloads as wl
+
+import gpukit
+from test_oracle_exchange import lattice_nbr
+
+pytestmark = pytest.mark.gpu
+NG = 4
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden", "balsara_table1.txt")
+
+
+def balsara_states(test_id):
+    out = {}
+    for line in open(GOLDEN):
+        if line.startswith("#") or not line.strip():
+            continue
+        t = line.split()
+        if int(t[0]) == test_id:
+            out[t[1]] = [float(x) for x in t[2:]]
+    return out["L"], out["R"]
+
+
+def riemann_chain(test_id, n, nbx):
+    """nbx blocks of n^3 in a row along x covering [0,1], discontinuity at x = 0.5; uniform in
+    y and z (each block is its own periodic neighbour there), outflow in x."""
+    L, R = balsara_states(test_id)
+    gam = L[0]
+    nt = n + 2 * NG
+    d = 1.0 / (n * nbx)
+    sh = ak.shapes(nbx, n)
+    U = [np.zeros(sh["cell"]) for _ in range(5)]
+    Bf = [np.zeros(sh[k]) for k in ("xf", "yf", "zf")]
+    for b in range(nbx):
+        xc = (b * n + np.arange(nt) - NG + 0.5) * d
+        left = xc < 0.5
+        q = [np.where(left, L[k], R[k]) for k in range(1, 9)]          # rho P vx vy vz Bx By Bz
+        rho, P, v, B = q[0], q[1], q[2:5], q[5:8]
+        lor = 1.0 / np.sqrt(1.0 - (v[0] ** 2 + v[1] ** 2 + v[2] ** 2))
+        o, zr = np.ones(nt), np.zeros(nt)
+        D, S, tau = wl._prim2cons_np(gam, [o, zr, zr, o, zr, o], rho, [lor * a for a in v], P, B)
+        for dst, src in zip(U, (D, S[0], S[1], S[2], tau)):
+            dst[b] = src[None, None, :]
+        Bf[0][b] = L[6]                                                  # B^x is the same on both sides
+        Bf[1][b] = B[1][None, None, :]
+        Bf[2][b] = B[2][None, None, :]
+    one, zero = np.ones(sh["cell"]), np.zeros(sh["cell"])
+    adm = [one, zero, zero, one, zero, one, one] + [zero] * 9
+    p = dict(nmb=nbx, n=n, gamma_ad=gam, rho_atm=1e-10, T_atm=1e-8, recon=1, riemann=0, fofc=0)
+    return dict(U=U, Bf=Bf, adm=adm, dx=np.full((nbx, 3), d), params=p, dt_fofc=0.0), d
+
+
+def run_tube(test_id, n, nbx, t_end=0.4, cfl=0.2, integrator=3, **override):
+    import torch
+    w, d = riemann_chain(test_id, n, nbx)
+    w["params"].update(override)
+    nsteps = int(np.ceil(t_end / (cfl * d)))
+    w["dt_fofc"] = t_end / nsteps
+    nbr = lattice_nbr((nbx, 1, 1), (False, True, True))
+    with gpukit.GpuStage(w) as g:
+        ak.ak_set_neighbors(g.ctx, nbr)
+        gflag = torch.zeros_like(g.flag)
+        ak.ak_advance(g.ctx, integrator, nsteps, t_end / nsteps, (1, 0, 0), g.U, g.Bf, g.W, gflag)
+        torch.cuda.synchronize()
+        W = [t.cpu().numpy() for t in g.W]
+        stats = g.stats()
+    s = slice(NG, NG + n)
+    line = lambda a: a[:, NG, NG, s].reshape(-1)                           # the interior cells along x
+    uniform = all(np.all(a[:, s, s, s] == a[:, NG:NG + 1, NG:NG + 1, s]) for a in W[:5])
+    return dict(rho=line(W[0]), P=line(W[4]), ux=line(W[1]), by=line(W[6]), uniform=uniform, stats=stats,
+                flagged=int(gflag.count_nonzero()))
+
+
+def coarsen(a):
+    return 0.5 * (a[0::2] + a[1::2])
+
+
+def tube_errors(test_id, n=16, nbxs=(4, 8, 16, 32)):
+    """L1 and L2 norms of rho(N) - coarsened rho(2N) for successive resolutions."""
+    runs = [run_tube(test_id, n, nbx) for nbx in nbxs]
+    e1, e2 = [], []
+    for a, b in zip(runs[:-1], runs[1:]):
+        diff = a["rho"] - coarsen(b["rho"])
+        e1.append(np.mean(np.abs(diff))); e2.append(np.sqrt(np.mean(diff ** 2)))
+    return runs, e1, e2
+
+
+# ---------------------------------------------------------------- cylindrical blast wave
+def blast_lattice(bx_field, n, nb):
+    """nb x nb x 1 blocks of n^3 covering [-6,6]^2 (uniform in z): rho_in = 1e-2, P_in = 1 inside
+    r_in = 0.8, ambient 1e-4 / 3e-5 outside r_out = 1, exponential decay (linear in the logarithm)
+    between; B = (Bx, 0, 0); fluid at rest; Gamma = 4/3."""
+    gam = 4.0 / 3.0
+    nt = n + 2 * NG
+    d = 12.0 / (n * nb)
+    nmb = nb * nb
+    sh = ak.shapes(nmb, n)
+    U = [np.zeros(sh["cell"]) for _ in range(5)]
+    Bf = [np.zeros(sh[k]) for k in ("xf", "yf", "zf")]
+    Bf[0][:] = bx_field
+    o, zr = np.ones((nt, nt)), np.zeros((nt, nt))
+    for by in range(nb):
+        for bx in range(nb):
+            m = by * nb + bx
+            xc = -6.0 + (bx * n + np.arange(nt) - NG + 0.5) * d
+            yc = -6.0 + (by * n + np.arange(nt) - NG + 0.5) * d
+            Y, X = np.meshgrid(yc, xc, indexing="ij")
+            r = np.sqrt(X * X + Y * Y)
+            f = np.clip((r - 0.8) / 0.2, 0.0, 1.0)                      # 0 inside r_in, 1 outside r_out
+            rho = np.exp((1.0 - f) * np.log(1e-2) + f * np.log(1e-4))
+            P = np.exp((1.0 - f) * np.log(1.0) + f * np.log(3e-5))
+            D, S, tau = wl._prim2cons_np(gam, [o, zr, zr, o, zr, o], rho, [zr, zr, zr], P, [bx_field * o, zr, zr])
+            for dst, src in zip(U, (D, S[0], S[1], S[2], tau)):
+                dst[m] = src[None, :, :]
+    one, zero = np.ones(sh["cell"]), np.zeros(sh["cell"])
+    adm = [one, zero, zero, one, zero, one, one] + [zero] * 9
+    p = dict(nmb=nmb, n=n, gamma_ad=gam, rho_atm=1e-10, T_atm=1e-8, f_thr=1.0, recon=2, riemann=1, fofc=1)
+    return dict(U=U, Bf=Bf, adm=adm, dx=np.full((nmb, 3), d), params=p, dt_fofc=0.0), d
+
+
+def run_blast(bx_field, n=20, nb=10, t_end=4.0, cfl=0.1, **override):
+    import torch
+    w, d = blast_lattice(bx_field, n, nb)
+    w["params"].update(override)
+    nsteps = int(np.ceil(t_end / (cfl * d)))
+    dt = t_end / nsteps
+    w["dt_fofc"] = dt
+    nbr = lattice_nbr((nb, nb, 1), (False, False, True))
+    s = slice(NG, NG + n)
+    with gpukit.GpuStage(w) as g:
+        ak.ak_set_neighbors(g.ctx, nbr)
+        gflag = torch.zeros_like(g.flag)
+        ak.ak_advance(g.ctx, 3, nsteps, dt, (1, 1, 0), g.U, g.Bf, g.W, gflag)
+        torch.cuda.synchronize()
+        W = [t.cpu().numpy() for t in g.W]
+        stats = g.stats()
+        flagged = int(gflag[:, s, s, s].count_nonzero())
+
+    def plane(a):                                                          # [nb*n, nb*n] at one z
+        a = a[:, NG, s, s].reshape(nb, nb, n, n)
+        return a.transpose(0, 2, 1, 3).reshape(nb * n, nb * n)
+    uniform_z = all(np.all(a[:, s, s, s] == a[:, NG:NG + 1, s, s]) for a in W[:5])
+    return dict(rho=plane(W[0]), P=plane(W[4]), ux=plane(W[1]), uy=plane(W[2]), stats=stats, flagged=flagged,
+                uniform_z=uniform_z, zones=nb * nb * n ** 3)
+
+
+# ================================================================ the tests
+@pytest.mark.parametrize("test_id", [1, 2, 3, 4, 5])
+def test_balsara_tubes_converge_at_first_order(test_id):
+    """LLF + PPM4, no FOFC, t = 0.5, the paper's resolutions 200/400/800 against its 1600-cell
+    run (80 blocks of 20^3 in a row, exchanged every stage).  'Approximate first-order convergence
+    for all tests' (the lowest resolutions of #3 and #5 are not yet convergent): the L1 order
+    of rho between 200 and 800 cells is about one; the run stays one-dimensional bit for bit and
+    needs no floor and no inversion failure ('never approaches atmosphere')."""
+    runs = [run_tube(test_id, 20, nbx, t_end=0.5) for nbx in (10, 20, 40, 80)]
+    ref = runs[-1]["rho"]
+    err = []
+    for r in runs[:-1]:
+        c = ref
+        while c.size > r["rho"].size:
+            c = coarsen(c)
+        err.append(np.mean(np.abs(r["rho"] - c)))
+    order = np.log2(err[0] / err[2]) / 2.0
+    assert err[0] > err[1] > err[2]
+    assert 0.75 < order < 1.6, (err, order)
+    for r in runs:
+        st = r["stats"]
+        assert r["uniform"] and np.isfinite(r["rho"]).all()
+        assert st["n_c2p_fail"] == 0 and st["n_cons_floor"] == 0 and st["n_prim_floor"] == 0
+        assert r["rho"].min() > 0.05 and r["P"].min() > 0.05
+
+
+def _front(a, thr):
+    n = a.shape[0]
+    x = (np.arange(n) + 0.5) * 12.0 / n - 6.0
+    return np.abs(x[a[n // 2] > thr]).max(), np.abs(x[a[:, n // 2] > thr]).max()
+
+
+def test_blast_wave_moderate_field_with_fofc():
+    """B_x = 0.1 (Figure 4) at the paper's 200^2 cells, HLLE + WENO-Z + RK3, CFL 0.1,
+    FOFC: the state at t = 4 is physical everywhere without any floor, the front has travelled
+    at nearly the speed of light (r_out + t = 5 bounds it), the solution keeps the symmetry of the data."""
+    r = run_blast(0.1)
+    P, rho, st = r["P"], r["rho"], r["stats"]
+    assert np.isfinite(P).all() and r["uniform_z"]
+    assert st["n_c2p_fail"] == 0 and st["n_cons_floor"] == 0 and st["n_prim_floor"] == 0
+    assert P.min() > 1e-5 and rho.min() > 3e-5
+    fx, fy = _front(P, 1e-4)
+    assert 4.5 < fx <= 5.0 + 0.06 and 4.5 < fy <= 5.0 + 0.06
+    assert np.abs(P - P[:, ::-1]).max() < 0.03 * P.max() and np.abs(P - P[::-1, :]).max() < 0.03 * P.max()
+    assert 0.0 < r["flagged"] < 0.3 * r["zones"]
+
+
+@pytest.mark.parametrize("dmp_M", [0.0, 1.1])
+def test_blast_wave_strong_field_stays_physical_with_fofc(dmp_M):
+    """B_x = 1 (Figure 5): with FOFC or FOFC+DMP (M = 1.1) no inversion fails and no cell
+    is reset to atmosphere."""
+    r = run_blast(1.0, dmp_M=dmp_M)
+    assert np.isfinite(r["P"]).all() and r["stats"]["n_c2p_fail"] == 0
+    assert r["rho"].min() > 1e-8 and r["P"].min() > 0.0 and r["P"].max() < 1.0
+    lor = np.sqrt(1.0 + r["ux"] ** 2 + r["uy"] ** 2)
+    assert lor.max() < 200.0
+
+
+def test_blast_wave_strong_field_without_fofc_disintegrates():
+    """'A test with WENOZ quickly disintegrated due to primitive inversion failures resetting
+    the solution to atmosphere' - the same run with the FOFC switched off."""
+    r = run_blast(1.0, fofc=0)
+    assert r["stats"]["n_c2p_fail"] > 100
+    assert int((r["rho"] <= 1.0000001e-10).sum()) > 0
