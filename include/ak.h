@@ -177,6 +177,24 @@ int ak_set_fofc_blend(ak_ctx*, const ak_cons* U0, double a, double b);
  * ghost fill — paper_2409_10384_b200/halo.py) and table entries may point at them. */
 int ak_set_neighbors(ak_ctx*, const int* nbr, int nmb_total);
 
+/* ---- ghost slabs for the exchange across GPUs (D:§12) ------------------------------
+ * A slab is the part of one block that a block which has it as neighbour `code` (the table index
+ * above: the offset from the reader to this block) reads in ak_fill_ghosts.  Per axis with offset o,
+ * cell-like indices [n, n+ng) for o = -1, [ng, 2ng) for o = +1, [ng, ng+n) for o = 0; along the normal
+ * of a face field [n, n+ng), [ng, 2ng+1), [ng, ng+n+1) (the faces it owns, plus face ie+1 where the
+ * reader may take it).  In the buffer a slab holds D~, S~x, S~y, S~z, tau~, then B~f^x, B~f^y, B~f^z,
+ * each box k-major.  ak_halo_slab_elems: doubles in one slab (host arithmetic; < 0 for a bad code).
+ * ak_halo_pack gathers ndesc slabs into buf, ak_halo_unpack scatters them back (into mirror blocks):
+ * desc = DEVICE int64 [ndesc][3] = {block, code, offset of the slab in buf in doubles}; block is an
+ * index into the arrays passed (0 <= block < the nmb_total of ak_set_neighbors, else nmb); a
+ * descriptor out of range is skipped.  buf = DEVICE doubles, caller-owned, 16-byte aligned.
+ * Asynchronous on the context's stream; only these slabs' elements are touched. */
+long long ak_halo_slab_elems(const ak_ctx*, int code);
+int ak_halo_pack(ak_ctx*, int ndesc, const long long* desc, const ak_cons* U, const ak_faceB_rw* Bf,
+                 double* buf);
+int ak_halo_unpack(ak_ctx*, int ndesc, const long long* desc, const double* buf, const ak_cons* U,
+                   const ak_faceB_rw* Bf);
+
 /* Fill the ghost cells of U~ and the ghost faces of B~f in place.  bc[d] = AK_BC_* per direction:
  * periodic (face ie+1 is made a copy of face is) or outflow (zero-gradient copies). */
 int ak_fill_ghosts(ak_ctx*, const int bc[3], const ak_cons* U, const ak_faceB_rw* Bf);

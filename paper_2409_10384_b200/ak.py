@@ -22,7 +22,7 @@ EXPORTS = ("ak_create", "ak_set_metric", "ak_con2prim", "ak_rhs", "ak_emf", "ak_
            "ak_get_flux", "ak_rhs_host", "ak_timing", "ak_kernel_ms", "ak_probe_copy",
            "ak_probe_fp64", "ak_destroy", "ak_strerror", "ak_version",
            "ak_set_fofc_blend", "ak_fill_ghosts", "ak_stage_update", "ak_advance", "ak_set_neighbors",
-           "ak_matter_sources")
+           "ak_matter_sources", "ak_halo_slab_elems", "ak_halo_pack", "ak_halo_unpack")
 BC_PERIODIC, BC_OUTFLOW = 0, 1
 
 _dp = C.POINTER(C.c_double)
@@ -104,6 +104,10 @@ def lib():
         L.ak_probe_copy.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_longlong, C.c_int, _dp]
         L.ak_probe_fp64.argtypes = [C.c_void_p, C.c_int, C.c_int, _dp]
         L.ak_destroy.argtypes = [C.c_void_p]
+        L.ak_halo_slab_elems.restype = C.c_longlong
+        L.ak_halo_slab_elems.argtypes = [C.c_void_p, C.c_int]
+        L.ak_halo_pack.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.POINTER(AkCons), C.POINTER(AkFaceB), C.c_void_p]
+        L.ak_halo_unpack.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.POINTER(AkCons), C.POINTER(AkFaceB)]
         L.ak_set_fofc_blend.argtypes = [C.c_void_p, C.POINTER(AkCons), C.c_double, C.c_double]
         L.ak_fill_ghosts.argtypes = [C.c_void_p, C.POINTER(C.c_int), C.POINTER(AkCons), C.POINTER(AkFaceB)]
         L.ak_stage_update.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_double, C.POINTER(AkCons),
@@ -276,6 +280,29 @@ def ak_set_neighbors(ctx, nbr, nmb_total=0):
         return
     a = np.ascontiguousarray(nbr, dtype=np.int32)
     _chk(lib().ak_set_neighbors(ctx, a.ctypes.data_as(C.POINTER(C.c_int)), int(nmb_total)), "ak_set_neighbors")
+
+
+def ak_halo_slab_elems(ctx, code):
+    """doubles in the ghost slab of neighbour code `code` (include/ak.h)."""
+    v = int(lib().ak_halo_slab_elems(ctx, int(code)))
+    if v < 0:
+        raise ValueError("ak_halo_slab_elems: bad neighbour code %r" % (code,))
+    return v
+
+
+def ak_halo_pack(ctx, desc, U, Bf, buf):
+    """desc: device int64 tensor [ndesc][3] = block, code, offset in buf; buf: device float64 tensor."""
+    u, b = _struct(AkCons, U), _struct(AkFaceB, Bf)
+    nd = 0 if desc is None else int(desc.shape[0])
+    _chk(lib().ak_halo_pack(ctx, nd, _ptr(desc), C.byref(u), C.byref(b), _ptr(buf)),
+         "ak_halo_pack")
+
+
+def ak_halo_unpack(ctx, desc, buf, U, Bf):
+    u, b = _struct(AkCons, U), _struct(AkFaceB, Bf)
+    nd = 0 if desc is None else int(desc.shape[0])
+    _chk(lib().ak_halo_unpack(ctx, nd, _ptr(desc), _ptr(buf), C.byref(u), C.byref(b)),
+         "ak_halo_unpack")
 
 
 def ak_matter_sources(ctx, W, out10):

@@ -58,6 +58,7 @@ struct ak_ctx {
   double* regU0[5]; double* regB0[3]; double* reg_dU[5]; double* regE[3]; unsigned char* reg_flag;
   bool have_reg;
   int* nbr;                     // device copy of the neighbour table (ak_set_neighbors), or NULL
+  int nmb_total;                // blocks in the caller's arrays (own + mirrors), 0 = nmb
   // pipelined host entry (ak_rhs_host): two lanes, each a child context over `lane_chunk` blocks
   // with its own stream and device staging; chunks alternate between the lanes
   double* host_dx;              // [nmb][3] host copy
@@ -758,12 +759,52 @@ int ak_fill_ghosts(ak_ctx* c, const int bc[3], const ak_cons* U, const ak_faceB_
   return AK_OK;
 }
 
+long long ak_halo_slab_elems(const ak_ctx* c, int code) {
+  if (!c || code < 0 || code > 26 || code == 13) return -1;
+  return slab_elems(code, c->P.n, c->P.is);
+}
+
+static int halo_slabs(ak_ctx* c, bool unpack, int ndesc, const long long* desc, const ak_cons* U,
+                      const ak_faceB_rw* Bf, double* buf) {
+  if (!c || ndesc < 0 || !U || !Bf || !U->D || !U->Sx || !U->Sy || !U->Sz || !U->tau || !Bf->bx || !Bf->by || !Bf->bz)
+    return AK_EINVAL;
+  if (ndesc == 0) return AK_OK;
+  if (!desc || !buf || (((uintptr_t)buf) & 15u) || (((uintptr_t)desc) & 7u)) return AK_EINVAL;
+  CK(cudaSetDevice(c->hp.device));
+  DrvFields f;
+  memset(&f, 0, sizeof(f));
+  f.U[0] = U->D; f.U[1] = U->Sx; f.U[2] = U->Sy; f.U[3] = U->Sz; f.U[4] = U->tau;
+  f.Bf[0] = Bf->bx; f.Bf[1] = Bf->by; f.Bf[2] = Bf->bz;
+  const int nblocks = c->nmb_total > c->P.nmb ? c->nmb_total : c->P.nmb;
+  // a face slab of a 32^3 block has 5*4*32*32 cells: 8 chunks of 256 threads make ~10 passes per field
+  const long long big = 5LL * c->P.is * c->P.n * c->P.n;
+  unsigned chunks = (unsigned)((big + 256 * 10 - 1) / (256 * 10));
+  if (chunks < 1) chunks = 1;
+  for (int q0 = 0; q0 < ndesc; q0 += 65535) {
+    const int nd = ndesc - q0 < 65535 ? ndesc - q0 : 65535;
+    const dim3 grid(chunks, (unsigned)nd);
+    if (unpack) k_halo_slabs<true><<<grid, 256, 0, c->stream>>>(c->P, f, desc + 3LL * q0, buf, nblocks);
+    else k_halo_slabs<false><<<grid, 256, 0, c->stream>>>(c->P, f, desc + 3LL * q0, buf, nblocks);
+  }
+  CK(cudaGetLastError());
+  return AK_OK;
+}
+
+int ak_halo_pack(ak_ctx* c, int ndesc, const long long* desc, const ak_cons* U, const ak_faceB_rw* Bf, double* buf) {
+  return halo_slabs(c, false, ndesc, desc, U, Bf, buf);
+}
+
+int ak_halo_unpack(ak_ctx* c, int ndesc, const long long* desc, const double* buf, const ak_cons* U,
+                   const ak_faceB_rw* Bf) {
+  return halo_slabs(c, true, ndesc, desc, U, Bf, const_cast<double*>(buf));
+}
+
 int ak_set_neighbors(ak_ctx* c, const int* nbr, int nmb_total) {
   if (!c) return AK_EINVAL;
   CK(cudaSetDevice(c->hp.device));
   if (!nbr) {
     CK(cudaStreamSynchronize(c->stream));
-    cudaFree(c->nbr); c->nbr = nullptr;
+    cudaFree(c->nbr); c->nbr = nullptr; c->nmb_total = 0;
     return AK_OK;
   }
   const long long cnt = 27LL * c->P.nmb;
@@ -773,6 +814,7 @@ int ak_set_neighbors(ak_ctx* c, const int* nbr, int nmb_total) {
   if (!c->nbr) CK(cudaMalloc(&c->nbr, sizeof(int) * cnt));
   CK(cudaMemcpyAsync(c->nbr, nbr, sizeof(int) * cnt, cudaMemcpyHostToDevice, c->stream));
   CK(cudaStreamSynchronize(c->stream));        // nbr is the caller's
+  c->nmb_total = nmb_total;
   return AK_OK;
 }
 

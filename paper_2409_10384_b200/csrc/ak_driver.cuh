@@ -180,4 +180,52 @@ __global__ void __launch_bounds__(256) k_exchange(const __grid_constant__ Par P,
   }
 }
 
+// ---------------------------------------------------------------- ghost slabs for the cross-GPU exchange
+// A slab is the part of one block that a block at the other end of neighbour code c reads in pass 0 of
+// k_exchange (c = (oz+1)*9+(oy+1)*3+(ox+1), the offset from the reader to this block).  Per axis with
+// offset o: cell-like indices [n, n+ng) for o = -1, [ng, 2ng) for o = +1, [ng, ng+n) for o = 0; along a
+// face field's normal [n, n+ng), [ng, 2ng+1), [ng, ng+n+1).  Order in the buffer: the five cell fields,
+// then B~f^x, B~f^y, B~f^z, each k-major.  include/ak.h: ak_halo_slab_elems, ak_halo_pack, ak_halo_unpack.
+__host__ __device__ __forceinline__ int slab_start(int o, int n, int ng) { return o < 0 ? n : ng; }
+__host__ __device__ __forceinline__ int slab_extent(int o, int n, int ng, bool normal) {
+  if (normal) return o < 0 ? ng : (o > 0 ? ng + 1 : n + 1);
+  return o != 0 ? ng : n;
+}
+__host__ __device__ inline long long slab_elems(int code, int n, int ng) {
+  const int o[3] = {code % 3 - 1, (code / 3) % 3 - 1, code / 9 - 1};
+  long long c[3], f[3];
+  for (int a = 0; a < 3; ++a) { c[a] = slab_extent(o[a], n, ng, false); f[a] = slab_extent(o[a], n, ng, true); }
+  return 5 * c[0] * c[1] * c[2] + f[0] * c[1] * c[2] + c[0] * f[1] * c[2] + c[0] * c[1] * f[2];
+}
+
+// desc[3*q + {0,1,2}] = block, code, offset of the slab in buf (elements).  grid (chunks, ndesc).
+template <bool UNPACK>
+__global__ void __launch_bounds__(256) k_halo_slabs(const __grid_constant__ Par P, const __grid_constant__ DrvFields f,
+                                                    const long long* __restrict__ desc, double* __restrict__ buf,
+                                                    int nblocks) {
+  const long long* dq = desc + 3LL * blockIdx.y;
+  const int m = (int)dq[0], code = (int)dq[1];
+  if (m < 0 || m >= nblocks || code < 0 || code > 26) return;
+  double* b = buf + dq[2];
+  const int o[3] = {code % 3 - 1, (code / 3) % 3 - 1, code / 9 - 1};
+  const int n = P.n, ng = P.is;
+  const int s0 = slab_start(o[0], n, ng), s1 = slab_start(o[1], n, ng), s2 = slab_start(o[2], n, ng);
+  const Ix ix{P.nt, P.px};
+  const int tid = blockIdx.x * blockDim.x + threadIdx.x, nth = gridDim.x * blockDim.x;
+#pragma unroll 1
+  for (int fld = 0; fld < 8; ++fld) {
+    const int D = fld - 5;                                   // normal of a face field, < 0 for cell fields
+    const int ex = slab_extent(o[0], n, ng, D == 0), ey = slab_extent(o[1], n, ng, D == 1),
+              ez = slab_extent(o[2], n, ng, D == 2);
+    const int cnt = ex * ey * ez;
+    double* fp = D < 0 ? f.U[fld] : f.Bf[D];
+    for (int e = tid; e < cnt; e += nth) {
+      const int i = e % ex, j = (e / ex) % ey, k = e / (ex * ey);
+      const long long g = D < 0 ? ix.cell(m, k + s2, j + s1, i + s0) : ix.face(D, m, k + s2, j + s1, i + s0);
+      if (UNPACK) fp[g] = b[e]; else b[e] = fp[g];
+    }
+    b += cnt;
+  }
+}
+
 }  // namespace ak

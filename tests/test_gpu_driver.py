@@ -242,8 +242,9 @@ def test_halo_advance_single_rank_equals_ak_advance():
 
 def test_two_shards_with_mirror_blocks_on_one_gpu():
     """Two shards of the eight-block domain, each with its own context (nmb = 4) and read-only mirror
-    blocks behind its own; the mirror refresh is done here by plain device copies in lock-step (one
-    GPU, no waiting kernels) in place of the NCCL point-to-point operations.  Equals the oracle."""
+    blocks behind its own (NaN until delivered).  The refresh is the slab path of halo.HaloPlan.refresh
+    with the NCCL point-to-point operations replaced by device copies between the packed buffers, in
+    lock-step (one GPU, no waiting kernels): ak_halo_pack -> copy -> ak_halo_unpack.  Equals the oracle."""
     import torch
     from paper_2409_10384_b200 import halo
     from test_oracle_exchange import lattice_nbr
@@ -258,7 +259,8 @@ def test_two_shards_with_mirror_blocks_on_one_gpu():
         plan = halo.HaloPlan(nbr, r, 2)
         lo, hi = plan.lo, plan.hi
         mk = lambda a: torch.cat([torch.from_numpy(np.ascontiguousarray(a[lo:hi])),
-                                  torch.zeros((plan.n_total - plan.n_own,) + a.shape[1:], dtype=torch.float64)]).to(dev)
+                                  torch.full((plan.n_total - plan.n_own,) + a.shape[1:], float("nan"),
+                                             dtype=torch.float64)]).to(dev)
         sh = ak.shapes(plan.n_own, dom["p"]["n"])
         z = lambda k: torch.zeros(sh[k], dtype=torch.float64, device=dev)
         st = dict(plan=plan, U=[mk(u) for u in dom["U"]], Bf=[mk(b) for b in dom["Bf"]],
@@ -271,13 +273,22 @@ def test_two_shards_with_mirror_blocks_on_one_gpu():
         st["ops"] = halo.AkOps(st["ctx"], plan, (0, 0, 0), st["W"], st["dU"], st["E"])
         ranks.append(st)
 
+    n = dom["p"]["n"]
+    for st in ranks:
+        sd, ss, rd, rs = st["plan"].slab_tables(n)
+        st["tables"] = (sd, ss, rd, rs)
+        st["bufs"] = st["ops"].halo_buffers(sum(l for _, l in ss.values()), sum(l for _, l in rs.values()))
+
     def refresh():
+        for st in ranks:
+            st["ops"].pack(st["tables"][0], st["U"], st["Bf"], st["bufs"][0])
         for me in ranks:
             other = ranks[1 - me["plan"].rank]
-            for q, g in enumerate(me["plan"].mirrors):
-                src = g - other["plan"].lo
-                for t_me, t_ot in zip(me["U"] + me["Bf"], other["U"] + other["Bf"]):
-                    t_me[me["plan"].n_own + q].copy_(t_ot[src])
+            (a, l), (b, l2) = me["tables"][3][other["plan"].rank], other["tables"][1][me["plan"].rank]
+            assert l == l2
+            me["bufs"][1][a:a + l].copy_(other["bufs"][0][b:b + l])
+        for st in ranks:
+            st["ops"].unpack(st["tables"][2], st["bufs"][1], st["U"], st["Bf"])
     try:
         dt = dom["dt"]
         for _ in range(2):
@@ -303,6 +314,53 @@ def test_two_shards_with_mirror_blocks_on_one_gpu():
     finally:
         for st in ranks:
             ak.ak_destroy(st["ctx"])
+
+
+@pytest.mark.parametrize("n", [6, 16, 32])
+def test_halo_pack_unpack_equal_numpy_slicing(n):
+    """ak_halo_pack / ak_halo_unpack against slicing the boxes out with numpy (the slab rule itself is
+    pinned to the oracle's exchange in test_multirank_cpu.py): all 26 codes of two blocks, buffer
+    bit for bit; unpacking into NaN blocks writes exactly the boxes."""
+    import torch
+    from paper_2409_10384_b200 import halo
+    from test_multirank_cpu import numpy_slabs
+    nmb = 3
+    sh = ak.shapes(nmb, n)
+    rng = np.random.default_rng(n)
+    keys = ["cell"] * 5 + ["xf", "yf", "zf"]
+    F = [rng.uniform(-1, 1, sh[k]) for k in keys]
+    desc, off = [], 0
+    ctx = ak.ak_create(ak.make_params(nmb=nmb, n=n, gamma_ad=2.0, rho_atm=1e-10, T_atm=1e-8), np.full((nmb, 3), 0.1))
+    try:
+        for blk in (2, 0):
+            for code in range(27):
+                if code == 13:
+                    continue
+                desc.append((blk, code, off))
+                ne = ak.ak_halo_slab_elems(ctx, code)
+                assert ne == halo.slab_elems(n, 4, code)
+                off += ne
+        desc = np.array(desc, dtype=np.int64)
+        ref = np.zeros(off)
+        numpy_slabs(desc, F, ref, n, unpack=False)
+        dF = _dev(F)
+        ddesc = torch.from_numpy(desc).cuda()
+        buf = torch.full((off,), float("nan"), dtype=torch.float64, device="cuda")
+        ak.ak_halo_pack(ctx, ddesc, dF[:5], dF[5:], buf)
+        torch.cuda.synchronize()
+        assert np.array_equal(buf.cpu().numpy(), ref)
+        G = [np.full(sh[k], np.nan) for k in keys]
+        numpy_slabs(desc, G, ref, n, unpack=True)
+        dG = [torch.full(sh[k], float("nan"), dtype=torch.float64, device="cuda") for k in keys]
+        ak.ak_halo_unpack(ctx, ddesc, buf, dG[:5], dG[5:])
+        torch.cuda.synchronize()
+        for a, b in zip(_np(dG), G):
+            assert np.array_equal(a, b, equal_nan=True)
+            assert np.isnan(a[1]).all() and not np.isnan(a[0]).all()
+        with pytest.raises(ValueError):
+            ak.ak_halo_slab_elems(ctx, 13)
+    finally:
+        ak.ak_destroy(ctx)
 
 
 # ---------------------------------------------------------------- the paper's loop advection (P:226-250)

@@ -119,12 +119,36 @@ def _eight_block_domain():
                 adm=[cat("adm", q) for q in range(16)], dx=np.full((8, 3), d), p=p, dt=0.15 * d)
 
 
+def numpy_slabs(desc, fields, buf, n, unpack, ng=4):
+    """pack/unpack by numpy slicing: the eight boxes of every (block, code) pair, k-major, in order."""
+    from paper_2409_10384_b200 import halo
+    for blk, code, off in desc:
+        for fld in range(8):
+            (sx, ex), (sy, ey), (sz, ez) = halo.slab_box(n, ng, int(code), fld)
+            view = fields[fld][blk, sz:sz + ez, sy:sy + ey, sx:sx + ex]
+            cnt = ex * ey * ez
+            if unpack:
+                view[...] = buf[off:off + cnt].reshape(ez, ey, ex)
+            else:
+                buf[off:off + cnt] = view.reshape(-1)
+            off += cnt
+
+
 class _OracleOps:
     """halo.advance `ops` backed by the CPU oracle (numpy views of the CPU tensors)."""
 
-    def __init__(self, par, plan, dx, adm, bc):
+    def __init__(self, par, plan, dx, adm, bc, n):
         from oracle import pyoracle as orc
-        self.orc, self.par, self.plan, self.dx, self.adm, self.bc = orc, par, plan, dx, adm, bc
+        self.orc, self.par, self.plan, self.dx, self.adm, self.bc, self.n = orc, par, plan, dx, adm, bc, n
+
+    def halo_buffers(self, nsend, nrecv):
+        return torch.zeros(nsend, dtype=torch.float64), torch.zeros(nrecv, dtype=torch.float64)
+
+    def pack(self, desc, U, Bf, buf):
+        numpy_slabs(desc, [u.numpy() for u in U] + [b.numpy() for b in Bf], buf.numpy(), self.n, unpack=False)
+
+    def unpack(self, desc, buf, U, Bf):
+        numpy_slabs(desc, [u.numpy() for u in U] + [b.numpy() for b in Bf], buf.numpy(), self.n, unpack=True)
 
     def fill(self, U, Bf):
         self.orc.exchange_ghosts(self.par, self.plan.local_nbr, self.bc, [u.numpy() for u in U], [b.numpy() for b in Bf])
@@ -142,7 +166,7 @@ class _OracleOps:
                               [u.numpy() for u in U], [x.numpy() for x in Bf], dU, E)
 
 
-def _halo_worker(rank, world, port, out):
+def _halo_worker(rank, world, port, out, whole_blocks=False):
     from oracle import pyoracle as orc
     from paper_2409_10384_b200 import halo
     from test_oracle_exchange import lattice_nbr
@@ -156,13 +180,15 @@ def _halo_worker(rank, world, port, out):
         lo, hi = plan.lo, plan.hi
 
         def with_mirrors(a):
-            t = torch.zeros((plan.n_total,) + a.shape[1:], dtype=torch.float64)
+            # mirrors start as NaN: anything the ghost fill reads of them must have been delivered
+            t = torch.full((plan.n_total,) + a.shape[1:], float("nan"), dtype=torch.float64)
             t[:plan.n_own] = torch.from_numpy(a[lo:hi])
             return t
         U = [with_mirrors(u) for u in dom["U"]]; Bf = [with_mirrors(b) for b in dom["Bf"]]
         par = orc.make_params(nmb=plan.n_own, **dom["p"])
-        ops = _OracleOps(par, plan, dom["dx"][lo:hi], [np.ascontiguousarray(a[lo:hi]) for a in dom["adm"]], (0, 0, 0))
-        halo.advance(plan, ops, 3, 2, dom["dt"], U, Bf)
+        ops = _OracleOps(par, plan, dom["dx"][lo:hi], [np.ascontiguousarray(a[lo:hi]) for a in dom["adm"]], (0, 0, 0),
+                         dom["p"]["n"])
+        halo.advance(plan, ops, 3, 2, dom["dt"], U, Bf, whole_blocks=whole_blocks)
         payload = dict(lo=lo, hi=hi, U=[u[:plan.n_own].numpy().copy() for u in U],
                        Bf=[b[:plan.n_own].numpy().copy() for b in Bf], mirrors=plan.mirrors)
         gathered = [None] * world if rank == 0 else None
@@ -193,7 +219,9 @@ def test_halo_plan_tables():
     assert one.n_total == 8 and not one.send and not one.recv and np.array_equal(one.local_nbr, nbr)
 
 
-def test_two_ranks_with_halo_exchange_equal_one_process():
+@pytest.mark.parametrize("whole_blocks", [False, True])
+def test_two_ranks_with_halo_exchange_equal_one_process(whole_blocks):
+    """ghost slabs (default) and whole-block mirrors both reproduce the single-process run bit for bit."""
     from oracle import pyoracle as orc
     from test_oracle_exchange import lattice_nbr
     orc.build()
@@ -201,7 +229,7 @@ def test_two_ranks_with_halo_exchange_equal_one_process():
     ctx = mp.get_context("spawn")
     q = ctx.Queue()
     port = _free_port()
-    procs = [ctx.Process(target=_halo_worker, args=(r, world, port, q)) for r in range(world)]
+    procs = [ctx.Process(target=_halo_worker, args=(r, world, port, q, whole_blocks)) for r in range(world)]
     for p in procs:
         p.start()
     gathered = q.get(timeout=300)
@@ -219,3 +247,51 @@ def test_two_ranks_with_halo_exchange_equal_one_process():
             assert np.array_equal(part["U"][v], U[v][lo:hi]), (lo, v)
         for c in range(3):
             assert np.array_equal(part["Bf"][c], Bf[c][lo:hi]), (lo, c)
+
+
+def test_slab_boxes_are_what_the_exchange_reads():
+    """Pin of the slab index rule (include/ak.h, halo.slab_box) against the oracle's ghost exchange: on
+    a periodic 3x3x3 lattice every element carries its own address; after orc.exchange_ghosts the
+    ghosts of block 0 tell which elements of which neighbour were read.  For every neighbour code
+    that set equals the slab box, except that a face field's box keeps face ie+1 along its normal
+    where the offset is 0 (read only when the reader has no upper image there)."""
+    from oracle import pyoracle as orc
+    from paper_2409_10384_b200 import halo
+    from test_oracle_exchange import lattice_nbr
+    n, ng, nmb = 6, 4, 27
+    nt = n + 2 * ng
+    sh = orc.shapes(nmb, n)
+    nbr = lattice_nbr((3, 3, 3), (True, True, True))
+    keys = ["cell"] * 5 + ["xf", "yf", "zf"]
+    fields = []
+    for k in keys:
+        per = int(np.prod(sh[k][1:]))
+        fields.append((np.arange(nmb)[:, None] * 1e6 + np.arange(per)[None, :]).reshape(sh[k]).astype(np.float64))
+    before = [f.copy() for f in fields]
+    orc.exchange_ghosts(orc.make_params(nmb=nmb, n=n), nbr, (0, 0, 0), fields[:5], fields[5:])
+    code_of = {int(nbr[0, c]): c for c in range(27) if c != 13}
+    assert len(code_of) == 26
+    for fld, k in enumerate(keys):
+        shape = sh[k][1:]
+        got = fields[fld][0]
+        changed = got != before[fld][0]
+        src_blk = (got[changed] // 1e6).astype(int)
+        src_idx = (got[changed] % 1e6).astype(int)
+        assert 0 not in set(src_blk.tolist())
+        for blk, code in code_of.items():
+            read = set(src_idx[src_blk == blk].tolist())
+            (sx, ex), (sy, ey), (sz, ez) = halo.slab_box(n, ng, code, fld)
+            box = np.zeros(shape, dtype=bool)
+            box[sz:sz + ez, sy:sy + ey, sx:sx + ex] = True
+            boxset = set(np.flatnonzero(box).tolist())
+            assert read <= boxset, (fld, code)
+            extra = boxset - read
+            if fld < 5:
+                assert not extra, (fld, code)
+            else:
+                a = fld - 5                                              # normal axis: 0 x, 1 y, 2 z
+                o = (code % 3 - 1, (code // 3) % 3 - 1, code // 9 - 1)[a]
+                idx = np.array(sorted(extra), dtype=int)
+                coord = np.unravel_index(idx, shape)[2 - a] if idx.size else idx
+                assert (o == 0 and np.all(coord == ng + n)) or idx.size == 0, (fld, code)
+        assert sum(halo.slab_elems(n, ng, c) for c in code_of.values()) > 0
