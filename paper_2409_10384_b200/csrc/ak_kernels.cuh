@@ -211,7 +211,10 @@ __global__ void __launch_bounds__(128, AK_FOFC_MINB) k_fofc_test(const __grid_co
   const double Ds = Us[0], ts = Us[4];
   int st = c2p_cell<false>(P, g, Us, Bc, W5);
   if (P.dmp_M > 0.0) {
-    double Dmin = f.U[0][c], Dmax = Dmin, tmin = f.U[4][c], tmax = tmin;
+    // fmin/fmax over the 27 cells (the centre is one of them) written as compare-and-select from
+    // +-inf: the same values for every input (a NaN is skipped either way; only the sign of a zero
+    // can differ, which no comparison below sees) at a third of the instructions of fmin/fmax.
+    double Dmin = CUDART_INF, Dmax = -CUDART_INF, tmin = CUDART_INF, tmax = -CUDART_INF;
     const long long sy = P.nt, sz = (long long)P.nt * P.nt;
 #ifndef AK_DMP_UNROLL
 #define AK_DMP_UNROLL 1
@@ -225,8 +228,8 @@ __global__ void __launch_bounds__(128, AK_FOFC_MINB) k_fofc_test(const __grid_co
         for (int ii = -1; ii <= 1; ++ii) {
           const long long cn = c + kk * sz + jj * sy + ii;
           const double d = f.U[0][cn], t = f.U[4][cn];
-          Dmin = fmin(Dmin, d); Dmax = fmax(Dmax, d);
-          tmin = fmin(tmin, t); tmax = fmax(tmax, t);
+          Dmin = d < Dmin ? d : Dmin; Dmax = d > Dmax ? d : Dmax;
+          tmin = t < tmin ? t : tmin; tmax = t > tmax ? t : tmax;
         }
     if (Ds < Dmin * P.dmp_iM || Ds > P.dmp_M * Dmax || ts < tmin * P.dmp_iM || ts > P.dmp_M * tmax)
       st |= ST_DMP;
