@@ -2,12 +2,6 @@
 // Build: nvcc -gencode arch=compute_100a,code=sm_100a --fmad=false -lineinfo (see build.py).
 #include "../../include/ak.h"
 #include "ak_source.cuh"
-#ifndef AK_FLUX_TILE
-#define AK_FLUX_TILE 0   // 1: shared-memory tiled sweeps (ak_flux_tile.cuh); measured slower, see profiles/
-#endif
-#if AK_FLUX_TILE
-#include "ak_flux_tile.cuh"
-#endif
 #ifndef AK_FLUX_TMA
 #define AK_FLUX_TMA 1   // 1: TMA-staged sweeps (ak_flux_tma.cuh) when n is even and a face row fits a block
 #endif
@@ -219,29 +213,6 @@ int launch_flux(ak_ctx* c, const Fields& f) {
       return AK_OK;
     }
   }
-#if AK_FLUX_TILE
-  // tile shape (ak_flux_tile.cuh): x sweeps take whole pencils, y/z sweeps 32 pencils x 8 cells
-  int NA, NB;
-#ifndef AK_TILE_NB_X
-#define AK_TILE_NB_X 16
-#endif
-#ifndef AK_TILE_NA_YZ
-#define AK_TILE_NA_YZ 8
-#endif
-  if (DIR == 0) { NA = n + 4 < TILE_MAX_THREADS ? n + 4 : TILE_MAX_THREADS; NB = TILE_MAX_THREADS / NA; if (NB > AK_TILE_NB_X) NB = AK_TILE_NB_X; }
-  else { NA = AK_TILE_NA_YZ; NB = 32; }
-  const long long np_all = (long long)c->P.nmb * (n + 2) * (n + 2);
-  const dim3 g(nblk(np_all, NB), (unsigned)((n + 3 + NA - 2) / (NA - 1)));
-  const int bd = NA * NB;
-  const size_t smem = sizeof(double) * TILE_SMEM_DOUBLES * bd;
-  switch (c->P.recon) {
-    case 0: k_flux_tile<DIR, 0><<<g, bd, smem, c->stream>>>(c->P, f, NA, NB); break;
-    case 1: k_flux_tile<DIR, 1><<<g, bd, smem, c->stream>>>(c->P, f, NA, NB); break;
-    case 3: k_flux_tile<DIR, 3><<<g, bd, smem, c->stream>>>(c->P, f, NA, NB); break;
-    case 4: k_flux_tile<DIR, 4><<<g, bd, smem, c->stream>>>(c->P, f, NA, NB); break;
-    default: k_flux_tile<DIR, 2><<<g, bd, smem, c->stream>>>(c->P, f, NA, NB); break;
-  }
-#else
   const long long nf = (long long)(n + 3) * (n + 2) * (n + 2) * c->P.nmb;
   const unsigned g = nblk(nf, 128);
   switch (c->P.recon) {
@@ -251,7 +222,6 @@ int launch_flux(ak_ctx* c, const Fields& f) {
     case 4: k_flux<DIR, 4><<<g, 128, 0, c->stream>>>(c->P, f); break;
     default: k_flux<DIR, 2><<<g, 128, 0, c->stream>>>(c->P, f); break;
   }
-#endif
   CK(cudaGetLastError());
   c->launches[KC_FX + DIR] += 1;
   return AK_OK;
