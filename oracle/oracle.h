@@ -45,6 +45,11 @@ typedef struct {
   double dmp_M;                  /* Eq. 12; <=0 off                          */
   int c2p_max_iter;
   double c2p_tol;
+  /* equation of state (oracle/eos.h): 0 ideal gas with gamma_ad; 1 piecewise-polytropic hybrid
+   * (reading R29) with pp_nseg (1..4) segments of exponent pp_gamma[i], the
+   * first with constant pp_K0, breakpoints pp_rho[0] < pp_rho[1] < ..., thermal gamma_th. */
+  int eos, pp_nseg;
+  double pp_K0, pp_gamma[4], pp_rho[3], gamma_th;
 } orc_params;
 
 /* status / flag bits */
@@ -61,6 +66,14 @@ void orc_metric_inverse(const double g[6], double* det, double* sdet, double gin
 void orc_prim2cons(double gamma_ad, const double g[6], const double prim[5],
                    const double B[3], double cons[5]);
 
+/* Same with the equation of state of p (ideal gas or hybrid). */
+void orc_prim2cons_eos(const orc_params* p, const double g[6], const double prim[5],
+                       const double B[3], double cons[5]);
+
+/* O1 for the EOS of p: out = {P(rho,eps), h-1 and c_s^2 at (rho, P(rho,eps)), P_c, eps_c}
+ * (P_c = eps_c = 0 for the ideal gas). */
+void orc_eos_point(const orc_params* p, double rho, double eps, double out[5]);
+
 /* O3: Ut = densitised {D,S_i,tau} (rewritten if floored and !check_only),
  * Btcc = densitised cell-centred B, W out = {rho,ux,uy,uz,P}.
  * Returns the status byte; *iters = master-function evaluations used. */
@@ -70,6 +83,9 @@ int orc_con2prim_cell(const orc_params* p, const double g[6], double Ut[5],
 /* O3 master function f(mu) exposed for the zero-at-true-root pin.
  * in: q, r2, bs2 (= B^2/D), rb2 (= (r_i B^i)^2 / D). */
 double orc_c2p_master(double gamma_ad, double q, double r2, double bs2, double rb2, double mu);
+/* the same for the EOS of p; D = undensitised conserved density (rho^ = D / W^). */
+double orc_c2p_master_eos(const orc_params* p, double D, double q, double r2, double bs2,
+                          double rb2, double mu);
 
 /* O4: q[5] = cells i-2..i+2; qm = value at the left face of cell i, qp at the right. */
 void orc_reconstruct(int kind, const double q[5], double* qm, double* qp);

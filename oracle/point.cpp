@@ -2,6 +2,7 @@
 // see oracle.h).  Build with -O2 -ffp-contract=off: every operation below is a single
 // IEEE fp64 +,-,*,/,sqrt,fmin,fmax or comparison, evaluated in the order written.
 #include "oracle.h"
+#include "eos.h"
 #include <cmath>
 
 namespace {
@@ -45,8 +46,9 @@ extern "C" void orc_metric_inverse(const double g[6], double* det, double* sdet,
 // Eq. 6 with the ideal gas h = 1 + Gamma/(Gamma-1) T, T = P/rho
 // ("temperature"; P = rho T pinned by P:283).  tau in the algebraically
 // identical cancellation-free form (DESIGN.md §3 O2).
-extern "C" void orc_prim2cons(double gamma_ad, const double g[6], const double prim[5],
-                              const double B[3], double cons[5]) {
+namespace {
+void prim2cons_eos(const OrcEos& e, const double g[6], const double prim[5], const double B[3],
+                   double cons[5]) {
   const double rho = prim[0], P = prim[4];
   const double u[3] = {prim[1], prim[2], prim[3]};
   double ul[3], Bl[3];
@@ -58,9 +60,7 @@ extern "C" void orc_prim2cons(double gamma_ad, const double g[6], const double p
   lower(g, B, Bl);
   const double B2 = dot(Bl, B);
   const double Bv = B[0] * vl[0] + B[1] * vl[1] + B[2] * vl[2];
-  const double gm1r = gamma_ad / (gamma_ad - 1.0);
-  const double T = P / rho;
-  const double hm1 = gm1r * T;
+  const double hm1 = eos_hm1(e, rho, P);
   const double h = 1.0 + hm1;
   const double D = rho * W;
   const double wtot = rho * h * W * W + B2;
@@ -70,12 +70,31 @@ extern "C" void orc_prim2cons(double gamma_ad, const double g[6], const double p
   cons[3] = wtot * vl[2] - Bv * Bl[2];
   cons[4] = D * (hm1 * W + usq / (1.0 + W)) + B2 - P - 0.5 * (Bv * Bv + B2 * iW * iW);
 }
+}  // namespace
+
+extern "C" void orc_prim2cons(double gamma_ad, const double g[6], const double prim[5],
+                              const double B[3], double cons[5]) {
+  orc_params ideal{};
+  ideal.gamma_ad = gamma_ad;
+  prim2cons_eos(orc_make_eos(&ideal), g, prim, B, cons);
+}
+extern "C" void orc_prim2cons_eos(const orc_params* p, const double g[6], const double prim[5],
+                                  const double B[3], double cons[5]) {
+  prim2cons_eos(orc_make_eos(p), g, prim, B, cons);
+}
+extern "C" void orc_eos_point(const orc_params* p, double rho, double eps, double out[5]) {
+  const OrcEos e = orc_make_eos(p);
+  out[0] = eos_P(e, rho, eps);
+  eos_hm1_cs2(e, rho, out[0], out[1], out[2]);
+  out[3] = 0.0; out[4] = 0.0;
+  if (e.kind == 1) { double Gi; eos_cold(e, rho, out[3], out[4], Gi); }
+}
 
 // ---------------------------------------------------------------- O3 -------
 // Master function of the bracketed 1-D solve for mu = 1/(W h) ("based on
 // the algorithm presented in Kastaun et al. (2021)").  h0 = 1 for the ideal gas.
 namespace {
-struct C2PState { double q, r2, bs2, rb2, v0sq, gm1; };
+struct C2PState { double q, r2, bs2, rb2, v0sq, gm1; const OrcEos* eos; double D; };
 struct C2PAux { double x, rbar2, qbar, vsq, iW, What, eps; };
 
 inline void c2p_aux(const C2PState& s, double mu, C2PAux& a) {
@@ -90,8 +109,18 @@ inline void c2p_aux(const C2PState& s, double mu, C2PAux& a) {
 inline double c2p_f(const C2PState& s, double mu) {
   C2PAux a;
   c2p_aux(s, mu, a);
-  const double eps = std::fmax(a.eps, 0.0);
-  const double ahat = s.gm1 * eps / (1.0 + eps);  // P/(rho(1+eps)) for P=(Gamma-1) rho eps
+  double eps, ahat;
+  if (s.eos->kind == 0) {
+    eps = std::fmax(a.eps, 0.0);
+    ahat = s.gm1 * eps / (1.0 + eps);  // P/(rho(1+eps)) for P=(Gamma-1) rho eps
+  } else {                             // general form: a^ = P(rho^, eps^) / (rho^ (1 + eps^))
+    const double rhohat = s.D * a.iW;
+    double Pc, epsc, Gi;
+    eos_cold(*s.eos, rhohat, Pc, epsc, Gi);
+    eps = std::fmax(a.eps, epsc);      // eps^ clamped into the EOS range (eps >= eps_c)
+    const double Phat = Pc + s.eos->gthm1 * rhohat * (eps - epsc);
+    ahat = Phat / (rhohat * (1.0 + eps));
+  }
   const double nuA = (1.0 + ahat) * (1.0 + eps) * a.iW;
   const double nuB = (1.0 + ahat) * (1.0 + a.qbar - mu * a.rbar2);
   return mu - 1.0 / (std::fmax(nuA, nuB) + mu * a.rbar2);
@@ -133,7 +162,16 @@ inline bool illinois(const C2PState& s, int which, double a, double b, double fa
 
 extern "C" double orc_c2p_master(double gamma_ad, double q, double r2, double bs2, double rb2,
                                  double mu) {
-  C2PState s{q, r2, bs2, rb2, r2 / (1.0 + r2), gamma_ad - 1.0};
+  orc_params ideal{};
+  ideal.gamma_ad = gamma_ad;
+  const OrcEos e = orc_make_eos(&ideal);
+  C2PState s{q, r2, bs2, rb2, r2 / (1.0 + r2), gamma_ad - 1.0, &e, 1.0};
+  return c2p_f(s, mu);
+}
+extern "C" double orc_c2p_master_eos(const orc_params* p, double D, double q, double r2, double bs2,
+                                     double rb2, double mu) {
+  const OrcEos e = orc_make_eos(p);
+  C2PState s{q, r2, bs2, rb2, r2 / (1.0 + r2), e.gm1, &e, D};
   return c2p_f(s, mu);
 }
 
@@ -141,9 +179,9 @@ extern "C" int orc_con2prim_cell(const orc_params* p, const double g[6], double 
                                  const double Btcc[3], double Wout[5], int check_only,
                                  int* iters) {
   int status = 0, nev = 0;
-  const double gm1 = p->gamma_ad - 1.0;
-  const double eps_atm = p->T_atm / gm1;
-  const double P_atm = p->rho_atm * p->T_atm;
+  const OrcEos eos = orc_make_eos(p);
+  const double gm1 = eos.gm1;
+  const double P_atm = eos_P_at_T(eos, p->rho_atm, p->T_atm);
   double det, sdet, gi[6];
   orc_metric_inverse(g, &det, &sdet, gi);
   const double isd = 1.0 / sdet;
@@ -171,11 +209,11 @@ extern "C" int orc_con2prim_cell(const orc_params* p, const double g[6], double 
   }
   if (solve && B2 > p->mag_max * D) { D = B2 / p->mag_max; status |= ORC_MAGCAP; }
   if (solve && atmo) {
-    rho = D; P = D * p->T_atm;   // u = 0
+    rho = D; P = eos_P_at_T(eos, D, p->T_atm);   // u = 0
     solve = false;
   }
   if (solve) {
-    const double tau_atm = D * eps_atm + 0.5 * B2;
+    const double tau_atm = D * eos_eps_at_T(eos, D, p->T_atm) + 0.5 * B2;
     if (tau < tau_atm) { tau = tau_atm; status |= ORC_TAUFLOOR; }
     // step 4
     const double iD = 1.0 / D;
@@ -191,6 +229,8 @@ extern "C" int orc_con2prim_cell(const orc_params* p, const double g[6], double 
     s.rb2 = rB * rB * iD;
     s.v0sq = s.r2 / (1.0 + s.r2);
     s.gm1 = gm1;
+    s.eos = &eos;
+    s.D = D;
     // step 5: bracket
     bool ok = true;
     double mu_hi = 1.0;
@@ -216,8 +256,7 @@ extern "C" int orc_con2prim_cell(const orc_params* p, const double g[6], double 
       C2PAux a;
       c2p_aux(s, mu, a);
       rho = D * a.iW;
-      const double T = gm1 * a.eps;
-      P = rho * T;
+      P = eos_P(eos, rho, a.eps);
       const double c = mu * rB * iD;
       const double mx = mu * a.x;
       ux = a.What * (mx * (ru[0] + c * B[0]));
@@ -233,15 +272,14 @@ extern "C" int orc_con2prim_cell(const orc_params* p, const double g[6], double 
   if (rho < p->f_thr * p->rho_atm) {
     rho = p->rho_atm; ux = uy = uz = 0.0; P = P_atm;
     status |= ORC_RHOFLOOR;
-  } else if (P < rho * p->T_atm) {
-    P = rho * p->T_atm;
+  } else if (eos_T_floor(eos, rho, p->T_atm, P)) {
     status |= ORC_TFLOOR;
   }
   Wout[0] = rho; Wout[1] = ux; Wout[2] = uy; Wout[3] = uz; Wout[4] = P;
   // step 8: "A similar policy holds for the conserved variables"
   if (status != 0 && !check_only) {
     double c5[5];
-    orc_prim2cons(p->gamma_ad, g, Wout, B, c5);
+    prim2cons_eos(eos, g, Wout, B, c5);
     for (int v = 0; v < 5; ++v) Ut[v] = sdet * c5[v];
   }
   if (iters) *iters = nev;
@@ -357,7 +395,7 @@ struct Side { double U[7], F[7], lm, lp; };
 
 // One side of the Riemann problem at a face of direction d (Eq. 8).
 // prim = {rho,u^x,u^y,u^z,P}; Bt1,Bt2 densitised transverse B; Bd undensitised normal B.
-inline void side_state(double gamma_ad, int d, const double g[6], double gdd, double sdet,
+inline void side_state(const OrcEos& eos, int d, const double g[6], double gdd, double sdet,
                        double isd, double alp, double ialp, const double bet[3],
                        const double prim[5], double Bt1t, double Bt2t, double Bd, Side& s) {
   const int t1 = (d + 1) % 3, t2 = (d + 2) % 3;
@@ -379,9 +417,8 @@ inline void side_state(double gamma_ad, int d, const double g[6], double gdd, do
   const double bl[3] = {Bl[0] * iW + Bv * ul[0], Bl[1] * iW + Bv * ul[1],
                         Bl[2] * iW + Bv * ul[2]};
   const double ab0 = W * Bv;                                       // alpha b^0 (Eq. 7a)
-  const double gm1r = gamma_ad / (gamma_ad - 1.0);
-  const double T = P / rho;
-  const double hm1 = gm1r * T;
+  double hm1, cs2;
+  eos_hm1_cs2(eos, rho, P, hm1, cs2);
   const double h = 1.0 + hm1;
   const double Ptot = P + 0.5 * b2;
   const double D = rho * W;
@@ -407,7 +444,6 @@ inline void side_state(double gamma_ad, int d, const double g[6], double gdd, do
   s.F[6] = sdet * (alp * (B[t2] * vh[d] - B[d] * vh[t2]));
   // signal speeds: fast-magnetosonic bound (DESIGN.md §3 O6)
   const double vsq = v[0] * vl[0] + v[1] * vl[1] + v[2] * vl[2];
-  const double cs2 = gamma_ad * T / h;                  // Gamma P / (rho h)
   const double rhoh = rho * h;
   const double va2 = b2 / (rhoh + b2);
   const double a2 = cs2 + va2 - cs2 * va2;
@@ -421,12 +457,12 @@ inline void side_state(double gamma_ad, int d, const double g[6], double gdd, do
 }
 
 // face-state floor of P:139 ("after reconstruction")
-inline void face_floor(const orc_params* p, double prim[5]) {
+inline void face_floor(const orc_params* p, const OrcEos& eos, double prim[5]) {
   if (prim[0] < p->f_thr * p->rho_atm) {
     prim[0] = p->rho_atm; prim[1] = 0.0; prim[2] = 0.0; prim[3] = 0.0;
-    prim[4] = p->rho_atm * p->T_atm;
-  } else if (prim[4] < prim[0] * p->T_atm) {
-    prim[4] = prim[0] * p->T_atm;
+    prim[4] = eos_P_at_T(eos, p->rho_atm, p->T_atm);
+  } else {
+    eos_T_floor(eos, prim[0], p->T_atm, prim[4]);
   }
 }
 }  // namespace
@@ -448,10 +484,11 @@ extern "C" void orc_face_flux(const orc_params* p, int dir, int riemann, const d
   const double Bd = Bfd * isd;
   double pl[5] = {WL[0], WL[1], WL[2], WL[3], WL[4]};
   double pr[5] = {WR[0], WR[1], WR[2], WR[3], WR[4]};
-  if (apply_floor) { face_floor(p, pl); face_floor(p, pr); }
+  const OrcEos eos = orc_make_eos(p);
+  if (apply_floor) { face_floor(p, eos, pl); face_floor(p, eos, pr); }
   Side L, R;
-  side_state(p->gamma_ad, dir, g, gdd, sdet, isd, alp, ialp, bet, pl, WL[5], WL[6], Bd, L);
-  side_state(p->gamma_ad, dir, g, gdd, sdet, isd, alp, ialp, bet, pr, WR[5], WR[6], Bd, R);
+  side_state(eos, dir, g, gdd, sdet, isd, alp, ialp, bet, pl, WL[5], WL[6], Bd, L);
+  side_state(eos, dir, g, gdd, sdet, isd, alp, ialp, bet, pr, WR[5], WR[6], Bd, R);
   if (lam) { lam[0] = L.lm; lam[1] = L.lp; lam[2] = R.lm; lam[3] = R.lp; }
   if (riemann == 1) {  // HLLE
     const double lL = std::fmin(0.0, std::fmin(L.lm, R.lm));

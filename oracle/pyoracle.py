@@ -16,7 +16,7 @@ _SRC = ["point.cpp", "stage.cpp", "driver.cpp"]
 
 def build(force=False):
     """g++ -O2 -ffp-contract=off: no FMA contraction, IEEE fp64 in the written order."""
-    srcs = [os.path.join(_HERE, s) for s in _SRC] + [os.path.join(_HERE, "oracle.h")]
+    srcs = [os.path.join(_HERE, s) for s in _SRC] + [os.path.join(_HERE, "oracle.h"), os.path.join(_HERE, "eos.h")]
     if not force and os.path.exists(_SO) and all(
             os.path.getmtime(_SO) >= os.path.getmtime(s) for s in srcs):
         return _SO
@@ -32,7 +32,9 @@ class OrcParams(C.Structure):
                 ("f_thr", C.c_double), ("mag_max", C.c_double),
                 ("recon", C.c_int), ("riemann", C.c_int), ("fofc", C.c_int),
                 ("fofc_riemann", C.c_int), ("dmp_M", C.c_double),
-                ("c2p_max_iter", C.c_int), ("c2p_tol", C.c_double)]
+                ("c2p_max_iter", C.c_int), ("c2p_tol", C.c_double),
+                ("eos", C.c_int), ("pp_nseg", C.c_int), ("pp_K0", C.c_double),
+                ("pp_gamma", C.c_double * 4), ("pp_rho", C.c_double * 3), ("gamma_th", C.c_double)]
 
 
 _lib = None
@@ -47,14 +49,26 @@ def lib():
         _lib.orc_c2p_master.restype = C.c_double
         _lib.orc_c2p_master.argtypes = [C.c_double] * 6
         _lib.orc_con2prim_cell.restype = C.c_int
+        _lib.orc_c2p_master_eos.restype = C.c_double
+        _lib.orc_c2p_master_eos.argtypes = [C.c_void_p] + [C.c_double] * 6
     return _lib
 
 
 def make_params(nmb=1, n=4, gamma_ad=2.0, rho_atm=1e-10, T_atm=1e-8, f_thr=1.0,
                 mag_max=float("inf"), recon=1, riemann=1, fofc=1, fofc_riemann=0, dmp_M=0.0,
-                c2p_max_iter=40, c2p_tol=1e-15, **_ignored):
-    return OrcParams(nmb, n, 4, gamma_ad, rho_atm, T_atm, f_thr, mag_max, recon, riemann,
-                     fofc, fofc_riemann, dmp_M, c2p_max_iter, c2p_tol)
+                c2p_max_iter=40, c2p_tol=1e-15, eos_hybrid=None, **_ignored):
+    """eos_hybrid: None (ideal gas with gamma_ad) or dict(K0, gammas, rho_breaks, gamma_th)."""
+    p = OrcParams(nmb, n, 4, gamma_ad, rho_atm, T_atm, f_thr, mag_max, recon, riemann,
+                  fofc, fofc_riemann, dmp_M, c2p_max_iter, c2p_tol)
+    if eos_hybrid is not None:
+        gam, rb = list(eos_hybrid["gammas"]), list(eos_hybrid.get("rho_breaks", []))
+        assert 1 <= len(gam) <= 4 and len(rb) == len(gam) - 1
+        p.eos, p.pp_nseg, p.pp_K0, p.gamma_th = 1, len(gam), eos_hybrid["K0"], eos_hybrid["gamma_th"]
+        for i, x in enumerate(gam):
+            p.pp_gamma[i] = x
+        for i, x in enumerate(rb):
+            p.pp_rho[i] = x
+    return p
 
 
 def _d(a):
@@ -98,6 +112,24 @@ def con2prim_cell(par, g, Ut, Btcc, check_only=False):
     st = lib().orc_con2prim_cell(C.byref(par), gp, Ut.ctypes.data_as(_dp), bp,
                                  W.ctypes.data_as(_dp), int(check_only), C.byref(it))
     return st, W, Ut, it.value
+
+
+def prim2cons_eos(par, g, prim, B):
+    g, gp = _d(g); prim, pp = _d(prim); B, bp = _d(B)
+    out = np.zeros(5)
+    lib().orc_prim2cons_eos(C.byref(par), gp, pp, bp, out.ctypes.data_as(_dp))
+    return out
+
+
+def eos_point(par, rho, eps):
+    """{P(rho,eps), h-1, c_s^2, P_c, eps_c} of the EOS in par."""
+    out = np.zeros(5)
+    lib().orc_eos_point(C.byref(par), C.c_double(rho), C.c_double(eps), out.ctypes.data_as(_dp))
+    return out
+
+
+def c2p_master_eos(par, D, q, r2, bs2, rb2, mu):
+    return lib().orc_c2p_master_eos(C.byref(par), D, q, r2, bs2, rb2, mu)
 
 
 def c2p_master(gamma_ad, q, r2, bs2, rb2, mu):

@@ -2,6 +2,7 @@
 // (+DMP), O8 constrained-transport corner EMFs, O9 flux divergence + geometric sources.
 // Test infrastructure only (see oracle.h).  Straight loops, one MeshBlock at a time.
 #include "oracle.h"
+#include "eos.h"
 #include <cmath>
 #include <cstring>
 #include <functional>
@@ -274,7 +275,7 @@ struct Stage {
           const double prim[5] = {W[0][c], W[1][c], W[2][c], W[3][c], W[4][c]};
           const double B[3] = {W[5][c] * isd, W[6][c] * isd, W[7][c] * isd};
           double cons[5];
-          orc_prim2cons(p->gamma_ad, g, prim, B, cons);
+          orc_prim2cons_eos(p, g, prim, B, cons);
           const double rho = prim[0], P = prim[4];
           const double u[3] = {prim[1], prim[2], prim[3]};
           const double ul[3] = {g[0] * u[0] + g[1] * u[1] + g[2] * u[2],
@@ -291,7 +292,7 @@ struct Stage {
           const double b2 = B2 * iW * iW + Bv * Bv;
           const double bl[3] = {Bl[0] * iW + Bv * ul[0], Bl[1] * iW + Bv * ul[1],
                                 Bl[2] * iW + Bv * ul[2]};
-          const double h = 1.0 + p->gamma_ad / (p->gamma_ad - 1.0) * (P / rho);
+          const double h = 1.0 + eos_hm1(orc_make_eos(p), rho, P);
           const double Ptot = P + 0.5 * b2;
           const double wt = rho * h + b2;
           // S_ij = (rho h + b^2) u_i u_j + Ptot g_ij - b_i b_j ; packed xx,xy,xz,yy,yz,zz
@@ -361,7 +362,7 @@ extern "C" void orc_matter_sources(const orc_params* p, const double* const W[8]
     const double prim[5] = {W[0][c], W[1][c], W[2][c], W[3][c], W[4][c]};
     const double B[3] = {W[5][c] * isd, W[6][c] * isd, W[7][c] * isd};
     double cons[5];
-    orc_prim2cons(p->gamma_ad, g, prim, B, cons);
+    orc_prim2cons_eos(p, g, prim, B, cons);
     const double rho = prim[0], P = prim[4];
     const double u[3] = {prim[1], prim[2], prim[3]};
     const double ul[3] = {g[0] * u[0] + g[1] * u[1] + g[2] * u[2], g[1] * u[0] + g[3] * u[1] + g[4] * u[2],
@@ -375,7 +376,7 @@ extern "C" void orc_matter_sources(const orc_params* p, const double* const W[8]
     const double Bv = B[0] * vl[0] + B[1] * vl[1] + B[2] * vl[2];
     const double b2 = B2 * iW * iW + Bv * Bv;
     const double bl[3] = {Bl[0] * iW + Bv * ul[0], Bl[1] * iW + Bv * ul[1], Bl[2] * iW + Bv * ul[2]};
-    const double h = 1.0 + p->gamma_ad / (p->gamma_ad - 1.0) * (P / rho);
+    const double h = 1.0 + eos_hm1(orc_make_eos(p), rho, P);
     const double Ptot = P + 0.5 * b2;
     const double wt = rho * h + b2;
     out[0][c] = cons[4] + cons[0];

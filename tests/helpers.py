@@ -19,7 +19,7 @@ def random_spd(rng, strength=0.3):
     return np.array([m[i, j] for (i, j) in SYM])
 
 
-def tensor_state(alpha, beta_u, g6, rho, v_u, P, B_u, Gamma):
+def tensor_state(alpha, beta_u, g6, rho, v_u, P, B_u, Gamma, h=None):
     """Conserved (D,S_i,tau,B^i) and flux matrices F[j] (j = direction) of
     (D,S_x,S_y,S_z,tau,B^x,B^y,B^z), all multiplied by sqrt(gamma), from T^{mu nu}, *F^{mu nu}."""
     gam = sym6_to_mat(g6)
@@ -37,7 +37,8 @@ def tensor_state(alpha, beta_u, g6, rho, v_u, P, B_u, Gamma):
     b0 = W * (B_u @ v_l) / alpha                       # Eq. 7a
     b = np.concatenate([[b0], (B_u + alpha * b0 * u[1:]) / W])   # Eq. 7b
     b2 = b @ g4 @ b
-    h = 1.0 + Gamma / (Gamma - 1.0) * P / rho
+    if h is None:                                       # ideal gas; else the caller's specific enthalpy
+        h = 1.0 + Gamma / (Gamma - 1.0) * P / rho
     T = (rho * h + b2) * np.outer(u, u) + (P + 0.5 * b2) * g4i - np.outer(b, b)   # Eq. 2
     Fd = np.outer(b, u) - np.outer(u, b)               # Eq. 3: (*F)^{mu nu}
     D = alpha * rho * u[0]
