@@ -165,6 +165,23 @@ int ak_rhs_host(ak_ctx*, const ak_cons* U, const ak_faceB* Bf, const ak_prim* W,
  * replaced) = the step-start register; U0 == NULL restores U* = U - dt_fofc div F. */
 int ak_set_fofc_blend(ak_ctx*, const ak_cons* U0, double a, double b);
 
+/* Equation of state (S:§8(f) rank 3; "supports ideal gases and piecewise polytropic hybrid
+ * EOSs"; the paper prints no formula, D:§10 reading R29 fixes it).  After this call every part of
+ * the stage (con2prim, floors, fluxes, FOFC test, sources, ak_matter_sources) uses
+ *   cold curve, segment i (rho_breaks[i-1] <= rho < rho_breaks[i]):
+ *     P_c = K_i rho^Gamma_i,  eps_c = a_i + K_i rho^(Gamma_i-1)/(Gamma_i-1),
+ *     K_0 = K0, a_0 = 0, K_i and a_i continuous at the breakpoints;
+ *   P = P_c + (gamma_th-1) rho (eps - eps_c);  T = (P - P_c)/rho (so T_atm floors the thermal part
+ *   and K0 = 0 is the ideal gas with Gamma = gamma_th);  h = 1 + eps + P/rho;
+ *   c_s^2 = (Gamma_i P_c + gamma_th (P - P_c))/(rho h);  atmosphere P = P_c(rho_atm) + rho_atm T_atm.
+ * nseg in 1..4; gammas = HOST [nseg], each > 1; rho_breaks = HOST [nseg-1], positive and increasing
+ * (ignored for nseg = 1); K0 >= 0; gamma_th > 1: else AK_EINVAL, nothing changed.  The arrays are
+ * copied.  ak_params.gamma_ad is then unused.  nseg = 0 returns to the ideal gas of ak_params.
+ * rho^Gamma is the device pow(): results agree with a libm evaluation to rounding, not bit for bit.
+ * The hybrid stage runs the plain (not TMA-staged) flux sweeps. */
+int ak_set_eos_hybrid(ak_ctx*, int nseg, double K0, const double* gammas, const double* rho_breaks,
+                      double gamma_th);
+
 /* Same-level neighbour table for ak_fill_ghosts / ak_advance (D:§12; "interblock
  * communication"): nbr = HOST int [nmb][27], entry (oz+1)*9+(oy+1)*3+(ox+1) = index of the block
  * adjacent at offset (ox,oy,oz) in {-1,0,1}^3, -1 = none (entry 13, the block itself, is ignored).

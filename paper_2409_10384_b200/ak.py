@@ -22,7 +22,8 @@ EXPORTS = ("ak_create", "ak_set_metric", "ak_con2prim", "ak_rhs", "ak_emf", "ak_
            "ak_get_flux", "ak_rhs_host", "ak_timing", "ak_kernel_ms", "ak_probe_copy",
            "ak_probe_fp64", "ak_destroy", "ak_strerror", "ak_version",
            "ak_set_fofc_blend", "ak_fill_ghosts", "ak_stage_update", "ak_advance", "ak_set_neighbors",
-           "ak_matter_sources", "ak_halo_slab_elems", "ak_halo_pack", "ak_halo_unpack")
+           "ak_matter_sources", "ak_halo_slab_elems", "ak_halo_pack", "ak_halo_unpack",
+           "ak_set_eos_hybrid")
 BC_PERIODIC, BC_OUTFLOW = 0, 1
 
 _dp = C.POINTER(C.c_double)
@@ -104,6 +105,7 @@ def lib():
         L.ak_probe_copy.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_longlong, C.c_int, _dp]
         L.ak_probe_fp64.argtypes = [C.c_void_p, C.c_int, C.c_int, _dp]
         L.ak_destroy.argtypes = [C.c_void_p]
+        L.ak_set_eos_hybrid.argtypes = [C.c_void_p, C.c_int, C.c_double, _dp, _dp, C.c_double]
         L.ak_halo_slab_elems.restype = C.c_longlong
         L.ak_halo_slab_elems.argtypes = [C.c_void_p, C.c_int]
         L.ak_halo_pack.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.POINTER(AkCons), C.POINTER(AkFaceB), C.c_void_p]
@@ -253,6 +255,16 @@ def ak_set_fofc_blend(ctx, U0, a=0.0, b=1.0):
     else:
         u = _struct(AkCons, U0)
         _chk(lib().ak_set_fofc_blend(ctx, C.byref(u), float(a), float(b)), "ak_set_fofc_blend")
+
+
+def ak_set_eos_hybrid(ctx, K0, gammas, rho_breaks=(), gamma_th=2.0):
+    """Piecewise-polytropic hybrid EOS (include/ak.h); gammas = () returns to the ideal gas."""
+    g = (C.c_double * max(len(gammas), 1))(*[float(x) for x in gammas])
+    r = (C.c_double * max(len(rho_breaks), 1))(*[float(x) for x in rho_breaks])
+    if len(gammas) > 0 and len(rho_breaks) != len(gammas) - 1:
+        raise ValueError("rho_breaks must hold len(gammas) - 1 values")
+    _chk(lib().ak_set_eos_hybrid(ctx, len(gammas), C.c_double(float(K0)), g, r, C.c_double(float(gamma_th))),
+         "ak_set_eos_hybrid")
 
 
 def ak_fill_ghosts(ctx, bc, U, Bf):

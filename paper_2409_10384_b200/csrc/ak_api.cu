@@ -99,6 +99,13 @@ int validate(const ak_params* p, const double* dx3) {
   return AK_OK;
 }
 
+// the equation-of-state part of Par (ak_set_eos_hybrid), for the child contexts of ak_rhs_host
+inline void copy_eos(Par& d, const Par& s) {
+  d.eos = s.eos; d.nseg = s.nseg; d.gth = s.gth; d.gthm1 = s.gthm1; d.P_atm = s.P_atm;
+  for (int i = 0; i < 4; ++i) { d.ppK[i] = s.ppK[i]; d.ppG[i] = s.ppG[i]; d.ppa[i] = s.ppa[i]; }
+  for (int i = 0; i < 3; ++i) d.pprb[i] = s.pprb[i];
+}
+
 inline unsigned nblk(long long n, int t) { return (unsigned)((n + t - 1) / t); }
 
 struct Timer {
@@ -157,8 +164,12 @@ bool set_prim(Fields& f, const ak_prim* W) {
 int launch_c2p(ak_ctx* c, const Fields& f, bool with_emf) {
   Timer t(c, KC_C2P);
   CK(cudaMemsetAsync(c->stats, 0, sizeof(unsigned long long) * 3, c->stream));
-  if (with_emf) k_con2prim<true><<<nblk(c->sz.cell, 128), 128, 0, c->stream>>>(c->P, f);
-  else k_con2prim<false><<<nblk(c->sz.cell, 128), 128, 0, c->stream>>>(c->P, f);
+  const unsigned g = nblk(c->sz.cell, 128);
+  if (c->P.eos) {
+    if (with_emf) k_con2prim<true, 1><<<g, 128, 0, c->stream>>>(c->P, f);
+    else k_con2prim<false, 1><<<g, 128, 0, c->stream>>>(c->P, f);
+  } else if (with_emf) k_con2prim<true><<<g, 128, 0, c->stream>>>(c->P, f);
+  else k_con2prim<false><<<g, 128, 0, c->stream>>>(c->P, f);
   c->launches[KC_C2P] += 1;
   CK(cudaGetLastError());
   return AK_OK;
@@ -186,7 +197,9 @@ int launch_flux(ak_ctx* c, const Fields& f) {
   constexpr int AK_FLUX_CELL = (AK_FLUX_CELL_MASK >> DIR) & 1;
   // threads per row of a tile: faces (k_flux_tma) or cells (k_flux_tma_cell)
   const int nfi = AK_FLUX_CELL ? (DIR == 0 ? n + 4 : e) : (DIR == 0 ? n + 3 : e);
-  if (AK_FLUX_TMA && n % 2 == 0 && nfi * (AK_FLUX_CELL && DIR != 0 ? 2 : 1) <= TMA_THREADS) {
+  // the hybrid EOS runs the plain one-thread-per-face sweep (the TMA tiles are tuned for, and
+  // instantiated with, the ideal gas of the paper's runs)
+  if (AK_FLUX_TMA && !c->P.eos && n % 2 == 0 && nfi * (AK_FLUX_CELL && DIR != 0 ? 2 : 1) <= TMA_THREADS) {
     // tile height: as many rows as fit the block, balanced over the extent it tiles
     const int nfd = DIR == 0 ? e : n + 3;
     const int namax = TMA_THREADS / nfi - (AK_FLUX_CELL && DIR != 0 ? 1 : 0);
@@ -215,12 +228,22 @@ int launch_flux(ak_ctx* c, const Fields& f) {
   }
   const long long nf = (long long)(n + 3) * (n + 2) * (n + 2) * c->P.nmb;
   const unsigned g = nblk(nf, 128);
-  switch (c->P.recon) {
-    case 0: k_flux<DIR, 0><<<g, 128, 0, c->stream>>>(c->P, f); break;
-    case 1: k_flux<DIR, 1><<<g, 128, 0, c->stream>>>(c->P, f); break;
-    case 3: k_flux<DIR, 3><<<g, 128, 0, c->stream>>>(c->P, f); break;
-    case 4: k_flux<DIR, 4><<<g, 128, 0, c->stream>>>(c->P, f); break;
-    default: k_flux<DIR, 2><<<g, 128, 0, c->stream>>>(c->P, f); break;
+  if (c->P.eos) {
+    switch (c->P.recon) {
+      case 0: k_flux<DIR, 0, 1><<<g, 128, 0, c->stream>>>(c->P, f); break;
+      case 1: k_flux<DIR, 1, 1><<<g, 128, 0, c->stream>>>(c->P, f); break;
+      case 3: k_flux<DIR, 3, 1><<<g, 128, 0, c->stream>>>(c->P, f); break;
+      case 4: k_flux<DIR, 4, 1><<<g, 128, 0, c->stream>>>(c->P, f); break;
+      default: k_flux<DIR, 2, 1><<<g, 128, 0, c->stream>>>(c->P, f); break;
+    }
+  } else {
+    switch (c->P.recon) {
+      case 0: k_flux<DIR, 0><<<g, 128, 0, c->stream>>>(c->P, f); break;
+      case 1: k_flux<DIR, 1><<<g, 128, 0, c->stream>>>(c->P, f); break;
+      case 3: k_flux<DIR, 3><<<g, 128, 0, c->stream>>>(c->P, f); break;
+      case 4: k_flux<DIR, 4><<<g, 128, 0, c->stream>>>(c->P, f); break;
+      default: k_flux<DIR, 2><<<g, 128, 0, c->stream>>>(c->P, f); break;
+    }
   }
   CK(cudaGetLastError());
   c->launches[KC_FX + DIR] += 1;
@@ -237,7 +260,8 @@ int launch_fofc(ak_ctx* c, const Fields& f, double dt) {
     CK(cudaMemsetAsync(c->count, 0, sizeof(unsigned) * 4, c->stream));
     CK(cudaMemsetAsync(c->stats + S_FOFC_CELLS, 0, sizeof(unsigned long long) * 2, c->stream));
     if (c->P.fofc) {
-      k_fofc_test<<<nblk(ntest, 128), 128, 0, c->stream>>>(c->P, f, dt);
+      if (c->P.eos) k_fofc_test<1><<<nblk(ntest, 128), 128, 0, c->stream>>>(c->P, f, dt);
+      else k_fofc_test<0><<<nblk(ntest, 128), 128, 0, c->stream>>>(c->P, f, dt);
       c->launches[KC_FOFC_TEST] += 1;
       CK(cudaGetLastError());
     }
@@ -245,9 +269,15 @@ int launch_fofc(ak_ctx* c, const Fields& f, double dt) {
   if (c->P.fofc) {
     Timer t(c, KC_FOFC_FIX);
     const unsigned g = (unsigned)(nf < 148LL * 8 * 128 ? nblk(nf, 128) : 148 * 8);
-    k_fofc_reflux<0><<<g, 128, 0, c->stream>>>(c->P, f);
-    k_fofc_reflux<1><<<g, 128, 0, c->stream>>>(c->P, f);
-    k_fofc_reflux<2><<<g, 128, 0, c->stream>>>(c->P, f);
+    if (c->P.eos) {
+      k_fofc_reflux<0, 1><<<g, 128, 0, c->stream>>>(c->P, f);
+      k_fofc_reflux<1, 1><<<g, 128, 0, c->stream>>>(c->P, f);
+      k_fofc_reflux<2, 1><<<g, 128, 0, c->stream>>>(c->P, f);
+    } else {
+      k_fofc_reflux<0><<<g, 128, 0, c->stream>>>(c->P, f);
+      k_fofc_reflux<1><<<g, 128, 0, c->stream>>>(c->P, f);
+      k_fofc_reflux<2><<<g, 128, 0, c->stream>>>(c->P, f);
+    }
     CK(cudaGetLastError());
     c->launches[KC_FOFC_FIX] += 3;
   }
@@ -271,7 +301,8 @@ int launch_ct(ak_ctx* c, const Fields& f, bool have_cell_emf) {
 int launch_src(ak_ctx* c, const Fields& f) {
   Timer t(c, KC_SRC);
   const long long n = c->P.n;
-  k_div_src<<<nblk(n * n * n * c->P.nmb, 128), 128, 0, c->stream>>>(c->P, f);
+  if (c->P.eos) k_div_src<1><<<nblk(n * n * n * c->P.nmb, 128), 128, 0, c->stream>>>(c->P, f);
+  else k_div_src<0><<<nblk(n * n * n * c->P.nmb, 128), 128, 0, c->stream>>>(c->P, f);
   CK(cudaGetLastError());
   c->launches[KC_SRC] += 1;
   return AK_OK;
@@ -436,6 +467,46 @@ int ak_set_metric(ak_ctx* c, const ak_adm* a) {
   return AK_OK;
 }
 
+int ak_set_eos_hybrid(ak_ctx* c, int nseg, double K0, const double* gammas, const double* rho_breaks,
+                      double gamma_th) {
+  if (!c) return AK_EINVAL;
+  Par& P = c->P;
+  if (nseg == 0) {              // back to the ideal gas of ak_params.gamma_ad
+    P.eos = 0; P.nseg = 0;
+    P.P_atm = P.rho_atm * P.T_atm;
+    c->have_flux = false;
+    for (int l = 0; l < 2; ++l) if (c->lane[l]) copy_eos(c->lane[l]->P, P);
+    return AK_OK;
+  }
+  if (nseg < 1 || nseg > 4 || !gammas || (nseg > 1 && !rho_breaks)) return AK_EINVAL;
+  if (!(std::isfinite(K0) && K0 >= 0.0) || !(std::isfinite(gamma_th) && gamma_th > 1.0)) return AK_EINVAL;
+  for (int i = 0; i < nseg; ++i)
+    if (!(std::isfinite(gammas[i]) && gammas[i] > 1.0)) return AK_EINVAL;
+  for (int i = 0; i + 1 < nseg; ++i)
+    if (!finite_pos(rho_breaks[i]) || (i > 0 && !(rho_breaks[i] > rho_breaks[i - 1]))) return AK_EINVAL;
+  // K_i and the offsets a_i of eps_c follow from continuity of P_c and eps_c at the breakpoints
+  P.eos = 1; P.nseg = nseg; P.gth = gamma_th; P.gthm1 = gamma_th - 1.0;
+  for (int i = 0; i < 4; ++i) { P.ppK[i] = 0.0; P.ppG[i] = 2.0; P.ppa[i] = 0.0; }
+  for (int i = 0; i < 3; ++i) P.pprb[i] = 0.0;
+  for (int i = 0; i < nseg; ++i) P.ppG[i] = gammas[i];
+  for (int i = 0; i + 1 < nseg; ++i) P.pprb[i] = rho_breaks[i];
+  P.ppK[0] = K0;
+  for (int i = 1; i < nseg; ++i) {
+    const double rb = P.pprb[i - 1], Ga = P.ppG[i - 1], Gb = P.ppG[i];
+    P.ppK[i] = P.ppK[i - 1] * std::pow(rb, Ga - Gb);
+    P.ppa[i] = P.ppa[i - 1] + P.ppK[i - 1] * std::pow(rb, Ga - 1.0) / (Ga - 1.0) -
+               P.ppK[i] * std::pow(rb, Gb - 1.0) / (Gb - 1.0);
+  }
+  // atmosphere pressure P(rho_atm, T_atm) = P_c(rho_atm) + rho_atm T_atm (host pow, as the device's
+  // differs from it by rounding only in the last place)
+  int s0 = 0;
+  while (s0 + 1 < nseg && P.rho_atm >= P.pprb[s0]) ++s0;
+  P.P_atm = P.ppK[s0] * std::pow(P.rho_atm, P.ppG[s0]) + P.rho_atm * P.T_atm;
+  c->have_flux = false;
+  for (int l = 0; l < 2; ++l) if (c->lane[l]) copy_eos(c->lane[l]->P, P);
+  return AK_OK;
+}
+
 int ak_con2prim(ak_ctx* c, const ak_cons* U, const ak_faceB* Bf, const ak_prim* W, unsigned char* status) {
   if (!c) return AK_EINVAL;
   if (!c->have_metric) return AK_ESTATE;
@@ -494,7 +565,8 @@ int ak_matter_sources(ak_ctx* c, const ak_prim* W, const ak_matter* out) {
   MatterOut o = {{out->E, out->Sx, out->Sy, out->Sz, out->Sxx, out->Sxy, out->Sxz, out->Syy, out->Syz, out->Szz}};
   for (int q = 0; q < 10; ++q) if (!o.q[q]) return AK_EINVAL;
   CK(cudaSetDevice(c->hp.device));
-  k_matter<<<nblk(c->sz.cell, 128), 128, 0, c->stream>>>(c->P, f, o);
+  if (c->P.eos) k_matter<1><<<nblk(c->sz.cell, 128), 128, 0, c->stream>>>(c->P, f, o);
+  else k_matter<0><<<nblk(c->sz.cell, 128), 128, 0, c->stream>>>(c->P, f, o);
   CK(cudaGetLastError());
   return AK_OK;
 }
@@ -562,6 +634,7 @@ static int rhs_host_pipelined(ak_ctx* c, int chunk, double* const hU[5], const d
       hp.stream = (void*)st;
       const int r = ak_create(&hp, c->host_dx, &c->lane[l]);
       if (r != AK_OK) { cudaStreamDestroy(st); return r; }
+      copy_eos(c->lane[l]->P, c->P);
       // staging kinds: 0..4 U (cell), 5..7 Bf (xf yf zf), 8..15 W (cell), 16..20 dU (cell), 21..23 E (ex ey ez)
       for (int q = 0; q < 24; ++q) {
         const int kind = q < 5 ? 0 : (q < 8 ? 1 + (q - 5) : (q < 21 ? 0 : 4 + (q - 21)));

@@ -22,6 +22,10 @@ struct Par {
   int max_iter;
   double tol;
   int recon, riemann, fofc, fofc_riemann;
+  // piecewise-polytropic hybrid EOS (ak_set_eos_hybrid; reading R29); eos = 0: ideal gas
+  int eos, nseg;
+  double ppK[4], ppG[4], ppa[4], pprb[3];   // K_i, Gamma_i, eps offsets a_i, breakpoints
+  double gth, gthm1;                        // Gamma_th, Gamma_th - 1
 };
 
 // All field pointers one stage touches (passed by value as a kernel parameter).
@@ -106,9 +110,86 @@ __device__ __forceinline__ double ddiv(double a, double b) {
   return z ? (b > 0.0 ? a : -a) : q;
 }
 
+// ------------------------------------------------------------------ O1: equation of state
+// EOS = 0: ideal gas, P = (Gamma-1) rho eps, T = P/rho, h - 1 = Gamma/(Gamma-1) T, c_s^2 = Gamma T / h.
+// EOS = 1: piecewise-polytropic hybrid (R29): cold curve P_c = K_i rho^Gamma_i,
+//   eps_c = a_i + P_c / ((Gamma_i - 1) rho) in the segment that holds rho; thermal part
+//   P - P_c = (Gamma_th - 1) rho (eps - eps_c); T = (P - P_c)/rho; h = 1 + eps + P/rho;
+//   c_s^2 = (Gamma_i P_c + Gamma_th (P - P_c)) / (rho h).
+__device__ __forceinline__ void eos_cold(const Par& P, double rho, double& Pc, double& epsc, double& Gi) {
+  int i = 0;
+  while (i + 1 < P.nseg && rho >= P.pprb[i]) ++i;
+  Gi = P.ppG[i];
+  Pc = P.ppK[i] * pow(rho, Gi);
+  epsc = P.ppa[i] + Pc / ((Gi - 1.0) * rho);
+}
+template <int EOS>
+__device__ __forceinline__ void eos_hm1_cs2(const Par& P, double rho, double pr, double& hm1, double& cs2) {
+  if (EOS == 0) {
+    const double T = pr / rho;
+    hm1 = P.gm1r * T;
+    const double h = 1.0 + hm1;
+    cs2 = P.Gam * T / h;
+  } else {
+    double Pc, epsc, Gi;
+    eos_cold(P, rho, Pc, epsc, Gi);
+    const double Pth = pr - Pc;
+    const double eps = epsc + Pth / (P.gthm1 * rho);
+    hm1 = eps + pr / rho;
+    const double h = 1.0 + hm1;
+    cs2 = (Gi * Pc + P.gth * Pth) / (rho * h);
+  }
+}
+template <int EOS>
+__device__ __forceinline__ double eos_hm1(const Par& P, double rho, double pr) {
+  if (EOS == 0) return P.gm1r * (pr / rho);
+  double hm1, cs2;
+  eos_hm1_cs2<EOS>(P, rho, pr, hm1, cs2);
+  return hm1;
+}
+// pressure / specific internal energy of matter of density rho at temperature T
+template <int EOS>
+__device__ __forceinline__ double eos_P_at_T(const Par& P, double rho, double T) {
+  if (EOS == 0) return rho * T;
+  double Pc, epsc, Gi;
+  eos_cold(P, rho, Pc, epsc, Gi);
+  return Pc + rho * T;
+}
+template <int EOS>
+__device__ __forceinline__ double eos_eps_at_T(const Par& P, double rho, double T) {
+  if (EOS == 0) return P.eps_atm;            // T_atm / (Gamma - 1): the only temperature asked for
+  double Pc, epsc, Gi;
+  eos_cold(P, rho, Pc, epsc, Gi);
+  return epsc + T / P.gthm1;
+}
+// P(rho, eps)
+template <int EOS>
+__device__ __forceinline__ double eos_P(const Par& P, double rho, double eps) {
+  if (EOS == 0) {
+    const double T = P.gm1 * eps;
+    return rho * T;
+  }
+  double Pc, epsc, Gi;
+  eos_cold(P, rho, Pc, epsc, Gi);
+  return Pc + P.gthm1 * rho * (eps - epsc);
+}
+// temperature floor: raises pr and returns true if T(rho, pr) < T_atm
+template <int EOS>
+__device__ __forceinline__ bool eos_T_floor(const Par& P, double rho, double& pr) {
+  if (EOS == 0) {
+    if (pr < rho * P.T_atm) { pr = rho * P.T_atm; return true; }
+    return false;
+  }
+  double Pc, epsc, Gi;
+  eos_cold(P, rho, Pc, epsc, Gi);
+  if (pr - Pc < rho * P.T_atm) { pr = Pc + rho * P.T_atm; return true; }
+  return false;
+}
+
 // ------------------------------------------------------------------ O2: prim -> cons (Eq. 6)
 // prim = rho, u^i = W v^i, P; B undensitised; cons = D, S_i, tau (undensitised).
 // tau in the cancellation-free form of DESIGN.md §3 O2.
+template <int EOS = 0>
 __device__ __forceinline__ void prim2cons(const Par& P, const Met3& g, double rho, const double u[3],
                                           double pr, const double B[3], double c[5]) {
   double ul[3], Bl[3];
@@ -120,8 +201,7 @@ __device__ __forceinline__ void prim2cons(const Par& P, const Met3& g, double rh
   lower(g, B, Bl);
   const double B2 = dot3(Bl, B);
   const double Bv = B[0] * vl[0] + B[1] * vl[1] + B[2] * vl[2];
-  const double T = pr / rho;
-  const double hm1 = P.gm1r * T;
+  const double hm1 = eos_hm1<EOS>(P, rho, pr);
   const double h = 1.0 + hm1;
   const double D = rho * W;
   const double wtot = rho * h * W * W + B2;
@@ -134,8 +214,10 @@ __device__ __forceinline__ void prim2cons(const Par& P, const Met3& g, double rh
 
 // ------------------------------------------------------------------ O3: con2prim
 // Bracketed 1-D solve for mu = 1/(W h) (scheme of Kastaun et al. 2021), h0 = 1.
+template <int EOS = 0>
 struct C2P {
   double q, r2, bs2, rb2, v0sq, gm1;
+  const Par* par; double D;    // EOS = 1 only: the EOS constants and the conserved density (rho^ = D / W^)
   // quantities at a trial mu
   double x, rbar2, qbar, vsq, iW, What, eps;
   __device__ __forceinline__ void aux(double mu) {
@@ -150,8 +232,18 @@ struct C2P {
   // master function f(mu)
   __device__ __forceinline__ double f(double mu) {
     aux(mu);
-    const double e = fmax(eps, 0.0);
-    const double ahat = ddiv(gm1 * e, 1.0 + e);
+    double e, ahat;
+    if (EOS == 0) {
+      e = fmax(eps, 0.0);
+      ahat = ddiv(gm1 * e, 1.0 + e);
+    } else {                     // general form a^ = P(rho^, eps^) / (rho^ (1 + eps^)), eps^ >= eps_c(rho^)
+      const double rhohat = D * iW;
+      double Pc, epsc, Gi;
+      eos_cold(*par, rhohat, Pc, epsc, Gi);
+      e = fmax(eps, epsc);
+      const double Phat = Pc + par->gthm1 * rhohat * (e - epsc);
+      ahat = Phat / (rhohat * (1.0 + e));
+    }
     const double nuA = (1.0 + ahat) * (1.0 + e) * iW;
     const double nuB = (1.0 + ahat) * (1.0 + qbar - mu * rbar2);
     return mu - 1.0 / (fmax(nuA, nuB) + mu * rbar2);
@@ -167,8 +259,8 @@ struct C2P {
 // Illinois-modified regula falsi on [a,b] with fa_ < 0 <= fb_.  AUX selects fa over f.
 // The iteration cap is uniform (a parameter), so a warp leaves the loop together at the
 // latest after max_iter evaluations.
-template <bool AUX>
-__device__ __forceinline__ bool illinois(C2P& s, double a, double b, double fa_, double fb_,
+template <bool AUX, int EOS>
+__device__ __forceinline__ bool illinois(C2P<EOS>& s, double a, double b, double fa_, double fb_,
                                          int max_iter, double tol, double& root) {
   int side = 0;
   double cprev = b;
@@ -202,20 +294,22 @@ __device__ __forceinline__ bool illinois(C2P& s, double a, double b, double fa_,
 #else
 #define AK_RARE __forceinline__
 #endif
-__device__ AK_RARE bool c2p_upper_bracket(C2P& s, int max_iter, double tol, double& mu_hi) {
-  return illinois<true>(s, 0.0, 1.0, -1.0, s.fa(1.0), max_iter, tol, mu_hi);
+template <int EOS>
+__device__ AK_RARE bool c2p_upper_bracket(C2P<EOS>& s, int max_iter, double tol, double& mu_hi) {
+  return illinois<true, EOS>(s, 0.0, 1.0, -1.0, s.fa(1.0), max_iter, tol, mu_hi);
 }
+template <int EOS>
 __device__ AK_RARE void c2p_write_back(const Par& P, const Met3& g, double sdet, double rho, double ux, double uy,
                                        double uz, double pr, const double B[3], double Ut[5]) {
   double c5[5];
   const double u[3] = {ux, uy, uz};
-  prim2cons(P, g, rho, u, pr, B, c5);
+  prim2cons<EOS>(P, g, rho, u, pr, B, c5);
   for (int v = 0; v < 5; ++v) Ut[v] = sdet * c5[v];
 }
 
 // One cell.  Ut = densitised D,S_i,tau (rewritten from the final primitives when WRITE_BACK
 // and the status is non-zero); Bt = densitised cell-centred B; W5 = rho,u^x,u^y,u^z,P.
-template <bool WRITE_BACK>
+template <bool WRITE_BACK, int EOS = 0>
 __device__ __forceinline__ int c2p_cell(const Par& P, const Met3& g, double Ut[5], const double Bt[3],
                                         double W5[5]) {
   int status = 0;
@@ -226,7 +320,7 @@ __device__ __forceinline__ int c2p_cell(const Par& P, const Met3& g, double Ut[5
   double D = Ut[0] * isd, tau = Ut[4] * isd;
   const double Sl[3] = {Ut[1] * isd, Ut[2] * isd, Ut[3] * isd};
   const double B[3] = {Bt[0] * isd, Bt[1] * isd, Bt[2] * isd};
-  double rho = P.rho_atm, ux = 0.0, uy = 0.0, uz = 0.0, pr = P.P_atm;
+  double rho = P.rho_atm, ux = 0.0, uy = 0.0, uz = 0.0, pr = P.P_atm;   // P_atm = P(rho_atm, T_atm) of the EOS
   bool solve = true;
   if (!(isfinite(D) && isfinite(Sl[0]) && isfinite(Sl[1]) && isfinite(Sl[2]) && isfinite(tau) &&
         isfinite(B[0]) && isfinite(B[1]) && isfinite(B[2]))) {
@@ -249,14 +343,15 @@ __device__ __forceinline__ int c2p_cell(const Par& P, const Met3& g, double Ut[5
   }
   if (solve && atmo) {
     rho = D;
-    pr = D * P.T_atm;
+    pr = eos_P_at_T<EOS>(P, D, P.T_atm);
     solve = false;
   }
   if (solve) {
-    const double tau_atm = D * P.eps_atm + 0.5 * B2;
+    const double tau_atm = D * eos_eps_at_T<EOS>(P, D, P.T_atm) + 0.5 * B2;
     if (tau < tau_atm) { tau = tau_atm; status |= ST_TAUFLOOR; }
     const double iD = 1.0 / D;
-    C2P s;
+    C2P<EOS> s;
+    s.par = &P; s.D = D;
     s.q = tau * iD;
     const double rl[3] = {Sl[0] * iD, Sl[1] * iD, Sl[2] * iD};
     const double ru[3] = {gu.xx * rl[0] + gu.xy * rl[1] + gu.xz * rl[2],
@@ -281,15 +376,14 @@ __device__ __forceinline__ int c2p_cell(const Par& P, const Met3& g, double Ut[5
       const double f_lo = s.f(0.0);
       if (!(f_hi >= 0.0) || !(f_lo < 0.0)) ok = false;
       else if (f_hi == 0.0) mu = mu_hi;
-      else ok = illinois<false>(s, 0.0, mu_hi, f_lo, f_hi, P.max_iter, P.tol, mu);
+      else ok = illinois<false, EOS>(s, 0.0, mu_hi, f_lo, f_hi, P.max_iter, P.tol, mu);
     }
     if (!ok) {
       status |= ST_FAIL;
     } else {
       s.aux(mu);
       rho = D * s.iW;
-      const double T = P.gm1 * s.eps;
-      pr = rho * T;
+      pr = eos_P<EOS>(P, rho, s.eps);
       const double c = mu * rB * iD;
       const double mx = mu * s.x;
       ux = s.What * (mx * (ru[0] + c * B[0]));
@@ -305,12 +399,11 @@ __device__ __forceinline__ int c2p_cell(const Par& P, const Met3& g, double Ut[5
   if (rho < P.thr) {
     rho = P.rho_atm; ux = uy = uz = 0.0; pr = P.P_atm;
     status |= ST_RHOFLOOR;
-  } else if (pr < rho * P.T_atm) {
-    pr = rho * P.T_atm;
+  } else if (eos_T_floor<EOS>(P, rho, pr)) {
     status |= ST_TFLOOR;
   }
   W5[0] = rho; W5[1] = ux; W5[2] = uy; W5[3] = uz; W5[4] = pr;
-  if (WRITE_BACK && status != 0) c2p_write_back(P, g, sdet, rho, ux, uy, uz, pr, B, Ut);
+  if (WRITE_BACK && status != 0) c2p_write_back<EOS>(P, g, sdet, rho, ux, uy, uz, pr, B, Ut);
   return status;
 }
 

@@ -125,19 +125,22 @@ __device__ __forceinline__ void face_geometry(const double mL[10], const double 
 }
 
 // face-state floor ("after reconstruction"); s = rho,ux,uy,uz,P,...
+template <int EOS = 0>
 __device__ __forceinline__ void face_floor(const Par& P, double s[7]) {
   if (s[0] < P.thr) {
     s[0] = P.rho_atm; s[1] = 0.0; s[2] = 0.0; s[3] = 0.0;
     s[4] = P.P_atm;
-  } else if (s[4] < s[0] * P.T_atm) {
-    s[4] = s[0] * P.T_atm;
+  } else if (EOS == 0) {
+    if (s[4] < s[0] * P.T_atm) s[4] = s[0] * P.T_atm;
+  } else {
+    eos_T_floor<EOS>(P, s[0], s[4]);
   }
 }
 
 // ------------------------------------------------------------------ O6: one side (Eq. 8)
 // s = rho,u^x,u^y,u^z,P,B~t1,B~t2 (transverse B densitised); Bd = undensitised normal B.
 // Out: densitised conserved U[7], densitised fluxes F[7], signal speeds lm, lp.
-template <int DIR>
+template <int DIR, int EOS = 0>
 __device__ __forceinline__ void side_state(const Par& P, const FaceGeo& G, const double s[7], double Bd,
                                            double U[7], double F[7], double& lm, double& lp) {
   constexpr int t1 = (DIR + 1) % 3, t2 = (DIR + 2) % 3;
@@ -158,8 +161,8 @@ __device__ __forceinline__ void side_state(const Par& P, const FaceGeo& G, const
   const double b2 = B2 * iW * iW + Bv * Bv;                                   // Eq. 7
   const double bl[3] = {Bl[0] * iW + Bv * ul[0], Bl[1] * iW + Bv * ul[1], Bl[2] * iW + Bv * ul[2]};
   const double ab0 = W * Bv;                                                  // alpha b^0
-  const double T = pr / rho;
-  const double hm1 = P.gm1r * T;
+  double hm1, cs2;
+  eos_hm1_cs2<EOS>(P, rho, pr, hm1, cs2);
   const double h = 1.0 + hm1;
   const double Ptot = pr + 0.5 * b2;
   const double D = rho * W;
@@ -185,7 +188,6 @@ __device__ __forceinline__ void side_state(const Par& P, const FaceGeo& G, const
   F[6] = G.sdet * (G.alp * (B[t2] * vh[DIR] - B[DIR] * vh[t2]));
   // fast-magnetosonic bound on the characteristic speeds (DESIGN.md §3 O6, reading R18)
   const double vsq = v[0] * vl[0] + v[1] * vl[1] + v[2] * vl[2];
-  const double cs2 = P.Gam * T / h;
   const double rhoh = rho * h;
   const double va2 = ddiv(b2, rhoh + b2);
   const double a2 = cs2 + va2 - cs2 * va2;
@@ -200,16 +202,16 @@ __device__ __forceinline__ void side_state(const Par& P, const FaceGeo& G, const
 
 // Face flux from left/right states (floored here when FLOOR), the face-normal B~ and the
 // two adjacent cells' metric.  RS: 0 LLF, 1 HLLE.
-template <int DIR, bool FLOOR>
+template <int DIR, bool FLOOR, int EOS = 0>
 __device__ __forceinline__ void face_flux(const Par& P, int rs, const double mL[10], const double mR[10],
                                           double sL[7], double sR[7], double Bfd, double Fo[7]) {
   FaceGeo G;
   face_geometry<DIR>(mL, mR, G);
   const double Bd = Bfd * G.isd;
-  if (FLOOR) { face_floor(P, sL); face_floor(P, sR); }
+  if (FLOOR) { face_floor<EOS>(P, sL); face_floor<EOS>(P, sR); }
   double UL[7], FL[7], UR[7], FR[7], lmL, lpL, lmR, lpR;
-  side_state<DIR>(P, G, sL, Bd, UL, FL, lmL, lpL);
-  side_state<DIR>(P, G, sR, Bd, UR, FR, lmR, lpR);
+  side_state<DIR, EOS>(P, G, sL, Bd, UL, FL, lmL, lpL);
+  side_state<DIR, EOS>(P, G, sR, Bd, UR, FR, lmR, lpR);
   if (rs == 1) {   // HLLE
     const double lL = fmin(0.0, fmin(lmL, lmR));
     const double lR = fmax(0.0, fmax(lpL, lpR));

@@ -64,7 +64,7 @@ __device__ __forceinline__ void load_met10(const Fields& f, long long c, double 
 // ---- K1 ------------------------------------------------------------------------------
 // EMF: also write the cell-centred EMFs of the final primitives (the arithmetic of k_cell_emf), so
 // that a stage that runs part (1) does not re-read W and the metric for them.
-template <bool EMF>
+template <bool EMF, int EOS = 0>
 __global__ void __launch_bounds__(128, AK_C2P_MINB) k_con2prim(const __grid_constant__ Par P,
                                                   const __grid_constant__ Fields f) {
   const int nt = P.nt;
@@ -88,7 +88,7 @@ __global__ void __launch_bounds__(128, AK_C2P_MINB) k_con2prim(const __grid_cons
   Bc[0] = 0.5 * (__ldg(f.Bf[0] + fx) + __ldg(f.Bf[0] + fx + 1));
   Bc[1] = 0.5 * (__ldg(f.Bf[1] + fy) + __ldg(f.Bf[1] + fy + nt));
   Bc[2] = 0.5 * (__ldg(f.Bf[2] + fz) + __ldg(f.Bf[2] + fz + (long long)nt * nt));
-  const int st = c2p_cell<true>(P, g, Ut, Bc, W5);
+  const int st = c2p_cell<true, EOS>(P, g, Ut, Bc, W5);
 #pragma unroll
   for (int v = 0; v < 5; ++v) f.W[v][c] = W5[v];
 #pragma unroll
@@ -132,7 +132,7 @@ __device__ __forceinline__ bool decode_face(const Par& P, long long idx, int& m,
 }
 
 // ---- K2 (v1: one thread per face; both one-sided reconstructions done by the thread) ----
-template <int DIR, int RECON>
+template <int DIR, int RECON, int EOS = 0>
 __global__ void __launch_bounds__(128, AK_FLUX_MINB) k_flux(const __grid_constant__ Par P,
                                               const __grid_constant__ Fields f) {
   int m, k, j, i;
@@ -162,7 +162,7 @@ __global__ void __launch_bounds__(128, AK_FLUX_MINB) k_flux(const __grid_constan
   load_met10(f, cl, mL);
   load_met10(f, cu, mR);
   const long long fi = ix.face(DIR, m, k, j, i);
-  face_flux<DIR, true>(P, P.riemann, mL, mR, sL, sR, __ldg(f.Bf[DIR] + fi), Fo);
+  face_flux<DIR, true, EOS>(P, P.riemann, mL, mR, sL, sR, __ldg(f.Bf[DIR] + fi), Fo);
 #pragma unroll
   for (int v = 0; v < 7; ++v) f.F[7 * DIR + v][fi] = Fo[v];
 }
@@ -190,6 +190,7 @@ __device__ __forceinline__ double div_flux(const Fields& f, const Ix& ix, int v,
 }
 
 // ---- K3: FOFC estimate and test (DMP Eq. 12) -------------------------------
+template <int EOS = 0>
 __global__ void __launch_bounds__(128, AK_FOFC_MINB) k_fofc_test(const __grid_constant__ Par P,
                                                    const __grid_constant__ Fields f, double dt) {
   int m, k, j, i;
@@ -209,7 +210,7 @@ __global__ void __launch_bounds__(128, AK_FOFC_MINB) k_fofc_test(const __grid_co
 #pragma unroll
   for (int v = 0; v < 3; ++v) Bc[v] = f.W[5 + v][c];
   const double Ds = Us[0], ts = Us[4];
-  int st = c2p_cell<false>(P, g, Us, Bc, W5);
+  int st = c2p_cell<false, EOS>(P, g, Us, Bc, W5);
   if (P.dmp_M > 0.0) {
     // fmin/fmax over the 27 cells (the centre is one of them) written as compare-and-select from
     // +-inf: the same values for every input (a NaN is skipped either way; only the sign of a zero
@@ -254,7 +255,7 @@ __global__ void __launch_bounds__(128, AK_FOFC_MINB) k_fofc_test(const __grid_co
 // (upper) is redone exactly once: by B's entry if B is flagged, else by A's.  So entry c handles
 // its lower DIR-face always and its upper DIR-face only when the upper neighbour is not flagged.
 // Thread t < 2 * count: which = t / count (0 lower, 1 upper) keeps warps uniform.
-template <int DIR>
+template <int DIR, int EOS = 0>
 __global__ void __launch_bounds__(128) k_fofc_reflux(const __grid_constant__ Par P,
                                                      const __grid_constant__ Fields f) {
   const unsigned cnt = f.count[3];
@@ -280,7 +281,7 @@ __global__ void __launch_bounds__(128) k_fofc_reflux(const __grid_constant__ Par
     load_met10(f, cl, mL);
     load_met10(f, cu, mR);
     const long long fi = ix.face(DIR, m, k, j, i);
-    face_flux<DIR, true>(P, P.fofc_riemann, mL, mR, sL, sR, __ldg(f.Bf[DIR] + fi), Fo);
+    face_flux<DIR, true, EOS>(P, P.fofc_riemann, mL, mR, sL, sR, __ldg(f.Bf[DIR] + fi), Fo);
 #pragma unroll
     for (int v = 0; v < 7; ++v) f.F[7 * DIR + v][fi] = Fo[v];
     ++nface;

@@ -9,6 +9,7 @@ namespace ak {
 #ifndef AK_SRC_MINB
 #define AK_SRC_MINB 4
 #endif
+template <int EOS = 0>
 __global__ void __launch_bounds__(128, AK_SRC_MINB) k_div_src(const __grid_constant__ Par P,
                                                  const __grid_constant__ Fields f) {
   const int n = P.n;
@@ -38,7 +39,7 @@ __global__ void __launch_bounds__(128, AK_SRC_MINB) k_div_src(const __grid_const
   const double u[3] = {f.W[1][c], f.W[2][c], f.W[3][c]};
   const double B[3] = {f.W[5][c] * isd, f.W[6][c] * isd, f.W[7][c] * isd};
   double cons[5];
-  prim2cons(P, g, rho, u, pr, B, cons);
+  prim2cons<EOS>(P, g, rho, u, pr, B, cons);
   double ul[3], Bl[3];
   lower(g, u, ul);
   const double usq = dot3(ul, u);
@@ -49,7 +50,7 @@ __global__ void __launch_bounds__(128, AK_SRC_MINB) k_div_src(const __grid_const
   const double Bv = B[0] * vl[0] + B[1] * vl[1] + B[2] * vl[2];
   const double b2 = B2 * iW * iW + Bv * Bv;
   const double bl[3] = {Bl[0] * iW + Bv * ul[0], Bl[1] * iW + Bv * ul[1], Bl[2] * iW + Bv * ul[2]};
-  const double h = 1.0 + P.Gam / (P.Gam - 1.0) * (pr / rho);
+  const double h = EOS == 0 ? 1.0 + P.Gam / (P.Gam - 1.0) * (pr / rho) : 1.0 + eos_hm1<EOS>(P, rho, pr);
   const double Ptot = pr + 0.5 * b2;
   const double wt = rho * h + b2;
   // S_ij = (rho h + b^2) u_i u_j + Ptot gamma_ij - b_i b_j
@@ -109,6 +110,7 @@ __global__ void __launch_bounds__(128, AK_SRC_MINB) k_div_src(const __grid_const
 // at every stored cell from the cell-centred primitives ----------------------------------------------
 struct MatterOut { double* q[10]; };   // E, Sx, Sy, Sz, Sxx, Sxy, Sxz, Syy, Syz, Szz
 
+template <int EOS = 0>
 __global__ void __launch_bounds__(128) k_matter(const __grid_constant__ Par P, const __grid_constant__ Fields f,
                                                 const __grid_constant__ MatterOut o) {
   const long long ncell = (long long)P.nmb * P.nt * P.nt * P.nt;
@@ -123,7 +125,7 @@ __global__ void __launch_bounds__(128) k_matter(const __grid_constant__ Par P, c
   const double u[3] = {f.W[1][c], f.W[2][c], f.W[3][c]};
   const double B[3] = {f.W[5][c] * isd, f.W[6][c] * isd, f.W[7][c] * isd};
   double cons[5];
-  prim2cons(P, g, rho, u, pr, B, cons);
+  prim2cons<EOS>(P, g, rho, u, pr, B, cons);
   double ul[3], Bl[3];
   lower(g, u, ul);
   const double usq = dot3(ul, u);
@@ -134,7 +136,7 @@ __global__ void __launch_bounds__(128) k_matter(const __grid_constant__ Par P, c
   const double Bv = B[0] * vl[0] + B[1] * vl[1] + B[2] * vl[2];
   const double b2 = B2 * iW * iW + Bv * Bv;
   const double bl[3] = {Bl[0] * iW + Bv * ul[0], Bl[1] * iW + Bv * ul[1], Bl[2] * iW + Bv * ul[2]};
-  const double h = 1.0 + P.Gam / (P.Gam - 1.0) * (pr / rho);
+  const double h = EOS == 0 ? 1.0 + P.Gam / (P.Gam - 1.0) * (pr / rho) : 1.0 + eos_hm1<EOS>(P, rho, pr);
   const double Ptot = pr + 0.5 * b2;
   const double wt = rho * h + b2;
   o.q[0][c] = cons[4] + cons[0];

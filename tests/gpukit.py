@@ -35,6 +35,9 @@ class GpuStage:
         self.params = ak.make_params(device=torch.device(dev).index or 0, stream=stream, **p)
         self.ctx = ak.ak_create(self.params, w["dx"])
         ak.ak_set_metric(self.ctx, self.adm)
+        hyb = p.get("eos_hybrid")
+        if hyb is not None:
+            ak.ak_set_eos_hybrid(self.ctx, hyb["K0"], hyb["gammas"], hyb.get("rho_breaks", ()), hyb["gamma_th"])
 
     def con2prim(self):
         ak.ak_con2prim(self.ctx, self.U, self.Bf, self.W, self.status)
