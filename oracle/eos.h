@@ -10,6 +10,8 @@
 //     "temperature" T = (P - P_c)/rho, so that K = 0 is the ideal gas with Gamma = Gamma_th;
 //     h = 1 + eps + P/rho,   c_s^2 = [Gamma_i P_c + Gamma_th (P - P_c)] / (rho h).
 // Every function below evaluates the ideal gas with exactly the operations of DESIGN.md §3.
+// Pins: tests/test_oracle_eos.py (T31).  Parity unpinned: which temperature the floors of P:139
+// act on for the hybrid EOS (the paper is silent; R29 takes the thermal one).
 #ifndef GRMHD_ORACLE_EOS_H
 #define GRMHD_ORACLE_EOS_H
 #include "oracle.h"
