@@ -297,7 +297,7 @@ def run_gpu(args, rank, local_rank, world):
     return dict(torch=torch, ak=ak, ctx=ctx, dev=dev, stream=stream, U=U, U0=U0, Bf=Bf, W=W, dU=dU, E=E, flag=flag,
                 status=status, sh=sh, nmb=nmb, n=n, ids=ids, zones=zones, dt_fofc=dt_fofc, params_d=params_d,
                 ms_step=ms_step, value=value, clocks=clocks, kms=kms, klaunch=klaunch, stats=stats, t_gen=t_gen,
-                spec=spec, world=world, dx=dx)
+                spec=spec, world=world, dx=dx, adm=adm)
 
 
 def run_e2e(R, steps):
@@ -406,6 +406,60 @@ def roofline(R, hbm_peak, peak_src):
     return rf, table, stage
 
 
+def run_fma(R, steps):
+    """the FMA-contracted perf build (libak_fma.so, same sources with
+    --fmad=true) timed on the same resident inputs, with its deviation from the product build
+    (which the parity tests hold bit-identical to the oracle) in units of BASELINE.json's tolerance
+    and the number of mask bytes that differ.  Runs before anything evolves the resident inputs."""
+    torch, ak = R["torch"], R["ak"]
+    from paper_2409_10384_b200 import build as akbuild
+    if not os.path.exists(akbuild.SO_FMA):
+        return dict(unavailable="libak_fma.so not built (python -m paper_2409_10384_b200.build --fma)")
+    dev, stream = R["dev"], R["stream"]
+
+    def one_stage(ctx):
+        for u, u0 in zip(R["U"], R["U0"]):
+            u.copy_(u0)
+        ak.ak_rhs(ctx, R["U"], R["Bf"], R["W"], 0, R["dt_fofc"], R["dU"], R["E"], R["flag"], R["status"])
+        torch.cuda.synchronize(dev)
+
+    one_stage(R["ctx"])
+    ref = [t.clone() for t in R["dU"] + R["E"]]
+    ref_flag, ref_status = R["flag"].clone(), R["status"].clone()
+    umax = [float(u.abs().max()) for u in R["U0"]]
+    ak.use_library(akbuild.SO_FMA)      # R["ctx"] stays alive; it is only used again after switching back
+    try:
+        par = ak.make_params(device=dev.index or 0, stream=stream.cuda_stream, **R["params_d"])
+        ctx = ak.ak_create(par, R["dx"])
+        ak.ak_set_metric(ctx, R["adm"])
+        one_stage(ctx)
+        atol = [1e-14 * m for m in umax] + [1e-14 * max(umax)] * 3
+        worst = 0.0
+        for a, b, at in zip(R["dU"] + R["E"], ref, atol):
+            worst = max(worst, float(((a - b).abs() / (at + 1e-11 * b.abs())).max()))
+        nflag = int((R["flag"] != ref_flag).sum())
+        nstatus = int((R["status"] != ref_status).sum())
+        del ref
+        for _ in range(3):
+            ak.ak_rhs(ctx, R["U"], R["Bf"], R["W"], 0, R["dt_fofc"], R["dU"], R["E"], R["flag"], R["status"])
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(dev)
+        e0.record(stream)
+        for _ in range(steps):
+            ak.ak_rhs(ctx, R["U"], R["Bf"], R["W"], 0, R["dt_fofc"], R["dU"], R["E"], R["flag"], R["status"])
+        e1.record(stream)
+        torch.cuda.synchronize(dev)
+        ms = e0.elapsed_time(e1) / steps
+        ak.ak_destroy(ctx)
+    finally:
+        ak.use_library(None)
+    return dict(build="--fmad=true", ms_per_step=round(ms, 4), value=R["zones"] / (ms * 1e-3), unit=UNIT,
+                speedup_vs_product=round(R["ms_step"] / ms, 4),
+                worst_deviation_over_tolerance=worst, tolerance="rel 1e-11, abs 1e-14 max|U| (dU/dt and EMFs)",
+                fofc_flag_bytes_differ=nflag, c2p_status_bytes_differ=nstatus,
+                note="context only: the reported value, parity tests and profiles are the --fmad=false build")
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -418,6 +472,7 @@ def main():
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="CPU-oracle sample budget per step")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-fma", action="store_true", help="skip the FMA-contracted perf-build leg")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -429,6 +484,7 @@ def main():
     hbm_peak, peak_src = measured_peaks()
     rf, table, stage = roofline(R, hbm_peak, peak_src)
     e2e = None if args.no_e2e else run_e2e(R, max(1, args.e2e_steps))
+    fma = None if (args.no_fma or world > 1) else run_fma(R, args.steps)
     rk3 = run_rk3(R)
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu:
@@ -455,7 +511,7 @@ def main():
                                 fofc_faces=st["n_fofc_faces"]),
                     clocks=R["clocks"], e2e=e2e, gpu_launches=int(sum(R["klaunch"].values())),
                     roofline=rf, kernels=table, stage_hbm=stage, cpu_baseline=cpu, rk3_step=rk3,
-                    gen_seconds=round(R["t_gen"], 1))
+                    fma_build=fma, gen_seconds=round(R["t_gen"], 1))
         print(json.dumps(line))
     R["ak"].ak_destroy(R["ctx"])
     if world > 1:

@@ -123,6 +123,16 @@ def lib():
     return _lib
 
 
+def use_library(path=None):
+    """Switch the binding to another build of the same library (None: the default libak.so), e.g. the
+    FMA-contracted libak_fma.so of build.py.  Contexts belong to the library that created them:
+    destroy them before switching."""
+    global _lib, SO_PATH
+    SO_PATH = path or os.environ.get("AK_LIBRARY") or os.path.join(_HERE, "libak.so")
+    _lib = None
+    return lib()
+
+
 def strerror(code):
     return lib().ak_strerror(int(code)).decode()
 
