@@ -251,7 +251,7 @@ def _c0_modes(seed):
     return modes
 
 
-C0_BSCALE = None  # filled lazily: rescales rms|B| to 0.1
+C0_BSCALE = {}  # per seed, filled lazily: rescales rms|B| to 0.1 (a function of the seed alone, not of call order)
 
 
 def _vecpot(name, spec, comp, x, y, z):
@@ -299,9 +299,9 @@ def _vecpot(name, spec, comp, x, y, z):
 
 
 def _c0_scale(spec):
-    global C0_BSCALE
-    if C0_BSCALE is None:
-        C0_BSCALE = 1.0
+    seed = spec["seed"]
+    if seed not in C0_BSCALE:
+        C0_BSCALE[seed] = 1.0
         # rms |curl A| on a fixed 32^3 sample of [0,1]^3 (analytic derivative by differences)
         n = 32
         c = (np.arange(n) + 0.5) / n
@@ -316,8 +316,8 @@ def _c0_scale(spec):
             return (A(comp, X + sh[0], Y + sh[1], Z + sh[2]) - A(comp, X - sh[0], Y - sh[1], Z - sh[2])) / (2 * h)
         Bx = d(2, 1) - d(1, 2); By = d(0, 2) - d(2, 0); Bz = d(1, 0) - d(0, 1)
         rms = np.sqrt(np.mean(Bx * Bx + By * By + Bz * Bz))
-        C0_BSCALE = 0.1 / rms
-    return C0_BSCALE
+        C0_BSCALE[seed] = 0.1 / rms
+    return C0_BSCALE[seed]
 
 
 # ------------------------------------------------------------------ Eq. 6 (generator's own)
