@@ -406,6 +406,46 @@ def roofline(R, hbm_peak, peak_src):
     return rf, table, stage
 
 
+HYBRID_EOS = dict(K0=100.0, gammas=[2.0, 2.6], rho_breaks=[6.4e-4], gamma_th=1.75)
+
+
+def run_hybrid(R, steps):
+    """Context: the same stage on the same resident inputs with the piecewise-polytropic hybrid EOS
+    (the cold curve of the generator's Gamma=2, K=100 polytrope with a
+    stiffer segment above half the central density).  Runs before anything evolves the inputs and
+    returns the context to the ideal gas."""
+    torch, ak, ctx = R["torch"], R["ak"], R["ctx"]
+    dev, stream = R["dev"], R["stream"]
+    for u, u0 in zip(R["U"], R["U0"]):
+        u.copy_(u0)
+    ak.ak_set_eos_hybrid(ctx, **HYBRID_EOS)
+    try:
+        for _ in range(3):
+            ak.ak_rhs(ctx, R["U"], R["Bf"], R["W"], 0, R["dt_fofc"], R["dU"], R["E"], R["flag"], R["status"])
+        ak.ak_timing(ctx, 1)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(dev)
+        e0.record(stream)
+        for _ in range(steps):
+            ak.ak_rhs(ctx, R["U"], R["Bf"], R["W"], 0, R["dt_fofc"], R["dU"], R["E"], R["flag"], R["status"])
+        e1.record(stream)
+        torch.cuda.synchronize(dev)
+        ms = e0.elapsed_time(e1) / steps
+        kms, klaunch = ak.ak_kernel_ms(ctx)
+        ak.ak_timing(ctx, 0)
+        st = ak.ak_get_stats(ctx)
+    finally:
+        ak.ak_set_eos_hybrid(ctx, 0.0, ())
+        for u, u0 in zip(R["U"], R["U0"]):
+            u.copy_(u0)
+    return dict(eos=HYBRID_EOS, ms_per_step=round(ms, 4), value=R["zones"] / (ms * 1e-3), unit=UNIT,
+                kernel_ms={k: round(v / steps, 4) for k, v in kms.items()},
+                fofc_flagged_fraction=round(st["n_fofc_cells"] / (R["nmb"] * (R["n"] + 2) ** 3), 6),
+                note="context only, per GPU: the workload's conserved states were built with the ideal gas, so under "
+                     "this EOS many more cells are floored and flagged than in the reported run (see the flagged "
+                     "fraction); rho^Gamma is pow() in con2prim and the FOFC test")
+
+
 def run_fma(R, steps):
     """the FMA-contracted perf build (libak_fma.so, same sources with
     --fmad=true) timed on the same resident inputs, with its deviation from the product build
@@ -485,6 +525,7 @@ def main():
     rf, table, stage = roofline(R, hbm_peak, peak_src)
     e2e = None if args.no_e2e else run_e2e(R, max(1, args.e2e_steps))
     fma = None if (args.no_fma or world > 1) else run_fma(R, args.steps)
+    hyb = None if (args.no_fma or world > 1) else run_hybrid(R, args.steps)
     rk3 = run_rk3(R)
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu:
@@ -511,7 +552,7 @@ def main():
                                 fofc_faces=st["n_fofc_faces"]),
                     clocks=R["clocks"], e2e=e2e, gpu_launches=int(sum(R["klaunch"].values())),
                     roofline=rf, kernels=table, stage_hbm=stage, cpu_baseline=cpu, rk3_step=rk3,
-                    fma_build=fma, gen_seconds=round(R["t_gen"], 1))
+                    fma_build=fma, hybrid_eos=hyb, gen_seconds=round(R["t_gen"], 1))
         print(json.dumps(line))
     R["ak"].ak_destroy(R["ctx"])
     if world > 1:

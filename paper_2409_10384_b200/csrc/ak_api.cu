@@ -45,7 +45,7 @@ struct ak_ctx {
   double* stg_U[5]; double* stg_Bf[3]; double* stg_W[8]; double* stg_dU[5]; double* stg_E[3];
   unsigned char* stg_flag; unsigned char* stg_status;
   bool have_stg;
-  bool tma_attr[3];
+  bool tma_attr[2][3];
   // FOFC stage blend (ak_set_fofc_blend)
   const double* blendU0[5]; double blend_a, blend_b;
   // stage-driver registers (ak_advance), allocated on first use
@@ -179,15 +179,21 @@ int launch_c2p(ak_ctx* c, const Fields& f, bool with_emf) {
 #define AK_FLUX_CELL_MASK 1   // bit d set: direction d uses the reconstruct-once variant k_flux_tma_cell
 #endif
 
-template <int DIR, int RECON>
-int launch_flux_tma(ak_ctx* c, const Fields& f, int NA, unsigned grid, int bd, size_t smem) {
-  auto kern = ((AK_FLUX_CELL_MASK >> DIR) & 1) ? k_flux_tma_cell<DIR, RECON> : k_flux_tma<DIR, RECON>;
-  if (!c->tma_attr[DIR]) {
+template <int DIR, int RECON, int EOS>
+int launch_flux_tma_eos(ak_ctx* c, const Fields& f, int NA, unsigned grid, int bd, size_t smem) {
+  auto kern = ((AK_FLUX_CELL_MASK >> DIR) & 1) ? k_flux_tma_cell<DIR, RECON, EOS> : k_flux_tma<DIR, RECON, EOS>;
+  if (!c->tma_attr[EOS][DIR]) {   // per instantiation in use: recon and n are fixed for the life of a context
     CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    c->tma_attr[DIR] = true;
+    c->tma_attr[EOS][DIR] = true;
   }
   kern<<<grid, bd, smem, c->stream>>>(c->P, f, NA);
   return AK_OK;
+}
+
+template <int DIR, int RECON>
+int launch_flux_tma(ak_ctx* c, const Fields& f, int NA, unsigned grid, int bd, size_t smem) {
+  return c->P.eos ? launch_flux_tma_eos<DIR, RECON, 1>(c, f, NA, grid, bd, smem)
+                  : launch_flux_tma_eos<DIR, RECON, 0>(c, f, NA, grid, bd, smem);
 }
 
 template <int DIR>
@@ -197,9 +203,7 @@ int launch_flux(ak_ctx* c, const Fields& f) {
   constexpr int AK_FLUX_CELL = (AK_FLUX_CELL_MASK >> DIR) & 1;
   // threads per row of a tile: faces (k_flux_tma) or cells (k_flux_tma_cell)
   const int nfi = AK_FLUX_CELL ? (DIR == 0 ? n + 4 : e) : (DIR == 0 ? n + 3 : e);
-  // the hybrid EOS runs the plain one-thread-per-face sweep (the TMA tiles are tuned for, and
-  // instantiated with, the ideal gas of the paper's runs)
-  if (AK_FLUX_TMA && !c->P.eos && n % 2 == 0 && nfi * (AK_FLUX_CELL && DIR != 0 ? 2 : 1) <= TMA_THREADS) {
+  if (AK_FLUX_TMA && n % 2 == 0 && nfi * (AK_FLUX_CELL && DIR != 0 ? 2 : 1) <= TMA_THREADS) {
     // tile height: as many rows as fit the block, balanced over the extent it tiles
     const int nfd = DIR == 0 ? e : n + 3;
     const int namax = TMA_THREADS / nfi - (AK_FLUX_CELL && DIR != 0 ? 1 : 0);

@@ -46,7 +46,7 @@ __device__ __forceinline__ void mbar_wait(uint64_t* b, unsigned parity) {
       "}\n" ::"r"(smem_u32(b)), "r"(parity) : "memory");
 }
 
-template <int DIR, int RECON>
+template <int DIR, int RECON, int EOS = 0>
 __global__ void __launch_bounds__(TMA_THREADS, AK_TMA_MINB)
 k_flux_tma(const __grid_constant__ Par P, const __grid_constant__ Fields f, int NA) {
   extern __shared__ __align__(128) double sm[];
@@ -127,7 +127,7 @@ k_flux_tma(const __grid_constant__ Par P, const __grid_constant__ Fields f, int 
     mL[q] = g[0];
     mR[q] = g[DIR == 0 ? 1 : nt];
   }
-  face_flux<DIR, true>(P, P.riemann, mL, mR, sL, sR, Bfd, Fo);
+  face_flux<DIR, true, EOS>(P, P.riemann, mL, mR, sL, sR, Bfd, Fo);
 #pragma unroll
   for (int v = 0; v < 7; ++v) f.F[7 * DIR + v][fi] = Fo[v];
 }
@@ -146,7 +146,7 @@ k_flux_tma(const __grid_constant__ Par P, const __grid_constant__ Fields f, int 
 #ifndef AK_TMAC_MINB
 #define AK_TMAC_MINB 2
 #endif
-template <int DIR, int RECON>
+template <int DIR, int RECON, int EOS = 0>
 __global__ void __launch_bounds__(TMA_THREADS, AK_TMAC_MINB)
 k_flux_tma_cell(const __grid_constant__ Par P, const __grid_constant__ Fields f, int NA) {
   extern __shared__ __align__(128) double sm[];
@@ -229,7 +229,7 @@ k_flux_tma_cell(const __grid_constant__ Par P, const __grid_constant__ Fields f,
     mL[q] = g[0];
     mR[q] = g[DIR == 0 ? 1 : nt];
   }
-  face_flux<DIR, true>(P, P.riemann, mL, mR, sL, qm, Bfd, Fo);
+  face_flux<DIR, true, EOS>(P, P.riemann, mL, mR, sL, qm, Bfd, Fo);
 #pragma unroll
   for (int v = 0; v < 7; ++v) f.F[7 * DIR + v][fi] = Fo[v];
 }
