@@ -31,6 +31,21 @@ __device__ __forceinline__ void warp_count(unsigned long long* ctr, bool pred) {
   if (m != 0 && (threadIdx.x & 31) == (__ffs(m) - 1)) atomicAdd(ctr, (unsigned long long)__popc(m));
 }
 
+// Register-free prefetch of a line a thread reads only after a long dependent computation: lapse and
+// shift for the cell EMFs after the con2prim solve (profiles/r1_v10_final.md: the largest long-scoreboard
+// stall of that kernel; measured 3.156 -> 3.117 ms on C4).  The same for the DMP neighbourhood of the
+// FOFC test measured 3 % slower and is not done.
+#ifndef AK_PREFETCH
+#define AK_PREFETCH 1   // 0: off, 1: prefetch.global.L1, 2: prefetch.global.L2
+#endif
+__device__ __forceinline__ void prefetch(const void* p) {
+#if AK_PREFETCH == 1
+  asm volatile("prefetch.global.L1 [%0];" ::"l"(p));
+#elif AK_PREFETCH == 2
+  asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+#endif
+}
+
 // ---- index helpers (layouts of include/ak.h) ------------------------------------------
 struct Ix {
   int nt, px;
@@ -82,6 +97,10 @@ __global__ void __launch_bounds__(128, AK_C2P_MINB) k_con2prim(const __grid_cons
   double Ut[5], Bc[3], W5[5];
 #pragma unroll
   for (int v = 0; v < 5; ++v) Ut[v] = f.U[v][c];
+  if (EMF) {
+#pragma unroll
+    for (int q = 6; q < 10; ++q) prefetch(f.adm[q] + c);   // lapse and shift, read after the solve
+  }
   const long long fx = row * P.px + i;
   const long long fy = (mk * (nt + 1) + j) * nt + i;
   const long long fz = (((long long)m * (nt + 1) + k) * nt + j) * nt + i;
