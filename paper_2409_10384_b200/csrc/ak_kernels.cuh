@@ -16,6 +16,9 @@ namespace ak {
 #ifndef AK_C2P_MINB
 #define AK_C2P_MINB 8
 #endif
+#ifndef AK_C2P_PARK
+#define AK_C2P_PARK 1   // k_con2prim parks the metric and B in shared memory across the root solve
+#endif
 #ifndef AK_FLUX_MINB
 #define AK_FLUX_MINB 5
 #endif
@@ -107,7 +110,34 @@ __global__ void __launch_bounds__(128, AK_C2P_MINB) k_con2prim(const __grid_cons
   Bc[0] = 0.5 * (__ldg(f.Bf[0] + fx) + __ldg(f.Bf[0] + fx + 1));
   Bc[1] = 0.5 * (__ldg(f.Bf[1] + fy) + __ldg(f.Bf[1] + fy + nt));
   Bc[2] = 0.5 * (__ldg(f.Bf[2] + fz) + __ldg(f.Bf[2] + fz + (long long)nt * nt));
+#if AK_C2P_PARK
+  // The metric and B are needed again only after the root solve.  Parked in shared memory they
+  // leave the registers for the solve; left to the compiler they are spilled to local memory,
+  // which is written through to L2 and partly on to DRAM (profiles/r1_v10_final.md): 3.12 -> 2.90 ms
+  // on C4.  Parking r^i and B^i inside c2p_cell as well, or in k_fofc_test, measured no gain / 1 % loss.
+  __shared__ double park[9][128];
+  park[0][threadIdx.x] = g.xx; park[1][threadIdx.x] = g.xy; park[2][threadIdx.x] = g.xz;
+  park[3][threadIdx.x] = g.yy; park[4][threadIdx.x] = g.yz; park[5][threadIdx.x] = g.zz;
+#pragma unroll
+  for (int v = 0; v < 3; ++v) park[6 + v][threadIdx.x] = Bc[v];
+  const int st = c2p_cell<false, EOS>(P, g, Ut, Bc, W5);
+  {
+    volatile double* pk = &park[0][threadIdx.x];
+    g.xx = pk[0]; g.xy = pk[128]; g.xz = pk[2 * 128]; g.yy = pk[3 * 128]; g.yz = pk[4 * 128]; g.zz = pk[5 * 128];
+#pragma unroll
+    for (int v = 0; v < 3; ++v) Bc[v] = pk[(6 + v) * 128];
+  }
+  if (st != 0) {   // "a similar policy holds for the conserved variables": rewrite them from the final primitives
+    double det, sdet;
+    Met3 gu;
+    metric_inverse(g, det, sdet, gu);
+    const double isd = 1.0 / sdet;
+    const double B[3] = {Bc[0] * isd, Bc[1] * isd, Bc[2] * isd};
+    c2p_write_back<EOS>(P, g, sdet, W5[0], W5[1], W5[2], W5[3], W5[4], B, Ut);
+  }
+#else
   const int st = c2p_cell<true, EOS>(P, g, Ut, Bc, W5);
+#endif
 #pragma unroll
   for (int v = 0; v < 5; ++v) f.W[v][c] = W5[v];
 #pragma unroll
