@@ -210,7 +210,11 @@ int launch_flux(ak_ctx* c, const Fields& f) {
     const int tiles = (nfd + namax - 1) / namax;
     const int NA = (nfd + tiles - 1) / tiles;
     const int maxW = DIR == 0 ? NA : NA + 5, maxM = DIR == 0 ? NA : NA + 1;
-    const size_t smem = sizeof(double) * ((size_t)(7 * maxW + 10 * maxM) * nt + (AK_FLUX_CELL ? 7 * TMA_THREADS : 0));
+    size_t smem = sizeof(double) * ((size_t)(7 * maxW + 10 * maxM) * nt + (AK_FLUX_CELL ? 7 * TMA_THREADS : 0));
+    if (!AK_FLUX_CELL && AK_FLUX_PARK) {   // k_flux_tma reuses the tile as 21 doubles of parking space per thread
+      const size_t park = sizeof(double) * 21 * (size_t)TMA_THREADS;
+      if (park > smem) smem = park;
+    }
     if (smem <= 200 * 1024) {
       const unsigned grid = (unsigned)((long long)c->P.nmb * e * tiles);
       // threads: one per face (or cell) of the tile, rounded up to whole warps

@@ -232,4 +232,55 @@ __device__ __forceinline__ void face_flux(const Par& P, int rs, const double mL[
   }
 }
 
+// The same face flux with the long-lived intermediates parked in shared memory instead of spilled to
+// local memory (which is written through to L2): the right state waits there while the left side is
+// evaluated, the left side's U and F while the right side is.  pk = this thread's column of a
+// [21][stride] array no other thread touches.  Same operations in the same order as face_flux<DIR, true>.
+template <int DIR, int EOS = 0>
+__device__ __forceinline__ void face_flux_parked(const Par& P, int rs, const FaceGeo& G, double sL[7], double sR[7],
+                                                 double Bfd, double Fo[7], double* park, int stride) {
+  volatile double* pk = park;
+  const double Bd = Bfd * G.isd;
+  face_floor<EOS>(P, sL); face_floor<EOS>(P, sR);
+#pragma unroll
+  for (int v = 0; v < 7; ++v) pk[v * stride] = sR[v];
+  double UR[7], FR[7], lmL, lpL, lmR, lpR;
+  {
+    double UL[7], FL[7];
+    side_state<DIR, EOS>(P, G, sL, Bd, UL, FL, lmL, lpL);
+#pragma unroll
+    for (int c = 0; c < 7; ++c) { pk[(7 + c) * stride] = UL[c]; pk[(14 + c) * stride] = FL[c]; }
+  }
+  {
+    double sRq[7];
+#pragma unroll
+    for (int v = 0; v < 7; ++v) sRq[v] = pk[v * stride];
+    side_state<DIR, EOS>(P, G, sRq, Bd, UR, FR, lmR, lpR);
+  }
+  if (rs == 1) {   // HLLE
+    const double lL = fmin(0.0, fmin(lmL, lmR));
+    const double lR = fmax(0.0, fmax(lpL, lpR));
+    const double dl = lR - lL;
+    if (dl == 0.0) {
+#pragma unroll
+      for (int c = 0; c < 7; ++c) Fo[c] = 0.5 * (pk[(14 + c) * stride] + FR[c]);
+    } else {
+      const double idl = 1.0 / dl;
+      const double lRL = lR * lL;
+#pragma unroll
+      for (int c = 0; c < 7; ++c) {
+        const double ULc = pk[(7 + c) * stride], FLc = pk[(14 + c) * stride];
+        Fo[c] = (lR * FLc - lL * FR[c] + lRL * (UR[c] - ULc)) * idl;
+      }
+    }
+  } else {         // LLF
+    const double lam = fmax(fmax(fabs(lmL), fabs(lpL)), fmax(fabs(lmR), fabs(lpR)));
+#pragma unroll
+    for (int c = 0; c < 7; ++c) {
+      const double ULc = pk[(7 + c) * stride], FLc = pk[(14 + c) * stride];
+      Fo[c] = 0.5 * (FLc + FR[c]) - 0.5 * lam * (UR[c] - ULc);
+    }
+  }
+}
+
 }  // namespace ak

@@ -17,6 +17,9 @@
 
 namespace ak {
 
+#ifndef AK_FLUX_PARK
+#define AK_FLUX_PARK 1   // k_flux_tma: intermediates of the Riemann solve parked in the (spent) tile
+#endif
 #ifndef AK_TMA_MINB
 #define AK_TMA_MINB 3
 #endif
@@ -103,31 +106,45 @@ k_flux_tma(const __grid_constant__ Par P, const __grid_constant__ Fields f, int 
     Bfd = __ldg(f.Bf[DIR] + fi);
   }
   mbar_wait(&mbar, 0);
+#if !AK_FLUX_PARK
   if (!active) return;
+#endif
   double sL[7], sR[7], mL[10], mR[10], Fo[7];
+  if (active) {
 #pragma unroll
-  for (int v = 0; v < 7; ++v) {
-    // six stencil cells f-3 .. f+2: along i in one row (x) or one per shared row (y, z)
-    const double* w = DIR == 0 ? sW + ((size_t)v * maxW + a) * nt + ii - 3 : sW + ((size_t)v * maxW + a) * nt + ii;
-    const int s = DIR == 0 ? 1 : nt;
-    if (RECON == 0) {
-      sL[v] = w[2 * s]; sR[v] = w[3 * s];
-    } else {
-      const double q0 = w[0], q1 = w[s], q2 = w[2 * s], q3 = w[3 * s], q4 = w[4 * s], q5 = w[5 * s];
-      double qm, qp;
-      recon<RECON>(q0, q1, q2, q3, q4, qm, qp);
-      sL[v] = qp;
-      recon<RECON>(q1, q2, q3, q4, q5, qm, qp);
-      sR[v] = qm;
+    for (int v = 0; v < 7; ++v) {
+      // six stencil cells f-3 .. f+2: along i in one row (x) or one per shared row (y, z)
+      const double* w = DIR == 0 ? sW + ((size_t)v * maxW + a) * nt + ii - 3 : sW + ((size_t)v * maxW + a) * nt + ii;
+      const int s = DIR == 0 ? 1 : nt;
+      if (RECON == 0) {
+        sL[v] = w[2 * s]; sR[v] = w[3 * s];
+      } else {
+        const double q0 = w[0], q1 = w[s], q2 = w[2 * s], q3 = w[3 * s], q4 = w[4 * s], q5 = w[5 * s];
+        double qm, qp;
+        recon<RECON>(q0, q1, q2, q3, q4, qm, qp);
+        sL[v] = qp;
+        recon<RECON>(q1, q2, q3, q4, q5, qm, qp);
+        sR[v] = qm;
+      }
+    }
+#pragma unroll
+    for (int q = 0; q < 10; ++q) {
+      const double* g = DIR == 0 ? sM + ((size_t)q * maxM + a) * nt + ii - 1 : sM + ((size_t)q * maxM + a) * nt + ii;
+      mL[q] = g[0];
+      mR[q] = g[DIR == 0 ? 1 : nt];
     }
   }
-#pragma unroll
-  for (int q = 0; q < 10; ++q) {
-    const double* g = DIR == 0 ? sM + ((size_t)q * maxM + a) * nt + ii - 1 : sM + ((size_t)q * maxM + a) * nt + ii;
-    mL[q] = g[0];
-    mR[q] = g[DIR == 0 ? 1 : nt];
-  }
+#if AK_FLUX_PARK
+  // every thread has read its stencils: the tile is reused as the parking space of face_flux_parked
+  // (21 doubles per thread; the launcher sizes the allocation for both uses)
+  FaceGeo G;
+  if (active) face_geometry<DIR>(mL, mR, G);
+  __syncthreads();
+  if (!active) return;
+  face_flux_parked<DIR, EOS>(P, P.riemann, G, sL, sR, Bfd, Fo, sm + t, (int)blockDim.x);
+#else
   face_flux<DIR, true, EOS>(P, P.riemann, mL, mR, sL, sR, Bfd, Fo);
+#endif
 #pragma unroll
   for (int v = 0; v < 7; ++v) f.F[7 * DIR + v][fi] = Fo[v];
 }
