@@ -160,8 +160,11 @@ k_flux_tma(const __grid_constant__ Par P, const __grid_constant__ Fields f, int 
 //   DIR = x : NA rows x (n+4) cells (i in [is-2, ie+2]); the first cell of a row has no face.
 //   DIR = y,z: (NA+1) cell rows x (n+2) lanes for NA face rows; the first cell row has no face.
 // Same shared slabs as k_flux_tma plus 7 doubles per thread for q^+.
+#ifndef AK_FLUXC_PARK
+#define AK_FLUXC_PARK 1   // Riemann intermediates parked in the spent tile after a second barrier
+#endif
 #ifndef AK_TMAC_MINB
-#define AK_TMAC_MINB 2
+#define AK_TMAC_MINB 3    // with parking 80 registers do (3 blocks/SM: 4.19 -> 4.11 ms on C4; 2 blocks at 128: 4.29)
 #endif
 template <int DIR, int RECON, int EOS = 0>
 __global__ void __launch_bounds__(TMA_THREADS, AK_TMAC_MINB)
@@ -235,18 +238,31 @@ k_flux_tma_cell(const __grid_constant__ Par P, const __grid_constant__ Fields f,
     }
   }
   __syncthreads();
+#if !AK_FLUXC_PARK
   if (!has_face) return;
+#endif
   const int back = DIR == 0 ? 1 : nci;                 // thread of the lower cell
   double sL[7], mL[10], mR[10], Fo[7];
+  if (has_face) {
 #pragma unroll
-  for (int v = 0; v < 7; ++v) sL[v] = sQ[v * TMA_THREADS + t - back];
+    for (int v = 0; v < 7; ++v) sL[v] = sQ[v * TMA_THREADS + t - back];
 #pragma unroll
-  for (int q = 0; q < 10; ++q) {
-    const double* g = DIR == 0 ? sM + ((size_t)q * maxM + a) * nt + ii - 1 : sM + ((size_t)q * maxM + a - 1) * nt + ii;
-    mL[q] = g[0];
-    mR[q] = g[DIR == 0 ? 1 : nt];
+    for (int q = 0; q < 10; ++q) {
+      const double* g = DIR == 0 ? sM + ((size_t)q * maxM + a) * nt + ii - 1 : sM + ((size_t)q * maxM + a - 1) * nt + ii;
+      mL[q] = g[0];
+      mR[q] = g[DIR == 0 ? 1 : nt];
+    }
   }
+#if AK_FLUXC_PARK
+  // second barrier: states and metric are in registers, the whole allocation becomes parking space
+  FaceGeo G;
+  if (has_face) face_geometry<DIR>(mL, mR, G);
+  __syncthreads();
+  if (!has_face) return;
+  face_flux_parked<DIR, EOS>(P, P.riemann, G, sL, qm, Bfd, Fo, sm + t, (int)blockDim.x);
+#else
   face_flux<DIR, true, EOS>(P, P.riemann, mL, mR, sL, qm, Bfd, Fo);
+#endif
 #pragma unroll
   for (int v = 0; v < 7; ++v) f.F[7 * DIR + v][fi] = Fo[v];
 }
