@@ -211,7 +211,7 @@ int launch_flux(ak_ctx* c, const Fields& f) {
     const int NA = (nfd + tiles - 1) / tiles;
     const int maxW = DIR == 0 ? NA : NA + 5, maxM = DIR == 0 ? NA : NA + 1;
     size_t smem = sizeof(double) * ((size_t)(7 * maxW + 10 * maxM) * nt + (AK_FLUX_CELL ? 7 * TMA_THREADS : 0));
-    if (AK_FLUX_CELL ? AK_FLUXC_PARK : AK_FLUX_PARK) {   // the tile is reused as 21 doubles of parking space per thread
+    if (AK_FLUX_CELL ? AK_FLUXC_PARK : AK_FLUX_PARK) {   // the spent tile is reused as 21 doubles of parking space per thread
       const size_t park = sizeof(double) * 21 * (size_t)TMA_THREADS;
       if (park > smem) smem = park;
     }

@@ -233,28 +233,29 @@ __device__ __forceinline__ void face_flux(const Par& P, int rs, const double mL[
 }
 
 // The same face flux with the long-lived intermediates parked in shared memory instead of spilled to
-// local memory (which is written through to L2): the right state waits there while the left side is
-// evaluated, the left side's U and F while the right side is.  pk = this thread's column of a
-// [21][stride] array no other thread touches.  Same operations in the same order as face_flux<DIR, true>.
+// local memory (which is written through to L2): the right state waits there (pkR, put there by the
+// caller, unfloored) while the left side is evaluated, the left side's U and F (pk, [14][stride]) while
+// the right side is.  Columns no other thread touches.  Same operations as face_flux<DIR, true>.
 template <int DIR, int EOS = 0>
-__device__ __forceinline__ void face_flux_parked(const Par& P, int rs, const FaceGeo& G, double sL[7], double sR[7],
-                                                 double Bfd, double Fo[7], double* park, int stride) {
+__device__ __forceinline__ void face_flux_parked(const Par& P, int rs, const FaceGeo& G, double sL[7],
+                                                 double* parkR, int strideR, double Bfd, double Fo[7],
+                                                 double* park, int stride) {
   volatile double* pk = park;
+  volatile double* pkR = parkR;
   const double Bd = Bfd * G.isd;
-  face_floor<EOS>(P, sL); face_floor<EOS>(P, sR);
-#pragma unroll
-  for (int v = 0; v < 7; ++v) pk[v * stride] = sR[v];
+  face_floor<EOS>(P, sL);
   double UR[7], FR[7], lmL, lpL, lmR, lpR;
   {
     double UL[7], FL[7];
     side_state<DIR, EOS>(P, G, sL, Bd, UL, FL, lmL, lpL);
 #pragma unroll
-    for (int c = 0; c < 7; ++c) { pk[(7 + c) * stride] = UL[c]; pk[(14 + c) * stride] = FL[c]; }
+    for (int c = 0; c < 7; ++c) { pk[c * stride] = UL[c]; pk[(7 + c) * stride] = FL[c]; }
   }
   {
     double sRq[7];
 #pragma unroll
-    for (int v = 0; v < 7; ++v) sRq[v] = pk[v * stride];
+    for (int v = 0; v < 7; ++v) sRq[v] = pkR[v * strideR];
+    face_floor<EOS>(P, sRq);
     side_state<DIR, EOS>(P, G, sRq, Bd, UR, FR, lmR, lpR);
   }
   if (rs == 1) {   // HLLE
@@ -263,13 +264,13 @@ __device__ __forceinline__ void face_flux_parked(const Par& P, int rs, const Fac
     const double dl = lR - lL;
     if (dl == 0.0) {
 #pragma unroll
-      for (int c = 0; c < 7; ++c) Fo[c] = 0.5 * (pk[(14 + c) * stride] + FR[c]);
+      for (int c = 0; c < 7; ++c) Fo[c] = 0.5 * (pk[(7 + c) * stride] + FR[c]);
     } else {
       const double idl = 1.0 / dl;
       const double lRL = lR * lL;
 #pragma unroll
       for (int c = 0; c < 7; ++c) {
-        const double ULc = pk[(7 + c) * stride], FLc = pk[(14 + c) * stride];
+        const double ULc = pk[c * stride], FLc = pk[(7 + c) * stride];
         Fo[c] = (lR * FLc - lL * FR[c] + lRL * (UR[c] - ULc)) * idl;
       }
     }
@@ -277,7 +278,7 @@ __device__ __forceinline__ void face_flux_parked(const Par& P, int rs, const Fac
     const double lam = fmax(fmax(fabs(lmL), fabs(lpL)), fmax(fabs(lmR), fabs(lpR)));
 #pragma unroll
     for (int c = 0; c < 7; ++c) {
-      const double ULc = pk[(7 + c) * stride], FLc = pk[(14 + c) * stride];
+      const double ULc = pk[c * stride], FLc = pk[(7 + c) * stride];
       Fo[c] = 0.5 * (FLc + FR[c]) - 0.5 * lam * (UR[c] - ULc);
     }
   }

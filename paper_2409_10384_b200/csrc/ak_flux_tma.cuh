@@ -141,7 +141,13 @@ k_flux_tma(const __grid_constant__ Par P, const __grid_constant__ Fields f, int 
   if (active) face_geometry<DIR>(mL, mR, G);
   __syncthreads();
   if (!active) return;
-  face_flux_parked<DIR, EOS>(P, P.riemann, G, sL, sR, Bfd, Fo, sm + t, (int)blockDim.x);
+  {   // (parking the right state behind the tile while it is reconstructed measured 3 % slower: more shared memory)
+    volatile double* pR = sm + 14 * (int)blockDim.x + t;
+#pragma unroll
+    for (int v = 0; v < 7; ++v) pR[v * (int)blockDim.x] = sR[v];
+  }
+  face_flux_parked<DIR, EOS>(P, P.riemann, G, sL, sm + 14 * (int)blockDim.x + t, (int)blockDim.x, Bfd, Fo, sm + t,
+                             (int)blockDim.x);
 #else
   face_flux<DIR, true, EOS>(P, P.riemann, mL, mR, sL, sR, Bfd, Fo);
 #endif
@@ -259,7 +265,13 @@ k_flux_tma_cell(const __grid_constant__ Par P, const __grid_constant__ Fields f,
   if (has_face) face_geometry<DIR>(mL, mR, G);
   __syncthreads();
   if (!has_face) return;
-  face_flux_parked<DIR, EOS>(P, P.riemann, G, sL, qm, Bfd, Fo, sm + t, (int)blockDim.x);
+  {
+    volatile double* pR = sm + 14 * (int)blockDim.x + t;
+#pragma unroll
+    for (int v = 0; v < 7; ++v) pR[v * (int)blockDim.x] = qm[v];
+  }
+  face_flux_parked<DIR, EOS>(P, P.riemann, G, sL, sm + 14 * (int)blockDim.x + t, (int)blockDim.x, Bfd, Fo, sm + t,
+                             (int)blockDim.x);
 #else
   face_flux<DIR, true, EOS>(P, P.riemann, mL, mR, sL, qm, Bfd, Fo);
 #endif
