@@ -51,8 +51,8 @@ FLUX_FP64_PER_FACE = {0: 634, 1: 928, 2: 1810, 3: 752, 4: 1600}   # 4 (PPMX): st
 FP64_PIPE_PEAK_TINST = 148 * 4 * 16 * 1.965e9 * 1e-12
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu capture
 # (profiles/r1_v11_final.md), keyed by (blocks, kernel class); other sizes: null.
-NCU_TRAFFIC_BYTES = {(768, "con2prim"): 12.077e9, (768, "flux_x"): 7.680e9, (768, "flux_y"): 8.243e9,
-                     (768, "flux_z"): 8.297e9, (768, "fofc_test"): 9.089e9, (768, "div_src"): 11.372e9}
+NCU_TRAFFIC_BYTES = {(768, "con2prim"): 12.073e9, (768, "flux_x"): 7.632e9, (768, "flux_y"): 8.180e9,
+                     (768, "flux_z"): 8.223e9, (768, "fofc_test"): 9.088e9, (768, "div_src"): 11.376e9}
 
 
 def kernel_units(nmb, n):
