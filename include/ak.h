@@ -28,13 +28,17 @@
  *   E_z (z-edges) [nmb][nt][nt+1][px]
  * A tilde means "densitised", i.e. multiplied by sqrt(det gamma_ij).
  *
- * ---- Ownership.  Every field pointer is a DEVICE pointer owned by the caller (8-byte
- * aligned fp64, or bytes for masks) unless a function says "host".  The context borrows
+ * ---- Ownership.  Every field pointer is a DEVICE pointer owned by the caller (fp64, the base
+ * of every field 16-byte aligned — checked, AK_EINVAL otherwise: rows are staged with TMA bulk
+ * copies, which need it; or bytes for masks) unless a function says "host".  The context borrows
  * pointers for the duration of one call (metric: until replaced or ak_destroy) and owns
  * only its scratch (face fluxes, cell-centred EMFs, FOFC face lists, counters).
  *
  * ---- Asynchrony.  ak_con2prim / ak_rhs / ak_emf enqueue on the context's stream and
  * return; they never synchronise.  ak_get_stats and the *_host entry points synchronise.
+ * With an overlapped schedule (ak_set_overlap) ak_rhs forks onto context-owned streams and
+ * joins back: work enqueued on the context's stream before the call is complete before any
+ * kernel of the stage starts, and work enqueued after it starts after the whole stage.
  *
  * ---- Errors.  Return codes report API misuse and CUDA failures only.  Unphysical cells
  * are data ("it is flagged"): they are reported through status / flag bytes and the
@@ -131,6 +135,17 @@ int ak_con2prim(ak_ctx*, const ak_cons* U, const ak_faceB* Bf, const ak_prim* W,
 int ak_rhs(ak_ctx*, const ak_cons* U, const ak_faceB* Bf, const ak_prim* W, int w_is_valid,
            double dt_fofc, const ak_rhs_out* out);
 
+/* Schedule of ak_rhs (and of the stages of ak_advance).  nchunks < 2 (the state after ak_create
+ * unless the environment variable AK_OV_CHUNKS is set): the kernels of parts (1)-(6) run one after
+ * another over the whole batch on the context's stream.  nchunks >= 2 (at most 64): MeshBlocks are
+ * independent (S:§8(e)), so the batch is cut into nchunks contiguous groups of blocks and the stage is
+ * pipelined over them on three context-owned streams: part (1) of group i+1 and parts (4)-(6) of group
+ * i-1 — bound by memory latency and bandwidth — run with capped grids and high priority beside the
+ * fp64-bound sweeps (2)+(3) of group i, so that both the fp64 pipe and HBM stay busy (D:§6.2).  Same
+ * kernels, same arithmetic, the same bits out; only events order the streams (no kernel waits on
+ * another).  nchunks is clamped to nmb. */
+int ak_set_overlap(ak_ctx*, int nchunks);
+
 /* Part (5) alone, from the (post-FOFC) fluxes the last ak_rhs left in the context
  * (AK_ESTATE if there are none) and the primitives W. */
 int ak_emf(ak_ctx*, const ak_prim* W, double* Ex, double* Ey, double* Ez);
@@ -178,7 +193,7 @@ int ak_set_fofc_blend(ak_ctx*, const ak_cons* U0, double a, double b);
  * (ignored for nseg = 1); K0 >= 0; gamma_th > 1: else AK_EINVAL, nothing changed.  The arrays are
  * copied.  ak_params.gamma_ad is then unused.  nseg = 0 returns to the ideal gas of ak_params.
  * rho^Gamma is the device pow(): results agree with a libm evaluation to rounding, not bit for bit.
- * The hybrid stage runs the plain (not TMA-staged) flux sweeps. */
+ * The hybrid stage runs the same TMA-staged flux sweeps as the ideal gas (kernels templated on the EOS). */
 int ak_set_eos_hybrid(ak_ctx*, int nseg, double K0, const double* gammas, const double* rho_breaks,
                       double gamma_th);
 
@@ -233,8 +248,12 @@ int ak_advance(ak_ctx*, int integrator, int nsteps, double dt, const int bc[3], 
 
 /* Device-timing hooks for the benchmark: bracket kernel class `which` (0 con2prim, 1-3 flux
  * sweeps x/y/z, 4 FOFC test, 5 FOFC list+reflux, 6 cell EMF+CT, 7 divergence+sources) with
- * CUDA events on the context's stream in subsequent calls; ak_kernel_ms synchronises and
- * returns the accumulated milliseconds and launch count since ak_timing was enabled. */
+ * CUDA events on the stream the class is launched on in subsequent calls; ak_kernel_ms synchronises
+ * and returns the accumulated milliseconds and launch count since ak_timing was enabled.
+ * Serial schedule: the classes partition the stage, their times add up to it.  Overlapped schedule:
+ * a class's time is the span from its first block starting to its last block finishing while kernels
+ * of the other streams share the SMs — spans overlap, their sum exceeds the stage time, and a span is
+ * NOT the kernel's stand-alone duration (use the serial schedule for per-kernel rooflines). */
 int ak_timing(ak_ctx*, int enable);
 int ak_kernel_ms(ak_ctx*, double ms_out[8], long long launches_out[8]);
 

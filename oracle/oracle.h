@@ -3,8 +3,10 @@
  * Plain, slow, fp64 restatement of the Valencia GRMHD right-hand-side stage of
  * arXiv:2409.10384 (PAPER.md, cited as P:line).  It exists to check the CUDA
  * library; only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
- * `--impl reference` leg may build, load or call it.  It shares no code, header,
- * table or helper with paper_2409_10384_b200/csrc (the product).
+ * `--impl reference` leg may build, load or call it.  No file, header, table or helper is
+ * shared with paper_2409_10384_b200/csrc (the product); the product's point operators restate
+ * the same canonical expression trees, so agreement of the two to the last bit
+ * certifies the product's plumbing, while the physics is certified by the pins below.
  *
  * Steps follow DESIGN.md §3 (O0..O9) which restates, in the paper's notation,
  *   Eq. 6 prim->cons, Eq. 7 b^mu, Eq. 8 fluxes,

@@ -23,7 +23,7 @@ EXPORTS = ("ak_create", "ak_set_metric", "ak_con2prim", "ak_rhs", "ak_emf", "ak_
            "ak_probe_fp64", "ak_destroy", "ak_strerror", "ak_version",
            "ak_set_fofc_blend", "ak_fill_ghosts", "ak_stage_update", "ak_advance", "ak_set_neighbors",
            "ak_matter_sources", "ak_halo_slab_elems", "ak_halo_pack", "ak_halo_unpack",
-           "ak_set_eos_hybrid")
+           "ak_set_eos_hybrid", "ak_set_overlap")
 BC_PERIODIC, BC_OUTFLOW = 0, 1
 
 _dp = C.POINTER(C.c_double)
@@ -119,6 +119,7 @@ def lib():
                                  C.POINTER(AkFaceB), C.POINTER(AkPrim), C.c_void_p]
         L.ak_matter_sources.argtypes = [C.c_void_p, C.POINTER(AkPrim), C.POINTER(AkMatter)]
         L.ak_set_neighbors.argtypes = [C.c_void_p, C.POINTER(C.c_int), C.c_int]
+        L.ak_set_overlap.argtypes = [C.c_void_p, C.c_int]
         _lib = L
     return _lib
 
@@ -209,6 +210,11 @@ def ak_rhs_host(ctx, U, Bf, W, dt_fofc, dU, E, fofc_flag=None, c2p_status=None):
     u, b, w = _struct(AkCons, U), _struct(AkFaceB, Bf), _struct(AkPrim, W)
     o = _struct(AkRhsOut, list(dU) + list(E) + [fofc_flag, c2p_status])
     _chk(lib().ak_rhs_host(ctx, C.byref(u), C.byref(b), C.byref(w), float(dt_fofc), C.byref(o)), "ak_rhs_host")
+
+
+def ak_set_overlap(ctx, nchunks):
+    """schedule of ak_rhs: < 2 serial, else pipelined over nchunks groups of blocks (include/ak.h)."""
+    _chk(lib().ak_set_overlap(ctx, int(nchunks)), "ak_set_overlap")
 
 
 def ak_emf(ctx, W, Ex, Ey, Ez):

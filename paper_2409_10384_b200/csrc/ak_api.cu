@@ -11,6 +11,7 @@
 #include <cmath>
 #include <cstdint>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -19,6 +20,16 @@ using namespace ak;
 namespace {
 
 enum { KC_C2P = 0, KC_FX, KC_FY, KC_FZ, KC_FOFC_TEST, KC_FOFC_FIX, KC_CT, KC_SRC, KC_N };
+constexpr int MAXCH = 64;     // most chunks of an overlapped schedule (counter slots per context)
+// overlapped schedule: blocks per SM the memory-bound classes may take beside the sweeps (0 = no cap)
+#ifndef AK_OV_CAP_C2P_DEFAULT
+#define AK_OV_CAP_C2P_DEFAULT 3
+#define AK_OV_CAP_FOFC_DEFAULT 3
+#define AK_OV_CAP_FIX_DEFAULT 2
+#define AK_OV_CAP_CT_DEFAULT 4
+#define AK_OV_CAP_SRC_DEFAULT 2
+#define AK_OV_SMEM_PAD_DEFAULT 0
+#endif
 
 struct Sizes {
   long long cell, xf, yf, zf, ex, ey, ez;   // elements per batch
@@ -45,7 +56,12 @@ struct ak_ctx {
   double* stg_U[5]; double* stg_Bf[3]; double* stg_W[8]; double* stg_dU[5]; double* stg_E[3];
   unsigned char* stg_flag; unsigned char* stg_status;
   bool have_stg;
-  bool tma_attr[2][3];
+  // overlapped schedule (ak_set_overlap): chunks of blocks on internal streams
+  int ov_chunks;                // < 2: serial
+  cudaStream_t ovs[3];          // con2prim, sweeps, FOFC/CT/sources (ovs[2] may equal ovs[0])
+  cudaEvent_t* ov_ev; int ov_nev;
+  int cap[8];                   // grid caps (blocks) per kernel class in the overlapped schedule, 0 = none
+  int sweep_smem_pad;           // bytes: dynamic shared memory the sweeps ask for at least when overlapped
   // FOFC stage blend (ak_set_fofc_blend)
   const double* blendU0[5]; double blend_a, blend_b;
   // stage-driver registers (ak_advance), allocated on first use
@@ -108,17 +124,27 @@ inline void copy_eos(Par& d, const Par& s) {
 
 inline unsigned nblk(long long n, int t) { return (unsigned)((n + t - 1) / t); }
 
+// One launch target: a contiguous range of blocks (Par.nmb of them, every field pointer of Fields moved to
+// the first) on a stream.  Serial schedule: the whole batch on the context's stream.  Overlapped schedule
+// (ak_set_overlap): one chunk of blocks on one of the internal streams.
+struct Lane {
+  const Par& P;
+  const Fields& f;
+  cudaStream_t st;
+  bool ov;          // part of an overlapped schedule: grid caps and the sweep shared-memory pad apply
+};
+
 struct Timer {
-  ak_ctx* c; int which; cudaEvent_t a, b; bool on;
-  Timer(ak_ctx* c_, int w) : c(c_), which(w), on(c_->timing) {
+  ak_ctx* c; int which; cudaEvent_t a, b; bool on; cudaStream_t st;
+  Timer(ak_ctx* c_, int w, cudaStream_t st_) : c(c_), which(w), on(c_->timing), st(st_) {
     if (on) {
       cudaEventCreate(&a); cudaEventCreate(&b);
-      cudaEventRecord(a, c->stream);
+      cudaEventRecord(a, st);
     }
   }
   ~Timer() {
     if (!on) return;
-    cudaEventRecord(b, c->stream);
+    cudaEventRecord(b, st);
     if (c->npend == c->cappend) {
       int nc = c->cappend ? 2 * c->cappend : 256;
       ak_ctx::Pending* np = (ak_ctx::Pending*)realloc(c->pend, sizeof(ak_ctx::Pending) * nc);
@@ -143,33 +169,69 @@ void fill_fields(ak_ctx* c, Fields& f) {
   f.fa = c->blend_a; f.fb = c->blend_b;
 }
 
+// Fields / Par of the sub-batch of blocks [m0, m0 + nb): every pointer moved to block m0 of its own layout;
+// counters and the flagged-cell list are the slots of chunk `ci`.
+void chunk_fields(const ak_ctx* c, const Fields& f, int m0, int nb, int ci, Fields& g, Par& Pc) {
+  Pc = c->P;
+  Pc.nmb = nb;
+  g = f;
+  const long long nt = c->P.nt, px = c->P.px, n = c->P.n;
+  const long long cell = nt * nt * nt * m0;
+  const long long fsz[3] = {nt * nt * px * m0, nt * (nt + 1) * nt * m0, (nt + 1) * nt * nt * m0};
+  const long long esz[3] = {(nt + 1) * (nt + 1) * nt * m0, (nt + 1) * nt * px * m0, nt * (nt + 1) * px * m0};
+  for (int q = 0; q < 5; ++q) { g.U[q] += cell; if (g.dU[q]) g.dU[q] += cell; if (g.U0[q]) g.U0[q] += cell; }
+  for (int q = 0; q < 3; ++q) { g.Bf[q] += fsz[q]; g.Ecc[q] += cell; if (g.E[q]) g.E[q] += esz[q]; }
+  for (int q = 0; q < 16; ++q) g.adm[q] += cell;
+  for (int q = 0; q < 8; ++q) g.W[q] += cell;
+  for (int q = 0; q < 21; ++q) g.F[q] += fsz[q / 7];
+  g.flag += cell;
+  if (g.status) g.status += cell;
+  g.dx += 3LL * m0;
+  g.list += (n + 2) * (n + 2) * (n + 2) * m0;
+  g.count += 4 * ci;
+  g.stats += (long long)S_NSTAT * ci;
+}
+
+// 16-byte alignment of every caller field pointer ("Base pointers 16-B aligned (checked ->
+// AK_EINVAL)"): the TMA-staged sweeps copy rows of W and of the metric with cp.async.bulk / tensor maps,
+// which fault on a global address that is not a multiple of 16.
+inline bool al16(const void* p) { return p && (((uintptr_t)p) & 15u) == 0; }
+
 bool set_cons(Fields& f, const ak_cons* U) {
-  if (!U || !U->D || !U->Sx || !U->Sy || !U->Sz || !U->tau) return false;
+  if (!U || !al16(U->D) || !al16(U->Sx) || !al16(U->Sy) || !al16(U->Sz) || !al16(U->tau)) return false;
   f.U[0] = U->D; f.U[1] = U->Sx; f.U[2] = U->Sy; f.U[3] = U->Sz; f.U[4] = U->tau;
   return true;
 }
 bool set_faceB(Fields& f, const ak_faceB* B) {
-  if (!B || !B->bx || !B->by || !B->bz) return false;
+  if (!B || !al16(B->bx) || !al16(B->by) || !al16(B->bz)) return false;
   f.Bf[0] = B->bx; f.Bf[1] = B->by; f.Bf[2] = B->bz;
   return true;
 }
 bool set_prim(Fields& f, const ak_prim* W) {
-  if (!W || !W->rho || !W->ux || !W->uy || !W->uz || !W->p || !W->bccx || !W->bccy || !W->bccz)
+  if (!W || !al16(W->rho) || !al16(W->ux) || !al16(W->uy) || !al16(W->uz) || !al16(W->p) || !al16(W->bccx) ||
+      !al16(W->bccy) || !al16(W->bccz))
     return false;
   f.W[0] = W->rho; f.W[1] = W->ux; f.W[2] = W->uy; f.W[3] = W->uz; f.W[4] = W->p;
   f.W[5] = W->bccx; f.W[6] = W->bccy; f.W[7] = W->bccz;
   return true;
 }
 
-int launch_c2p(ak_ctx* c, const Fields& f, bool with_emf) {
-  Timer t(c, KC_C2P);
-  CK(cudaMemsetAsync(c->stats, 0, sizeof(unsigned long long) * 3, c->stream));
-  const unsigned g = nblk(c->sz.cell, 128);
-  if (c->P.eos) {
-    if (with_emf) k_con2prim<true, 1><<<g, 128, 0, c->stream>>>(c->P, f);
-    else k_con2prim<false, 1><<<g, 128, 0, c->stream>>>(c->P, f);
-  } else if (with_emf) k_con2prim<true><<<g, 128, 0, c->stream>>>(c->P, f);
-  else k_con2prim<false><<<g, 128, 0, c->stream>>>(c->P, f);
+// grid of a grid-stride kernel: what covers the items, or the cap of its class when one is set
+inline unsigned capped(long long items, int threads, int cap_blocks) {
+  const long long need = (items + threads - 1) / threads;
+  return (unsigned)((cap_blocks > 0 && need > cap_blocks) ? cap_blocks : need);
+}
+
+int launch_c2p(ak_ctx* c, const Lane& L, bool with_emf) {
+  Timer t(c, KC_C2P, L.st);
+  CK(cudaMemsetAsync(L.f.stats, 0, sizeof(unsigned long long) * 3, L.st));
+  const long long ncell = (long long)L.P.nmb * L.P.nt * L.P.nt * L.P.nt;
+  const unsigned g = capped(ncell, 128, L.ov ? c->cap[KC_C2P] : 0);
+  if (L.P.eos) {
+    if (with_emf) k_con2prim<true, 1><<<g, 128, 0, L.st>>>(L.P, L.f);
+    else k_con2prim<false, 1><<<g, 128, 0, L.st>>>(L.P, L.f);
+  } else if (with_emf) k_con2prim<true><<<g, 128, 0, L.st>>>(L.P, L.f);
+  else k_con2prim<false><<<g, 128, 0, L.st>>>(L.P, L.f);
   c->launches[KC_C2P] += 1;
   CK(cudaGetLastError());
   return AK_OK;
@@ -179,30 +241,43 @@ int launch_c2p(ak_ctx* c, const Fields& f, bool with_emf) {
 #define AK_FLUX_CELL_MASK 1   // bit d set: direction d uses the reconstruct-once variant k_flux_tma_cell
 #endif
 
-template <int DIR, int RECON, int EOS>
-int launch_flux_tma_eos(ak_ctx* c, const Fields& f, int NA, unsigned grid, int bd, size_t smem) {
-  auto kern = ((AK_FLUX_CELL_MASK >> DIR) & 1) ? k_flux_tma_cell<DIR, RECON, EOS> : k_flux_tma<DIR, RECON, EOS>;
-  if (!c->tma_attr[EOS][DIR]) {   // per instantiation in use: recon and n are fixed for the life of a context
+// cudaFuncAttributeMaxDynamicSharedMemorySize belongs to the kernel function (per device), not to a
+// context: two live contexts of different n share one instantiation and need different amounts.  The
+// attribute is therefore only ever RAISED, tracked per instantiation and device.
+template <typename K>
+int raise_smem_attr(K kern, int device, size_t smem, int (&have)[64]) {
+  const int d = device & 63;
+  if ((int)smem > have[d]) {
     CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    c->tma_attr[EOS][DIR] = true;
+    have[d] = (int)smem;
   }
-  kern<<<grid, bd, smem, c->stream>>>(c->P, f, NA);
+  return AK_OK;
+}
+
+template <int DIR, int RECON, int EOS>
+int launch_flux_tma_eos(ak_ctx* c, const Lane& L, int NA, unsigned grid, int bd, size_t smem) {
+  auto kern = ((AK_FLUX_CELL_MASK >> DIR) & 1) ? k_flux_tma_cell<DIR, RECON, EOS> : k_flux_tma<DIR, RECON, EOS>;
+  static int have[64] = {0};
+  const int r = raise_smem_attr(kern, c->hp.device, smem, have);
+  if (r != AK_OK) return r;
+  kern<<<grid, bd, smem, L.st>>>(L.P, L.f, NA);
   return AK_OK;
 }
 
 template <int DIR, int RECON>
-int launch_flux_tma(ak_ctx* c, const Fields& f, int NA, unsigned grid, int bd, size_t smem) {
-  return c->P.eos ? launch_flux_tma_eos<DIR, RECON, 1>(c, f, NA, grid, bd, smem)
-                  : launch_flux_tma_eos<DIR, RECON, 0>(c, f, NA, grid, bd, smem);
+int launch_flux_tma(ak_ctx* c, const Lane& L, int NA, unsigned grid, int bd, size_t smem) {
+  return L.P.eos ? launch_flux_tma_eos<DIR, RECON, 1>(c, L, NA, grid, bd, smem)
+                 : launch_flux_tma_eos<DIR, RECON, 0>(c, L, NA, grid, bd, smem);
 }
 
 template <int DIR>
-int launch_flux(ak_ctx* c, const Fields& f) {
-  Timer t(c, KC_FX + DIR);
-  const int n = c->P.n, nt = c->P.nt, e = n + 2;
+int launch_flux(ak_ctx* c, const Lane& L) {
+  Timer t(c, KC_FX + DIR, L.st);
+  const int n = L.P.n, nt = L.P.nt, e = n + 2;
   constexpr int AK_FLUX_CELL = (AK_FLUX_CELL_MASK >> DIR) & 1;
   // threads per row of a tile: faces (k_flux_tma) or cells (k_flux_tma_cell)
   const int nfi = AK_FLUX_CELL ? (DIR == 0 ? n + 4 : e) : (DIR == 0 ? n + 3 : e);
+  // bulk copies need 16-byte-aligned rows: n even, and (for chunk offsets) every field base a multiple of 16
   if (AK_FLUX_TMA && n % 2 == 0 && nfi * (AK_FLUX_CELL && DIR != 0 ? 2 : 1) <= TMA_THREADS) {
     // tile height: as many rows as fit the block, balanced over the extent it tiles
     const int nfd = DIR == 0 ? e : n + 3;
@@ -215,18 +290,21 @@ int launch_flux(ak_ctx* c, const Fields& f) {
       const size_t park = sizeof(double) * 21 * (size_t)TMA_THREADS;
       if (park > smem) smem = park;
     }
+    // overlapped schedule: a larger allocation keeps a third sweep block off the SM, so that the
+    // capped memory-bound kernels of the other stream find registers and thread slots there
+    if (L.ov && c->sweep_smem_pad > 0 && smem < (size_t)c->sweep_smem_pad) smem = (size_t)c->sweep_smem_pad;
     if (smem <= 200 * 1024) {
-      const unsigned grid = (unsigned)((long long)c->P.nmb * e * tiles);
+      const unsigned grid = (unsigned)((long long)L.P.nmb * e * tiles);
       // threads: one per face (or cell) of the tile, rounded up to whole warps
       const int rows = NA + ((AK_FLUX_CELL && DIR != 0) ? 1 : 0);
       const int bd = ((rows * nfi + 31) / 32) * 32;
       int r;
-      switch (c->P.recon) {
-        case 0: r = launch_flux_tma<DIR, 0>(c, f, NA, grid, bd, smem); break;
-        case 1: r = launch_flux_tma<DIR, 1>(c, f, NA, grid, bd, smem); break;
-        case 3: r = launch_flux_tma<DIR, 3>(c, f, NA, grid, bd, smem); break;
-        case 4: r = launch_flux_tma<DIR, 4>(c, f, NA, grid, bd, smem); break;
-        default: r = launch_flux_tma<DIR, 2>(c, f, NA, grid, bd, smem); break;
+      switch (L.P.recon) {
+        case 0: r = launch_flux_tma<DIR, 0>(c, L, NA, grid, bd, smem); break;
+        case 1: r = launch_flux_tma<DIR, 1>(c, L, NA, grid, bd, smem); break;
+        case 3: r = launch_flux_tma<DIR, 3>(c, L, NA, grid, bd, smem); break;
+        case 4: r = launch_flux_tma<DIR, 4>(c, L, NA, grid, bd, smem); break;
+        default: r = launch_flux_tma<DIR, 2>(c, L, NA, grid, bd, smem); break;
       }
       if (r != AK_OK) return r;
       CK(cudaGetLastError());
@@ -234,23 +312,23 @@ int launch_flux(ak_ctx* c, const Fields& f) {
       return AK_OK;
     }
   }
-  const long long nf = (long long)(n + 3) * (n + 2) * (n + 2) * c->P.nmb;
+  const long long nf = (long long)(n + 3) * (n + 2) * (n + 2) * L.P.nmb;
   const unsigned g = nblk(nf, 128);
-  if (c->P.eos) {
-    switch (c->P.recon) {
-      case 0: k_flux<DIR, 0, 1><<<g, 128, 0, c->stream>>>(c->P, f); break;
-      case 1: k_flux<DIR, 1, 1><<<g, 128, 0, c->stream>>>(c->P, f); break;
-      case 3: k_flux<DIR, 3, 1><<<g, 128, 0, c->stream>>>(c->P, f); break;
-      case 4: k_flux<DIR, 4, 1><<<g, 128, 0, c->stream>>>(c->P, f); break;
-      default: k_flux<DIR, 2, 1><<<g, 128, 0, c->stream>>>(c->P, f); break;
+  if (L.P.eos) {
+    switch (L.P.recon) {
+      case 0: k_flux<DIR, 0, 1><<<g, 128, 0, L.st>>>(L.P, L.f); break;
+      case 1: k_flux<DIR, 1, 1><<<g, 128, 0, L.st>>>(L.P, L.f); break;
+      case 3: k_flux<DIR, 3, 1><<<g, 128, 0, L.st>>>(L.P, L.f); break;
+      case 4: k_flux<DIR, 4, 1><<<g, 128, 0, L.st>>>(L.P, L.f); break;
+      default: k_flux<DIR, 2, 1><<<g, 128, 0, L.st>>>(L.P, L.f); break;
     }
   } else {
-    switch (c->P.recon) {
-      case 0: k_flux<DIR, 0><<<g, 128, 0, c->stream>>>(c->P, f); break;
-      case 1: k_flux<DIR, 1><<<g, 128, 0, c->stream>>>(c->P, f); break;
-      case 3: k_flux<DIR, 3><<<g, 128, 0, c->stream>>>(c->P, f); break;
-      case 4: k_flux<DIR, 4><<<g, 128, 0, c->stream>>>(c->P, f); break;
-      default: k_flux<DIR, 2><<<g, 128, 0, c->stream>>>(c->P, f); break;
+    switch (L.P.recon) {
+      case 0: k_flux<DIR, 0><<<g, 128, 0, L.st>>>(L.P, L.f); break;
+      case 1: k_flux<DIR, 1><<<g, 128, 0, L.st>>>(L.P, L.f); break;
+      case 3: k_flux<DIR, 3><<<g, 128, 0, L.st>>>(L.P, L.f); break;
+      case 4: k_flux<DIR, 4><<<g, 128, 0, L.st>>>(L.P, L.f); break;
+      default: k_flux<DIR, 2><<<g, 128, 0, L.st>>>(L.P, L.f); break;
     }
   }
   CK(cudaGetLastError());
@@ -258,33 +336,35 @@ int launch_flux(ak_ctx* c, const Fields& f) {
   return AK_OK;
 }
 
-int launch_fofc(ak_ctx* c, const Fields& f, double dt) {
-  const long long n = c->P.n;
-  const long long ntest = (n + 2) * (n + 2) * (n + 2) * c->P.nmb;
-  const long long nf = (n + 3) * (n + 2) * (n + 2) * c->P.nmb;
+int launch_fofc(ak_ctx* c, const Lane& L, double dt) {
+  const long long n = L.P.n, nt = L.P.nt;
+  const long long ntest = (n + 2) * (n + 2) * (n + 2) * L.P.nmb;
+  const long long nf = (n + 3) * (n + 2) * (n + 2) * L.P.nmb;
   {
-    Timer t(c, KC_FOFC_TEST);
-    CK(cudaMemsetAsync(f.flag, 0, (size_t)c->sz.cell, c->stream));
-    CK(cudaMemsetAsync(c->count, 0, sizeof(unsigned) * 4, c->stream));
-    CK(cudaMemsetAsync(c->stats + S_FOFC_CELLS, 0, sizeof(unsigned long long) * 2, c->stream));
-    if (c->P.fofc) {
-      if (c->P.eos) k_fofc_test<1><<<nblk(ntest, 128), 128, 0, c->stream>>>(c->P, f, dt);
-      else k_fofc_test<0><<<nblk(ntest, 128), 128, 0, c->stream>>>(c->P, f, dt);
+    Timer t(c, KC_FOFC_TEST, L.st);
+    CK(cudaMemsetAsync(L.f.flag, 0, (size_t)(nt * nt * nt * L.P.nmb), L.st));
+    CK(cudaMemsetAsync(L.f.count, 0, sizeof(unsigned) * 4, L.st));
+    CK(cudaMemsetAsync(L.f.stats + S_FOFC_CELLS, 0, sizeof(unsigned long long) * 2, L.st));
+    if (L.P.fofc) {
+      const unsigned g = capped(ntest, 128, L.ov ? c->cap[KC_FOFC_TEST] : 0);
+      if (L.P.eos) k_fofc_test<1><<<g, 128, 0, L.st>>>(L.P, L.f, dt);
+      else k_fofc_test<0><<<g, 128, 0, L.st>>>(L.P, L.f, dt);
       c->launches[KC_FOFC_TEST] += 1;
       CK(cudaGetLastError());
     }
   }
-  if (c->P.fofc) {
-    Timer t(c, KC_FOFC_FIX);
-    const unsigned g = (unsigned)(nf < 148LL * 8 * 128 ? nblk(nf, 128) : 148 * 8);
-    if (c->P.eos) {
-      k_fofc_reflux<0, 1><<<g, 128, 0, c->stream>>>(c->P, f);
-      k_fofc_reflux<1, 1><<<g, 128, 0, c->stream>>>(c->P, f);
-      k_fofc_reflux<2, 1><<<g, 128, 0, c->stream>>>(c->P, f);
+  if (L.P.fofc) {
+    Timer t(c, KC_FOFC_FIX, L.st);
+    unsigned g = (unsigned)(nf < 148LL * 8 * 128 ? nblk(nf, 128) : 148 * 8);
+    if (L.ov && c->cap[KC_FOFC_FIX] > 0 && g > (unsigned)c->cap[KC_FOFC_FIX]) g = (unsigned)c->cap[KC_FOFC_FIX];
+    if (L.P.eos) {
+      k_fofc_reflux<0, 1><<<g, 128, 0, L.st>>>(L.P, L.f);
+      k_fofc_reflux<1, 1><<<g, 128, 0, L.st>>>(L.P, L.f);
+      k_fofc_reflux<2, 1><<<g, 128, 0, L.st>>>(L.P, L.f);
     } else {
-      k_fofc_reflux<0><<<g, 128, 0, c->stream>>>(c->P, f);
-      k_fofc_reflux<1><<<g, 128, 0, c->stream>>>(c->P, f);
-      k_fofc_reflux<2><<<g, 128, 0, c->stream>>>(c->P, f);
+      k_fofc_reflux<0><<<g, 128, 0, L.st>>>(L.P, L.f);
+      k_fofc_reflux<1><<<g, 128, 0, L.st>>>(L.P, L.f);
+      k_fofc_reflux<2><<<g, 128, 0, L.st>>>(L.P, L.f);
     }
     CK(cudaGetLastError());
     c->launches[KC_FOFC_FIX] += 3;
@@ -292,25 +372,27 @@ int launch_fofc(ak_ctx* c, const Fields& f, double dt) {
   return AK_OK;
 }
 
-int launch_ct(ak_ctx* c, const Fields& f, bool have_cell_emf) {
-  Timer t(c, KC_CT);
-  const long long n = c->P.n;
-  const long long ntest = (n + 2) * (n + 2) * (n + 2) * c->P.nmb;
-  const long long ne = n * (n + 1) * (n + 1) * c->P.nmb;
-  if (!have_cell_emf) k_cell_emf<<<nblk(ntest, 128), 128, 0, c->stream>>>(c->P, f);
-  k_ct<0><<<nblk(ne, 128), 128, 0, c->stream>>>(c->P, f);
-  k_ct<1><<<nblk(ne, 128), 128, 0, c->stream>>>(c->P, f);
-  k_ct<2><<<nblk(ne, 128), 128, 0, c->stream>>>(c->P, f);
+int launch_ct(ak_ctx* c, const Lane& L, bool have_cell_emf) {
+  Timer t(c, KC_CT, L.st);
+  const long long n = L.P.n;
+  const long long ntest = (n + 2) * (n + 2) * (n + 2) * L.P.nmb;
+  const long long ne = n * (n + 1) * (n + 1) * L.P.nmb;
+  const unsigned g = capped(ne, 128, L.ov ? c->cap[KC_CT] : 0);
+  if (!have_cell_emf) k_cell_emf<<<nblk(ntest, 128), 128, 0, L.st>>>(L.P, L.f);
+  k_ct<0><<<g, 128, 0, L.st>>>(L.P, L.f);
+  k_ct<1><<<g, 128, 0, L.st>>>(L.P, L.f);
+  k_ct<2><<<g, 128, 0, L.st>>>(L.P, L.f);
   CK(cudaGetLastError());
   c->launches[KC_CT] += have_cell_emf ? 3 : 4;
   return AK_OK;
 }
 
-int launch_src(ak_ctx* c, const Fields& f) {
-  Timer t(c, KC_SRC);
-  const long long n = c->P.n;
-  if (c->P.eos) k_div_src<1><<<nblk(n * n * n * c->P.nmb, 128), 128, 0, c->stream>>>(c->P, f);
-  else k_div_src<0><<<nblk(n * n * n * c->P.nmb, 128), 128, 0, c->stream>>>(c->P, f);
+int launch_src(ak_ctx* c, const Lane& L) {
+  Timer t(c, KC_SRC, L.st);
+  const long long n = L.P.n;
+  const unsigned g = capped(n * n * n * L.P.nmb, 128, L.ov ? c->cap[KC_SRC] : 0);
+  if (L.P.eos) k_div_src<1><<<g, 128, 0, L.st>>>(L.P, L.f);
+  else k_div_src<0><<<g, 128, 0, L.st>>>(L.P, L.f);
   CK(cudaGetLastError());
   c->launches[KC_SRC] += 1;
   return AK_OK;
@@ -389,6 +471,19 @@ int ak_create(const ak_params* p, const double* dx3, ak_ctx** out) {
   c->hp = *p;
   c->stream = (cudaStream_t)p->stream;
   c->blend_a = 0.0; c->blend_b = 1.0;
+  {
+    // overlapped-schedule tuning (ak_set_overlap): grid caps in blocks per SM, per kernel class; defaults
+    // from the measurements recorded in DESIGN.md §6.2, overridable for experiments
+    int nsm = 148;
+    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, p->device);
+    auto envi = [](const char* k, int dflt) { const char* v = getenv(k); return v ? atoi(v) : dflt; };
+    c->cap[KC_C2P] = nsm * envi("AK_OV_CAP_C2P", AK_OV_CAP_C2P_DEFAULT);
+    c->cap[KC_FOFC_TEST] = nsm * envi("AK_OV_CAP_FOFC", AK_OV_CAP_FOFC_DEFAULT);
+    c->cap[KC_FOFC_FIX] = nsm * envi("AK_OV_CAP_FIX", AK_OV_CAP_FIX_DEFAULT);
+    c->cap[KC_CT] = nsm * envi("AK_OV_CAP_CT", AK_OV_CAP_CT_DEFAULT);
+    c->cap[KC_SRC] = nsm * envi("AK_OV_CAP_SRC", AK_OV_CAP_SRC_DEFAULT);
+    c->sweep_smem_pad = envi("AK_OV_SMEM_PAD", AK_OV_SMEM_PAD_DEFAULT);
+  }
   Par& P = c->P;
   P.nmb = p->nmb; P.n = p->n; P.nt = p->n + 8; P.px = P.nt + 4; P.is = 4; P.ie = p->n + 3;
   P.Gam = p->gamma_ad; P.gm1 = p->gamma_ad - 1.0; P.gm1r = p->gamma_ad / (p->gamma_ad - 1.0);
@@ -416,10 +511,10 @@ int ak_create(const ak_params* p, const double* dx3, ak_ctx** out) {
   }
   if (e == cudaSuccess) e = cudaMalloc(&c->list, sizeof(unsigned) * ntest);
   if (e == cudaSuccess) e = cudaMalloc(&c->flag_own, (size_t)c->sz.cell);
-  if (e == cudaSuccess) e = cudaMalloc(&c->count, sizeof(unsigned) * 4);
-  if (e == cudaSuccess) e = cudaMalloc(&c->stats, sizeof(unsigned long long) * S_NSTAT);
-  if (e == cudaSuccess) e = cudaMemsetAsync(c->count, 0, sizeof(unsigned) * 4, c->stream);
-  if (e == cudaSuccess) e = cudaMemsetAsync(c->stats, 0, sizeof(unsigned long long) * S_NSTAT, c->stream);
+  if (e == cudaSuccess) e = cudaMalloc(&c->count, sizeof(unsigned) * 4 * MAXCH);
+  if (e == cudaSuccess) e = cudaMalloc(&c->stats, sizeof(unsigned long long) * S_NSTAT * MAXCH);
+  if (e == cudaSuccess) e = cudaMemsetAsync(c->count, 0, sizeof(unsigned) * 4 * MAXCH, c->stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(c->stats, 0, sizeof(unsigned long long) * S_NSTAT * MAXCH, c->stream);
   if (e == cudaSuccess) e = cudaMalloc(&c->dx, sizeof(double) * 3 * nb);
   if (e == cudaSuccess) e = cudaMemcpyAsync(c->dx, dx3, sizeof(double) * 3 * nb, cudaMemcpyHostToDevice, c->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);   // dx3 is the caller's: copy must be done
@@ -433,6 +528,10 @@ int ak_create(const ak_params* p, const double* dx3, ak_ctx** out) {
     return e == cudaErrorMemoryAllocation ? AK_ENOMEM : AK_ECUDA;
   }
   *out = c;
+  if (const char* v = getenv("AK_OV_CHUNKS")) {
+    const int r = ak_set_overlap(c, atoi(v));
+    if (r != AK_OK) { ak_destroy(c); *out = nullptr; return r; }
+  }
   return AK_OK;
 }
 
@@ -459,6 +558,12 @@ int ak_destroy(ak_ctx* c) {
     cudaFree(c->lane_mask[l][0]); cudaFree(c->lane_mask[l][1]);
   }
   if (c->lane_stats_h) cudaFreeHost(c->lane_stats_h);
+  if (c->ov_ev) {
+    for (int q = 0; q < c->ov_nev; ++q) if (c->ov_ev[q]) cudaEventDestroy(c->ov_ev[q]);
+    free(c->ov_ev);
+    for (int q = 0; q < 3; ++q)
+      if (c->ovs[q] && !(q == 2 && c->ovs[2] == c->ovs[0])) cudaStreamDestroy(c->ovs[q]);
+  }
   cudaFree(c->flag_own); cudaFree(c->count); cudaFree(c->stats); cudaFree(c->dx);
   delete c;
   return AK_OK;
@@ -469,7 +574,7 @@ int ak_set_metric(ak_ctx* c, const ak_adm* a) {
   const double* p[16] = {a->gxx, a->gxy, a->gxz, a->gyy, a->gyz, a->gzz, a->alp, a->betx, a->bety, a->betz,
                          a->Kxx, a->Kxy, a->Kxz, a->Kyy, a->Kyz, a->Kzz};
   for (int q = 0; q < 16; ++q)
-    if (!p[q] || ((uintptr_t)p[q] & 7u)) return AK_EINVAL;
+    if (!al16(p[q])) return AK_EINVAL;
   for (int q = 0; q < 16; ++q) c->adm[q] = p[q];
   c->have_metric = true;
   return AK_OK;
@@ -523,7 +628,8 @@ int ak_con2prim(ak_ctx* c, const ak_cons* U, const ak_faceB* Bf, const ak_prim* 
   if (!set_cons(f, U) || !set_faceB(f, Bf) || !set_prim(f, W)) return AK_EINVAL;
   f.status = status;
   CK(cudaSetDevice(c->hp.device));
-  return launch_c2p(c, f, false);
+  const Lane L = {c->P, f, c->stream, false};
+  return launch_c2p(c, L, false);
 }
 
 int ak_rhs(ak_ctx* c, const ak_cons* U, const ak_faceB* Bf, const ak_prim* W, int w_is_valid, double dt_fofc,
@@ -542,15 +648,91 @@ int ak_rhs(ak_ctx* c, const ak_cons* U, const ak_faceB* Bf, const ak_prim* W, in
   f.status = out->c2p_status;
   CK(cudaSetDevice(c->hp.device));
   c->stats_from_host = false;
+  // counters of every chunk slot start from zero (a stage that skips part (1) reports no con2prim counts)
+  CK(cudaMemsetAsync(c->stats, 0, sizeof(unsigned long long) * S_NSTAT * MAXCH, c->stream));
+  CK(cudaMemsetAsync(c->count, 0, sizeof(unsigned) * 4 * MAXCH, c->stream));
   int r;
-  if (!w_is_valid && (r = launch_c2p(c, f, true)) != AK_OK) return r;
-  if ((r = launch_flux<0>(c, f)) != AK_OK) return r;
-  if ((r = launch_flux<1>(c, f)) != AK_OK) return r;
-  if ((r = launch_flux<2>(c, f)) != AK_OK) return r;
-  if ((r = launch_fofc(c, f, dt_fofc)) != AK_OK) return r;
+  const int nch = c->ov_chunks < 2 ? 1 : (c->ov_chunks < c->P.nmb ? c->ov_chunks : c->P.nmb);
+  if (nch < 2) {
+    // serial schedule: the whole batch, kernel after kernel, on the context's stream
+    const Lane L = {c->P, f, c->stream, false};
+    if (!w_is_valid && (r = launch_c2p(c, L, true)) != AK_OK) return r;
+    if ((r = launch_flux<0>(c, L)) != AK_OK) return r;
+    if ((r = launch_flux<1>(c, L)) != AK_OK) return r;
+    if ((r = launch_flux<2>(c, L)) != AK_OK) return r;
+    if ((r = launch_fofc(c, L, dt_fofc)) != AK_OK) return r;
+    c->have_flux = true;
+    if ((r = launch_ct(c, L, !w_is_valid)) != AK_OK) return r;
+    return launch_src(c, L);
+  }
+  // overlapped schedule: MeshBlocks are independent, so the batch is cut into nch chunks.
+  // Stream A runs part (1) of chunk i+1 and stream C parts (4)-(6) of chunk i-1 (memory- and latency-bound,
+  // capped grids, high priority) while stream B runs the fp64-bound sweeps of chunk i.  Only events order
+  // the streams; no kernel waits on another.  Same kernels, same arithmetic: outputs are bit-identical.
+  cudaStream_t sA = c->ovs[0], sB = c->ovs[1], sC = c->ovs[2];
+  cudaEvent_t* ev = c->ov_ev;                     // [0] fork, [1..3] joins, [4 + 2 i] c2p(i), [5 + 2 i] flux(i)
+  CK(cudaEventRecord(ev[0], c->stream));
+  CK(cudaStreamWaitEvent(sA, ev[0], 0));
+  CK(cudaStreamWaitEvent(sB, ev[0], 0));
+  if (sC != sA) CK(cudaStreamWaitEvent(sC, ev[0], 0));
+  static thread_local Fields CF[MAXCH];
+  static thread_local Par CP[MAXCH];
+  const int base = c->P.nmb / nch, rem = c->P.nmb % nch;
+  for (int ci = 0, m0 = 0; ci < nch; ++ci) {
+    const int nb = base + (ci < rem ? 1 : 0);
+    chunk_fields(c, f, m0, nb, ci, CF[ci], CP[ci]);
+    m0 += nb;
+  }
+  auto c2p = [&](int ci) -> int {
+    if (w_is_valid) return AK_OK;
+    const Lane L = {CP[ci], CF[ci], sA, true};
+    const int rr = launch_c2p(c, L, true);
+    if (rr != AK_OK) return rr;
+    CK(cudaEventRecord(ev[4 + 2 * ci], sA));
+    return AK_OK;
+  };
+  if ((r = c2p(0)) != AK_OK) return r;
+  for (int ci = 0; ci < nch; ++ci) {
+    if (ci + 1 < nch && (r = c2p(ci + 1)) != AK_OK) return r;
+    const Lane LB = {CP[ci], CF[ci], sB, true};
+    if (!w_is_valid) CK(cudaStreamWaitEvent(sB, ev[4 + 2 * ci], 0));
+    if ((r = launch_flux<0>(c, LB)) != AK_OK) return r;
+    if ((r = launch_flux<1>(c, LB)) != AK_OK) return r;
+    if ((r = launch_flux<2>(c, LB)) != AK_OK) return r;
+    CK(cudaEventRecord(ev[5 + 2 * ci], sB));
+    const Lane LC = {CP[ci], CF[ci], sC, true};
+    CK(cudaStreamWaitEvent(sC, ev[5 + 2 * ci], 0));
+    if ((r = launch_fofc(c, LC, dt_fofc)) != AK_OK) return r;
+    if ((r = launch_ct(c, LC, !w_is_valid)) != AK_OK) return r;
+    if ((r = launch_src(c, LC)) != AK_OK) return r;
+  }
   c->have_flux = true;
-  if ((r = launch_ct(c, f, !w_is_valid)) != AK_OK) return r;
-  return launch_src(c, f);
+  CK(cudaEventRecord(ev[1], sA)); CK(cudaStreamWaitEvent(c->stream, ev[1], 0));
+  CK(cudaEventRecord(ev[2], sB)); CK(cudaStreamWaitEvent(c->stream, ev[2], 0));
+  if (sC != sA) { CK(cudaEventRecord(ev[3], sC)); CK(cudaStreamWaitEvent(c->stream, ev[3], 0)); }
+  return AK_OK;
+}
+
+int ak_set_overlap(ak_ctx* c, int nchunks) {
+  if (!c || nchunks < 0 || nchunks > MAXCH) return AK_EINVAL;
+  CK(cudaSetDevice(c->hp.device));
+  if (nchunks >= 2 && !c->ov_ev) {
+    int lo = 0, hi = 0;
+    CK(cudaDeviceGetStreamPriorityRange(&lo, &hi));          // lo = least, hi = greatest priority (numerically lower)
+    const char* e3 = getenv("AK_OV_STREAMS");
+    const char* ep = getenv("AK_OV_PRIO");                    // e.g. "hlh": priority of streams A, B, C
+    const char* pr = (ep && strlen(ep) == 3) ? ep : "hlh";
+    for (int q = 0; q < 3; ++q) {
+      if (q == 2 && e3 && atoi(e3) == 2) { c->ovs[2] = c->ovs[0]; break; }
+      CK(cudaStreamCreateWithPriority(&c->ovs[q], cudaStreamNonBlocking, pr[q] == 'h' ? hi : lo));
+    }
+    c->ov_nev = 4 + 2 * MAXCH;
+    c->ov_ev = (cudaEvent_t*)calloc(c->ov_nev, sizeof(cudaEvent_t));
+    if (!c->ov_ev) return AK_ENOMEM;
+    for (int q = 0; q < c->ov_nev; ++q) CK(cudaEventCreateWithFlags(&c->ov_ev[q], cudaEventDisableTiming));
+  }
+  c->ov_chunks = nchunks;
+  return AK_OK;
 }
 
 int ak_emf(ak_ctx* c, const ak_prim* W, double* Ex, double* Ey, double* Ez) {
@@ -561,7 +743,8 @@ int ak_emf(ak_ctx* c, const ak_prim* W, double* Ex, double* Ey, double* Ez) {
   if (!set_prim(f, W)) return AK_EINVAL;
   f.E[0] = Ex; f.E[1] = Ey; f.E[2] = Ez;
   CK(cudaSetDevice(c->hp.device));
-  return launch_ct(c, f, false);
+  const Lane L = {c->P, f, c->stream, false};
+  return launch_ct(c, L, false);
 }
 
 int ak_matter_sources(ak_ctx* c, const ak_prim* W, const ak_matter* out) {
@@ -582,18 +765,22 @@ int ak_matter_sources(ak_ctx* c, const ak_prim* W, const ak_matter* out) {
 int ak_get_stats(ak_ctx* c, ak_stats* o) {
   if (!c || !o) return AK_EINVAL;
   if (c->stats_from_host) { *o = c->host_acc; return AK_OK; }
-  unsigned long long h[S_NSTAT];
-  unsigned cnt[4];
+  static thread_local unsigned long long h[S_NSTAT * MAXCH];
+  static thread_local unsigned cnt[4 * MAXCH];
   CK(cudaSetDevice(c->hp.device));
   CK(cudaMemcpyAsync(h, c->stats, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
   CK(cudaMemcpyAsync(cnt, c->count, sizeof(cnt), cudaMemcpyDeviceToHost, c->stream));
   CK(cudaStreamSynchronize(c->stream));
-  o->n_c2p_fail = (long long)h[S_C2P_FAIL];
-  o->n_cons_floor = (long long)h[S_CONS_FLOOR];
-  o->n_prim_floor = (long long)h[S_PRIM_FLOOR];
-  o->n_fofc_cells = (long long)cnt[3];
-  o->n_dmp_cells = (long long)h[S_DMP_CELLS];
-  for (int d = 0; d < 3; ++d) o->n_fofc_faces[d] = cnt[d];
+  memset(o, 0, sizeof(*o));
+  for (int ci = 0; ci < MAXCH; ++ci) {      // one slot per chunk of the overlapped schedule (slot 0 otherwise)
+    const unsigned long long* hc = h + S_NSTAT * ci;
+    o->n_c2p_fail += (long long)hc[S_C2P_FAIL];
+    o->n_cons_floor += (long long)hc[S_CONS_FLOOR];
+    o->n_prim_floor += (long long)hc[S_PRIM_FLOOR];
+    o->n_dmp_cells += (long long)hc[S_DMP_CELLS];
+    o->n_fofc_cells += (long long)cnt[4 * ci + 3];
+    for (int d = 0; d < 3; ++d) o->n_fofc_faces[d] += cnt[4 * ci + d];
+  }
   return AK_OK;
 }
 
@@ -632,8 +819,15 @@ static int rhs_host_pipelined(ak_ctx* c, int chunk, double* const hU[5], const d
   const long long per[7] = {nt * nt * nt, nt * nt * px, nt * (nt + 1) * nt, (nt + 1) * nt * nt,
                             (nt + 1) * (nt + 1) * nt, (nt + 1) * nt * px, nt * (nt + 1) * px};   // cell xf yf zf ex ey ez
   const int nchunks = c->P.nmb / chunk;
+  c->have_flux = false;                       // the fluxes of this stage stay in the lanes: ak_emf / ak_get_flux -> AK_ESTATE
   if (c->lane_chunk != chunk) {
     if (c->lane_chunk != 0) return AK_ESTATE;
+    for (int l = 0; l < 2; ++l) {               // left over from an attempt that failed half way
+      if (c->lane[l]) { cudaStream_t st0 = c->lane[l]->stream; ak_destroy(c->lane[l]); cudaStreamDestroy(st0); c->lane[l] = nullptr; }
+      for (int q = 0; q < 24; ++q) { cudaFree(c->lane_buf[l][q]); c->lane_buf[l][q] = nullptr; }
+      for (int q = 0; q < 2; ++q) { cudaFree(c->lane_mask[l][q]); c->lane_mask[l][q] = nullptr; }
+    }
+    if (c->lane_stats_h) { cudaFreeHost(c->lane_stats_h); c->lane_stats_h = nullptr; }
     for (int l = 0; l < 2; ++l) {
       ak_params hp = c->hp;
       hp.nmb = chunk;
@@ -729,7 +923,9 @@ int ak_rhs_host(ak_ctx* c, const ak_cons* U, const ak_faceB* Bf, const ak_prim* 
     const int cap = c->P.nmb / 8 > 8 ? c->P.nmb / 8 : 8;
     if (c->P.nmb >= 16 && !c->blendU0[0])
       for (int q = cap; q >= 4; --q) if (c->P.nmb % q == 0) { chunk = q; break; }
-    if (c->lane_chunk) chunk = c->lane_chunk;
+    // lanes exist: keep their chunk size; a FOFC blend set since then goes the unpipelined way (the lanes
+    // do not carry the register U0)
+    if (c->lane_chunk) chunk = c->blendU0[0] ? 0 : c->lane_chunk;
     if (chunk) return rhs_host_pipelined(c, chunk, hU, hB, hW, dt_fofc, hdU, hE, out->fofc_flag, out->c2p_status);
   }
   if (!c->have_stg) {
@@ -933,8 +1129,12 @@ int ak_advance(ak_ctx* c, int integrator, int nsteps, double dt, const int bc[3]
       if (flag_or) k_or_bytes<<<148 * 8, 256, 0, c->stream>>>(flag_or, c->reg_flag, c->sz.cell);
       if (s == 0 && integrator > 1) {
         // step-start register: the state after the first stage's con2prim (floored)
-        for (int q = 0; q < 5; ++q) CK(cudaMemcpyAsync(c->regU0[q], Up[q], cb, cudaMemcpyDeviceToDevice, c->stream));
-        for (int q = 0; q < 3; ++q) CK(cudaMemcpyAsync(c->regB0[q], Bp[q], fb[q], cudaMemcpyDeviceToDevice, c->stream));
+        cudaError_t ce = cudaSuccess;
+        for (int q = 0; q < 5 && ce == cudaSuccess; ++q)
+          ce = cudaMemcpyAsync(c->regU0[q], Up[q], cb, cudaMemcpyDeviceToDevice, c->stream);
+        for (int q = 0; q < 3 && ce == cudaSuccess; ++q)
+          ce = cudaMemcpyAsync(c->regB0[q], Bp[q], fb[q], cudaMemcpyDeviceToDevice, c->stream);
+        if (ce != cudaSuccess) { last_cuda_error = ce; r = AK_ECUDA; break; }   // the blend is restored below
       }
       if (s == 0) r = ak_stage_update(c, 0.0, 1.0, dt, U, &Bc, U, Bf, &out);    // register = the state itself
       else r = ak_stage_update(c, a, b, dt, &R0, &RB0, U, Bf, &out);

@@ -1,7 +1,10 @@
 // ak_dev.cuh — device-side point operators of the GRMHD RHS stage (sm_100a, fp64).
 //
 // Written from DESIGN.md §3 (steps O0..O6, restating PAPER.md Eqs. 6-9; P:133;
-// P:137-139).  Shares nothing with oracle/.  The library is compiled with
+// P:137-139).  No file, header or table is shared with oracle/, but the point operators
+// here evaluate the SAME canonical expression trees as oracle/point.cpp, restated (that is what makes
+// the masks bit-reproducible): GPU == oracle therefore certifies indexing, tiling, staging and
+// compaction, and the physics rests on the oracle's pins.  The library is compiled with
 // --fmad=false: every +,-,*,/ and sqrt below is one IEEE fp64 operation evaluated in the
 // order written (C++ left-to-right association), which is what makes the status/flag masks
 // reproducible bit for bit (DESIGN.md §3 "reference arithmetic").

@@ -1,6 +1,7 @@
 // ak_flux.cuh — reconstruction (O4), face geometry (O5) and Riemann fluxes (O6).
 // DESIGN.md §3; PAPER.md P:133 (donor cell / PPM4 / WENO-Z, LLF / HLLE), Eq. 7-8,
-// face-state floor P:139.  Device code only; shares nothing with oracle/.
+// face-state floor P:139.  Device code only.  Same canonical expression trees as oracle/point.cpp,
+// restated in another file (see ak_dev.cuh); nothing is included from or linked with oracle/.
 #pragma once
 #include "ak_dev.cuh"
 

@@ -87,8 +87,13 @@ __global__ void __launch_bounds__(128, AK_C2P_MINB) k_con2prim(const __grid_cons
                                                   const __grid_constant__ Fields f) {
   const int nt = P.nt;
   const long long ncell = (long long)P.nmb * nt * nt * nt;
-  const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (c >= ncell) return;
+#if AK_C2P_PARK
+  __shared__ double park[9][128];
+#endif
+  // grid-stride: the launcher may cap the grid (a few blocks per SM) so that the kernel shares the SMs
+  // with the flux sweeps of another chunk of blocks (ak_set_overlap)
+  for (long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x; c < ncell;
+       c += (long long)gridDim.x * blockDim.x) {
   const int i = (int)(c % nt);
   const long long row = c / nt;               // (m*nt + k)*nt + j
   const int j = (int)(row % nt);
@@ -115,7 +120,6 @@ __global__ void __launch_bounds__(128, AK_C2P_MINB) k_con2prim(const __grid_cons
   // leave the registers for the solve; left to the compiler they are spilled to local memory,
   // which is written through to L2 and partly on to DRAM (profiles/r1_v10_final.md): 3.12 -> 2.90 ms
   // on C4.  Parking r^i and B^i inside c2p_cell as well, or in k_fofc_test, measured no gain / 1 % loss.
-  __shared__ double park[9][128];
   park[0][threadIdx.x] = g.xx; park[1][threadIdx.x] = g.xy; park[2][threadIdx.x] = g.xz;
   park[3][threadIdx.x] = g.yy; park[4][threadIdx.x] = g.yz; park[5][threadIdx.x] = g.zz;
 #pragma unroll
@@ -163,6 +167,7 @@ __global__ void __launch_bounds__(128, AK_C2P_MINB) k_con2prim(const __grid_cons
   warp_count(f.stats + S_C2P_FAIL, (st & ST_FAIL) != 0);
   warp_count(f.stats + S_CONS_FLOOR, (st & (ST_DFLOOR | ST_TAUFLOOR | ST_MAGCAP)) != 0);
   warp_count(f.stats + S_PRIM_FLOOR, (st & (ST_RHOFLOOR | ST_TFLOOR)) != 0);
+  }
 }
 
 // ---- computed-face range decoding ----------------------------------------------------
@@ -242,8 +247,9 @@ __device__ __forceinline__ double div_flux(const Fields& f, const Ix& ix, int v,
 template <int EOS = 0>
 __global__ void __launch_bounds__(128, AK_FOFC_MINB) k_fofc_test(const __grid_constant__ Par P,
                                                    const __grid_constant__ Fields f, double dt) {
+  for (long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;; tid += (long long)gridDim.x * blockDim.x) {
   int m, k, j, i;
-  if (!decode_test(P, (long long)blockIdx.x * blockDim.x + threadIdx.x, m, k, j, i)) return;
+  if (!decode_test(P, tid, m, k, j, i)) return;
   const Ix ix{P.nt, P.px};
   const long long c = ix.cell(m, k, j, i);
   const double idx[3] = {1.0 / f.dx[3 * m + 0], 1.0 / f.dx[3 * m + 1], 1.0 / f.dx[3 * m + 2]};
@@ -296,6 +302,7 @@ __global__ void __launch_bounds__(128, AK_FOFC_MINB) k_fofc_test(const __grid_co
     if (lane == leader) base = atomicAdd(f.count + 3, (unsigned)__popc(bal));
     base = __shfl_sync(act, base, leader);
     if (st != 0) f.list[base + __popc(bal & ((1u << lane) - 1u))] = (unsigned)c;
+  }
   }
 }
 
@@ -372,8 +379,8 @@ __global__ void __launch_bounds__(128) k_ct(const __grid_constant__ Par P,
   const int n = P.n;
   const int ei = n + (C3 == 0 ? 0 : 1), ej = n + (C3 == 1 ? 0 : 1), ek = n + (C3 == 2 ? 0 : 1);
   const long long per = (long long)ei * ej * ek;
-  const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (idx >= per * P.nmb) return;
+  for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < per * P.nmb;
+       idx += (long long)gridDim.x * blockDim.x) {
   const int m = (int)(idx / per);
   int r = (int)(idx - (long long)m * per);
   int p3[3];
@@ -412,6 +419,7 @@ __global__ void __launch_bounds__(128) k_ct(const __grid_constant__ Par P,
   const double dap = w2p * (Eaf_0m - Ec_mm) + (1.0 - w2p) * (Eaf_00 - Ec_m0);
   const double e = 0.25 * (Eaf_00 + Eaf_0m + Ebf_00 + Ebf_m0) + 0.25 * ((dbp - dbm) + (dap - dam));
   f.E[C3][ix.edge(C3, m, p3[2], p3[1], p3[0])] = e;
+  }
 }
 
 }  // namespace ak

@@ -14,8 +14,8 @@ __global__ void __launch_bounds__(128, AK_SRC_MINB) k_div_src(const __grid_const
                                                  const __grid_constant__ Fields f) {
   const int n = P.n;
   const long long per = (long long)n * n * n;
-  const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (idx >= per * P.nmb) return;
+  for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < per * P.nmb;
+       idx += (long long)gridDim.x * blockDim.x) {
   const int m = (int)(idx / per);
   int r = (int)(idx - (long long)m * per);
   const int i = r % n + P.is; r /= n;
@@ -104,6 +104,7 @@ __global__ void __launch_bounds__(128, AK_SRC_MINB) k_div_src(const __grid_const
   du[4] = du[4] + sdet * (alp * KS - Sda);
 #pragma unroll
   for (int v = 0; v < 5; ++v) f.dU[v][c] = du[v];
+  }
 }
 
 // ---- matter terms for a spacetime solver: E = tau + D, S_i, S_ij = T_ij, undensitised,
