@@ -32,13 +32,18 @@ UNIT = "zone-updates/s"
 
 # Algorithmic bytes per processed element of each kernel class:
 # compulsory reads + writes of fp64 fields (8 B each), one pass, no re-reads.
-#   con2prim : 5 U + 3x(nt+1)/nt face B + 6 gamma in, 8 W out (+1 B status)  per stored cell
+#   con2prim : 5 U + 3x(nt+1)/nt face B + 6 gamma in, 8 W out (+1 B status)  per stored cell,
+#              plus the cell-centred EMFs it writes from registers in the timed (w_is_valid = 0) path:
+#              alpha, beta^i in, 3 E_cc out                                    per test cell
 #   flux_d   : 8 W-class (7 recon vars) + 10 metric + 1 Bf in, 7 F out       per computed face
 #   fofc_test: 5 U + 15 F(x2 faces shared -> 15) + 6 gamma + 3 Bcc in, 1 B out per test cell
-#   ct       : cell EMF (3 u + 3 Bcc + 10 metric in, 3 out per test cell) + per edge 2 F_B + 2 F_D + 1 Ecc in, 1 out
+#   ct       : per edge 2 F_B + 2 F_D + 1 Ecc in, 1 out  (the cell EMFs are con2prim's: k_cell_emf is not
+#              launched when part (1) runs)
 #   div_src  : 15 F + 8 W + 16 adm in, 5 out                                 per interior zone
 ALG_BYTES = dict(con2prim=(5 + 3 + 6 + 8) * 8 + 1, flux=(7 + 10 + 1 + 7) * 8, fofc_test=(5 + 15 + 6 + 3) * 8 + 1,
-                 cell_emf=(6 + 10 + 3) * 8, ct_edge=(2 + 2 + 1 + 1) * 8, div_src=(15 + 8 + 16 + 5) * 8)
+                 cell_emf_fused=(4 + 3) * 8, ct_edge=(2 + 2 + 1 + 1) * 8, div_src=(15 + 8 + 16 + 5) * 8)
+# flop per element as the survey counted them (an FMA = 2), recon 1 PPM4 / 2 WENO-Z
+SURVEY_FLOP_PER_FACE = {1: 830, 2: 1250}
 
 
 # fp64-pipe instructions one face of a flux sweep needs (recon 0 donor, 1 PPM4, 2 WENO-Z; HLLE/LLF
@@ -64,9 +69,9 @@ def kernel_units(nmb, n):
 
 def kernel_alg_bytes(nmb, n):
     u = kernel_units(nmb, n)
-    b = dict(con2prim=u["con2prim"] * ALG_BYTES["con2prim"], flux_x=u["flux"] * ALG_BYTES["flux"],
-             fofc_test=u["fofc_test"] * ALG_BYTES["fofc_test"],
-             ct=u["cell_emf"] * ALG_BYTES["cell_emf"] + u["ct_edge"] * ALG_BYTES["ct_edge"],
+    b = dict(con2prim=u["con2prim"] * ALG_BYTES["con2prim"] + u["cell_emf"] * ALG_BYTES["cell_emf_fused"],
+             flux_x=u["flux"] * ALG_BYTES["flux"], fofc_test=u["fofc_test"] * ALG_BYTES["fofc_test"],
+             ct=u["ct_edge"] * ALG_BYTES["ct_edge"],
              div_src=u["div_src"] * ALG_BYTES["div_src"], fofc_fix=0)
     b["flux_y"] = b["flux_z"] = b["flux_x"]
     return b
@@ -228,6 +233,12 @@ def run_gpu(args, rank, local_rank, world):
     config = args.config
     spec = wl.config_spec(config)
     ids, nmb = pick_blocks(config, args.blocks)
+    if args.scaling == "strong" and world > 1:
+        # strong scaling: the config's block list is sharded over the ranks (contiguous ranges)
+        from paper_2409_10384_b200 import shard
+        all_ids = np.arange(wl.n_blocks(config)) if ids is None else ids
+        ids = shard.rank_block_ids(all_ids, rank, world, True)
+        nmb = len(ids)
     n = spec["params"]["n"]
     sh = ak.shapes(nmb, n)
     f64 = torch.float64
@@ -258,6 +269,8 @@ def run_gpu(args, rank, local_rank, world):
     par = ak.make_params(device=local_rank, stream=stream.cuda_stream, **params_d)
     ctx = ak.ak_create(par, dx)
     ak.ak_set_metric(ctx, adm)
+    if args.overlap >= 2:
+        ak.ak_set_overlap(ctx, args.overlap)
     zones = nmb * n ** 3
 
     def step():
@@ -293,17 +306,22 @@ def run_gpu(args, rank, local_rank, world):
         dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
     ms_total = float(tmax.item())
     ms_step = ms_total / args.steps
-    value = world * zones / (ms_step * 1e-3)
+    ztot = torch.tensor([float(zones)], dtype=f64, device=dev)
+    if world > 1:
+        dist.all_reduce(ztot, op=dist.ReduceOp.SUM)          # zones all ranks processed (weak: world x zones)
+    value = float(ztot.item()) / (ms_step * 1e-3)
     return dict(torch=torch, ak=ak, ctx=ctx, dev=dev, stream=stream, U=U, U0=U0, Bf=Bf, W=W, dU=dU, E=E, flag=flag,
                 status=status, sh=sh, nmb=nmb, n=n, ids=ids, zones=zones, dt_fofc=dt_fofc, params_d=params_d,
                 ms_step=ms_step, value=value, clocks=clocks, kms=kms, klaunch=klaunch, stats=stats, t_gen=t_gen,
-                spec=spec, world=world, dx=dx, adm=adm)
+                spec=spec, world=world, dx=dx, adm=adm, zones_total=float(ztot.item()),
+                schedule="overlapped, %d chunks (ak_set_overlap)" % args.overlap if args.overlap >= 2 else "serial")
 
 
 def run_e2e(R, steps):
     """Same metric through the C-ABI call with HOST buffers (ak_rhs_host): every step copies the
-    step's inputs U~, B~f from pinned host memory, runs parts 1-6 and reads back U~ (floored cells),
-    W, dU/dt, E and both masks.  The frozen metric snapshot stays resident (ak_set_metric)."""
+    step's inputs U~, B~f from pinned host memory, runs parts 1-6 and reads back the step's results: U~
+    (floored cells), dU/dt, E and both masks (the primitives W are an intermediate of the stage and stay on
+    the device: W = NULL).  The frozen metric snapshot stays resident (ak_set_metric)."""
     torch, ak = R["torch"], R["ak"]
     sh = R["sh"]
     pin = lambda k, dt=torch.float64: torch.zeros(sh[k], dtype=dt).pin_memory()
@@ -312,14 +330,13 @@ def run_e2e(R, steps):
     for h, d in zip(hU + hB, R["U0"] + R["Bf"]):
         h.copy_(d)
     hU0 = [h.clone() for h in hU]
-    hW = [pin("cell") for _ in range(8)]
     hdU = [pin("cell") for _ in range(5)]
     hE = [pin("ex"), pin("ey"), pin("ez")]
     hflag, hst = pin("cell", torch.uint8), pin("cell", torch.uint8)
     nbytes = lambda ts: int(sum(t.numel() * t.element_size() for t in ts))
     h2d = nbytes(hU + hB)
-    d2h = nbytes(hU + hW + hdU + hE + [hflag, hst])
-    call = lambda: ak.ak_rhs_host(R["ctx"], hU, hB, hW, R["dt_fofc"], hdU, hE, hflag, hst)
+    d2h = nbytes(hU + hdU + hE + [hflag, hst])
+    call = lambda: ak.ak_rhs_host(R["ctx"], hU, hB, None, R["dt_fofc"], hdU, hE, hflag, hst)
     call()                                                   # warm-up: allocates staging
     ts = []
     for _ in range(steps):
@@ -333,7 +350,7 @@ def run_e2e(R, steps):
     if R["world"] > 1:
         import torch.distributed as dist
         dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    val = R["world"] * R["zones"] * steps / float(tmax.item())
+    val = R["zones_total"] * steps / float(tmax.item())
     # the host path must give what the device path gave
     same = all(bool(torch.equal(h, d.cpu())) for h, d in zip(hdU, R["dU"]))
     return dict(value=val, unit=UNIT, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h, steps=steps,
@@ -381,8 +398,13 @@ def roofline(R, hbm_peak, peak_src):
     del a, b
     fp64_fma = ak.ak_probe_fp64(R["ctx"], 1, 3)
     fp64_nofma = ak.ak_probe_fp64(R["ctx"], 0, 3)
+    # no class may be credited with more bytes per second than the copy kernel moves (stale accounting check)
+    over = [k for k in table if table[k]["alg_gbs"] and table[k]["alg_gbs"] > copy_gbs]
     rf_common = dict(peak_source=peak_src, same_run_copy_gbs=round(copy_gbs, 1),
                      same_run_fp64_ginst=dict(fma=round(fp64_fma, 1), mul_add=round(fp64_nofma, 1)),
+                     peak_measured=dict(fp64_tflops_fma=round(2e-3 * fp64_fma, 2), fp64_tinst_mul_add=round(1e-3 * fp64_nofma, 2),
+                                        note="same-run ak_probe_fp64: independent DFMA / DMUL+DADD streams"),
+                     classes_above_copy_peak=over,
                      hbm=dict(achieved=table[dom]["alg_gbs"], peak=hbm_peak, unit="GB/s",
                               frac=round(table[dom]["alg_gbs"] / hbm_peak, 4) if table[dom]["alg_gbs"] else None))
     if dom.startswith("flux"):
@@ -394,6 +416,14 @@ def roofline(R, hbm_peak, peak_src):
         rf = dict(kernel=dom, bound="alu", achieved=round(ach, 3), peak=FP64_PIPE_PEAK_TINST, unit="Tinst/s (fp64 pipe)",
                   frac=round(ach / FP64_PIPE_PEAK_TINST, 4), traffic=NCU_TRAFFIC_BYTES.get((R["nmb"], dom)),
                   alg_ops_per_face=FLUX_FP64_PER_FACE[R["spec"]["params"]["recon"]], **rf_common)
+        sf = SURVEY_FLOP_PER_FACE.get(R["spec"]["params"]["recon"])
+        if sf:
+            # the survey's own unit: useful flops per face, against the no-FMA issue peak (the product is
+            # built --fmad=false: one flop per instruction) and against the FMA peak the same-run probe measures
+            tf = sf * kernel_units(R["nmb"], R["n"])["flux"] / (ms * 1e-3) * 1e-12
+            rf["survey"] = dict(flop_per_face=sf, achieved_tflops=round(tf, 3),
+                                frac_of_no_fma_issue_peak=round(tf / FP64_PIPE_PEAK_TINST, 4),
+                                frac_of_measured_fma_peak=round(tf / (2e-3 * fp64_fma), 4))
     else:
         ach = table[dom]["alg_gbs"]
         rf = dict(kernel=dom, bound="hbm", achieved=ach, peak=hbm_peak, unit="GB/s",
@@ -404,6 +434,66 @@ def roofline(R, hbm_peak, peak_src):
                  alg_gbs=round(stage_bytes / (R["ms_step"] * 1e-3) * 1e-9, 1))
     stage["frac_of_hbm_peak"] = round(stage["alg_gbs"] / hbm_peak, 4)
     return rf, table, stage
+
+
+def _time_stage(R, steps, **kw):
+    torch, ak = R["torch"], R["ak"]
+    call = lambda: ak.ak_rhs(R["ctx"], R["U"], R["Bf"], R["W"], 0, R["dt_fofc"], R["dU"], R["E"], R["flag"], R["status"], **kw)
+    for _ in range(3):
+        call()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize(R["dev"])
+    e0.record(R["stream"])
+    for _ in range(steps):
+        call()
+    e1.record(R["stream"])
+    torch.cuda.synchronize(R["dev"])
+    return e0.elapsed_time(e1) / steps
+
+
+def run_overlap(R, steps, nchunks=8):
+    """Context: the same stage under the overlapped schedule (ak_set_overlap: chunks of blocks pipelined over
+    three streams so that the memory-bound kernels of one chunk share the SMs with the fp64-bound sweeps of
+    another).  Outputs must be the bits of the serial schedule; the time is reported whichever way it falls
+    (profiles/r2_overlap.md: co-running does not pay on this path)."""
+    torch, ak = R["torch"], R["ak"]
+    if R["schedule"] != "serial":
+        return None
+    ak.ak_rhs(R["ctx"], R["U"], R["Bf"], R["W"], 0, R["dt_fofc"], R["dU"], R["E"], R["flag"], R["status"])   # serial
+    torch.cuda.synchronize(R["dev"])
+    ref = [t.clone() for t in R["dU"] + R["E"]] + [R["flag"].clone()]
+    ak.ak_set_overlap(R["ctx"], nchunks)
+    try:
+        ms = _time_stage(R, steps)
+        same = all(bool(torch.equal(a, b)) for a, b in zip(R["dU"] + R["E"] + [R["flag"]], ref))
+    finally:
+        ak.ak_set_overlap(R["ctx"], 0)
+    return dict(chunks=nchunks, ms_per_step=round(ms, 4), serial_ms_per_step=round(R["ms_step"], 4),
+                bit_identical_to_serial=same, note="context only; the reported value is the serial schedule")
+
+
+def run_matter(R, steps):
+    """Context: the matter terms E, S_i, S_ij for a spacetime solver as a fused
+    epilogue of the divergence+source kernel (ak_rhs_out.matter, interior cells) against the stand-alone
+    pass over all stored cells (ak_matter_sources)."""
+    torch, ak = R["torch"], R["ak"]
+    M = [torch.zeros_like(R["W"][0]) for _ in range(10)]
+    ms_fused = _time_stage(R, steps, matter=M)
+    ms_plain = _time_stage(R, steps)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ak.ak_matter_sources(R["ctx"], R["W"], M)
+    torch.cuda.synchronize(R["dev"])
+    e0.record(R["stream"])
+    for _ in range(steps):
+        ak.ak_matter_sources(R["ctx"], R["W"], M)
+    e1.record(R["stream"])
+    torch.cuda.synchronize(R["dev"])
+    del M
+    return dict(stage_ms_with_epilogue=round(ms_fused, 4), stage_ms_without=round(ms_plain, 4),
+                epilogue_cost_ms=round(ms_fused - ms_plain, 4),
+                standalone_kernel_ms=round(e0.elapsed_time(e1) / steps, 4),
+                note="fused: 10 stores per interior zone from registers K6 already holds; stand-alone: "
+                     "re-reads W and the metric over all nt^3 cells")
 
 
 HYBRID_EOS = dict(K0=40.0, gammas=[2.0, 2.2], rho_breaks=[6.4e-4], gamma_th=2.0)
@@ -513,6 +603,10 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-fma", action="store_true", help="skip the FMA-contracted perf-build leg")
+    ap.add_argument("--no-extra", action="store_true", help="skip the context legs (overlap, matter, rk3)")
+    ap.add_argument("--scaling", default="weak", choices=("weak", "strong"),
+                    help="N > 1: every rank its own batch (weak) or the config's blocks sharded over ranks (strong)")
+    ap.add_argument("--overlap", type=int, default=0, help="time the stage with ak_set_overlap(N) (default: serial)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -526,19 +620,25 @@ def main():
     e2e = None if args.no_e2e else run_e2e(R, max(1, args.e2e_steps))
     fma = None if (args.no_fma or world > 1) else run_fma(R, args.steps)
     hyb = None if (args.no_fma or world > 1) else run_hybrid(R, args.steps)
-    rk3 = run_rk3(R)
+    ovl = None if (args.no_extra or world > 1) else run_overlap(R, args.steps)
+    mat = None if (args.no_extra or world > 1) else run_matter(R, args.steps)
+    rk3 = None if args.no_extra else run_rk3(R)
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu:
         zones, cores, sample, step = oracle_sample(args.config, target_s=args.cpu_seconds)
         t = step()
         cpu = dict(value=zones / t, unit=UNIT, cores=cores, kind="oracle", sample=sample, seconds=round(t, 2))
+        # the oracle also on one thread
+        z1, c1, s1, step1 = oracle_sample(args.config, target_s=min(6.0, args.cpu_seconds), cores=1)
+        t1 = step1()
+        cpu["single_thread"] = dict(value=z1 / t1, unit=UNIT, cores=1, sample=s1, seconds=round(t1, 2))
     if rank == 0:
         spec = R["spec"]
         st = R["stats"]
         ntest = R["nmb"] * (R["n"] + 2) ** 3
         line = dict(metric=METRIC, value=R["value"], unit=UNIT, n_gpus=world, steps=args.steps,
-                    warmup=max(args.warmup, 3), ms_per_step=R["ms_step"], higher_is_better=True, scaling="weak",
-                    vs_baseline=None, dtype="f64", data="synthetic", impl="ak",
+                    warmup=max(args.warmup, 3), ms_per_step=R["ms_step"], higher_is_better=True, scaling=args.scaling,
+                    vs_baseline=None, dtype="f64", data="synthetic", impl="ak", schedule=R["schedule"],
                     config=dict(workload="%s (BASELINE.json configs[%s]): %d MeshBlocks of %d^3 + 4 ghosts per GPU, "
                                 "%s/%s, FOFC %s, DMP M=%s" % (
                                     args.config, args.config[1], R["nmb"], R["n"],
@@ -552,7 +652,8 @@ def main():
                                 fofc_faces=st["n_fofc_faces"]),
                     clocks=R["clocks"], e2e=e2e, gpu_launches=int(sum(R["klaunch"].values())),
                     roofline=rf, kernels=table, stage_hbm=stage, cpu_baseline=cpu, rk3_step=rk3,
-                    fma_build=fma, hybrid_eos=hyb, gen_seconds=round(R["t_gen"], 1))
+                    fma_build=fma, hybrid_eos=hyb, overlap_schedule=ovl, matter_epilogue=mat,
+                    gen_seconds=round(R["t_gen"], 1))
         print(json.dumps(line))
     R["ak"].ak_destroy(R["ctx"])
     if world > 1:

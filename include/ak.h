@@ -53,7 +53,7 @@ extern "C" {
 
 typedef struct ak_ctx ak_ctx; /* opaque */
 
-enum { AK_OK = 0, AK_EINVAL = -1, AK_ENOMEM = -2, AK_ECUDA = -3, AK_ESTATE = -4 };
+enum { AK_OK = 0, AK_EINVAL = -1, AK_ENOMEM = -2, AK_ECUDA = -3, AK_ESTATE = -4, AK_EHOOK = -5 };
 enum { AK_RECON_DC = 0, AK_RECON_PPM4 = 1, AK_RECON_WENOZ = 2, AK_RECON_PLM = 3, AK_RECON_PPMX = 4 };
 enum { AK_RS_LLF = 0, AK_RS_HLLE = 1 };
 enum { AK_BC_PERIODIC = 0, AK_BC_OUTFLOW = 1 };                  /* stage driver, D:§11 */
@@ -97,6 +97,10 @@ typedef struct {
   const double *gxx, *gxy, *gxz, *gyy, *gyz, *gzz, *alp, *betx, *bety, *betz,
                *Kxx, *Kxy, *Kxz, *Kyy, *Kyz, *Kzz;
 } ak_adm;                          /* cell fields: gamma_ij, alpha, beta^i, K_ij (Eq. 5)      */
+/* Matter terms a spacetime (Z4c) right-hand side needs from the fluid (P:119 "E = tau + D ...
+ * S_ij = T_ij"): E, S_i, S_ij, undensitised.  Ten caller-owned device cell fields. */
+typedef struct { double *E, *Sx, *Sy, *Sz, *Sxx, *Sxy, *Sxz, *Syy, *Syz, *Szz; } ak_matter;
+
 typedef struct {
   double *dD, *dSx, *dSy, *dSz, *dtau; /* cell fields; interior cells written, rest untouched */
   double *Ex, *Ey, *Ez;                /* edge fields; edges of interior cells written        */
@@ -104,6 +108,12 @@ typedef struct {
                                        /* tested range); may be NULL                          */
   unsigned char* c2p_status;           /* [nmb][nt^3] bytes, written when part (1) runs;      */
                                        /* may be NULL                                         */
+  const ak_matter* matter;             /* may be NULL.  Else part (6) also writes the matter  */
+                                       /* terms of the stage's primitives on the INTERIOR     */
+                                       /* cells (the rest untouched): a fused epilogue of the */
+                                       /* divergence+source kernel, which holds E, S_i, S_ij  */
+                                       /* in registers (S:§8(f) rank 4).  Same bits as        */
+                                       /* ak_matter_sources.  Must be NULL for ak_rhs_host.   */
 } ak_rhs_out;
 
 typedef struct {
@@ -150,10 +160,9 @@ int ak_set_overlap(ak_ctx*, int nchunks);
  * (AK_ESTATE if there are none) and the primitives W. */
 int ak_emf(ak_ctx*, const ak_prim* W, double* Ex, double* Ey, double* Ez);
 
-/* Matter terms a spacetime (Z4c) right-hand side needs from the fluid (P:119 "E = tau + D ...
- * S_ij = T_ij"): E, S_i, S_ij, undensitised, at every stored cell, from the primitives W
- * and the metric set with ak_set_metric.  Ten caller-owned device cell fields. */
-typedef struct { double *E, *Sx, *Sy, *Sz, *Sxx, *Sxy, *Sxz, *Syy, *Syz, *Szz; } ak_matter;
+/* The matter terms (ak_matter above) at EVERY stored cell, ghosts included, from the primitives W and
+ * the metric set with ak_set_metric: the stand-alone pass; ak_rhs_out.matter gives the interior cells
+ * for free inside a stage. */
 int ak_matter_sources(ak_ctx*, const ak_prim* W, const ak_matter* out);
 
 /* Copy the device counters to the host.  Synchronises the stream. */
@@ -168,7 +177,11 @@ int ak_get_flux(ak_ctx*, int dir, int comp, double* dst);
  * W, out are host pointers (pinned memory recommended); the metric must already be set with
  * ak_set_metric (device pointers: the snapshot is frozen across stages).  Copies U and Bf
  * to context-owned device staging, runs parts (1)-(6), copies back U (floored cells), W,
- * dU, E and the two masks, and synchronises.  Staging is allocated on first use. */
+ * dU, E and the two masks, and synchronises.  Staging is allocated on first use.
+ * W == NULL (or all eight members NULL): the primitives are an intermediate of the stage and are not
+ * copied back (3.1 of the 8.5 GB a C4 stage would otherwise return).  Batches of >= 16 blocks are
+ * pipelined in chunks over two internal streams so that H2D, kernels and D2H overlap; the fluxes of such
+ * a stage stay in the pipeline's contexts (ak_emf / ak_get_flux afterwards: AK_ESTATE). */
 int ak_rhs_host(ak_ctx*, const ak_cons* U, const ak_faceB* Bf, const ak_prim* W,
                 double dt_fofc, const ak_rhs_out* out);
 
@@ -245,6 +258,16 @@ int ak_stage_update(ak_ctx*, double a, double b, double dt, const ak_cons* U0, c
  * of the FOFC flags of every stage (caller zeroes it). */
 int ak_advance(ak_ctx*, int integrator, int nsteps, double dt, const int bc[3], const ak_cons* U,
                const ak_faceB_rw* Bf, const ak_prim* W, unsigned char* flag_or);
+
+/* ak_advance with a caller hook: refresh(user) is called on the HOST before every ghost fill (each
+ * stage, and the fill at the end) — the point where a multi-GPU driver refreshes the mirror blocks of
+ * ak_set_neighbors (pack, NCCL send/recv, unpack, all enqueued on the context's stream by the hook;
+ * D:§12).  The stage sequence and the Shu-Osher weights stay inside the library.  A non-zero
+ * return aborts with AK_EHOOK (the FOFC blend is restored).  refresh == NULL: ak_advance. */
+typedef int (*ak_refresh_fn)(void* user);
+int ak_advance_hooked(ak_ctx*, int integrator, int nsteps, double dt, const int bc[3], const ak_cons* U,
+                      const ak_faceB_rw* Bf, const ak_prim* W, unsigned char* flag_or,
+                      ak_refresh_fn refresh, void* user);
 
 /* Device-timing hooks for the benchmark: bracket kernel class `which` (0 con2prim, 1-3 flux
  * sweeps x/y/z, 4 FOFC test, 5 FOFC list+reflux, 6 cell EMF+CT, 7 divergence+sources) with

@@ -177,6 +177,10 @@ extern "C" void orc_advance_nbr(const orc_params* p, const double* dx, int integ
                                 double dt, const int bc[3], const int* nbr, double* const U[5],
                                 double* const Bf[3], const double* const adm[16], double* const W[8],
                                 unsigned char* flag_or, int nthreads);
+extern "C" int orc_advance_hooked(const orc_params* p, const double* dx, int integrator, int nsteps,
+                                  double dt, const int bc[3], const int* nbr, double* const U[5],
+                                  double* const Bf[3], const double* const adm[16], double* const W[8],
+                                  unsigned char* flag_or, int nthreads, int (*refresh)(void*), void* user);
 
 extern "C" void orc_advance(const orc_params* p, const double* dx, int integrator, int nsteps,
                             double dt, const int bc[3], double* const U[5], double* const Bf[3],
@@ -189,6 +193,15 @@ extern "C" void orc_advance_nbr(const orc_params* p, const double* dx, int integ
                                 double dt, const int bc[3], const int* nbr, double* const U[5],
                                 double* const Bf[3], const double* const adm[16], double* const W[8],
                                 unsigned char* flag_or, int nthreads) {
+  orc_advance_hooked(p, dx, integrator, nsteps, dt, bc, nbr, U, Bf, adm, W, flag_or, nthreads, nullptr, nullptr);
+}
+
+// The same loop with a caller hook run before every ghost fill (every stage, and the final fill): where a
+// multi-rank driver refreshes the mirror blocks its neighbour table points at.  A non-zero return aborts.
+extern "C" int orc_advance_hooked(const orc_params* p, const double* dx, int integrator, int nsteps,
+                                  double dt, const int bc[3], const int* nbr, double* const U[5],
+                                  double* const Bf[3], const double* const adm[16], double* const W[8],
+                                  unsigned char* flag_or, int nthreads, int (*refresh)(void*), void* user) {
   const Lay L(p->n, p->ng);
   const long nt = L.nt, px = L.px, nb = p->nmb;
   const long ncell = nb * nt * nt * nt;
@@ -206,6 +219,7 @@ extern "C" void orc_advance_nbr(const orc_params* p, const double* dx, int integ
   for (int step = 0; step < nsteps; ++step)
     for (int s = 0; s < ns; ++s) {
       const double a = A[ns - 1][s], b = B[ns - 1][s];
+      if (refresh) { const int hr = refresh(user); if (hr != 0) return hr; }
       if (nbr) orc_exchange_ghosts(p, nbr, bc, U, Bf); else orc_fill_ghosts(p, bc, U, Bf);
       orc_rhs_blend(p, dx, U, Bf, adm, W, 0, dt, s == 0 ? nullptr : U0, a, b, dU, E, flag.data(),
                     nullptr, nthreads);
@@ -223,5 +237,7 @@ extern "C" void orc_advance_nbr(const orc_params* p, const double* dx, int integ
         orc_stage_update(p, dx, a, b, dt, U0, B0, U, Bf, dU, E);
       }
     }
+  if (refresh) { const int hr = refresh(user); if (hr != 0) return hr; }
   if (nbr) orc_exchange_ghosts(p, nbr, bc, U, Bf); else orc_fill_ghosts(p, bc, U, Bf);
+  return 0;
 }

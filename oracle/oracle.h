@@ -158,6 +158,12 @@ void orc_advance(const orc_params* p, const double* dx, int integrator, int nste
  * (oz+1)*9+(oy+1)*3+(ox+1), -1 = none; sides without a face neighbour get bc[d]. */
 void orc_exchange_ghosts(const orc_params* p, const int* nbr, const int bc[3], double* const U[5],
                          double* const Bf[3]);
+/* ... with a caller hook run on the host before every ghost fill (multi-rank drivers refresh their
+ * mirror blocks there); returns the hook's first non-zero value, else 0. */
+int orc_advance_hooked(const orc_params* p, const double* dx, int integrator, int nsteps, double dt,
+                       const int bc[3], const int* nbr, double* const U[5], double* const Bf[3],
+                       const double* const adm[16], double* const W[8], unsigned char* flag_or,
+                       int nthreads, int (*refresh)(void*), void* user);
 void orc_advance_nbr(const orc_params* p, const double* dx, int integrator, int nsteps, double dt,
                      const int bc[3], const int* nbr, double* const U[5], double* const Bf[3],
                      const double* const adm[16], double* const W[8], unsigned char* flag_or,

@@ -263,6 +263,34 @@ def advance_nbr(par, dx, integrator, nsteps, dt, bc, nbr, U, Bf, adm, nthreads=1
     return W, flag
 
 
+def advance_hooked(par, dx, integrator, nsteps, dt, bc, nbr, U, Bf, adm, refresh, nthreads=1):
+    """advance_nbr with a Python callable run before every ghost fill; U, Bf may hold mirror blocks
+    behind the par.nmb evolved ones (nbr = local table pointing at them)."""
+    sh = shapes(par.nmb, par.n)
+    dx = np.ascontiguousarray(dx, dtype=np.float64).reshape(par.nmb, 3)
+    W = [np.zeros(sh["cell"]) for _ in range(8)]
+    flag = np.zeros(sh["cell"], dtype=np.uint8)
+    a, ap = _nbr(nbr, par.nmb)
+    err = []
+
+    def _cb(_user):
+        try:
+            refresh()
+            return 0
+        except BaseException as e:      # never unwind through C
+            err.append(e)
+            return 1
+    cb = C.CFUNCTYPE(C.c_int, C.c_void_p)(_cb)
+    lib().orc_advance_hooked.restype = C.c_int
+    rc = lib().orc_advance_hooked(C.byref(par), dx.ctypes.data_as(_dp), int(integrator), int(nsteps), C.c_double(dt),
+                                  _ib(bc), ap, _ptrs(U), _ptrs(Bf), _ptrs(adm), _ptrs(W),
+                                  flag.ctypes.data_as(C.c_void_p), int(nthreads), cb, None)
+    if err:
+        raise err[0]
+    assert rc == 0
+    return W, flag
+
+
 def matter_sources(par, W, g6):
     """E, S_i, S_ij (10 cell arrays, undensitised) from the primitives."""
     sh = shapes(par.nmb, par.n)

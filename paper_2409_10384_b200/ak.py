@@ -13,7 +13,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 SO_PATH = os.environ.get("AK_LIBRARY") or os.path.join(_HERE, "libak.so")   # AK_LIBRARY: another build of the same library
 
-AK_OK, AK_EINVAL, AK_ENOMEM, AK_ECUDA, AK_ESTATE = 0, -1, -2, -3, -4
+AK_OK, AK_EINVAL, AK_ENOMEM, AK_ECUDA, AK_ESTATE, AK_EHOOK = 0, -1, -2, -3, -4, -5
 RECON_DC, RECON_PPM4, RECON_WENOZ, RECON_PLM, RECON_PPMX = 0, 1, 2, 3, 4
 RS_LLF, RS_HLLE = 0, 1
 ST_DFLOOR, ST_TAUFLOOR, ST_MAGCAP, ST_RHOFLOOR, ST_TFLOOR, ST_FAIL, ST_DMP = 1, 2, 4, 8, 16, 32, 64
@@ -23,7 +23,7 @@ EXPORTS = ("ak_create", "ak_set_metric", "ak_con2prim", "ak_rhs", "ak_emf", "ak_
            "ak_probe_fp64", "ak_destroy", "ak_strerror", "ak_version",
            "ak_set_fofc_blend", "ak_fill_ghosts", "ak_stage_update", "ak_advance", "ak_set_neighbors",
            "ak_matter_sources", "ak_halo_slab_elems", "ak_halo_pack", "ak_halo_unpack",
-           "ak_set_eos_hybrid", "ak_set_overlap")
+           "ak_set_eos_hybrid", "ak_set_overlap", "ak_advance_hooked")
 BC_PERIODIC, BC_OUTFLOW = 0, 1
 
 _dp = C.POINTER(C.c_double)
@@ -57,7 +57,7 @@ class AkAdm(C.Structure):
 
 class AkRhsOut(C.Structure):
     _fields_ = [(k, C.c_void_p) for k in ("dD", "dSx", "dSy", "dSz", "dtau", "Ex", "Ey", "Ez",
-                                          "fofc_flag", "c2p_status")]
+                                          "fofc_flag", "c2p_status", "matter")]
 
 
 class AkMatter(C.Structure):
@@ -68,6 +68,9 @@ class AkStats(C.Structure):
     _fields_ = [("n_c2p_fail", C.c_longlong), ("n_cons_floor", C.c_longlong),
                 ("n_prim_floor", C.c_longlong), ("n_fofc_cells", C.c_longlong),
                 ("n_dmp_cells", C.c_longlong), ("n_fofc_faces", C.c_longlong * 3)]
+
+
+REFRESH_FN = C.CFUNCTYPE(C.c_int, C.c_void_p)      # ak_refresh_fn of include/ak.h
 
 
 class AkError(RuntimeError):
@@ -117,6 +120,8 @@ def lib():
                                       C.POINTER(AkRhsOut)]
         L.ak_advance.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double, C.POINTER(C.c_int), C.POINTER(AkCons),
                                  C.POINTER(AkFaceB), C.POINTER(AkPrim), C.c_void_p]
+        L.ak_advance_hooked.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double, C.POINTER(C.c_int), C.POINTER(AkCons),
+                                        C.POINTER(AkFaceB), C.POINTER(AkPrim), C.c_void_p, REFRESH_FN, C.c_void_p]
         L.ak_matter_sources.argtypes = [C.c_void_p, C.POINTER(AkPrim), C.POINTER(AkMatter)]
         L.ak_set_neighbors.argtypes = [C.c_void_p, C.POINTER(C.c_int), C.c_int]
         L.ak_set_overlap.argtypes = [C.c_void_p, C.c_int]
@@ -198,17 +203,22 @@ def ak_con2prim(ctx, U, Bf, W, status=None):
     _chk(lib().ak_con2prim(ctx, C.byref(u), C.byref(b), C.byref(w), _ptr(status)), "ak_con2prim")
 
 
-def ak_rhs(ctx, U, Bf, W, w_is_valid, dt_fofc, dU, E, fofc_flag=None, c2p_status=None):
+def ak_rhs(ctx, U, Bf, W, w_is_valid, dt_fofc, dU, E, fofc_flag=None, c2p_status=None, matter=None):
+    """matter: None or ten device cell fields E, S_i, S_ij written on interior cells by part (6)."""
     u, b, w = _struct(AkCons, U), _struct(AkFaceB, Bf), _struct(AkPrim, W)
-    o = _struct(AkRhsOut, list(dU) + list(E) + [fofc_flag, c2p_status])
+    m = _struct(AkMatter, matter) if matter is not None else None
+    o = _struct(AkRhsOut, list(dU) + list(E) + [fofc_flag, c2p_status, None])
+    if m is not None:
+        o.matter = C.cast(C.pointer(m), C.c_void_p)
     _chk(lib().ak_rhs(ctx, C.byref(u), C.byref(b), C.byref(w), int(w_is_valid), float(dt_fofc), C.byref(o)),
          "ak_rhs")
 
 
 def ak_rhs_host(ctx, U, Bf, W, dt_fofc, dU, E, fofc_flag=None, c2p_status=None):
-    """same stage with HOST buffers (numpy arrays or pinned CPU tensors)."""
-    u, b, w = _struct(AkCons, U), _struct(AkFaceB, Bf), _struct(AkPrim, W)
-    o = _struct(AkRhsOut, list(dU) + list(E) + [fofc_flag, c2p_status])
+    """same stage with HOST buffers (numpy arrays or pinned CPU tensors); W = None: primitives not returned."""
+    u, b = _struct(AkCons, U), _struct(AkFaceB, Bf)
+    w = _struct(AkPrim, W) if W is not None else AkPrim()
+    o = _struct(AkRhsOut, list(dU) + list(E) + [fofc_flag, c2p_status, None])
     _chk(lib().ak_rhs_host(ctx, C.byref(u), C.byref(b), C.byref(w), float(dt_fofc), C.byref(o)), "ak_rhs_host")
 
 
@@ -290,7 +300,7 @@ def ak_fill_ghosts(ctx, bc, U, Bf):
 
 def ak_stage_update(ctx, a, b, dt, U0, B0, U, Bf, dU, E):
     u0, b0, u, bf = _struct(AkCons, U0), _struct(AkFaceB, B0), _struct(AkCons, U), _struct(AkFaceB, Bf)
-    o = _struct(AkRhsOut, list(dU) + list(E) + [None, None])
+    o = _struct(AkRhsOut, list(dU) + list(E) + [None, None, None])
     _chk(lib().ak_stage_update(ctx, float(a), float(b), float(dt), C.byref(u0), C.byref(b0), C.byref(u),
                                C.byref(bf), C.byref(o)), "ak_stage_update")
 
@@ -299,6 +309,26 @@ def ak_advance(ctx, integrator, nsteps, dt, bc, U, Bf, W, flag_or=None):
     u, bf, w = _struct(AkCons, U), _struct(AkFaceB, Bf), _struct(AkPrim, W)
     _chk(lib().ak_advance(ctx, int(integrator), int(nsteps), float(dt), _bc(bc), C.byref(u), C.byref(bf),
                           C.byref(w), _ptr(flag_or)), "ak_advance")
+
+
+def ak_advance_hooked(ctx, integrator, nsteps, dt, bc, U, Bf, W, flag_or=None, refresh=None):
+    """ak_advance with `refresh()` (a Python callable or None) run before every ghost fill."""
+    u, bf, w = _struct(AkCons, U), _struct(AkFaceB, Bf), _struct(AkPrim, W)
+    err = []
+
+    def _cb(_user):
+        try:
+            refresh()
+            return 0
+        except BaseException as e:      # never unwind through C
+            err.append(e)
+            return 1
+    cb = REFRESH_FN(_cb) if refresh is not None else C.cast(None, REFRESH_FN)
+    code = lib().ak_advance_hooked(ctx, int(integrator), int(nsteps), float(dt), _bc(bc), C.byref(u), C.byref(bf),
+                                   C.byref(w), _ptr(flag_or), cb, None)
+    if err:
+        raise err[0]
+    _chk(code, "ak_advance_hooked")
 
 
 def ak_set_neighbors(ctx, nbr, nmb_total=0):

@@ -186,6 +186,7 @@ void chunk_fields(const ak_ctx* c, const Fields& f, int m0, int nb, int ci, Fiel
   for (int q = 0; q < 21; ++q) g.F[q] += fsz[q / 7];
   g.flag += cell;
   if (g.status) g.status += cell;
+  if (g.M[0]) for (int q = 0; q < 10; ++q) g.M[q] += cell;
   g.dx += 3LL * m0;
   g.list += (n + 2) * (n + 2) * (n + 2) * m0;
   g.count += 4 * ci;
@@ -227,7 +228,14 @@ int launch_c2p(ak_ctx* c, const Lane& L, bool with_emf) {
   CK(cudaMemsetAsync(L.f.stats, 0, sizeof(unsigned long long) * 3, L.st));
   const long long ncell = (long long)L.P.nmb * L.P.nt * L.P.nt * L.P.nt;
   const unsigned g = capped(ncell, 128, L.ov ? c->cap[KC_C2P] : 0);
-  if (L.P.eos) {
+  const bool stride = (long long)g * 128 < ncell;       // a capped grid needs the grid-stride form
+  if (stride) {
+    if (L.P.eos) {
+      if (with_emf) k_con2prim<true, 1, true><<<g, 128, 0, L.st>>>(L.P, L.f);
+      else k_con2prim<false, 1, true><<<g, 128, 0, L.st>>>(L.P, L.f);
+    } else if (with_emf) k_con2prim<true, 0, true><<<g, 128, 0, L.st>>>(L.P, L.f);
+    else k_con2prim<false, 0, true><<<g, 128, 0, L.st>>>(L.P, L.f);
+  } else if (L.P.eos) {
     if (with_emf) k_con2prim<true, 1><<<g, 128, 0, L.st>>>(L.P, L.f);
     else k_con2prim<false, 1><<<g, 128, 0, L.st>>>(L.P, L.f);
   } else if (with_emf) k_con2prim<true><<<g, 128, 0, L.st>>>(L.P, L.f);
@@ -347,7 +355,10 @@ int launch_fofc(ak_ctx* c, const Lane& L, double dt) {
     CK(cudaMemsetAsync(L.f.stats + S_FOFC_CELLS, 0, sizeof(unsigned long long) * 2, L.st));
     if (L.P.fofc) {
       const unsigned g = capped(ntest, 128, L.ov ? c->cap[KC_FOFC_TEST] : 0);
-      if (L.P.eos) k_fofc_test<1><<<g, 128, 0, L.st>>>(L.P, L.f, dt);
+      if ((long long)g * 128 < ntest) {
+        if (L.P.eos) k_fofc_test<1, true><<<g, 128, 0, L.st>>>(L.P, L.f, dt);
+        else k_fofc_test<0, true><<<g, 128, 0, L.st>>>(L.P, L.f, dt);
+      } else if (L.P.eos) k_fofc_test<1><<<g, 128, 0, L.st>>>(L.P, L.f, dt);
       else k_fofc_test<0><<<g, 128, 0, L.st>>>(L.P, L.f, dt);
       c->launches[KC_FOFC_TEST] += 1;
       CK(cudaGetLastError());
@@ -379,9 +390,15 @@ int launch_ct(ak_ctx* c, const Lane& L, bool have_cell_emf) {
   const long long ne = n * (n + 1) * (n + 1) * L.P.nmb;
   const unsigned g = capped(ne, 128, L.ov ? c->cap[KC_CT] : 0);
   if (!have_cell_emf) k_cell_emf<<<nblk(ntest, 128), 128, 0, L.st>>>(L.P, L.f);
-  k_ct<0><<<g, 128, 0, L.st>>>(L.P, L.f);
-  k_ct<1><<<g, 128, 0, L.st>>>(L.P, L.f);
-  k_ct<2><<<g, 128, 0, L.st>>>(L.P, L.f);
+  if ((long long)g * 128 < ne) {
+    k_ct<0, true><<<g, 128, 0, L.st>>>(L.P, L.f);
+    k_ct<1, true><<<g, 128, 0, L.st>>>(L.P, L.f);
+    k_ct<2, true><<<g, 128, 0, L.st>>>(L.P, L.f);
+  } else {
+    k_ct<0><<<g, 128, 0, L.st>>>(L.P, L.f);
+    k_ct<1><<<g, 128, 0, L.st>>>(L.P, L.f);
+    k_ct<2><<<g, 128, 0, L.st>>>(L.P, L.f);
+  }
   CK(cudaGetLastError());
   c->launches[KC_CT] += have_cell_emf ? 3 : 4;
   return AK_OK;
@@ -391,7 +408,10 @@ int launch_src(ak_ctx* c, const Lane& L) {
   Timer t(c, KC_SRC, L.st);
   const long long n = L.P.n;
   const unsigned g = capped(n * n * n * L.P.nmb, 128, L.ov ? c->cap[KC_SRC] : 0);
-  if (L.P.eos) k_div_src<1><<<g, 128, 0, L.st>>>(L.P, L.f);
+  if ((long long)g * 128 < n * n * n * L.P.nmb) {
+    if (L.P.eos) k_div_src<1, true><<<g, 128, 0, L.st>>>(L.P, L.f);
+    else k_div_src<0, true><<<g, 128, 0, L.st>>>(L.P, L.f);
+  } else if (L.P.eos) k_div_src<1><<<g, 128, 0, L.st>>>(L.P, L.f);
   else k_div_src<0><<<g, 128, 0, L.st>>>(L.P, L.f);
   CK(cudaGetLastError());
   c->launches[KC_SRC] += 1;
@@ -452,6 +472,7 @@ const char* ak_strerror(int code) {
     case AK_ENOMEM: return "out of device memory";
     case AK_ECUDA: return last_cuda_error != cudaSuccess ? cudaGetErrorString(last_cuda_error) : "CUDA error";
     case AK_ESTATE: return "call out of order (metric or fluxes missing)";
+    case AK_EHOOK: return "the caller's refresh hook reported a failure";
     default: return "unknown error code";
   }
 }
@@ -646,6 +667,11 @@ int ak_rhs(ak_ctx* c, const ak_cons* U, const ak_faceB* Bf, const ak_prim* W, in
   f.E[0] = out->Ex; f.E[1] = out->Ey; f.E[2] = out->Ez;
   if (out->fofc_flag) f.flag = out->fofc_flag;
   f.status = out->c2p_status;
+  if (out->matter) {
+    const ak_matter* mo = out->matter;
+    double* mp[10] = {mo->E, mo->Sx, mo->Sy, mo->Sz, mo->Sxx, mo->Sxy, mo->Sxz, mo->Syy, mo->Syz, mo->Szz};
+    for (int q = 0; q < 10; ++q) { if (!al16(mp[q])) return AK_EINVAL; f.M[q] = mp[q]; }
+  }
   CK(cudaSetDevice(c->hp.device));
   c->stats_from_host = false;
   // counters of every chunk slot start from zero (a stage that skips part (1) reports no con2prim counts)
@@ -867,14 +893,14 @@ static int rhs_host_pipelined(ak_ctx* c, int chunk, double* const hU[5], const d
     const ak_cons dU_ = {b[0], b[1], b[2], b[3], b[4]};
     const ak_faceB dB_ = {b[5], b[6], b[7]};
     const ak_prim dW_ = {b[8], b[9], b[10], b[11], b[12], b[13], b[14], b[15]};
-    const ak_rhs_out dO = {b[16], b[17], b[18], b[19], b[20], b[21], b[22], b[23], c->lane_mask[l][0], c->lane_mask[l][1]};
+    const ak_rhs_out dO = {b[16], b[17], b[18], b[19], b[20], b[21], b[22], b[23], c->lane_mask[l][0], c->lane_mask[l][1], nullptr};
     const int r = ak_rhs(k, &dU_, &dB_, &dW_, 0, dt_fofc, &dO);
     if (r != AK_OK) return r;
     for (int q = 0; q < 5; ++q) {
       CK(cudaMemcpyAsync(hU[q] + m0 * per[0], b[q], sizeof(double) * per[0] * chunk, cudaMemcpyDeviceToHost, st));
       CK(cudaMemcpyAsync(hdU[q] + m0 * per[0], b[16 + q], sizeof(double) * per[0] * chunk, cudaMemcpyDeviceToHost, st));
     }
-    for (int q = 0; q < 8; ++q)
+    for (int q = 0; q < 8 && hW[0]; ++q)
       CK(cudaMemcpyAsync(hW[q] + m0 * per[0], b[8 + q], sizeof(double) * per[0] * chunk, cudaMemcpyDeviceToHost, st));
     for (int q = 0; q < 3; ++q)
       CK(cudaMemcpyAsync(hE[q] + m0 * per[4 + q], b[21 + q], sizeof(double) * per[4 + q] * chunk, cudaMemcpyDeviceToHost, st));
@@ -903,7 +929,7 @@ static int rhs_host_pipelined(ak_ctx* c, int chunk, double* const hU[5], const d
 
 int ak_rhs_host(ak_ctx* c, const ak_cons* U, const ak_faceB* Bf, const ak_prim* W, double dt_fofc,
                 const ak_rhs_out* out) {
-  if (!c || !U || !Bf || !W || !out) return AK_EINVAL;
+  if (!c || !U || !Bf || !out || out->matter) return AK_EINVAL;
   if (!c->have_metric) return AK_ESTATE;
   CK(cudaSetDevice(c->hp.device));
   const size_t cb = sizeof(double) * c->sz.cell;
@@ -911,12 +937,16 @@ int ak_rhs_host(ak_ctx* c, const ak_cons* U, const ak_faceB* Bf, const ak_prim* 
   const size_t eb[3] = {sizeof(double) * c->sz.ex, sizeof(double) * c->sz.ey, sizeof(double) * c->sz.ez};
   double* hU[5] = {U->D, U->Sx, U->Sy, U->Sz, U->tau};
   const double* hB[3] = {Bf->bx, Bf->by, Bf->bz};
-  double* hW[8] = {W->rho, W->ux, W->uy, W->uz, W->p, W->bccx, W->bccy, W->bccz};
+  // W == NULL (or all eight members NULL): the primitives stay on the device and are not copied back
+  double* hW[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  if (W) { hW[0] = W->rho; hW[1] = W->ux; hW[2] = W->uy; hW[3] = W->uz; hW[4] = W->p; hW[5] = W->bccx; hW[6] = W->bccy; hW[7] = W->bccz; }
+  int nW = 0;
+  for (int q = 0; q < 8; ++q) nW += hW[q] != nullptr;
+  if (nW != 0 && nW != 8) return AK_EINVAL;
   double* hdU[5] = {out->dD, out->dSx, out->dSy, out->dSz, out->dtau};
   double* hE[3] = {out->Ex, out->Ey, out->Ez};
   for (int q = 0; q < 5; ++q) if (!hU[q] || !hdU[q]) return AK_EINVAL;
   for (int q = 0; q < 3; ++q) if (!hB[q] || !hE[q]) return AK_EINVAL;
-  for (int q = 0; q < 8; ++q) if (!hW[q]) return AK_EINVAL;
   {
     // chunk = the largest divisor of nmb not above max(8, nmb / 8); small batches go in one piece
     int chunk = 0;
@@ -944,14 +974,14 @@ int ak_rhs_host(ak_ctx* c, const ak_cons* U, const ak_faceB* Bf, const ak_prim* 
   ak_faceB dB_ = {c->stg_Bf[0], c->stg_Bf[1], c->stg_Bf[2]};
   ak_prim dW_ = {c->stg_W[0], c->stg_W[1], c->stg_W[2], c->stg_W[3], c->stg_W[4], c->stg_W[5], c->stg_W[6], c->stg_W[7]};
   ak_rhs_out dO = {c->stg_dU[0], c->stg_dU[1], c->stg_dU[2], c->stg_dU[3], c->stg_dU[4],
-                   c->stg_E[0], c->stg_E[1], c->stg_E[2], c->stg_flag, c->stg_status};
+                   c->stg_E[0], c->stg_E[1], c->stg_E[2], c->stg_flag, c->stg_status, nullptr};
   const int r = ak_rhs(c, &dU_, &dB_, &dW_, 0, dt_fofc, &dO);
   if (r != AK_OK) return r;
   for (int q = 0; q < 5; ++q) {
     CK(cudaMemcpyAsync(hU[q], c->stg_U[q], cb, cudaMemcpyDeviceToHost, c->stream));
     CK(cudaMemcpyAsync(hdU[q], c->stg_dU[q], cb, cudaMemcpyDeviceToHost, c->stream));
   }
-  for (int q = 0; q < 8; ++q) CK(cudaMemcpyAsync(hW[q], c->stg_W[q], cb, cudaMemcpyDeviceToHost, c->stream));
+  for (int q = 0; q < 8 && hW[0]; ++q) CK(cudaMemcpyAsync(hW[q], c->stg_W[q], cb, cudaMemcpyDeviceToHost, c->stream));
   for (int q = 0; q < 3; ++q) CK(cudaMemcpyAsync(hE[q], c->stg_E[q], eb[q], cudaMemcpyDeviceToHost, c->stream));
   if (out->fofc_flag) CK(cudaMemcpyAsync(out->fofc_flag, c->stg_flag, (size_t)c->sz.cell, cudaMemcpyDeviceToHost, c->stream));
   if (out->c2p_status) CK(cudaMemcpyAsync(out->c2p_status, c->stg_status, (size_t)c->sz.cell, cudaMemcpyDeviceToHost, c->stream));
@@ -1092,6 +1122,12 @@ int ak_stage_update(ak_ctx* c, double a, double b, double dt, const ak_cons* U0,
 
 int ak_advance(ak_ctx* c, int integrator, int nsteps, double dt, const int bc[3], const ak_cons* U,
                const ak_faceB_rw* Bf, const ak_prim* W, unsigned char* flag_or) {
+  return ak_advance_hooked(c, integrator, nsteps, dt, bc, U, Bf, W, flag_or, nullptr, nullptr);
+}
+
+int ak_advance_hooked(ak_ctx* c, int integrator, int nsteps, double dt, const int bc[3], const ak_cons* U,
+                      const ak_faceB_rw* Bf, const ak_prim* W, unsigned char* flag_or, ak_refresh_fn refresh,
+                      void* user) {
   if (!c || integrator < 1 || integrator > 3 || nsteps < 0 || !std::isfinite(dt) || !bc_ok(bc) || !U || !Bf || !W)
     return AK_EINVAL;
   if (!c->have_metric) return AK_ESTATE;
@@ -1114,7 +1150,7 @@ int ak_advance(ak_ctx* c, int integrator, int nsteps, double dt, const int bc[3]
   const ak_faceB RB0 = {c->regB0[0], c->regB0[1], c->regB0[2]};
   const ak_faceB Bc = {Bf->bx, Bf->by, Bf->bz};
   const ak_rhs_out out = {c->reg_dU[0], c->reg_dU[1], c->reg_dU[2], c->reg_dU[3], c->reg_dU[4],
-                          c->regE[0], c->regE[1], c->regE[2], c->reg_flag, nullptr};
+                          c->regE[0], c->regE[1], c->regE[2], c->reg_flag, nullptr, nullptr};
   // the caller's blend setting is restored afterwards
   const double* sv[5]; for (int q = 0; q < 5; ++q) sv[q] = c->blendU0[q];
   const double sa = c->blend_a, sb = c->blend_b;
@@ -1122,6 +1158,7 @@ int ak_advance(ak_ctx* c, int integrator, int nsteps, double dt, const int bc[3]
   for (int step = 0; step < nsteps && r == AK_OK; ++step)
     for (int s = 0; s < integrator && r == AK_OK; ++s) {
       const double a = A[integrator - 1][s], b = B[integrator - 1][s];
+      if (refresh && refresh(user) != 0) { r = AK_EHOOK; break; }
       if ((r = ak_fill_ghosts(c, bc, U, Bf)) != AK_OK) break;
       if (s == 0) r = ak_set_fofc_blend(c, nullptr, 0.0, 1.0); else r = ak_set_fofc_blend(c, &R0, a, b);
       if (r != AK_OK) break;
@@ -1142,6 +1179,7 @@ int ak_advance(ak_ctx* c, int integrator, int nsteps, double dt, const int bc[3]
   for (int q = 0; q < 5; ++q) c->blendU0[q] = sv[q];
   c->blend_a = sa; c->blend_b = sb;
   if (r != AK_OK) return r;
+  if (refresh && refresh(user) != 0) return AK_EHOOK;
   return ak_fill_ghosts(c, bc, U, Bf);
 }
 

@@ -49,6 +49,7 @@ struct Fields {
   unsigned long long* stats;    // device counters (see ak_api.cu)
   const double* U0[5];          // FOFC estimate of a later RK stage: U* = fa U0 + fb (U - dt div F);
   double fa, fb;                // U0[0] == nullptr: U* = U - dt div F (R9)
+  double* M[10];                // matter terms E, S_i, S_ij written by K6 on interior cells (M[0] == nullptr: none)
 };
 
 enum { ST_DFLOOR = 1, ST_TAUFLOOR = 2, ST_MAGCAP = 4, ST_RHOFLOOR = 8, ST_TFLOOR = 16,

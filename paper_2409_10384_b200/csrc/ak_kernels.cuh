@@ -82,7 +82,9 @@ __device__ __forceinline__ void load_met10(const Fields& f, long long c, double 
 // ---- K1 ------------------------------------------------------------------------------
 // EMF: also write the cell-centred EMFs of the final primitives (the arithmetic of k_cell_emf), so
 // that a stage that runs part (1) does not re-read W and the metric for them.
-template <bool EMF, int EOS = 0>
+// STRIDE: grid-stride loop for a capped grid (overlapped schedule only; the plain one-cell-per-thread
+// form is 0.05-0.12 ms faster on C4 and is what the serial schedule launches)
+template <bool EMF, int EOS = 0, bool STRIDE = false>
 __global__ void __launch_bounds__(128, AK_C2P_MINB) k_con2prim(const __grid_constant__ Par P,
                                                   const __grid_constant__ Fields f) {
   const int nt = P.nt;
@@ -92,8 +94,9 @@ __global__ void __launch_bounds__(128, AK_C2P_MINB) k_con2prim(const __grid_cons
 #endif
   // grid-stride: the launcher may cap the grid (a few blocks per SM) so that the kernel shares the SMs
   // with the flux sweeps of another chunk of blocks (ak_set_overlap)
-  for (long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x; c < ncell;
-       c += (long long)gridDim.x * blockDim.x) {
+  long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  do {
+  if (c >= ncell) return;
   const int i = (int)(c % nt);
   const long long row = c / nt;               // (m*nt + k)*nt + j
   const int j = (int)(row % nt);
@@ -167,7 +170,8 @@ __global__ void __launch_bounds__(128, AK_C2P_MINB) k_con2prim(const __grid_cons
   warp_count(f.stats + S_C2P_FAIL, (st & ST_FAIL) != 0);
   warp_count(f.stats + S_CONS_FLOOR, (st & (ST_DFLOOR | ST_TAUFLOOR | ST_MAGCAP)) != 0);
   warp_count(f.stats + S_PRIM_FLOOR, (st & (ST_RHOFLOOR | ST_TFLOOR)) != 0);
-  }
+  c += (long long)gridDim.x * blockDim.x;
+  } while (STRIDE);
 }
 
 // ---- computed-face range decoding ----------------------------------------------------
@@ -244,10 +248,11 @@ __device__ __forceinline__ double div_flux(const Fields& f, const Ix& ix, int v,
 }
 
 // ---- K3: FOFC estimate and test (DMP Eq. 12) -------------------------------
-template <int EOS = 0>
+template <int EOS = 0, bool STRIDE = false>
 __global__ void __launch_bounds__(128, AK_FOFC_MINB) k_fofc_test(const __grid_constant__ Par P,
                                                    const __grid_constant__ Fields f, double dt) {
-  for (long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;; tid += (long long)gridDim.x * blockDim.x) {
+  long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  do {
   int m, k, j, i;
   if (!decode_test(P, tid, m, k, j, i)) return;
   const Ix ix{P.nt, P.px};
@@ -303,7 +308,8 @@ __global__ void __launch_bounds__(128, AK_FOFC_MINB) k_fofc_test(const __grid_co
     base = __shfl_sync(act, base, leader);
     if (st != 0) f.list[base + __popc(bal & ((1u << lane) - 1u))] = (unsigned)c;
   }
-  }
+  tid += (long long)gridDim.x * blockDim.x;
+  } while (STRIDE);
 }
 
 // ---- K4: first-order re-solve of the faces of the flagged cells ("recalculate the fluxes
@@ -372,15 +378,16 @@ __global__ void __launch_bounds__(128) k_cell_emf(const __grid_constant__ Par P,
 
 // ---- K5: corner EMFs, component C3 (Gardiner & Stone 2005; DESIGN.md §3 O8) ------------------
 // a, b cyclic after C3.  Edge (ia, ib, ic): ia, ib in [is, ie+1], ic in [is, ie].
-template <int C3>
+template <int C3, bool STRIDE = false>
 __global__ void __launch_bounds__(128) k_ct(const __grid_constant__ Par P,
                                             const __grid_constant__ Fields f) {
   constexpr int a = (C3 + 1) % 3, b = (C3 + 2) % 3;
   const int n = P.n;
   const int ei = n + (C3 == 0 ? 0 : 1), ej = n + (C3 == 1 ? 0 : 1), ek = n + (C3 == 2 ? 0 : 1);
   const long long per = (long long)ei * ej * ek;
-  for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < per * P.nmb;
-       idx += (long long)gridDim.x * blockDim.x) {
+  long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  do {
+  if (idx >= per * P.nmb) return;
   const int m = (int)(idx / per);
   int r = (int)(idx - (long long)m * per);
   int p3[3];
@@ -419,7 +426,8 @@ __global__ void __launch_bounds__(128) k_ct(const __grid_constant__ Par P,
   const double dap = w2p * (Eaf_0m - Ec_mm) + (1.0 - w2p) * (Eaf_00 - Ec_m0);
   const double e = 0.25 * (Eaf_00 + Eaf_0m + Ebf_00 + Ebf_m0) + 0.25 * ((dbp - dbm) + (dap - dam));
   f.E[C3][ix.edge(C3, m, p3[2], p3[1], p3[0])] = e;
-  }
+  idx += (long long)gridDim.x * blockDim.x;
+  } while (STRIDE);
 }
 
 }  // namespace ak

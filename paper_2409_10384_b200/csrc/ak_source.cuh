@@ -9,13 +9,14 @@ namespace ak {
 #ifndef AK_SRC_MINB
 #define AK_SRC_MINB 4
 #endif
-template <int EOS = 0>
+template <int EOS = 0, bool STRIDE = false>
 __global__ void __launch_bounds__(128, AK_SRC_MINB) k_div_src(const __grid_constant__ Par P,
                                                  const __grid_constant__ Fields f) {
   const int n = P.n;
   const long long per = (long long)n * n * n;
-  for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < per * P.nmb;
-       idx += (long long)gridDim.x * blockDim.x) {
+  long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  do {
+  if (idx >= per * P.nmb) return;
   const int m = (int)(idx / per);
   int r = (int)(idx - (long long)m * per);
   const int i = r % n + P.is; r /= n;
@@ -64,6 +65,15 @@ __global__ void __launch_bounds__(128, AK_SRC_MINB) k_div_src(const __grid_const
     Sdd[I6[q]][J6[q]] = s; Sdd[J6[q]][I6[q]] = s;
     gim[I6[q]][J6[q]] = gi6[q]; gim[J6[q]][I6[q]] = gi6[q];
   }
+  // fused epilogue (S:§8(f) rank 4): the matter terms a spacetime (Z4c) right-hand side needs
+  // are E = tau + D, S_i and S_ij = T_ij of exactly this state -- written here, from the registers that hold
+  // them, instead of by a second pass over W and the metric (k_matter; same expressions, same bits)
+  if (f.M[0]) {
+    f.M[0][c] = cons[4] + cons[0];
+    f.M[1][c] = cons[1]; f.M[2][c] = cons[2]; f.M[3][c] = cons[3];
+    f.M[4][c] = Sdd[0][0]; f.M[5][c] = Sdd[0][1]; f.M[6][c] = Sdd[0][2];
+    f.M[7][c] = Sdd[1][1]; f.M[8][c] = Sdd[1][2]; f.M[9][c] = Sdd[2][2];
+  }
   // S^{ij} = gamma^{ik} S_kl gamma^{lj}
   double T[3][3], Suu[6];
 #pragma unroll
@@ -104,7 +114,8 @@ __global__ void __launch_bounds__(128, AK_SRC_MINB) k_div_src(const __grid_const
   du[4] = du[4] + sdet * (alp * KS - Sda);
 #pragma unroll
   for (int v = 0; v < 5; ++v) f.dU[v][c] = du[v];
-  }
+  idx += (long long)gridDim.x * blockDim.x;
+  } while (STRIDE);
 }
 
 // ---- matter terms for a spacetime solver: E = tau + D, S_i, S_ij = T_ij, undensitised,

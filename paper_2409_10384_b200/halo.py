@@ -9,9 +9,10 @@ mirrors like local blocks.  What travels is the ghost SLAB of each (block, neigh
 (include/ak.h: ak_halo_pack / ak_halo_unpack): one packed buffer and one message per peer and
 direction.  HaloPlan.exchange (whole blocks, nothing packed) is kept as the plain alternative.
 
-This module holds no arithmetic of the method: it builds index tables, moves bytes and sequences
-calls.  The stage operations are passed in (`ops`), so the same loop drives the CUDA library on
-GPUs and, in tests/test_multirank_cpu.py, the CPU oracle on gloo.
+This module holds no arithmetic and no sequencing of the method: it builds index tables and moves
+bytes.  The Runge-Kutta stage loop is the library's (ak_advance_hooked calls back here before every
+ghost fill); `ops` says whose loop runs, so the same plan drives the CUDA library on GPUs and, in
+tests/test_multirank_cpu.py, the CPU oracle on gloo.
 """
 import numpy as np
 
@@ -144,32 +145,15 @@ class HaloPlan:
             w.wait()
 
 
-# Shu-Osher weights: U <- a U0 + b (U + dt L(U))
-RK_A = {1: (0.0,), 2: (0.0, 0.5), 3: (0.0, 0.75, 1.0 / 3.0)}
-RK_B = {1: (1.0,), 2: (1.0, 0.5), 3: (1.0, 0.25, 2.0 / 3.0)}
-
-
 def advance(plan, ops, integrator, nsteps, dt, U, Bf, whole_blocks=False):
-    """The loop of ak_advance with a mirror refresh before every ghost fill.
-    ops: fill(U, Bf); rhs(U, Bf, U0_or_None, a, b, dt) -> (dU, E); update(a, b, dt, U0, B0, U, Bf, dU, E);
-         snapshot(U, Bf) -> (U0, B0) copies of the owned blocks' state; and what HaloPlan.refresh needs.
+    """nsteps steps of SSP-RK<integrator> over this rank's blocks with a mirror refresh before every ghost
+    fill.  The stage sequence (fill -> rhs with the stage's FOFC blend -> Shu-Osher update, with CT) is
+    not written here: it lives behind the boundary (ak_advance_hooked; the oracle's orc_advance_hooked in
+    the CPU tests), which calls back into `refresh` at the right places.
+    ops: advance(integrator, nsteps, dt, U, Bf, refresh), and what HaloPlan.refresh needs.
     whole_blocks: refresh the mirrors with HaloPlan.exchange instead of ghost slabs."""
     refresh = (lambda: plan.exchange(list(U) + list(Bf))) if whole_blocks else (lambda: plan.refresh(ops, U, Bf))
-    U0 = B0 = None
-    for _ in range(nsteps):
-        for s in range(integrator):
-            a, b = RK_A[integrator][s], RK_B[integrator][s]
-            refresh()
-            ops.fill(U, Bf)
-            dU, E = ops.rhs(U, Bf, None if s == 0 else U0, a, b, dt)
-            if s == 0 and integrator > 1:
-                U0, B0 = ops.snapshot(U, Bf)
-            if s == 0:
-                ops.update(0.0, 1.0, dt, U, Bf, U, Bf, dU, E)
-            else:
-                ops.update(a, b, dt, U0, B0, U, Bf, dU, E)
-    refresh()
-    ops.fill(U, Bf)
+    ops.advance(integrator, nsteps, dt, U, Bf, refresh)
 
 
 class AkOps:
@@ -208,17 +192,5 @@ class AkOps:
         if len(desc):
             self.ak.ak_halo_unpack(self.ctx, self._dev_desc(desc), buf, U, Bf)
 
-    def fill(self, U, Bf):
-        self.ak.ak_fill_ghosts(self.ctx, self.bc, U, Bf)
-
-    def rhs(self, U, Bf, U0, a, b, dt):
-        self.ak.ak_set_fofc_blend(self.ctx, U0, a, b)
-        self.ak.ak_rhs(self.ctx, U, Bf, self.W, 0, dt, self.dU, self.E, self.flag, None)
-        self.ak.ak_set_fofc_blend(self.ctx, None)
-        return self.dU, self.E
-
-    def snapshot(self, U, Bf):
-        return [u.clone() for u in U], [b.clone() for b in Bf]
-
-    def update(self, a, b, dt, U0, B0, U, Bf, dU, E):
-        self.ak.ak_stage_update(self.ctx, a, b, dt, U0, B0, U, Bf, dU, E)
+    def advance(self, integrator, nsteps, dt, U, Bf, refresh):
+        self.ak.ak_advance_hooked(self.ctx, integrator, nsteps, dt, self.bc, U, Bf, self.W, self.flag, refresh)

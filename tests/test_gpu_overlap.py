@@ -1,0 +1,192 @@
+"""GPU tests of round 2's boundary work: the overlapped schedule of ak_rhs (ak_set_overlap) gives the
+bits of the serial schedule and of the oracle; misaligned field pointers are AK_EINVAL, not a device
+fault; two live contexts of different block size share the TMA sweep instantiations safely."""
+import copy
+
+import numpy as np
+import pytest
+
+from oracle import pyoracle as orc
+from paper_2409_10384_b200 import workloads as wl
+
+import gpukit
+
+pytestmark = pytest.mark.gpu
+
+
+def _noise_batch(nblocks, n, seed0, frac=0.03):
+    """a batch of independent noise blocks (floors, flags, re-fluxed faces in every block)."""
+    ws = [wl.make_test_noise_block(seed=seed0 + b, n=n, frac=frac) for b in range(nblocks)]
+    w = copy.deepcopy(ws[0])
+    for k in ("U", "Bf", "adm"):
+        w[k] = [np.concatenate([x[k][q] for x in ws], axis=0) for q in range(len(ws[0][k]))]
+    w["dx"] = np.concatenate([x["dx"] for x in ws], axis=0)
+    w["params"] = dict(w["params"]); w["params"]["nmb"] = nblocks
+    w["dt_fofc"] = 2.0 * ws[0]["dt_fofc"]
+    return w
+
+
+@pytest.mark.parametrize("nchunks", [2, 3, 64])
+@pytest.mark.parametrize("eos", [None, dict(K0=0.15, gammas=[1.8, 2.4, 2.1], rho_breaks=[0.3, 1.0], gamma_th=1.6)])
+def test_overlapped_schedule_equals_serial_and_oracle(nchunks, eos):
+    """7 blocks in 2 / 3 (uneven) / 7 (clamped from 64) chunks; WENO-Z, HLLE, FOFC + DMP."""
+    import torch
+    from paper_2409_10384_b200 import ak
+    w = _noise_batch(7, 8, seed0=40)
+    over = dict(recon=2, dmp_M=1.1)
+    if eos is not None:
+        over["eos_hybrid"] = eos
+    U_in = [u.copy() for u in w["U"]]
+    with gpukit.GpuStage(copy.deepcopy(w), **over) as a, gpukit.GpuStage(copy.deepcopy(w), **over) as b:
+        a.rhs()
+        ak.ak_set_overlap(b.ctx, nchunks)
+        b.rhs()
+        ra, rb = a.result(), b.result()
+        for k in ("dU", "E", "W", "U"):
+            for x, y in zip(ra[k], rb[k]):
+                assert np.array_equal(x, y), k
+        assert np.array_equal(ra["flag"], rb["flag"]) and np.array_equal(ra["status"], rb["status"])
+        assert a.stats() == b.stats()
+        fa, fb = a.flux(), b.flux()
+        for x, y in zip(fa, fb):
+            assert np.array_equal(x, y)
+        # CT alone from the fluxes the overlapped stage left behind
+        E2 = [torch.zeros_like(e) for e in b.E]
+        ak.ak_emf(b.ctx, b.W, *E2)
+        torch.cuda.synchronize()
+        for x, y in zip(E2, b.E):
+            assert torch.equal(x, y)
+        # w_is_valid = 1 under overlap
+        b.rhs(w_is_valid=True)
+        rc = b.result()
+        for k in ("dU", "E"):
+            for x, y in zip(ra[k], rc[k]):
+                assert np.array_equal(x, y), k
+        sb = b.stats()
+        assert sb["n_c2p_fail"] == 0 and sb["n_cons_floor"] == 0      # part (1) skipped: no con2prim counts
+        assert sb["n_fofc_cells"] == a.stats()["n_fofc_cells"]
+        # back to the serial schedule
+        ak.ak_set_overlap(b.ctx, 0)
+        b.rhs(w_is_valid=True)
+        rd = b.result()
+        for x, y in zip(ra["dU"] + ra["E"], rd["dU"] + rd["E"]):
+            assert np.array_equal(x, y)
+    p = dict(w["params"]); p.update(over)
+    o = orc.rhs(orc.make_params(**p), w["dx"], w["U"], w["Bf"], w["adm"], w["dt_fofc"], nthreads=8)
+    o["U"] = w["U"]
+    gpukit.assert_parity(rb, o, U_in, label="overlap %d" % nchunks)
+    assert np.count_nonzero(o["flag"]) > 0
+
+
+def test_overlapped_advance_equals_serial():
+    """ak_advance (RK3, stage-blended FOFC estimate) under the overlapped schedule: same bits."""
+    import torch
+    from paper_2409_10384_b200 import ak
+    w = _noise_batch(4, 8, seed0=70, frac=0.01)
+    res = []
+    for nchunks in (0, 3):
+        with gpukit.GpuStage(copy.deepcopy(w), recon=2, dmp_M=1.1) as g:
+            ak.ak_set_overlap(g.ctx, nchunks)
+            fl = torch.zeros_like(g.flag)
+            ak.ak_advance(g.ctx, 3, 2, 0.02 / 8, (0, 1, 0), g.U, g.Bf, g.W, fl)
+            torch.cuda.synchronize()
+            res.append([t.cpu().numpy() for t in g.U + g.Bf + g.W] + [fl.cpu().numpy()])
+    for x, y in zip(*res):
+        assert np.array_equal(x, y)
+    assert np.count_nonzero(res[0][-1]) > 0
+
+
+def test_set_overlap_validation():
+    from paper_2409_10384_b200 import ak
+    w = wl.make_blocks("C0")
+    with gpukit.GpuStage(copy.deepcopy(w)) as g:
+        for bad in (-1, 65):
+            assert ak.lib().ak_set_overlap(g.ctx, bad) == ak.AK_EINVAL
+        assert ak.lib().ak_set_overlap(None, 2) == ak.AK_EINVAL
+        ak.ak_set_overlap(g.ctx, 8)           # one block: clamps to the serial schedule
+        g.rhs()
+        ra = g.result()
+    with gpukit.GpuStage(copy.deepcopy(w)) as h:
+        h.rhs()
+        rb = h.result()
+    for x, y in zip(ra["dU"] + ra["E"], rb["dU"] + rb["E"]):
+        assert np.array_equal(x, y)
+
+
+def test_misaligned_field_pointer_is_einval():
+    """base pointers 16-byte aligned, checked -> AK_EINVAL.  A view that starts one double
+    into an allocation is 8-byte aligned only; the TMA bulk copies would fault on it."""
+    import ctypes as C
+    import torch
+    from paper_2409_10384_b200 import ak
+    w = wl.make_blocks("C0")
+    with gpukit.GpuStage(copy.deepcopy(w)) as g:
+        def off(t):                       # same shape, base address + 8 bytes
+            big = torch.zeros(t.numel() + 2, dtype=t.dtype, device=t.device)
+            v = big[1:1 + t.numel()].view(t.shape)
+            assert v.data_ptr() % 16 == 8
+            return v
+        L = ak.lib()
+        u, b, wp = ak._struct(ak.AkCons, g.U), ak._struct(ak.AkFaceB, g.Bf), ak._struct(ak.AkPrim, g.W)
+        o = ak._struct(ak.AkRhsOut, g.dU + g.E + [g.flag, g.status, None])
+        assert L.ak_rhs(g.ctx, C.byref(u), C.byref(b), C.byref(wp), 0, 0.01, C.byref(o)) == ak.AK_OK
+        for which in ("U", "Bf", "W"):
+            args = dict(U=list(g.U), Bf=list(g.Bf), W=list(g.W))
+            args[which][1] = off(args[which][1])
+            u, b, wp = ak._struct(ak.AkCons, args["U"]), ak._struct(ak.AkFaceB, args["Bf"]), ak._struct(ak.AkPrim, args["W"])
+            assert L.ak_rhs(g.ctx, C.byref(u), C.byref(b), C.byref(wp), 0, 0.01, C.byref(o)) == ak.AK_EINVAL, which
+            assert L.ak_con2prim(g.ctx, C.byref(u), C.byref(b), C.byref(wp), None) == ak.AK_EINVAL, which
+        adm = list(g.adm); adm[7] = off(adm[7])
+        s = ak._struct(ak.AkAdm, adm)
+        assert L.ak_set_metric(g.ctx, C.byref(s)) == ak.AK_EINVAL
+        torch.cuda.synchronize()          # nothing faulted
+        g.rhs()                           # the context still works with its (aligned) arrays
+
+
+def test_two_contexts_of_different_block_size_interleaved():
+    """cudaFuncAttributeMaxDynamicSharedMemorySize belongs to the kernel function, not the context: a
+    32^3 context (larger x-sweep tile), then a 16^3 context, then the 32^3 one again — same WENO-Z
+    instantiations, different shared-memory needs.  (the attribute must never be lowered.)"""
+    w32 = wl.make_blocks("C2", blocks=[21])
+    w16 = wl.make_test_noise_block(seed=5, n=16, frac=0.01)
+    with gpukit.GpuStage(copy.deepcopy(w16), recon=2) as small0:
+        small0.rhs()
+        r16_first = small0.result()
+    with gpukit.GpuStage(copy.deepcopy(w32)) as big, gpukit.GpuStage(copy.deepcopy(w16), recon=2) as small:
+        big.rhs()
+        r1 = big.result()
+        small.rhs()
+        r16 = small.result()
+        big.rhs(w_is_valid=True)
+        r2 = big.result()
+        small.rhs(w_is_valid=True)
+    for x, y in zip(r1["dU"] + r1["E"], r2["dU"] + r2["E"]):
+        assert np.array_equal(x, y)
+    for x, y in zip(r16["dU"] + r16["E"], r16_first["dU"] + r16_first["E"]):
+        assert np.array_equal(x, y)
+
+
+def test_host_entry_without_primitives():
+    """ak_rhs_host with W = NULL returns dU/dt, E, masks and floored U as before and skips the copy of the
+    primitives (small batch: plain path; 32 blocks: the two-lane pipeline)."""
+    import torch
+    from paper_2409_10384_b200 import ak
+    for w in (wl.make_test_noise_block(seed=13, n=8, frac=0.02), wl.make_blocks("C3", blocks=list(range(192, 224)))):
+        with gpukit.GpuStage(copy.deepcopy(w)) as a:
+            a.rhs()
+            ra = a.result()
+            sh = a.sh
+            hU = [u.copy() for u in w["U"]]
+            hdU = [np.zeros(sh["cell"]) for _ in range(5)]
+            hE = [np.zeros(sh[k]) for k in ("ex", "ey", "ez")]
+            hflag = np.zeros(sh["cell"], dtype=np.uint8); hst = np.zeros(sh["cell"], dtype=np.uint8)
+            ak.ak_rhs_host(a.ctx, hU, w["Bf"], None, w["dt_fofc"], hdU, hE, hflag, hst)
+            for x, y in zip(hdU + hE + hU, ra["dU"] + ra["E"] + ra["U"]):
+                assert np.array_equal(x, y)
+            assert np.array_equal(hflag, ra["flag"]) and np.array_equal(hst, ra["status"])
+            # a partly filled W is a usage error
+            import ctypes as C
+            u, b = ak._struct(ak.AkCons, hU), ak._struct(ak.AkFaceB, w["Bf"])
+            wp = ak.AkPrim(); wp.rho = hdU[0].ctypes.data
+            o = ak._struct(ak.AkRhsOut, hdU + hE + [hflag, hst, None])
+            assert ak.lib().ak_rhs_host(a.ctx, C.byref(u), C.byref(b), C.byref(wp), 0.01, C.byref(o)) == ak.AK_EINVAL

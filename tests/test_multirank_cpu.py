@@ -150,20 +150,10 @@ class _OracleOps:
     def unpack(self, desc, buf, U, Bf):
         numpy_slabs(desc, [u.numpy() for u in U] + [b.numpy() for b in Bf], buf.numpy(), self.n, unpack=True)
 
-    def fill(self, U, Bf):
-        self.orc.exchange_ghosts(self.par, self.plan.local_nbr, self.bc, [u.numpy() for u in U], [b.numpy() for b in Bf])
-
-    def rhs(self, U, Bf, U0, a, b, dt):
-        r = self.orc.rhs_blend(self.par, self.dx, [u.numpy() for u in U], [x.numpy() for x in Bf], self.adm, dt,
-                               None if U0 is None else [u.numpy() for u in U0], a, b)
-        return r["dU"], r["E"]
-
-    def snapshot(self, U, Bf):
-        return [u.clone() for u in U], [b.clone() for b in Bf]
-
-    def update(self, a, b, dt, U0, B0, U, Bf, dU, E):
-        self.orc.stage_update(self.par, self.dx, a, b, dt, [u.numpy() for u in U0], [x.numpy() for x in B0],
-                              [u.numpy() for u in U], [x.numpy() for x in Bf], dU, E)
+    def advance(self, integrator, nsteps, dt, U, Bf, refresh):
+        # U, Bf: n_total blocks (own + mirrors), numpy views of the CPU tensors, advanced in place
+        self.orc.advance_hooked(self.par, self.dx, integrator, nsteps, dt, self.bc, self.plan.local_nbr,
+                                [u.numpy() for u in U], [b.numpy() for b in Bf], self.adm, refresh)
 
 
 def _halo_worker(rank, world, port, out, whole_blocks=False):
