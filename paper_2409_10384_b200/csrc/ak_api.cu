@@ -6,6 +6,7 @@
 #define AK_FLUX_TMA 1   // 1: TMA-staged sweeps (ak_flux_tma.cuh) when n is even and a face row fits a block
 #endif
 #include "ak_flux_tma.cuh"
+#include "ak_flux_pencil.cuh"
 #include "ak_driver.cuh"
 
 #include <cmath>
@@ -29,6 +30,9 @@ constexpr int MAXCH = 64;     // most chunks of an overlapped schedule (counter 
 #define AK_OV_CAP_CT_DEFAULT 4
 #define AK_OV_CAP_SRC_DEFAULT 2
 #define AK_OV_SMEM_PAD_DEFAULT 0
+#endif
+#ifndef AK_PENCIL_WI_DEFAULT
+#define AK_PENCIL_WI_DEFAULT 0      // x-lanes per block of the y/z pencil sweeps (even; 0 = k_flux_tma tiles)
 #endif
 
 struct Sizes {
@@ -62,6 +66,7 @@ struct ak_ctx {
   cudaEvent_t* ov_ev; int ov_nev;
   int cap[8];                   // grid caps (blocks) per kernel class in the overlapped schedule, 0 = none
   int sweep_smem_pad;           // bytes: dynamic shared memory the sweeps ask for at least when overlapped
+  int pencil_wi;                // y/z sweeps: x-lanes per block of k_flux_pencil (0: tile kernels k_flux_tma)
   // FOFC stage blend (ak_set_fofc_blend)
   const double* blendU0[5]; double blend_a, blend_b;
   // stage-driver registers (ak_advance), allocated on first use
@@ -278,10 +283,113 @@ int launch_flux_tma(ak_ctx* c, const Lane& L, int NA, unsigned grid, int bd, siz
                  : launch_flux_tma_eos<DIR, RECON, 0>(c, L, NA, grid, bd, smem);
 }
 
+// ---- y/z sweeps on whole pencils with tensor-map TMA (ak_flux_pencil.cuh) -------------------------------
+typedef CUresult (*TmapEncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                 const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                 CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+// the driver's encoder through the runtime (no link against libcuda); NULL if this driver has none
+TmapEncodeFn tmap_encoder() {
+  static TmapEncodeFn fn = nullptr;
+  static bool tried = false;
+  if (!tried) {
+    tried = true;
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+        q == cudaDriverEntryPointSuccess)
+      fn = (TmapEncodeFn)p;
+    cudaGetLastError();
+  }
+  return fn;
+}
+
+template <int DIR>
+bool pencil_maps(const Par& P, const Fields& f, int WI, PencilMaps& M) {
+  TmapEncodeFn enc = tmap_encoder();
+  if (!enc) return false;
+  constexpr int t1 = (DIR + 1) % 3, t2 = (DIR + 2) % 3;
+  const cuuint64_t nt = (cuuint64_t)P.nt;
+  const cuuint64_t dims[3] = {nt, nt, nt * (cuuint64_t)P.nmb};
+  const cuuint64_t strides[2] = {nt * 8, nt * nt * 8};                  // bytes, dimensions 1 and 2
+  const cuuint32_t box[3] = {(cuuint32_t)WI, DIR == 1 ? (cuuint32_t)nt : 1u, DIR == 1 ? 1u : (cuuint32_t)nt};
+  const cuuint32_t estr[3] = {1, 1, 1};
+  auto one = [&](CUtensorMap* m, const double* base) {
+    return enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<double*>(base), dims, strides, box, estr,
+               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+  };
+  const int var[7] = {0, 1, 2, 3, 4, 5 + t1, 5 + t2};
+  for (int v = 0; v < 7; ++v) if (!one(&M.w[v], f.W[var[v]])) return false;
+  for (int q = 0; q < 10; ++q) {
+    const int fld = q == 0 ? 6 : (q < 4 ? 6 + q : q - 4);               // alp, betx..betz, gxx..gzz
+    if (!one(&M.m[q], f.adm[fld])) return false;
+  }
+  return true;
+}
+
+template <int DIR, int RECON, int EOS>
+int launch_pencil_eos(ak_ctx* c, const Lane& L, const PencilMaps& M, int WI, int tile_d, int i_first, int ntile_i,
+                      unsigned grid, int bd, size_t smem) {
+  auto kern = k_flux_pencil<DIR, RECON, EOS>;
+  static int have[64] = {0};
+  const int r = raise_smem_attr(kern, c->hp.device, smem, have);
+  if (r != AK_OK) return r;
+  kern<<<grid, bd, smem, L.st>>>(L.P, L.f, M, WI, tile_d, i_first, ntile_i);
+  return AK_OK;
+}
+
+// returns AK_OK when launched, 1 when the pencil kernel does not apply (caller falls back)
+template <int DIR>
+int launch_pencil(ak_ctx* c, const Lane& L) {
+  const int n = L.P.n, nt = L.P.nt;
+  if (c->pencil_wi < 2 || n % 2 != 0) return 1;
+  // x-lanes [is-1, ie+1] = [3, n+4] in tiles of WI lanes starting at the even lane 2 (a box must start on
+  // a 16-byte boundary: an odd first lane faults).  WI: even, at most the configured width, the block within
+  // AK_PENCIL_MAXT threads, least lanes wasted, the wider the better.
+  const int i_first = 2, lanes = n + 3;
+  int WI = 0, waste = 1 << 30;
+  for (int w = 4; w <= c->pencil_wi; w += 2) {
+    if (((w * (n + 4) + 31) / 32) * 32 > AK_PENCIL_MAXT) break;
+    const int ws = (lanes + w - 1) / w * w - lanes;
+    if (ws <= waste) { waste = ws; WI = w; }
+  }
+  if (WI == 0) return 1;
+  const int bd = ((WI * (n + 4) + 31) / 32) * 32;
+  PencilMaps M;
+  if (!pencil_maps<DIR>(L.P, L.f, WI, M)) return 1;
+  const int ntile_i = (lanes + WI - 1) / WI;
+  const int tile_d = ((nt * WI + 15) / 16) * 16;
+  size_t dbl = (size_t)17 * tile_d + (size_t)7 * bd;
+  if ((size_t)21 * bd > dbl) dbl = (size_t)21 * bd;
+  const size_t smem = sizeof(double) * dbl;
+  if (smem > 200 * 1024) return 1;
+  const unsigned grid = (unsigned)((long long)L.P.nmb * (n + 2) * ntile_i);
+  int r;
+#define AK_PENCIL_CASE(RC)                                                                                       \
+  r = L.P.eos ? launch_pencil_eos<DIR, RC, 1>(c, L, M, WI, tile_d, i_first, ntile_i, grid, bd, smem)            \
+              : launch_pencil_eos<DIR, RC, 0>(c, L, M, WI, tile_d, i_first, ntile_i, grid, bd, smem)
+  switch (L.P.recon) {
+    case 0: AK_PENCIL_CASE(0); break;
+    case 1: AK_PENCIL_CASE(1); break;
+    case 3: AK_PENCIL_CASE(3); break;
+    case 4: AK_PENCIL_CASE(4); break;
+    default: AK_PENCIL_CASE(2); break;
+  }
+#undef AK_PENCIL_CASE
+  if (r != AK_OK) return r;
+  CK(cudaGetLastError());
+  return AK_OK;
+}
+
 template <int DIR>
 int launch_flux(ak_ctx* c, const Lane& L) {
   Timer t(c, KC_FX + DIR, L.st);
   const int n = L.P.n, nt = L.P.nt, e = n + 2;
+  if (DIR != 0 && c->pencil_wi > 0) {
+    const int pr = launch_pencil<(DIR == 0 ? 1 : DIR)>(c, L);
+    if (pr == AK_OK) { c->launches[KC_FX + DIR] += 1; return AK_OK; }
+    if (pr != 1) return pr;
+  }
   constexpr int AK_FLUX_CELL = (AK_FLUX_CELL_MASK >> DIR) & 1;
   // threads per row of a tile: faces (k_flux_tma) or cells (k_flux_tma_cell)
   const int nfi = AK_FLUX_CELL ? (DIR == 0 ? n + 4 : e) : (DIR == 0 ? n + 3 : e);
@@ -504,6 +612,7 @@ int ak_create(const ak_params* p, const double* dx3, ak_ctx** out) {
     c->cap[KC_CT] = nsm * envi("AK_OV_CAP_CT", AK_OV_CAP_CT_DEFAULT);
     c->cap[KC_SRC] = nsm * envi("AK_OV_CAP_SRC", AK_OV_CAP_SRC_DEFAULT);
     c->sweep_smem_pad = envi("AK_OV_SMEM_PAD", AK_OV_SMEM_PAD_DEFAULT);
+    c->pencil_wi = envi("AK_PENCIL_WI", AK_PENCIL_WI_DEFAULT);
   }
   Par& P = c->P;
   P.nmb = p->nmb; P.n = p->n; P.nt = p->n + 8; P.px = P.nt + 4; P.is = 4; P.ie = p->n + 3;

@@ -252,6 +252,26 @@ struct C2P {
     const double nuB = (1.0 + ahat) * (1.0 + qbar - mu * rbar2);
     return mu - 1.0 / (fmax(nuA, nuB) + mu * rbar2);
   }
+  // f(0), ideal gas: the master function at mu = +0 without the operations whose results are then known
+  // exactly -- x = 1/(1 + 0 bs2) = 1, W^ = 1/sqrt(1 - 0) = 1, (+-0)/2 = +-0 -- i.e. two reciprocals, a square
+  // root and a division fewer; every other operation of aux()/f() is kept as written (products with 0.0
+  // included, so that signed zeros come out as they do in the full evaluation): the same bits.  Needs finite
+  // r2, bs2, rb2 and v^2 = fmin(0 rbar2, v0sq) == 0 (f0_ok); leaves the trial state (x .. eps) alone.
+  __device__ __forceinline__ bool f0_ok() const {
+    const double rb0 = r2 + 0.0 * rb2;
+    return EOS == 0 && isfinite(r2) && isfinite(bs2) && isfinite(rb2) && fmin(0.0 * rb0, v0sq) == 0.0;
+  }
+  __device__ __forceinline__ double f0() const {
+    const double rb0 = r2 + 0.0 * rb2;                              // rbar2
+    const double qb0 = q - 0.5 * bs2 - 0.0 * (bs2 * r2 - rb2);      // qbar
+    const double vs0 = fmin(0.0 * rb0, v0sq);                       // +-0
+    const double ep0 = (qb0 - 0.0 * rb0) + vs0;                     // W^ (qbar - mu rbar2) + (v^2 W^2)/(1 + W^)
+    const double e = fmax(ep0, 0.0);
+    const double ahat = ddiv(gm1 * e, 1.0 + e);
+    const double nuA = (1.0 + ahat) * (1.0 + e);
+    const double nuB = (1.0 + ahat) * (1.0 + qb0 - 0.0 * rb0);
+    return 0.0 - 1.0 / (fmax(nuA, nuB) + 0.0 * rb0);
+  }
   // auxiliary function whose root bounds mu from above when r >= h0
   __device__ __forceinline__ double fa(double mu) const {
     const double xx = 1.0 / (1.0 + mu * bs2);
@@ -377,15 +397,21 @@ __device__ __forceinline__ int c2p_cell(const Par& P, const Met3& g, double Ut[5
     double mu = 0.0;
     if (ok) {
       const double f_hi = s.f(mu_hi);
-      const double f_lo = s.f(0.0);
+      // f(0) by its shortcut where that is exact; it does not touch the trial state, which then still
+      // belongs to mu_hi
+      bool state_hi = true;
+      double f_lo;
+      if (s.f0_ok()) f_lo = s.f0();
+      else { f_lo = s.f(0.0); state_hi = false; }
       if (!(f_hi >= 0.0) || !(f_lo < 0.0)) ok = false;
-      else if (f_hi == 0.0) mu = mu_hi;
+      else if (f_hi == 0.0) { mu = mu_hi; if (!state_hi) s.aux(mu); }
       else ok = illinois<false, EOS>(s, 0.0, mu_hi, f_lo, f_hi, P.max_iter, P.tol, mu);
     }
     if (!ok) {
       status |= ST_FAIL;
     } else {
-      s.aux(mu);
+      // the trial state (x, rbar2, qbar, W^, eps) is that of mu already: the root finder returns the last
+      // point it evaluated, so aux(mu) would recompute the same values (one reciprocal pair, sqrt, division)
       rho = D * s.iW;
       pr = eos_P<EOS>(P, rho, s.eps);
       const double c = mu * rB * iD;
