@@ -23,7 +23,8 @@ EXPORTS = ("ak_create", "ak_set_metric", "ak_con2prim", "ak_rhs", "ak_emf", "ak_
            "ak_probe_fp64", "ak_destroy", "ak_strerror", "ak_version",
            "ak_set_fofc_blend", "ak_fill_ghosts", "ak_stage_update", "ak_advance", "ak_set_neighbors",
            "ak_matter_sources", "ak_halo_slab_elems", "ak_halo_pack", "ak_halo_unpack",
-           "ak_set_eos_hybrid", "ak_set_overlap", "ak_advance_hooked")
+           "ak_set_eos_hybrid", "ak_set_overlap", "ak_advance_hooked",
+           "ak_set_exact_shortcuts")
 BC_PERIODIC, BC_OUTFLOW = 0, 1
 
 _dp = C.POINTER(C.c_double)
@@ -125,6 +126,7 @@ def lib():
         L.ak_matter_sources.argtypes = [C.c_void_p, C.POINTER(AkPrim), C.POINTER(AkMatter)]
         L.ak_set_neighbors.argtypes = [C.c_void_p, C.POINTER(C.c_int), C.c_int]
         L.ak_set_overlap.argtypes = [C.c_void_p, C.c_int]
+        L.ak_set_exact_shortcuts.argtypes = [C.c_void_p, C.c_int]
         _lib = L
     return _lib
 
@@ -220,6 +222,11 @@ def ak_rhs_host(ctx, U, Bf, W, dt_fofc, dU, E, fofc_flag=None, c2p_status=None):
     w = _struct(AkPrim, W) if W is not None else AkPrim()
     o = _struct(AkRhsOut, list(dU) + list(E) + [fofc_flag, c2p_status, None])
     _chk(lib().ak_rhs_host(ctx, C.byref(u), C.byref(b), C.byref(w), float(dt_fofc), C.byref(o)), "ak_rhs_host")
+
+
+def ak_set_exact_shortcuts(ctx, mask):
+    """bit 0: skip the reconstruction of all-zero fields, bit 1: static-cell con2prim (include/ak.h)."""
+    _chk(lib().ak_set_exact_shortcuts(ctx, int(mask)), "ak_set_exact_shortcuts")
 
 
 def ak_set_overlap(ctx, nchunks):

@@ -623,6 +623,8 @@ int ak_create(const ak_params* p, const double* dx3, ak_ctx** out) {
   P.dmp_M = p->dmp_M; P.dmp_iM = p->dmp_M > 0.0 ? 1.0 / p->dmp_M : 0.0;
   P.max_iter = p->c2p_max_iter; P.tol = p->c2p_tol;
   P.recon = p->recon; P.riemann = p->riemann; P.fofc = p->fofc; P.fofc_riemann = p->fofc_riemann;
+  P.shortcuts = 3;
+  if (const char* v = getenv("AK_EXACT_SHORTCUTS")) P.shortcuts = atoi(v) & 3;
   const long long nt = P.nt, px = P.px, nb = P.nmb;
   c->sz.cell = nb * nt * nt * nt;
   c->sz.xf = nb * nt * nt * px; c->sz.yf = nb * nt * (nt + 1) * nt; c->sz.zf = nb * (nt + 1) * nt * nt;
@@ -848,6 +850,13 @@ int ak_rhs(ak_ctx* c, const ak_cons* U, const ak_faceB* Bf, const ak_prim* W, in
   return AK_OK;
 }
 
+int ak_set_exact_shortcuts(ak_ctx* c, int mask) {
+  if (!c || mask < 0 || mask > 3) return AK_EINVAL;
+  c->P.shortcuts = mask;
+  for (int l = 0; l < 2; ++l) if (c->lane[l]) c->lane[l]->P.shortcuts = mask;
+  return AK_OK;
+}
+
 int ak_set_overlap(ak_ctx* c, int nchunks) {
   if (!c || nchunks < 0 || nchunks > MAXCH) return AK_EINVAL;
   CK(cudaSetDevice(c->hp.device));
@@ -972,6 +981,7 @@ static int rhs_host_pipelined(ak_ctx* c, int chunk, double* const hU[5], const d
       const int r = ak_create(&hp, c->host_dx, &c->lane[l]);
       if (r != AK_OK) { cudaStreamDestroy(st); return r; }
       copy_eos(c->lane[l]->P, c->P);
+      c->lane[l]->P.shortcuts = c->P.shortcuts;
       // staging kinds: 0..4 U (cell), 5..7 Bf (xf yf zf), 8..15 W (cell), 16..20 dU (cell), 21..23 E (ex ey ez)
       for (int q = 0; q < 24; ++q) {
         const int kind = q < 5 ? 0 : (q < 8 ? 1 + (q - 5) : (q < 21 ? 0 : 4 + (q - 21)));

@@ -25,6 +25,8 @@ struct Par {
   int max_iter;
   double tol;
   int recon, riemann, fofc, fofc_riemann;
+  int shortcuts;                // exact data-dependent shortcuts (ak_set_exact_shortcuts): bit 0 reconstruction of
+                                // all-zero fields, bit 1 root solve of static unmagnetised cells; same bits out
   // piecewise-polytropic hybrid EOS (ak_set_eos_hybrid; reading R29); eos = 0: ideal gas
   int eos, nseg;
   double ppK[4], ppG[4], ppa[4], pprb[3];   // K_i, Gamma_i, eps offsets a_i, breakpoints
@@ -224,6 +226,10 @@ struct C2P {
   const Par* par; double D;    // EOS = 1 only: the EOS constants and the conserved density (rho^ = D / W^)
   // quantities at a trial mu
   double x, rbar2, qbar, vsq, iW, What, eps;
+  // static unmagnetised cell (r2 = bs2 = rb2 = 0): x = W^ = 1, rbar2 = 0, eps = qbar = q for every mu, so
+  // f(mu) = mu - inv with inv = 1/nu the same number at every evaluation: after one full evaluation
+  // (which leaves inv and the trial state behind) the root finder runs on that one subtraction
+  bool stat; double inv;
   __device__ __forceinline__ void aux(double mu) {
     x = 1.0 / (1.0 + mu * bs2);
     rbar2 = r2 * x * x + mu * x * (1.0 + x) * rb2;
@@ -235,6 +241,7 @@ struct C2P {
   }
   // master function f(mu)
   __device__ __forceinline__ double f(double mu) {
+    if (stat) return mu - inv;
     aux(mu);
     double e, ahat;
     if (EOS == 0) {
@@ -250,7 +257,8 @@ struct C2P {
     }
     const double nuA = (1.0 + ahat) * (1.0 + e) * iW;
     const double nuB = (1.0 + ahat) * (1.0 + qbar - mu * rbar2);
-    return mu - 1.0 / (fmax(nuA, nuB) + mu * rbar2);
+    inv = 1.0 / (fmax(nuA, nuB) + mu * rbar2);
+    return mu - inv;
   }
   // f(0), ideal gas: the master function at mu = +0 without the operations whose results are then known
   // exactly -- x = 1/(1 + 0 bs2) = 1, W^ = 1/sqrt(1 - 0) = 1, (+-0)/2 = +-0 -- i.e. two reciprocals, a square
@@ -387,6 +395,7 @@ __device__ __forceinline__ int c2p_cell(const Par& P, const Met3& g, double Ut[5
     s.rb2 = rB * rB * iD;
     s.v0sq = ddiv(s.r2, 1.0 + s.r2);
     s.gm1 = P.gm1;
+    s.stat = false; s.inv = 0.0;
     bool ok = true;
     double mu_hi = 1.0;
     if (!(s.r2 < 1.0)) {
@@ -397,11 +406,15 @@ __device__ __forceinline__ int c2p_cell(const Par& P, const Met3& g, double Ut[5
     double mu = 0.0;
     if (ok) {
       const double f_hi = s.f(mu_hi);
+      // S = 0 and B = 0 exactly (static atmosphere, the bulk of a merger grid): every later evaluation is
+      // mu - inv with the inv this one left behind (q > 0 keeps eps = qbar away from a signed zero)
+      s.stat = (P.shortcuts & 2) && s.r2 == 0.0 && s.bs2 == 0.0 && s.rb2 == 0.0 && s.q > 0.0;
       // f(0) by its shortcut where that is exact; it does not touch the trial state, which then still
       // belongs to mu_hi
       bool state_hi = true;
       double f_lo;
-      if (s.f0_ok()) f_lo = s.f0();
+      if (s.stat) f_lo = 0.0 - s.inv;
+      else if (s.f0_ok()) f_lo = s.f0();
       else { f_lo = s.f(0.0); state_hi = false; }
       if (!(f_hi >= 0.0) || !(f_lo < 0.0)) ok = false;
       else if (f_hi == 0.0) { mu = mu_hi; if (!state_hi) s.aux(mu); }

@@ -59,7 +59,8 @@ k_flux_pencil(const __grid_constant__ Par P, const __grid_constant__ Fields f,
   const int o = bid % e + P.is - 1;       // fixed transverse index: k (y sweep) or j (z sweep)
   const int m = bid / e;
   const int i0 = i_first + ti * WI;       // first x-lane of the tile
-  if (t == 0) { mbar_init(&mbar, 1); mbar_init(&mbarM, 1); }
+  __shared__ unsigned nzacc;
+  if (t == 0) { mbar_init(&mbar, 1); mbar_init(&mbarM, 1); nzacc = 0; }
   __syncthreads();
   if (t == 0) {
     const int c1 = DIR == 1 ? 0 : o, c2 = DIR == 1 ? m * nt + o : m * nt;
@@ -84,6 +85,7 @@ k_flux_pencil(const __grid_constant__ Par P, const __grid_constant__ Fields f,
     Bfd = __ldg(f.Bf[DIR] + fi);
   }
   mbar_wait(&mbar, 0);
+  const unsigned nzm = (RECON != 0 && (P.shortcuts & 1)) ? tile_nonzero_mask(sW, tile_d, nt * WI, &nzacc) : ALWAYS_NZ;
   double qm[7];
   if (active) {
 #pragma unroll
@@ -91,6 +93,7 @@ k_flux_pencil(const __grid_constant__ Par P, const __grid_constant__ Fields f,
       const double* w = sW + v * tile_d + t;     // cell cc-2 of this lane; cells cc-2 .. cc+2 at stride WI
       double qp;
       if (RECON == 0) { qm[v] = qp = w[2 * WI]; }
+      else if (!((nzm >> v) & 1u)) { qm[v] = qp = 0.0; }     // the field is +0.0 on the whole tile
       else recon<RECON>(w[0], w[WI], w[2 * WI], w[3 * WI], w[4 * WI], qm[v], qp);
       sQ[v * (int)blockDim.x + t] = qp;
     }

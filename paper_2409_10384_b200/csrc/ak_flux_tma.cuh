@@ -49,6 +49,26 @@ __device__ __forceinline__ void mbar_wait(uint64_t* b, unsigned parity) {
       "}\n" ::"r"(smem_u32(b)), "r"(parity) : "memory");
 }
 
+// Which of the five often-zero fields of a staged tile (slots 1, 2, 3 = u^i and 5, 6 = the transverse B~cc)
+// hold anything but +0.0: bit s of the result.  A field that is +0.0 on the whole tile reconstructs to
+// +0.0 on both sides of every face, for every scheme here, so its reconstruction can be
+// skipped: static atmosphere (u = 0) and unmagnetised regions (B = 0) are most of a merger grid.  All
+// threads of the block call this (one barrier); `acc` is a shared word that thread 0 zeroed before an
+// earlier barrier.
+__device__ __forceinline__ unsigned tile_nonzero_mask(const double* sW, int slot_stride, int count, unsigned* acc) {
+  unsigned nz = 0;
+  for (int q = threadIdx.x; q < count; q += (int)blockDim.x) {
+#pragma unroll
+    for (int s = 1; s < 7; ++s)
+      if (s != 4) nz |= (unsigned)(__double_as_longlong(sW[(size_t)s * slot_stride + q]) != 0LL) << s;
+  }
+  nz = __reduce_or_sync(0xffffffffu, nz);
+  if ((threadIdx.x & 31) == 0 && nz) atomicOr(acc, nz);
+  __syncthreads();
+  return *acc | 0x11u;                  // slots 0 (rho) and 4 (P) are never zero: always reconstructed
+}
+constexpr unsigned ALWAYS_NZ = 0x7fu;   // every slot reconstructed (shortcut off)
+
 template <int DIR, int RECON, int EOS = 0>
 __global__ void __launch_bounds__(TMA_THREADS, AK_TMA_MINB)
 k_flux_tma(const __grid_constant__ Par P, const __grid_constant__ Fields f, int NA) {
@@ -76,7 +96,8 @@ k_flux_tma(const __grid_constant__ Par P, const __grid_constant__ Fields f, int 
   else if (DIR == 1) { baseW = ix.cell(m, o, d0 - 3, 0); baseM = ix.cell(m, o, d0 - 1, 0); rs = nt; }
   else { baseW = ix.cell(m, d0 - 3, o, 0); baseM = ix.cell(m, d0 - 1, o, 0); rs = (long long)nt * nt; }
   const unsigned rowb = (unsigned)(nt * sizeof(double));
-  if (t == 0) mbar_init(&mbar, 1);
+  __shared__ unsigned nzacc;
+  if (t == 0) { mbar_init(&mbar, 1); nzacc = 0; }
   __syncthreads();
   if (t == 0) mbar_arrive_expect_tx(&mbar, (unsigned)(7 * nW + 10 * nM) * rowb);
   // ---- one bulk copy per (field, row)
@@ -106,6 +127,7 @@ k_flux_tma(const __grid_constant__ Par P, const __grid_constant__ Fields f, int 
     Bfd = __ldg(f.Bf[DIR] + fi);
   }
   mbar_wait(&mbar, 0);
+  const unsigned nzm = (RECON != 0 && (P.shortcuts & 1)) ? tile_nonzero_mask(sW, maxW * nt, nW * nt, &nzacc) : ALWAYS_NZ;
 #if !AK_FLUX_PARK
   if (!active) return;
 #endif
@@ -118,6 +140,8 @@ k_flux_tma(const __grid_constant__ Par P, const __grid_constant__ Fields f, int 
       const int s = DIR == 0 ? 1 : nt;
       if (RECON == 0) {
         sL[v] = w[2 * s]; sR[v] = w[3 * s];
+      } else if (!((nzm >> v) & 1u)) {
+        sL[v] = 0.0; sR[v] = 0.0;           // the field is +0.0 on the whole tile
       } else {
         const double q0 = w[0], q1 = w[s], q2 = w[2 * s], q3 = w[3 * s], q4 = w[4 * s], q5 = w[5 * s];
         double qm, qp;
@@ -198,7 +222,8 @@ k_flux_tma_cell(const __grid_constant__ Par P, const __grid_constant__ Fields f,
   else if (DIR == 1) { baseW = ix.cell(m, o, d0 - 3, 0); baseM = ix.cell(m, o, d0 - 1, 0); rs = nt; }
   else { baseW = ix.cell(m, d0 - 3, o, 0); baseM = ix.cell(m, d0 - 1, o, 0); rs = (long long)nt * nt; }
   const unsigned rowb = (unsigned)(nt * sizeof(double));
-  if (t == 0) mbar_init(&mbar, 1);
+  __shared__ unsigned nzacc;
+  if (t == 0) { mbar_init(&mbar, 1); nzacc = 0; }
   __syncthreads();
   if (t == 0) mbar_arrive_expect_tx(&mbar, (unsigned)(7 * nW + 10 * nM) * rowb);
   const int ncW = 7 * nW, nc = ncW + 10 * nM;
@@ -230,6 +255,7 @@ k_flux_tma_cell(const __grid_constant__ Par P, const __grid_constant__ Fields f,
     Bfd = __ldg(f.Bf[DIR] + fi);
   }
   mbar_wait(&mbar, 0);
+  const unsigned nzm = (RECON != 0 && (P.shortcuts & 1)) ? tile_nonzero_mask(sW, maxW * nt, nW * nt, &nzacc) : ALWAYS_NZ;
   double qm[7];
   if (active) {
 #pragma unroll
@@ -239,6 +265,7 @@ k_flux_tma_cell(const __grid_constant__ Par P, const __grid_constant__ Fields f,
       const int s = DIR == 0 ? 1 : nt;
       double qp;
       if (RECON == 0) { qm[v] = qp = w[2 * s]; }
+      else if (!((nzm >> v) & 1u)) { qm[v] = qp = 0.0; }     // the field is +0.0 on the whole tile
       else recon<RECON>(w[0], w[s], w[2 * s], w[3 * s], w[4 * s], qm[v], qp);
       sQ[v * TMA_THREADS + t] = qp;
     }

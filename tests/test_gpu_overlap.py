@@ -190,3 +190,63 @@ def test_host_entry_without_primitives():
             wp = ak.AkPrim(); wp.rho = hdU[0].ctypes.data
             o = ak._struct(ak.AkRhsOut, hdU + hE + [hflag, hst, None])
             assert ak.lib().ak_rhs_host(a.ctx, C.byref(u), C.byref(b), C.byref(wp), 0.01, C.byref(o)) == ak.AK_EINVAL
+
+
+@pytest.mark.parametrize("name,blocks,over", [
+    ("C2", [0, 21, 22, 41, 42, 63], dict()),                     # atmosphere blocks (u = 0, B = 0 exactly), star rims
+    ("C1", [0, 7], dict(recon=2)),                               # static star: every velocity exactly zero
+    ("C1", [0, 7], dict(recon=4, riemann=0)),
+    ("C3", [192 + 21, 64 + 21, 21], dict(recon=3)),              # nothing is zero: the shortcuts never fire
+])
+def test_exact_shortcuts_leave_every_bit_unchanged(name, blocks, over):
+    """ak_set_exact_shortcuts: skipping the reconstruction of fields that are +0.0 on a whole tile and
+    running the root find of static unmagnetised cells on f(mu) = mu - const are exact: mask 0 (full
+    arithmetic), 1, 2 and 3 give the same bits in every output, fluxes included, and equal the oracle."""
+    from paper_2409_10384_b200 import ak
+    w = wl.make_blocks(name, blocks=blocks)
+    U_in = [u.copy() for u in w["U"]]
+    res = []
+    for mask in (0, 1, 2, 3):
+        with gpukit.GpuStage(copy.deepcopy(w), **over) as g:
+            ak.ak_set_exact_shortcuts(g.ctx, mask)
+            g.rhs()
+            res.append((g.result(), g.flux(), g.stats()))
+    r0, f0, s0 = res[0]
+    for r, fl, st in res[1:]:
+        for k in ("dU", "E", "W", "U"):
+            for x, y in zip(r0[k], r[k]):
+                assert np.array_equal(x, y), k
+        assert np.array_equal(r0["flag"], r["flag"]) and np.array_equal(r0["status"], r["status"])
+        for x, y in zip(f0, fl):
+            assert np.array_equal(x, y)
+        assert st == s0
+    p = dict(w["params"]); p.update(over)
+    o = orc.rhs(orc.make_params(**p), w["dx"], w["U"], w["Bf"], w["adm"], w["dt_fofc"], nthreads=8)
+    o["U"] = w["U"]
+    gpukit.assert_parity(res[-1][0], o, U_in, label=name + " shortcuts")
+
+
+def test_exact_shortcuts_with_signed_zeros_and_partly_zero_fields():
+    """Hand-made primitives through ak_rhs(w_is_valid = 1): u^x = -0.0 in some cells (not +0.0: must be
+    reconstructed), u^z zero except one cell, B~cc zero on half the block, u^y = +0.0 everywhere.  Mask 0
+    and 3 must agree bit for bit, signs of zeros in the fluxes included."""
+    import torch
+    from paper_2409_10384_b200 import ak
+    w = wl.make_test_noise_block(seed=3, n=8, frac=0.0)
+    outs = []
+    for mask in (0, 3):
+        with gpukit.GpuStage(copy.deepcopy(w), recon=2, dmp_M=1.1) as g:
+            ak.ak_set_exact_shortcuts(g.ctx, mask)
+            g.con2prim()
+            nt = 16
+            g.W[1].zero_(); g.W[1][0, 5:9, 3:7, 2:12] = -0.0
+            g.W[2].zero_()
+            g.W[3].zero_(); g.W[3][0, 8, 8, 8] = 0.01
+            g.W[5][0, :, :, : nt // 2] = 0.0; g.W[6][0, : nt // 2] = 0.0; g.W[7].zero_()
+            g.rhs(w_is_valid=True)
+            outs.append((g.result(), g.flux()))
+    (ra, fa), (rb, fb) = outs
+    for x, y in zip(ra["dU"] + ra["E"] + fa, rb["dU"] + rb["E"] + fb):
+        assert np.array_equal(x, y)
+        assert np.array_equal(np.signbit(x), np.signbit(y))
+    assert np.array_equal(ra["flag"], rb["flag"])
