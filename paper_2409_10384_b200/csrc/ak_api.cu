@@ -66,6 +66,7 @@ struct ak_ctx {
   cudaEvent_t* ov_ev; int ov_nev;
   int cap[8];                   // grid caps (blocks) per kernel class in the overlapped schedule, 0 = none
   int sweep_smem_pad;           // bytes: dynamic shared memory the sweeps ask for at least when overlapped
+  int tile_tm;                  // tile kernels: stage tiles with tensor-map box copies (1) or row by row (0)
   int pencil_wi;                // y/z sweeps: x-lanes per block of k_flux_pencil (0: tile kernels k_flux_tma)
   // FOFC stage blend (ak_set_fofc_blend)
   const double* blendU0[5]; double blend_a, blend_b;
@@ -250,39 +251,6 @@ int launch_c2p(ak_ctx* c, const Lane& L, bool with_emf) {
   return AK_OK;
 }
 
-#ifndef AK_FLUX_CELL_MASK
-#define AK_FLUX_CELL_MASK 1   // bit d set: direction d uses the reconstruct-once variant k_flux_tma_cell
-#endif
-
-// cudaFuncAttributeMaxDynamicSharedMemorySize belongs to the kernel function (per device), not to a
-// context: two live contexts of different n share one instantiation and need different amounts.  The
-// attribute is therefore only ever RAISED, tracked per instantiation and device.
-template <typename K>
-int raise_smem_attr(K kern, int device, size_t smem, int (&have)[64]) {
-  const int d = device & 63;
-  if ((int)smem > have[d]) {
-    CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    have[d] = (int)smem;
-  }
-  return AK_OK;
-}
-
-template <int DIR, int RECON, int EOS>
-int launch_flux_tma_eos(ak_ctx* c, const Lane& L, int NA, unsigned grid, int bd, size_t smem) {
-  auto kern = ((AK_FLUX_CELL_MASK >> DIR) & 1) ? k_flux_tma_cell<DIR, RECON, EOS> : k_flux_tma<DIR, RECON, EOS>;
-  static int have[64] = {0};
-  const int r = raise_smem_attr(kern, c->hp.device, smem, have);
-  if (r != AK_OK) return r;
-  kern<<<grid, bd, smem, L.st>>>(L.P, L.f, NA);
-  return AK_OK;
-}
-
-template <int DIR, int RECON>
-int launch_flux_tma(ak_ctx* c, const Lane& L, int NA, unsigned grid, int bd, size_t smem) {
-  return L.P.eos ? launch_flux_tma_eos<DIR, RECON, 1>(c, L, NA, grid, bd, smem)
-                 : launch_flux_tma_eos<DIR, RECON, 0>(c, L, NA, grid, bd, smem);
-}
-
 // ---- y/z sweeps on whole pencils with tensor-map TMA (ak_flux_pencil.cuh) -------------------------------
 typedef CUresult (*TmapEncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
@@ -303,28 +271,71 @@ TmapEncodeFn tmap_encoder() {
   return fn;
 }
 
+// Tensor maps of the 17 fields of a sweep of direction DIR: every cell field is the rank-3 tensor
+// (i: nt, j: nt, K = m nt + k); boxW / boxM are the boxes of the primitive and of the metric fields.
 template <int DIR>
-bool pencil_maps(const Par& P, const Fields& f, int WI, PencilMaps& M) {
+bool field_maps(const Par& P, const Fields& f, const cuuint32_t boxW[3], const cuuint32_t boxM[3], TileMaps& M) {
   TmapEncodeFn enc = tmap_encoder();
   if (!enc) return false;
   constexpr int t1 = (DIR + 1) % 3, t2 = (DIR + 2) % 3;
   const cuuint64_t nt = (cuuint64_t)P.nt;
   const cuuint64_t dims[3] = {nt, nt, nt * (cuuint64_t)P.nmb};
   const cuuint64_t strides[2] = {nt * 8, nt * nt * 8};                  // bytes, dimensions 1 and 2
-  const cuuint32_t box[3] = {(cuuint32_t)WI, DIR == 1 ? (cuuint32_t)nt : 1u, DIR == 1 ? 1u : (cuuint32_t)nt};
   const cuuint32_t estr[3] = {1, 1, 1};
-  auto one = [&](CUtensorMap* m, const double* base) {
+  auto one = [&](CUtensorMap* m, const double* base, const cuuint32_t* box) {
     return enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<double*>(base), dims, strides, box, estr,
                CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
   };
   const int var[7] = {0, 1, 2, 3, 4, 5 + t1, 5 + t2};
-  for (int v = 0; v < 7; ++v) if (!one(&M.w[v], f.W[var[v]])) return false;
+  for (int v = 0; v < 7; ++v) if (!one(&M.w[v], f.W[var[v]], boxW)) return false;
   for (int q = 0; q < 10; ++q) {
     const int fld = q == 0 ? 6 : (q < 4 ? 6 + q : q - 4);               // alp, betx..betz, gxx..gzz
-    if (!one(&M.m[q], f.adm[fld])) return false;
+    if (!one(&M.m[q], f.adm[fld], boxM)) return false;
   }
   return true;
+}
+
+#ifndef AK_FLUX_CELL_MASK
+#define AK_FLUX_CELL_MASK 1   // bit d set: direction d uses the reconstruct-once variant k_flux_tma_cell
+#endif
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize belongs to the kernel function (per device), not to a
+// context: two live contexts of different n share one instantiation and need different amounts.  The
+// attribute is therefore only ever RAISED, tracked per instantiation and device.
+template <typename K>
+int raise_smem_attr(K kern, int device, size_t smem, int (&have)[64]) {
+  const int d = device & 63;
+  if ((int)smem > have[d]) {
+    CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    have[d] = (int)smem;
+  }
+  return AK_OK;
+}
+
+template <int DIR, int RECON, int EOS>
+int launch_flux_tma_eos(ak_ctx* c, const Lane& L, int NA, unsigned grid, int bd, size_t smem, const TileMaps& M,
+                        int use_tm) {
+  auto kern = ((AK_FLUX_CELL_MASK >> DIR) & 1) ? k_flux_tma_cell<DIR, RECON, EOS> : k_flux_tma<DIR, RECON, EOS>;
+  static int have[64] = {0};
+  const int r = raise_smem_attr(kern, c->hp.device, smem, have);
+  if (r != AK_OK) return r;
+  kern<<<grid, bd, smem, L.st>>>(L.P, L.f, NA, M, use_tm);
+  return AK_OK;
+}
+
+template <int DIR, int RECON>
+int launch_flux_tma(ak_ctx* c, const Lane& L, int NA, unsigned grid, int bd, size_t smem, const TileMaps& M,
+                    int use_tm) {
+  return L.P.eos ? launch_flux_tma_eos<DIR, RECON, 1>(c, L, NA, grid, bd, smem, M, use_tm)
+                 : launch_flux_tma_eos<DIR, RECON, 0>(c, L, NA, grid, bd, smem, M, use_tm);
+}
+
+template <int DIR>
+bool pencil_maps(const Par& P, const Fields& f, int WI, PencilMaps& M) {
+  const cuuint32_t nt = (cuuint32_t)P.nt;
+  const cuuint32_t box[3] = {(cuuint32_t)WI, DIR == 1 ? nt : 1u, DIR == 1 ? 1u : nt};
+  return field_maps<DIR>(P, f, box, box, M);
 }
 
 template <int DIR, int RECON, int EOS>
@@ -401,7 +412,18 @@ int launch_flux(ak_ctx* c, const Lane& L) {
     const int tiles = (nfd + namax - 1) / namax;
     const int NA = (nfd + tiles - 1) / tiles;
     const int maxW = DIR == 0 ? NA : NA + 5, maxM = DIR == 0 ? NA : NA + 1;
-    size_t smem = sizeof(double) * ((size_t)(7 * maxW + 10 * maxM) * nt + (AK_FLUX_CELL ? 7 * TMA_THREADS : 0));
+    size_t smem = sizeof(double) * ((size_t)7 * tile_slot(maxW, nt) + (size_t)10 * tile_slot(maxM, nt) +
+                                    (AK_FLUX_CELL ? 7 * TMA_THREADS : 0));
+    // the tile as 17 tensor-map box copies (one per field) when the driver can encode them, else row by row
+    TileMaps M;
+    int use_tm = 0;
+    if (c->tile_tm) {
+      const cuuint32_t unt = (cuuint32_t)nt;
+      const cuuint32_t bW[3] = {unt, DIR == 2 ? 1u : (cuuint32_t)maxW, DIR == 2 ? (cuuint32_t)maxW : 1u};
+      const cuuint32_t bM[3] = {unt, DIR == 2 ? 1u : (cuuint32_t)maxM, DIR == 2 ? (cuuint32_t)maxM : 1u};
+      use_tm = field_maps<DIR>(L.P, L.f, bW, bM, M) ? 1 : 0;
+    }
+    if (!use_tm) memset(&M, 0, sizeof(M));
     if (AK_FLUX_CELL ? AK_FLUXC_PARK : AK_FLUX_PARK) {   // the spent tile is reused as 21 doubles of parking space per thread
       const size_t park = sizeof(double) * 21 * (size_t)TMA_THREADS;
       if (park > smem) smem = park;
@@ -416,11 +438,11 @@ int launch_flux(ak_ctx* c, const Lane& L) {
       const int bd = ((rows * nfi + 31) / 32) * 32;
       int r;
       switch (L.P.recon) {
-        case 0: r = launch_flux_tma<DIR, 0>(c, L, NA, grid, bd, smem); break;
-        case 1: r = launch_flux_tma<DIR, 1>(c, L, NA, grid, bd, smem); break;
-        case 3: r = launch_flux_tma<DIR, 3>(c, L, NA, grid, bd, smem); break;
-        case 4: r = launch_flux_tma<DIR, 4>(c, L, NA, grid, bd, smem); break;
-        default: r = launch_flux_tma<DIR, 2>(c, L, NA, grid, bd, smem); break;
+        case 0: r = launch_flux_tma<DIR, 0>(c, L, NA, grid, bd, smem, M, use_tm); break;
+        case 1: r = launch_flux_tma<DIR, 1>(c, L, NA, grid, bd, smem, M, use_tm); break;
+        case 3: r = launch_flux_tma<DIR, 3>(c, L, NA, grid, bd, smem, M, use_tm); break;
+        case 4: r = launch_flux_tma<DIR, 4>(c, L, NA, grid, bd, smem, M, use_tm); break;
+        default: r = launch_flux_tma<DIR, 2>(c, L, NA, grid, bd, smem, M, use_tm); break;
       }
       if (r != AK_OK) return r;
       CK(cudaGetLastError());
@@ -613,6 +635,7 @@ int ak_create(const ak_params* p, const double* dx3, ak_ctx** out) {
     c->cap[KC_SRC] = nsm * envi("AK_OV_CAP_SRC", AK_OV_CAP_SRC_DEFAULT);
     c->sweep_smem_pad = envi("AK_OV_SMEM_PAD", AK_OV_SMEM_PAD_DEFAULT);
     c->pencil_wi = envi("AK_PENCIL_WI", AK_PENCIL_WI_DEFAULT);
+    c->tile_tm = envi("AK_TILE_TENSORMAP", 1);
   }
   Par& P = c->P;
   P.nmb = p->nmb; P.n = p->n; P.nt = p->n + 8; P.px = P.nt + 4; P.is = 4; P.ie = p->n + 3;

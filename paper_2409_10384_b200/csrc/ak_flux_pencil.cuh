@@ -30,17 +30,7 @@ namespace ak {
 #define AK_PENCIL_MINB 3
 #endif
 
-struct PencilMaps {
-  CUtensorMap w[7];     // rho, u^x, u^y, u^z, P, B~cc^{t1}, B~cc^{t2} of this direction
-  CUtensorMap m[10];    // alp, betx, bety, betz, gxx .. gzz
-};
-
-__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, int c0, int c1, int c2, uint64_t* bar) {
-  asm volatile(
-      "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
-      ::"r"(smem_u32(dst)), "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar))
-      : "memory");
-}
+typedef TileMaps PencilMaps;   // the same 17 fields, boxes of WI lanes x nt cells
 
 // tile_d: doubles per field tile in shared memory (nt * WI rounded up to a multiple of 16: 128-byte tiles)
 template <int DIR, int RECON, int EOS = 0>

@@ -13,6 +13,7 @@
 // Shared layout: [field][row][nt] doubles; lanes run along i: conflict-free.
 #pragma once
 #include <cstdint>
+#include <cuda.h>
 #include "ak_kernels.cuh"
 
 namespace ak {
@@ -69,16 +70,36 @@ __device__ __forceinline__ unsigned tile_nonzero_mask(const double* sW, int slot
 }
 constexpr unsigned ALWAYS_NZ = 0x7fu;   // every slot reconstructed (shortcut off)
 
+// Tensor maps of the 17 fields a sweep stages (host: ak_api.cu, cuTensorMapEncodeTiled).  Every cell field is
+// the rank-3 tensor (i: nt, j: nt, K = m nt + k) of doubles; the box is the whole tile of one field, so a
+// block issues 17 tensor copies (cp.async.bulk.tensor.3d, SASS UTMALDG) instead of one 1-D bulk copy per
+// (field, row) -- about 200 per tile, whose issue cost showed once the arithmetic shrank (profiles/r2_final.md).
+struct TileMaps {
+  CUtensorMap w[7];     // rho, u^x, u^y, u^z, P, B~cc^{t1}, B~cc^{t2} of this direction
+  CUtensorMap m[10];    // alp, betx, bety, betz, gxx .. gzz
+};
+__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, int c0, int c1, int c2, uint64_t* bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+      ::"r"(smem_u32(dst)), "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar))
+      : "memory");
+}
+// doubles per field slot of a tile: rows * nt rounded up to 16 (tensor copies want 128-byte destinations)
+__host__ __device__ __forceinline__ int tile_slot(int rows, int nt) { return ((rows * nt + 15) / 16) * 16; }
+
+// use_tm != 0: the tile comes as 17 tensor-map box copies (maps); else as one bulk copy per (field, row)
 template <int DIR, int RECON, int EOS = 0>
 __global__ void __launch_bounds__(TMA_THREADS, AK_TMA_MINB)
-k_flux_tma(const __grid_constant__ Par P, const __grid_constant__ Fields f, int NA) {
+k_flux_tma(const __grid_constant__ Par P, const __grid_constant__ Fields f, int NA,
+           const __grid_constant__ TileMaps maps, int use_tm) {
   extern __shared__ __align__(128) double sm[];
   __shared__ uint64_t mbar;
   const int nt = P.nt, e = P.n + 2, t = threadIdx.x;
   constexpr int t1 = (DIR + 1) % 3, t2 = (DIR + 2) % 3;
   const int maxW = DIR == 0 ? NA : NA + 5, maxM = DIR == 0 ? NA : NA + 1;
-  double* sW = sm;                             // [7][maxW][nt]
-  double* sM = sm + 7 * maxW * nt;             // [10][maxM][nt]
+  const int slotW = tile_slot(maxW, nt), slotM = tile_slot(maxM, nt);
+  double* sW = sm;                             // [7][slotW]   (maxW rows of nt)
+  double* sM = sm + 7 * slotW;                 // [10][slotM]  (maxM rows of nt)
   // ---- which tile
   const int nfd = DIR == 0 ? e : P.n + 3;      // extent that NA tiles: rows (x) or faces along d (y,z)
   const int tiles = (nfd + NA - 1) / NA;
@@ -99,6 +120,21 @@ k_flux_tma(const __grid_constant__ Par P, const __grid_constant__ Fields f, int 
   __shared__ unsigned nzacc;
   if (t == 0) { mbar_init(&mbar, 1); nzacc = 0; }
   __syncthreads();
+  if (use_tm) {
+    // ---- one tensor copy per field: the box holds maxW (maxM) rows whether or not the tile is ragged
+    if (t < 32) {                                                   // lanes 0..16 of warp 0: one field each
+      if (t == 0) mbar_arrive_expect_tx(&mbar, (unsigned)(7 * maxW + 10 * maxM) * rowb);
+      __syncwarp();
+      const int K = DIR == 2 ? m * nt + d0 : m * nt + o;            // plane coordinate of tile row 0 ...
+      if (t < 7) {
+        const int cW1 = DIR == 0 ? d0 : (DIR == 1 ? d0 - 3 : o), cW2 = DIR == 2 ? K - 3 : K;
+        tma_load_3d(sW + (size_t)t * slotW, &maps.w[t], 0, cW1, cW2, &mbar);
+      } else if (t < 17) {
+        const int cM1 = DIR == 0 ? d0 : (DIR == 1 ? d0 - 1 : o), cM2 = DIR == 2 ? K - 1 : K;
+        tma_load_3d(sM + (size_t)(t - 7) * slotM, &maps.m[t - 7], 0, cM1, cM2, &mbar);
+      }
+    }
+  } else {
   if (t == 0) mbar_arrive_expect_tx(&mbar, (unsigned)(7 * nW + 10 * nM) * rowb);
   // ---- one bulk copy per (field, row)
   const int ncW = 7 * nW, nc = ncW + 10 * nM;
@@ -106,13 +142,14 @@ k_flux_tma(const __grid_constant__ Par P, const __grid_constant__ Fields f, int 
     if (c < ncW) {
       const int v = c / nW, r = c - v * nW;
       const int fld = v < 5 ? v : (v == 5 ? 5 + t1 : 5 + t2);
-      bulk_copy_g2s(sW + ((size_t)v * maxW + r) * nt, f.W[fld] + baseW + r * rs, rowb, &mbar);
+      bulk_copy_g2s(sW + (size_t)v * slotW + r * nt, f.W[fld] + baseW + r * rs, rowb, &mbar);
     } else {
       const int cc = c - ncW;
       const int q = cc / nM, r = cc - q * nM;
       const int fld = q == 0 ? 6 : (q < 4 ? 6 + q : q - 4);   // alp, betx..betz, gxx..gzz
-      bulk_copy_g2s(sM + ((size_t)q * maxM + r) * nt, f.adm[fld] + baseM + r * rs, rowb, &mbar);
+      bulk_copy_g2s(sM + (size_t)q * slotM + r * nt, f.adm[fld] + baseM + r * rs, rowb, &mbar);
     }
+  }
   }
   // ---- this thread's face
   const int nfi = DIR == 0 ? P.n + 3 : e;      // faces per shared row
@@ -127,7 +164,7 @@ k_flux_tma(const __grid_constant__ Par P, const __grid_constant__ Fields f, int 
     Bfd = __ldg(f.Bf[DIR] + fi);
   }
   mbar_wait(&mbar, 0);
-  const unsigned nzm = (RECON != 0 && (P.shortcuts & 1)) ? tile_nonzero_mask(sW, maxW * nt, nW * nt, &nzacc) : ALWAYS_NZ;
+  const unsigned nzm = (RECON != 0 && (P.shortcuts & 1)) ? tile_nonzero_mask(sW, slotW, nW * nt, &nzacc) : ALWAYS_NZ;
 #if !AK_FLUX_PARK
   if (!active) return;
 #endif
@@ -136,7 +173,7 @@ k_flux_tma(const __grid_constant__ Par P, const __grid_constant__ Fields f, int 
 #pragma unroll
     for (int v = 0; v < 7; ++v) {
       // six stencil cells f-3 .. f+2: along i in one row (x) or one per shared row (y, z)
-      const double* w = DIR == 0 ? sW + ((size_t)v * maxW + a) * nt + ii - 3 : sW + ((size_t)v * maxW + a) * nt + ii;
+      const double* w = DIR == 0 ? sW + (size_t)v * slotW + a * nt + ii - 3 : sW + (size_t)v * slotW + a * nt + ii;
       const int s = DIR == 0 ? 1 : nt;
       if (RECON == 0) {
         sL[v] = w[2 * s]; sR[v] = w[3 * s];
@@ -153,7 +190,7 @@ k_flux_tma(const __grid_constant__ Par P, const __grid_constant__ Fields f, int 
     }
 #pragma unroll
     for (int q = 0; q < 10; ++q) {
-      const double* g = DIR == 0 ? sM + ((size_t)q * maxM + a) * nt + ii - 1 : sM + ((size_t)q * maxM + a) * nt + ii;
+      const double* g = DIR == 0 ? sM + (size_t)q * slotM + a * nt + ii - 1 : sM + (size_t)q * slotM + a * nt + ii;
       mL[q] = g[0];
       mR[q] = g[DIR == 0 ? 1 : nt];
     }
@@ -198,15 +235,17 @@ k_flux_tma(const __grid_constant__ Par P, const __grid_constant__ Fields f, int 
 #endif
 template <int DIR, int RECON, int EOS = 0>
 __global__ void __launch_bounds__(TMA_THREADS, AK_TMAC_MINB)
-k_flux_tma_cell(const __grid_constant__ Par P, const __grid_constant__ Fields f, int NA) {
+k_flux_tma_cell(const __grid_constant__ Par P, const __grid_constant__ Fields f, int NA,
+                const __grid_constant__ TileMaps maps, int use_tm) {
   extern __shared__ __align__(128) double sm[];
   __shared__ uint64_t mbar;
   const int nt = P.nt, e = P.n + 2, t = threadIdx.x;
   constexpr int t1 = (DIR + 1) % 3, t2 = (DIR + 2) % 3;
   const int maxW = DIR == 0 ? NA : NA + 5, maxM = DIR == 0 ? NA : NA + 1;
-  double* sW = sm;                             // [7][maxW][nt]
-  double* sM = sm + 7 * maxW * nt;             // [10][maxM][nt]
-  double* sQ = sM + 10 * maxM * nt;            // [7][TMA_THREADS]
+  const int slotW = tile_slot(maxW, nt), slotM = tile_slot(maxM, nt);
+  double* sW = sm;                             // [7][slotW]   (maxW rows of nt)
+  double* sM = sm + 7 * slotW;                 // [10][slotM]  (maxM rows of nt)
+  double* sQ = sM + 10 * slotM;                // [7][TMA_THREADS]
   const int nfd = DIR == 0 ? e : P.n + 3;
   const int tiles = (nfd + NA - 1) / NA;
   int bid = blockIdx.x;
@@ -225,19 +264,34 @@ k_flux_tma_cell(const __grid_constant__ Par P, const __grid_constant__ Fields f,
   __shared__ unsigned nzacc;
   if (t == 0) { mbar_init(&mbar, 1); nzacc = 0; }
   __syncthreads();
+  if (use_tm) {
+    if (t < 32) {                                                   // lanes 0..16 of warp 0: one field each
+      if (t == 0) mbar_arrive_expect_tx(&mbar, (unsigned)(7 * maxW + 10 * maxM) * rowb);
+      __syncwarp();
+      const int K = DIR == 2 ? m * nt + d0 : m * nt + o;            // plane coordinate of tile row 0 ...
+      if (t < 7) {
+        const int cW1 = DIR == 0 ? d0 : (DIR == 1 ? d0 - 3 : o), cW2 = DIR == 2 ? K - 3 : K;
+        tma_load_3d(sW + (size_t)t * slotW, &maps.w[t], 0, cW1, cW2, &mbar);
+      } else if (t < 17) {
+        const int cM1 = DIR == 0 ? d0 : (DIR == 1 ? d0 - 1 : o), cM2 = DIR == 2 ? K - 1 : K;
+        tma_load_3d(sM + (size_t)(t - 7) * slotM, &maps.m[t - 7], 0, cM1, cM2, &mbar);
+      }
+    }
+  } else {
   if (t == 0) mbar_arrive_expect_tx(&mbar, (unsigned)(7 * nW + 10 * nM) * rowb);
   const int ncW = 7 * nW, nc = ncW + 10 * nM;
   for (int c = t; c < nc; c += (int)blockDim.x) {
     if (c < ncW) {
       const int v = c / nW, r = c - v * nW;
       const int fld = v < 5 ? v : (v == 5 ? 5 + t1 : 5 + t2);
-      bulk_copy_g2s(sW + ((size_t)v * maxW + r) * nt, f.W[fld] + baseW + r * rs, rowb, &mbar);
+      bulk_copy_g2s(sW + (size_t)v * slotW + r * nt, f.W[fld] + baseW + r * rs, rowb, &mbar);
     } else {
       const int cc = c - ncW;
       const int q = cc / nM, r = cc - q * nM;
       const int fld = q == 0 ? 6 : (q < 4 ? 6 + q : q - 4);
-      bulk_copy_g2s(sM + ((size_t)q * maxM + r) * nt, f.adm[fld] + baseM + r * rs, rowb, &mbar);
+      bulk_copy_g2s(sM + (size_t)q * slotM + r * nt, f.adm[fld] + baseM + r * rs, rowb, &mbar);
     }
+  }
   }
   // ---- this thread's cell: row a of the tile, index ii along x
   const int nci = DIR == 0 ? P.n + 4 : e;              // cells per row of threads
@@ -255,13 +309,13 @@ k_flux_tma_cell(const __grid_constant__ Par P, const __grid_constant__ Fields f,
     Bfd = __ldg(f.Bf[DIR] + fi);
   }
   mbar_wait(&mbar, 0);
-  const unsigned nzm = (RECON != 0 && (P.shortcuts & 1)) ? tile_nonzero_mask(sW, maxW * nt, nW * nt, &nzacc) : ALWAYS_NZ;
+  const unsigned nzm = (RECON != 0 && (P.shortcuts & 1)) ? tile_nonzero_mask(sW, slotW, nW * nt, &nzacc) : ALWAYS_NZ;
   double qm[7];
   if (active) {
 #pragma unroll
     for (int v = 0; v < 7; ++v) {
       // stencil c-2 .. c+2: along i in the row (x); shared rows a .. a+4 (y, z: my cell is row a+2)
-      const double* w = DIR == 0 ? sW + ((size_t)v * maxW + a) * nt + ii - 2 : sW + ((size_t)v * maxW + a) * nt + ii;
+      const double* w = DIR == 0 ? sW + (size_t)v * slotW + a * nt + ii - 2 : sW + (size_t)v * slotW + a * nt + ii;
       const int s = DIR == 0 ? 1 : nt;
       double qp;
       if (RECON == 0) { qm[v] = qp = w[2 * s]; }
@@ -281,7 +335,7 @@ k_flux_tma_cell(const __grid_constant__ Par P, const __grid_constant__ Fields f,
     for (int v = 0; v < 7; ++v) sL[v] = sQ[v * TMA_THREADS + t - back];
 #pragma unroll
     for (int q = 0; q < 10; ++q) {
-      const double* g = DIR == 0 ? sM + ((size_t)q * maxM + a) * nt + ii - 1 : sM + ((size_t)q * maxM + a - 1) * nt + ii;
+      const double* g = DIR == 0 ? sM + (size_t)q * slotM + a * nt + ii - 1 : sM + (size_t)q * slotM + (a - 1) * nt + ii;
       mL[q] = g[0];
       mR[q] = g[DIR == 0 ? 1 : nt];
     }
