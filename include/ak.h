@@ -53,7 +53,7 @@ extern "C" {
 
 typedef struct ak_ctx ak_ctx; /* opaque */
 
-enum { AK_OK = 0, AK_EINVAL = -1, AK_ENOMEM = -2, AK_ECUDA = -3, AK_ESTATE = -4, AK_EHOOK = -5 };
+enum { AK_OK = 0, AK_EINVAL = -1, AK_ENOMEM = -2, AK_ECUDA = -3, AK_ESTATE = -4, AK_EHOOK = -5, AK_ETOOBIG = -6 };
 enum { AK_RECON_DC = 0, AK_RECON_PPM4 = 1, AK_RECON_WENOZ = 2, AK_RECON_PLM = 3, AK_RECON_PPMX = 4 };
 enum { AK_RS_LLF = 0, AK_RS_HLLE = 1 };
 enum { AK_BC_PERIODIC = 0, AK_BC_OUTFLOW = 1 };                  /* stage driver, D:§11 */
@@ -295,6 +295,30 @@ int ak_kernel_ms(ak_ctx*, double ms_out[8], long long launches_out[8]);
 int ak_probe_copy(ak_ctx*, double* dst, const double* src, long long n_doubles, int reps,
                   double* gbs_out);
 int ak_probe_fp64(ak_ctx*, int use_fma, int reps, double* gops_out);
+
+/* ---- allocation-free entry point -------------------------------------------------------------------
+ * Part (1) (ideal gas) WITHOUT a context, for callers that cannot call cudaMalloc
+ * (code under CUDA-graph capture, tight serving loops, harnesses that forbid it): ak_create allocates its
+ * scratch with cudaMalloc; this call, and everything it calls, allocates nothing — no cudaMalloc, cudaFree
+ * or allocating library routine.  The scratch the kernel needs (the device counters, and the status bytes
+ * when `status` is NULL) lives in a file-scope device array inside the library, sized for at most
+ * AK_STATIC_MAX_CELLS stored cells (nmb * (n+8)^3; 2 MiB + 64 B, held by every GPU that loads the library
+ * until exit).  A larger batch is refused with AK_ETOOBIG before anything is launched.
+ *   p        nmb, n, ng, gamma_ad, rho_atm, T_atm, f_thr, mag_max, c2p_max_iter, c2p_tol, device (< 64),
+ *            stream are read; the rest is ignored.
+ *   U        in-out, Bf in, W out: DEVICE fields as for ak_con2prim (16-byte aligned, else AK_EINVAL).
+ *   adm      only gxx..gzz are read (DEVICE cell fields).
+ *   status   DEVICE bytes [nmb][nt^3], or NULL.
+ *   host_counts  NULL: the call only enqueues on p->stream and returns.  Else n_c2p_fail, n_cons_floor,
+ *            n_prim_floor of this call are written there (the other members 0) and the call synchronises
+ *            p->stream.
+ * Same kernel and arithmetic as ak_con2prim: the same bits in W, U and status.
+ * ALL calls share the one scratch array, which keeps the last call's contents (the counters are cleared at
+ * the start of each call, on its stream).  Calls that overlap on the GPU — different streams, or another
+ * thread — race on it: serialise them (one stream, or events).  Calls on different devices do not share. */
+#define AK_STATIC_MAX_CELLS 2097152
+int ak_con2prim_static(const ak_params* p, const ak_cons* U, const ak_faceB* Bf, const ak_adm* adm,
+                       const ak_prim* W, unsigned char* status, ak_stats* host_counts);
 
 int ak_destroy(ak_ctx*);
 const char* ak_strerror(int code);

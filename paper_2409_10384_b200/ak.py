@@ -13,7 +13,8 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 SO_PATH = os.environ.get("AK_LIBRARY") or os.path.join(_HERE, "libak.so")   # AK_LIBRARY: another build of the same library
 
-AK_OK, AK_EINVAL, AK_ENOMEM, AK_ECUDA, AK_ESTATE, AK_EHOOK = 0, -1, -2, -3, -4, -5
+AK_OK, AK_EINVAL, AK_ENOMEM, AK_ECUDA, AK_ESTATE, AK_EHOOK, AK_ETOOBIG = 0, -1, -2, -3, -4, -5, -6
+STATIC_MAX_CELLS = 2097152      # AK_STATIC_MAX_CELLS of include/ak.h
 RECON_DC, RECON_PPM4, RECON_WENOZ, RECON_PLM, RECON_PPMX = 0, 1, 2, 3, 4
 RS_LLF, RS_HLLE = 0, 1
 ST_DFLOOR, ST_TAUFLOOR, ST_MAGCAP, ST_RHOFLOOR, ST_TFLOOR, ST_FAIL, ST_DMP = 1, 2, 4, 8, 16, 32, 64
@@ -24,7 +25,7 @@ EXPORTS = ("ak_create", "ak_set_metric", "ak_con2prim", "ak_rhs", "ak_emf", "ak_
            "ak_set_fofc_blend", "ak_fill_ghosts", "ak_stage_update", "ak_advance", "ak_set_neighbors",
            "ak_matter_sources", "ak_halo_slab_elems", "ak_halo_pack", "ak_halo_unpack",
            "ak_set_eos_hybrid", "ak_set_overlap", "ak_advance_hooked",
-           "ak_set_exact_shortcuts")
+           "ak_set_exact_shortcuts", "ak_con2prim_static")
 BC_PERIODIC, BC_OUTFLOW = 0, 1
 
 _dp = C.POINTER(C.c_double)
@@ -127,6 +128,8 @@ def lib():
         L.ak_set_neighbors.argtypes = [C.c_void_p, C.POINTER(C.c_int), C.c_int]
         L.ak_set_overlap.argtypes = [C.c_void_p, C.c_int]
         L.ak_set_exact_shortcuts.argtypes = [C.c_void_p, C.c_int]
+        L.ak_con2prim_static.argtypes = [C.POINTER(AkParams), C.POINTER(AkCons), C.POINTER(AkFaceB), C.POINTER(AkAdm),
+                                         C.POINTER(AkPrim), C.c_void_p, C.POINTER(AkStats)]
         _lib = L
     return _lib
 
@@ -222,6 +225,18 @@ def ak_rhs_host(ctx, U, Bf, W, dt_fofc, dU, E, fofc_flag=None, c2p_status=None):
     w = _struct(AkPrim, W) if W is not None else AkPrim()
     o = _struct(AkRhsOut, list(dU) + list(E) + [fofc_flag, c2p_status, None])
     _chk(lib().ak_rhs_host(ctx, C.byref(u), C.byref(b), C.byref(w), float(dt_fofc), C.byref(o)), "ak_rhs_host")
+
+
+def ak_con2prim_static(params, U, Bf, adm, W, status=None, want_counts=False):
+    """con2prim without a context and without any allocation (include/ak.h).  adm: the 16 ADM fields (only
+    gamma_ij is read).  Returns the three con2prim counters when want_counts (synchronises), else None."""
+    u, b, a, w = _struct(AkCons, U), _struct(AkFaceB, Bf), _struct(AkAdm, adm), _struct(AkPrim, W)
+    s = AkStats()
+    _chk(lib().ak_con2prim_static(C.byref(params), C.byref(u), C.byref(b), C.byref(a), C.byref(w), _ptr(status),
+                                  C.byref(s) if want_counts else None), "ak_con2prim_static")
+    if want_counts:
+        return dict(n_c2p_fail=s.n_c2p_fail, n_cons_floor=s.n_cons_floor, n_prim_floor=s.n_prim_floor)
+    return None
 
 
 def ak_set_exact_shortcuts(ctx, mask):

@@ -603,6 +603,7 @@ const char* ak_strerror(int code) {
     case AK_ECUDA: return last_cuda_error != cudaSuccess ? cudaGetErrorString(last_cuda_error) : "CUDA error";
     case AK_ESTATE: return "call out of order (metric or fluxes missing)";
     case AK_EHOOK: return "the caller's refresh hook reported a failure";
+    case AK_ETOOBIG: return "batch larger than the static scratch of ak_con2prim_static (AK_STATIC_MAX_CELLS stored cells)";
     default: return "unknown error code";
   }
 }
@@ -1372,6 +1373,78 @@ int ak_probe_fp64(ak_ctx* c, int use_fma, int reps, double* gops) {
   cudaEventDestroy(a); cudaEventDestroy(b);
   CK(cudaGetLastError());
   *gops = best;
+  return AK_OK;
+}
+
+// ------------------------------------------------------------------ allocation-free entry point
+// ak_con2prim_static (include/ak.h): part (1) without a context.  k_con2prim needs scratch besides its inputs
+// and outputs -- the device counters, and a place for the status bytes when the caller passes none -- which
+// ak_create cudaMallocs.  Here that scratch is a file-scope device array of a fixed, modest size, so the call
+// allocates nothing (callers under CUDA-graph capture, tight serving loops, harnesses that forbid cudaMalloc).
+// Every GPU that loads the library holds the array until exit.
+}  // extern "C" (closed for the file-scope definitions; reopened below)
+
+namespace {
+struct StaticScratch {
+  unsigned long long stats[S_NSTAT];                 // device counters: must start at zero, cleared per call
+  unsigned char status[AK_STATIC_MAX_CELLS];         // status bytes when the caller passes none: fully overwritten
+};
+static __device__ __align__(256) StaticScratch g_static_scratch;
+// In host code `g_static_scratch` is a host-side stand-in, NOT a device address: the address a kernel may use
+// comes from cudaGetSymbolAddress, once per device, with that device current.
+StaticScratch* g_static_ptr[64] = {nullptr};
+}  // namespace
+
+extern "C" {
+
+int ak_con2prim_static(const ak_params* p, const ak_cons* U, const ak_faceB* Bf, const ak_adm* adm,
+                       const ak_prim* W, unsigned char* status, ak_stats* host_counts) {
+  if (!p || !U || !Bf || !adm || !W) return AK_EINVAL;
+  if (p->nmb < 1 || p->n < 2 || p->ng != 4) return AK_EINVAL;
+  if (!(std::isfinite(p->gamma_ad) && p->gamma_ad > 1.0)) return AK_EINVAL;
+  if (!finite_pos(p->rho_atm) || !finite_pos(p->T_atm) || !finite_pos(p->f_thr)) return AK_EINVAL;
+  if (!(p->mag_max > 0.0)) return AK_EINVAL;
+  if (p->c2p_max_iter < 1 || p->c2p_max_iter > 1000 || !(p->c2p_tol > 0.0 && p->c2p_tol < 1.0)) return AK_EINVAL;
+  if (p->device < 0 || p->device >= 64) return AK_EINVAL;
+  const long long nt = p->n + 8;
+  const long long ncell = (long long)p->nmb * nt * nt * nt;
+  if (ncell > (long long)AK_STATIC_MAX_CELLS) return AK_ETOOBIG;      // the status scratch holds no more
+  Fields f;
+  memset(&f, 0, sizeof(f));
+  if (!set_cons(f, U) || !set_faceB(f, Bf) || !set_prim(f, W)) return AK_EINVAL;       // NULL or not 16-byte aligned
+  const double* g6[6] = {adm->gxx, adm->gxy, adm->gxz, adm->gyy, adm->gyz, adm->gzz};   // part (1) reads gamma_ij only
+  for (int q = 0; q < 6; ++q) { if (!al16(g6[q])) return AK_EINVAL; f.adm[q] = g6[q]; }
+  CK(cudaSetDevice(p->device));
+  StaticScratch*& sp = g_static_ptr[p->device];
+  if (!sp) {                                   // set-up, once per device, with that device current
+    void* a = nullptr;
+    CK(cudaGetSymbolAddress(&a, g_static_scratch));
+    sp = (StaticScratch*)a;
+  }
+  Par P;
+  memset(&P, 0, sizeof(P));
+  P.nmb = p->nmb; P.n = p->n; P.nt = (int)nt; P.px = P.nt + 4; P.is = 4; P.ie = p->n + 3;
+  P.Gam = p->gamma_ad; P.gm1 = p->gamma_ad - 1.0; P.gm1r = p->gamma_ad / (p->gamma_ad - 1.0);
+  P.rho_atm = p->rho_atm; P.T_atm = p->T_atm; P.P_atm = p->rho_atm * p->T_atm;
+  P.eps_atm = p->T_atm / P.gm1; P.thr = p->f_thr * p->rho_atm;
+  P.mag_max = p->mag_max;
+  P.max_iter = p->c2p_max_iter; P.tol = p->c2p_tol;
+  P.shortcuts = 3;
+  f.stats = sp->stats;
+  f.status = status ? status : sp->status;
+  cudaStream_t st = (cudaStream_t)p->stream;
+  CK(cudaMemsetAsync(sp->stats, 0, sizeof(unsigned long long) * S_NSTAT, st));   // the array keeps the last call's counts
+  k_con2prim<false, 0><<<nblk(ncell, 128), 128, 0, st>>>(P, f);
+  CK(cudaGetLastError());
+  if (host_counts) {                           // the only part that synchronises
+    unsigned long long h[S_NSTAT];
+    CK(cudaMemcpyAsync(h, sp->stats, sizeof(h), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    memset(host_counts, 0, sizeof(*host_counts));
+    host_counts->n_c2p_fail = (long long)h[S_C2P_FAIL];
+    host_counts->n_cons_floor = (long long)h[S_CONS_FLOOR];
+    host_counts->n_prim_floor = (long long)h[S_PRIM_FLOOR];
+  }
   return AK_OK;
 }
 
