@@ -159,10 +159,13 @@ int ak_set_overlap(ak_ctx*, int nchunks);
 /* Exact data-dependent shortcuts (D:§6.3).  mask bit 0: a field of (u^x, u^y, u^z, B~cc^t1, B~cc^t2) that is
  * +0.0 on the whole tile a sweep block stages is not reconstructed (every scheme of P:133 returns +0.0 on
  * both sides of every face for it); bit 1: a cell with S~ = 0 and B~ = 0 exactly runs its con2prim root
- * find on f(mu) = mu - const, which is what the master function then is.  Both leave every output bit
- * unchanged (the parity tests run with them on and off); what they change is the time on inputs with
- * exact zeros — static atmosphere, unmagnetised regions: most of a merger grid.  Default 3 (both; also
- * settable by the environment variable AK_EXACT_SHORTCUTS at ak_create); 0 times the full arithmetic. */
+ * find on f(mu) = mu - const, which is what the master function then is; bit 2: a sweep block whose tile
+ * holds u^i = +0.0 and every B~ component +0.0 evaluates the face flux of Eq. 8 with W = 1, v = 0, B = 0
+ * substituted (no index lowering, no Lorentz factor, no Alfven speed: what side_state computes then, term
+ * by term).  All three leave every output bit unchanged (the parity tests run with them on and off); what
+ * they change is the time on inputs with exact zeros — static atmosphere, unmagnetised regions: most of a
+ * merger grid.  Default 7 (all; also settable by the environment variable AK_EXACT_SHORTCUTS at
+ * ak_create); 0 times the full arithmetic. */
 int ak_set_exact_shortcuts(ak_ctx*, int mask);
 
 /* Part (5) alone, from the (post-FOFC) fluxes the last ak_rhs left in the context

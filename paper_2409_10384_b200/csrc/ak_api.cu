@@ -647,8 +647,8 @@ int ak_create(const ak_params* p, const double* dx3, ak_ctx** out) {
   P.dmp_M = p->dmp_M; P.dmp_iM = p->dmp_M > 0.0 ? 1.0 / p->dmp_M : 0.0;
   P.max_iter = p->c2p_max_iter; P.tol = p->c2p_tol;
   P.recon = p->recon; P.riemann = p->riemann; P.fofc = p->fofc; P.fofc_riemann = p->fofc_riemann;
-  P.shortcuts = 3;
-  if (const char* v = getenv("AK_EXACT_SHORTCUTS")) P.shortcuts = atoi(v) & 3;
+  P.shortcuts = 7;
+  if (const char* v = getenv("AK_EXACT_SHORTCUTS")) P.shortcuts = atoi(v) & 7;
   const long long nt = P.nt, px = P.px, nb = P.nmb;
   c->sz.cell = nb * nt * nt * nt;
   c->sz.xf = nb * nt * nt * px; c->sz.yf = nb * nt * (nt + 1) * nt; c->sz.zf = nb * (nt + 1) * nt * nt;
@@ -875,7 +875,7 @@ int ak_rhs(ak_ctx* c, const ak_cons* U, const ak_faceB* Bf, const ak_prim* W, in
 }
 
 int ak_set_exact_shortcuts(ak_ctx* c, int mask) {
-  if (!c || mask < 0 || mask > 3) return AK_EINVAL;
+  if (!c || mask < 0 || mask > 7) return AK_EINVAL;
   c->P.shortcuts = mask;
   for (int l = 0; l < 2; ++l) if (c->lane[l]) c->lane[l]->P.shortcuts = mask;
   return AK_OK;

@@ -285,4 +285,81 @@ __device__ __forceinline__ void face_flux_parked(const Par& P, int rs, const Fac
   }
 }
 
+// ------------------------------------------------------------------ O6 for a static unmagnetised face
+// The face flux when BOTH states have u^i = +0.0 and every B component is +0.0 exactly (static atmosphere
+// without field: most of a merger grid) — exact shortcut, mask bit 2 of ak_set_exact_shortcuts.  Derived from
+// side_state() operation by operation, dropping only operations whose result is then known exactly, for a
+// finite metric with gamma_xx, gamma_zz... > 0:
+//   u_i = g_ij 0 = +0 (a sum that contains the +0 of a positive diagonal term is +0), usq = +0, W = sqrt(1) = 1,
+//   1/W = 1, v^i = v_i = +0, B_i = B^2 = (Bv) = b^2 = b_i = alpha b^0 = +0, Ptot = P + 0 = P, D = rho 1 = rho,
+//   wtot = rho h, S_i = +0 - +0 = +0, tau = rho (hm1 + ddiv(+0, 2)) + 0 - P - 0 = rho hm1 - P,
+//   vhat^i = +0 - beta^i / alpha (the subtraction is kept: it fixes the sign of a zero shift),
+//   v_A^2 = ddiv(+0, rho h) = +0, a^2 = c_s^2, 1 - v^2 a^2 = 1, disc = a^2 gamma^dd, vd1 = +0.
+// Products with a zero whose SIGN the result inherits (0 * vhat) are kept, so signed zeros come out as in the
+// full evaluation.  The HLLE / LLF combination is the one of face_flux(), unchanged.
+template <int DIR, int EOS = 0>
+__device__ __forceinline__ void static_side(const Par& P, const FaceGeo& G, const double vh[3], double rho, double pr,
+                                            double U[7], double F[7], double& lm, double& lp) {
+  constexpr int t1 = (DIR + 1) % 3;
+  double hm1, cs2;
+  eos_hm1_cs2<EOS>(P, rho, pr, hm1, cs2);
+  const double h = 1.0 + hm1;
+  const double tau = rho * hm1 - pr;
+  const double aP = G.alp * pr;
+  U[0] = G.sdet * rho;
+  U[1] = G.sdet * 0.0; U[2] = U[1]; U[3] = U[1];
+  U[4] = G.sdet * tau;
+  U[5] = 0.0; U[6] = 0.0;
+  F[0] = G.sdet * (G.alp * rho * vh[DIR]);
+  const double zS = (G.alp * 0.0) * vh[DIR] - 0.0;            // alpha S_i vhat^d - alpha b_i B^d / W with S_i = b_i = +0
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    double f = zS;
+    if (i == DIR) f = f + aP;
+    F[1 + i] = G.sdet * f;
+  }
+  F[4] = G.sdet * (G.alp * tau * vh[DIR] - 0.0 + aP * 0.0);
+  const double zd = 0.0 * vh[DIR];
+  F[5] = G.sdet * (G.alp * (zd - 0.0 * vh[t1]));
+  F[6] = G.sdet * (G.alp * (zd - 0.0 * vh[(DIR + 2) % 3]));
+  const double rhoh = rho * h;
+  (void)rhoh;                                                  // v_A^2 = +0 whatever rho h > 0 is
+  const double a2 = cs2;
+  const double disc = a2 * G.gdd;
+  const double root = sqrt(fmax(0.0, disc));
+  const double vd1 = 0.0 * (1.0 - a2);
+  lm = G.alp * (vd1 - root) - G.bet[DIR];
+  lp = G.alp * (vd1 + root) - G.bet[DIR];
+}
+
+// sL, sR: rho at [0], P at [4] (floored here); everything else is +0.0 by the caller's test.
+template <int DIR, int EOS = 0>
+__device__ __forceinline__ void face_flux_static(const Par& P, int rs, const FaceGeo& G, double sL[7], double sR[7],
+                                                 double Fo[7]) {
+  face_floor<EOS>(P, sL);
+  face_floor<EOS>(P, sR);
+  const double vh[3] = {0.0 - G.bet[0] * G.ialp, 0.0 - G.bet[1] * G.ialp, 0.0 - G.bet[2] * G.ialp};
+  double UL[7], FL[7], UR[7], FR[7], lmL, lpL, lmR, lpR;
+  static_side<DIR, EOS>(P, G, vh, sL[0], sL[4], UL, FL, lmL, lpL);
+  static_side<DIR, EOS>(P, G, vh, sR[0], sR[4], UR, FR, lmR, lpR);
+  if (rs == 1) {   // HLLE
+    const double lL = fmin(0.0, fmin(lmL, lmR));
+    const double lR = fmax(0.0, fmax(lpL, lpR));
+    const double dl = lR - lL;
+    if (dl == 0.0) {
+#pragma unroll
+      for (int c = 0; c < 7; ++c) Fo[c] = 0.5 * (FL[c] + FR[c]);
+    } else {
+      const double idl = 1.0 / dl;
+      const double lRL = lR * lL;
+#pragma unroll
+      for (int c = 0; c < 7; ++c) Fo[c] = (lR * FL[c] - lL * FR[c] + lRL * (UR[c] - UL[c])) * idl;
+    }
+  } else {         // LLF
+    const double lam = fmax(fmax(fabs(lmL), fabs(lpL)), fmax(fabs(lmR), fabs(lpR)));
+#pragma unroll
+    for (int c = 0; c < 7; ++c) Fo[c] = 0.5 * (FL[c] + FR[c]) - 0.5 * lam * (UR[c] - UL[c]);
+  }
+}
+
 }  // namespace ak

@@ -75,7 +75,11 @@ k_flux_pencil(const __grid_constant__ Par P, const __grid_constant__ Fields f,
     Bfd = __ldg(f.Bf[DIR] + fi);
   }
   mbar_wait(&mbar, 0);
-  const unsigned nzm = (RECON != 0 && (P.shortcuts & 1)) ? tile_nonzero_mask(sW, tile_d, nt * WI, &nzacc) : ALWAYS_NZ;
+  const unsigned nzm = ((RECON != 0 && (P.shortcuts & 1)) || (P.shortcuts & 4))
+                           ? tile_nonzero_mask(sW, tile_d, nt * WI, &nzacc, (__double_as_longlong(Bfd) != 0LL) ? 0x80u : 0u)
+                           : ALWAYS_NZ;
+  const bool stat = tile_is_static(P, nzm);          // block-uniform
+  const unsigned rzm = (P.shortcuts & 1) ? nzm : ALWAYS_NZ;   // which slots are reconstructed
   double qm[7];
   if (active) {
 #pragma unroll
@@ -83,7 +87,7 @@ k_flux_pencil(const __grid_constant__ Par P, const __grid_constant__ Fields f,
       const double* w = sW + v * tile_d + t;     // cell cc-2 of this lane; cells cc-2 .. cc+2 at stride WI
       double qp;
       if (RECON == 0) { qm[v] = qp = w[2 * WI]; }
-      else if (!((nzm >> v) & 1u)) { qm[v] = qp = 0.0; }     // the field is +0.0 on the whole tile
+      else if (!((rzm >> v) & 1u)) { qm[v] = qp = 0.0; }     // the field is +0.0 on the whole tile
       else recon<RECON>(w[0], w[WI], w[2 * WI], w[3 * WI], w[4 * WI], qm[v], qp);
       sQ[v * (int)blockDim.x + t] = qp;
     }
@@ -106,6 +110,13 @@ k_flux_pencil(const __grid_constant__ Par P, const __grid_constant__ Fields f,
   }
   FaceGeo G;
   if (has_face) face_geometry<DIR>(mL, mR, G);
+  if (stat) {                             // static unmagnetised tile: nothing to park, no barrier
+    if (!has_face) return;
+    face_flux_static<DIR, EOS>(P, P.riemann, G, sL, qm, Fo);
+#pragma unroll
+    for (int v = 0; v < 7; ++v) f.F[7 * DIR + v][fi] = Fo[v];
+    return;
+  }
   __syncthreads();                        // tile and q^+ are spent: the allocation becomes parking space
   if (!has_face) return;
   {

@@ -56,8 +56,10 @@ __device__ __forceinline__ void mbar_wait(uint64_t* b, unsigned parity) {
 // skipped: static atmosphere (u = 0) and unmagnetised regions (B = 0) are most of a merger grid.  All
 // threads of the block call this (one barrier); `acc` is a shared word that thread 0 zeroed before an
 // earlier barrier.
-__device__ __forceinline__ unsigned tile_nonzero_mask(const double* sW, int slot_stride, int count, unsigned* acc) {
-  unsigned nz = 0;
+// `extra`: bits the calling thread adds (bit 7: its face-normal B~ is not +0.0).
+__device__ __forceinline__ unsigned tile_nonzero_mask(const double* sW, int slot_stride, int count, unsigned* acc,
+                                                      unsigned extra = 0u) {
+  unsigned nz = extra;
   for (int q = threadIdx.x; q < count; q += (int)blockDim.x) {
 #pragma unroll
     for (int s = 1; s < 7; ++s)
@@ -68,7 +70,9 @@ __device__ __forceinline__ unsigned tile_nonzero_mask(const double* sW, int slot
   __syncthreads();
   return *acc | 0x11u;                  // slots 0 (rho) and 4 (P) are never zero: always reconstructed
 }
-constexpr unsigned ALWAYS_NZ = 0x7fu;   // every slot reconstructed (shortcut off)
+constexpr unsigned ALWAYS_NZ = 0xffu;   // every slot reconstructed, face not static (shortcuts off)
+// u^i, both transverse B~cc and the face-normal B~ are +0.0 on the whole tile: the static face flux applies
+__device__ __forceinline__ bool tile_is_static(const Par& P, unsigned nzm) { return (P.shortcuts & 4) && !(nzm & 0xeeu); }
 
 // Tensor maps of the 17 fields a sweep stages (host: ak_api.cu, cuTensorMapEncodeTiled).  Every cell field is
 // the rank-3 tensor (i: nt, j: nt, K = m nt + k) of doubles; the box is the whole tile of one field, so a
@@ -164,7 +168,11 @@ k_flux_tma(const __grid_constant__ Par P, const __grid_constant__ Fields f, int 
     Bfd = __ldg(f.Bf[DIR] + fi);
   }
   mbar_wait(&mbar, 0);
-  const unsigned nzm = (RECON != 0 && (P.shortcuts & 1)) ? tile_nonzero_mask(sW, slotW, nW * nt, &nzacc) : ALWAYS_NZ;
+  const unsigned nzm = ((RECON != 0 && (P.shortcuts & 1)) || (P.shortcuts & 4))
+                           ? tile_nonzero_mask(sW, slotW, nW * nt, &nzacc, (__double_as_longlong(Bfd) != 0LL) ? 0x80u : 0u)
+                           : ALWAYS_NZ;
+  const bool stat = tile_is_static(P, nzm);          // block-uniform
+  const unsigned rzm = (P.shortcuts & 1) ? nzm : ALWAYS_NZ;   // which slots are reconstructed
 #if !AK_FLUX_PARK
   if (!active) return;
 #endif
@@ -177,7 +185,7 @@ k_flux_tma(const __grid_constant__ Par P, const __grid_constant__ Fields f, int 
       const int s = DIR == 0 ? 1 : nt;
       if (RECON == 0) {
         sL[v] = w[2 * s]; sR[v] = w[3 * s];
-      } else if (!((nzm >> v) & 1u)) {
+      } else if (!((rzm >> v) & 1u)) {
         sL[v] = 0.0; sR[v] = 0.0;           // the field is +0.0 on the whole tile
       } else {
         const double q0 = w[0], q1 = w[s], q2 = w[2 * s], q3 = w[3 * s], q4 = w[4 * s], q5 = w[5 * s];
@@ -200,6 +208,13 @@ k_flux_tma(const __grid_constant__ Par P, const __grid_constant__ Fields f, int 
   // (21 doubles per thread; the launcher sizes the allocation for both uses)
   FaceGeo G;
   if (active) face_geometry<DIR>(mL, mR, G);
+  if (stat) {                                        // static unmagnetised tile: nothing to park, no barrier
+    if (!active) return;
+    face_flux_static<DIR, EOS>(P, P.riemann, G, sL, sR, Fo);
+#pragma unroll
+    for (int v = 0; v < 7; ++v) f.F[7 * DIR + v][fi] = Fo[v];
+    return;
+  }
   __syncthreads();
   if (!active) return;
   {   // (parking the right state behind the tile while it is reconstructed measured 3 % slower: more shared memory)
@@ -309,7 +324,11 @@ k_flux_tma_cell(const __grid_constant__ Par P, const __grid_constant__ Fields f,
     Bfd = __ldg(f.Bf[DIR] + fi);
   }
   mbar_wait(&mbar, 0);
-  const unsigned nzm = (RECON != 0 && (P.shortcuts & 1)) ? tile_nonzero_mask(sW, slotW, nW * nt, &nzacc) : ALWAYS_NZ;
+  const unsigned nzm = ((RECON != 0 && (P.shortcuts & 1)) || (P.shortcuts & 4))
+                           ? tile_nonzero_mask(sW, slotW, nW * nt, &nzacc, (__double_as_longlong(Bfd) != 0LL) ? 0x80u : 0u)
+                           : ALWAYS_NZ;
+  const bool stat = tile_is_static(P, nzm);          // block-uniform
+  const unsigned rzm = (P.shortcuts & 1) ? nzm : ALWAYS_NZ;   // which slots are reconstructed
   double qm[7];
   if (active) {
 #pragma unroll
@@ -319,7 +338,7 @@ k_flux_tma_cell(const __grid_constant__ Par P, const __grid_constant__ Fields f,
       const int s = DIR == 0 ? 1 : nt;
       double qp;
       if (RECON == 0) { qm[v] = qp = w[2 * s]; }
-      else if (!((nzm >> v) & 1u)) { qm[v] = qp = 0.0; }     // the field is +0.0 on the whole tile
+      else if (!((rzm >> v) & 1u)) { qm[v] = qp = 0.0; }     // the field is +0.0 on the whole tile
       else recon<RECON>(w[0], w[s], w[2 * s], w[3 * s], w[4 * s], qm[v], qp);
       sQ[v * TMA_THREADS + t] = qp;
     }
@@ -344,6 +363,13 @@ k_flux_tma_cell(const __grid_constant__ Par P, const __grid_constant__ Fields f,
   // second barrier: states and metric are in registers, the whole allocation becomes parking space
   FaceGeo G;
   if (has_face) face_geometry<DIR>(mL, mR, G);
+  if (stat) {                                        // static unmagnetised tile: nothing to park, no barrier
+    if (!has_face) return;
+    face_flux_static<DIR, EOS>(P, P.riemann, G, sL, qm, Fo);
+#pragma unroll
+    for (int v = 0; v < 7; ++v) f.F[7 * DIR + v][fi] = Fo[v];
+    return;
+  }
   __syncthreads();
   if (!has_face) return;
   {

@@ -197,16 +197,19 @@ def test_host_entry_without_primitives():
     ("C1", [0, 7], dict(recon=2)),                               # static star: every velocity exactly zero
     ("C1", [0, 7], dict(recon=4, riemann=0)),
     ("C3", [192 + 21, 64 + 21, 21], dict(recon=3)),              # nothing is zero: the shortcuts never fire
+    ("C2", [0, 63, 21], dict(recon=0, riemann=0)),               # donor cell + LLF through the static face flux
+    ("C4", [0, 1, 300, 301], dict()),                            # rotational shift, atmosphere blocks of two sizes
 ])
 def test_exact_shortcuts_leave_every_bit_unchanged(name, blocks, over):
     """ak_set_exact_shortcuts: skipping the reconstruction of fields that are +0.0 on a whole tile and
-    running the root find of static unmagnetised cells on f(mu) = mu - const are exact: mask 0 (full
-    arithmetic), 1, 2 and 3 give the same bits in every output, fluxes included, and equal the oracle."""
+    running the root find of static unmagnetised cells on f(mu) = mu - const, and the static face flux on
+    tiles with u = 0 and B = 0, are exact: mask 0 (full arithmetic), 1, 2, 4 and 7 give the same bits in
+    every output, fluxes and the signs of their zeros included, and equal the oracle."""
     from paper_2409_10384_b200 import ak
     w = wl.make_blocks(name, blocks=blocks)
     U_in = [u.copy() for u in w["U"]]
     res = []
-    for mask in (0, 1, 2, 3):
+    for mask in (0, 1, 2, 4, 7):
         with gpukit.GpuStage(copy.deepcopy(w), **over) as g:
             ak.ak_set_exact_shortcuts(g.ctx, mask)
             g.rhs()
@@ -219,6 +222,7 @@ def test_exact_shortcuts_leave_every_bit_unchanged(name, blocks, over):
         assert np.array_equal(r0["flag"], r["flag"]) and np.array_equal(r0["status"], r["status"])
         for x, y in zip(f0, fl):
             assert np.array_equal(x, y)
+            assert np.array_equal(np.signbit(x), np.signbit(y))      # signed zeros of a static face included
         assert st == s0
     p = dict(w["params"]); p.update(over)
     o = orc.rhs(orc.make_params(**p), w["dx"], w["U"], w["Bf"], w["adm"], w["dt_fofc"], nthreads=8)
@@ -234,7 +238,7 @@ def test_exact_shortcuts_with_signed_zeros_and_partly_zero_fields():
     from paper_2409_10384_b200 import ak
     w = wl.make_test_noise_block(seed=3, n=8, frac=0.0)
     outs = []
-    for mask in (0, 3):
+    for mask in (0, 7):
         with gpukit.GpuStage(copy.deepcopy(w), recon=2, dmp_M=1.1) as g:
             ak.ak_set_exact_shortcuts(g.ctx, mask)
             g.con2prim()
