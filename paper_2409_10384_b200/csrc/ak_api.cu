@@ -66,6 +66,7 @@ struct ak_ctx {
   cudaEvent_t* ov_ev; int ov_nev;
   int cap[8];                   // grid caps (blocks) per kernel class in the overlapped schedule, 0 = none
   int sweep_smem_pad;           // bytes: dynamic shared memory the sweeps ask for at least when overlapped
+  unsigned int* zflags;         // [nmb] per-block zero-field flags written by k_con2prim (Fields::zflags)
   int tile_tm;                  // tile kernels: stage tiles with tensor-map box copies (1) or row by row (0)
   int pencil_wi;                // y/z sweeps: x-lanes per block of k_flux_pencil (0: tile kernels k_flux_tma)
   // FOFC stage blend (ak_set_fofc_blend)
@@ -191,6 +192,7 @@ void chunk_fields(const ak_ctx* c, const Fields& f, int m0, int nb, int ci, Fiel
   for (int q = 0; q < 8; ++q) g.W[q] += cell;
   for (int q = 0; q < 21; ++q) g.F[q] += fsz[q / 7];
   g.flag += cell;
+  if (g.zflags) g.zflags += m0;
   if (g.status) g.status += cell;
   if (g.M[0]) for (int q = 0; q < 10; ++q) g.M[q] += cell;
   g.dx += 3LL * m0;
@@ -232,6 +234,7 @@ inline unsigned capped(long long items, int threads, int cap_blocks) {
 int launch_c2p(ak_ctx* c, const Lane& L, bool with_emf) {
   Timer t(c, KC_C2P, L.st);
   CK(cudaMemsetAsync(L.f.stats, 0, sizeof(unsigned long long) * 3, L.st));
+  if (L.f.zflags) CK(cudaMemsetAsync(L.f.zflags, 0, sizeof(unsigned) * L.P.nmb, L.st));   // this pass sets the bits
   const long long ncell = (long long)L.P.nmb * L.P.nt * L.P.nt * L.P.nt;
   const unsigned g = capped(ncell, 128, L.ov ? c->cap[KC_C2P] : 0);
   const bool stride = (long long)g * 128 < ncell;       // a capped grid needs the grid-stride form
@@ -671,6 +674,8 @@ int ak_create(const ak_params* p, const double* dx3, ak_ctx** out) {
   if (e == cudaSuccess) e = cudaMalloc(&c->stats, sizeof(unsigned long long) * S_NSTAT * MAXCH);
   if (e == cudaSuccess) e = cudaMemsetAsync(c->count, 0, sizeof(unsigned) * 4 * MAXCH, c->stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(c->stats, 0, sizeof(unsigned long long) * S_NSTAT * MAXCH, c->stream);
+  if (e == cudaSuccess) e = cudaMalloc(&c->zflags, sizeof(unsigned) * nb);
+  if (e == cudaSuccess) e = cudaMemsetAsync(c->zflags, 0xff, sizeof(unsigned) * nb, c->stream);
   if (e == cudaSuccess) e = cudaMalloc(&c->dx, sizeof(double) * 3 * nb);
   if (e == cudaSuccess) e = cudaMemcpyAsync(c->dx, dx3, sizeof(double) * 3 * nb, cudaMemcpyHostToDevice, c->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);   // dx3 is the caller's: copy must be done
@@ -720,7 +725,7 @@ int ak_destroy(ak_ctx* c) {
     for (int q = 0; q < 3; ++q)
       if (c->ovs[q] && !(q == 2 && c->ovs[2] == c->ovs[0])) cudaStreamDestroy(c->ovs[q]);
   }
-  cudaFree(c->flag_own); cudaFree(c->count); cudaFree(c->stats); cudaFree(c->dx);
+  cudaFree(c->flag_own); cudaFree(c->count); cudaFree(c->stats); cudaFree(c->dx); cudaFree(c->zflags);
   delete c;
   return AK_OK;
 }
@@ -802,6 +807,9 @@ int ak_rhs(ak_ctx* c, const ak_cons* U, const ak_faceB* Bf, const ak_prim* W, in
   f.E[0] = out->Ex; f.E[1] = out->Ey; f.E[2] = out->Ez;
   if (out->fofc_flag) f.flag = out->fofc_flag;
   f.status = out->c2p_status;
+  // per-block zero-field flags: part (1) of this call writes them, the later parts read them; primitives the
+  // caller supplies (w_is_valid) come without
+  f.zflags = w_is_valid ? nullptr : c->zflags;
   if (out->matter) {
     const ak_matter* mo = out->matter;
     double* mp[10] = {mo->E, mo->Sx, mo->Sy, mo->Sz, mo->Sxx, mo->Sxy, mo->Sxz, mo->Syy, mo->Syz, mo->Szz};

@@ -52,6 +52,8 @@ struct Fields {
   const double* U0[5];          // FOFC estimate of a later RK stage: U* = fa U0 + fb (U - dt div F);
   double fa, fb;                // U0[0] == nullptr: U* = U - dt div F (R9)
   double* M[10];                // matter terms E, S_i, S_ij written by K6 on interior cells (M[0] == nullptr: none)
+  unsigned int* zflags;         // [nmb] bit q set: primitive field W[q] (q = 1..3 u^i, 5..7 B~cc^i) of that block holds
+                                // a value that is not +0.0 (written by k_con2prim, conservative); nullptr: unknown
 };
 
 enum { ST_DFLOOR = 1, ST_TAUFLOOR = 2, ST_MAGCAP = 4, ST_RHOFLOOR = 8, ST_TFLOOR = 16,

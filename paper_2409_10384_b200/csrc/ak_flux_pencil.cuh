@@ -86,8 +86,8 @@ k_flux_pencil(const __grid_constant__ Par P, const __grid_constant__ Fields f,
     for (int v = 0; v < 7; ++v) {
       const double* w = sW + v * tile_d + t;     // cell cc-2 of this lane; cells cc-2 .. cc+2 at stride WI
       double qp;
-      if (RECON == 0) { qm[v] = qp = w[2 * WI]; }
-      else if (!((rzm >> v) & 1u)) { qm[v] = qp = 0.0; }     // the field is +0.0 on the whole tile
+      if (!((rzm >> v) & 1u)) { qm[v] = qp = 0.0; }          // the field is +0.0 on the whole tile
+      else if (RECON == 0) { qm[v] = qp = w[2 * WI]; }
       else recon<RECON>(w[0], w[WI], w[2 * WI], w[3 * WI], w[4 * WI], qm[v], qp);
       sQ[v * (int)blockDim.x + t] = qp;
     }

@@ -57,18 +57,31 @@ __device__ __forceinline__ void mbar_wait(uint64_t* b, unsigned parity) {
 // threads of the block call this (one barrier); `acc` is a shared word that thread 0 zeroed before an
 // earlier barrier.
 // `extra`: bits the calling thread adds (bit 7: its face-normal B~ is not +0.0).
+// `loaded`: slots that were staged at all (a slot the block's zero flags ruled out is not in shared memory and
+// counts as zero).
 __device__ __forceinline__ unsigned tile_nonzero_mask(const double* sW, int slot_stride, int count, unsigned* acc,
-                                                      unsigned extra = 0u) {
+                                                      unsigned extra = 0u, unsigned loaded = 0x7fu) {
   unsigned nz = extra;
-  for (int q = threadIdx.x; q < count; q += (int)blockDim.x) {
+  if (loaded & 0x6eu) {
+    for (int q = threadIdx.x; q < count; q += (int)blockDim.x) {
 #pragma unroll
-    for (int s = 1; s < 7; ++s)
-      if (s != 4) nz |= (unsigned)(__double_as_longlong(sW[(size_t)s * slot_stride + q]) != 0LL) << s;
+      for (int s = 1; s < 7; ++s)
+        if (s != 4 && ((loaded >> s) & 1u)) nz |= (unsigned)(__double_as_longlong(sW[(size_t)s * slot_stride + q]) != 0LL) << s;
+    }
   }
   nz = __reduce_or_sync(0xffffffffu, nz);
   if ((threadIdx.x & 31) == 0 && nz) atomicOr(acc, nz);
   __syncthreads();
   return *acc | 0x11u;                  // slots 0 (rho) and 4 (P) are never zero: always reconstructed
+}
+// Slots of a sweep of direction DIR that have to be staged, from the block's zero flags (Fields::zflags, written
+// by k_con2prim): slot 0 rho, 1..3 u^i, 4 P, 5 / 6 the transverse B~cc.
+template <int DIR>
+__device__ __forceinline__ unsigned slots_to_load(const Par& P, const Fields& f, int m) {
+  if (!f.zflags || !(P.shortcuts & 1)) return 0x7fu;
+  constexpr int t1 = (DIR + 1) % 3, t2 = (DIR + 2) % 3;
+  const unsigned z = f.zflags[m];
+  return 0x11u | (z & 0x0eu) | (((z >> (5 + t1)) & 1u) << 5) | (((z >> (5 + t2)) & 1u) << 6);
 }
 constexpr unsigned ALWAYS_NZ = 0xffu;   // every slot reconstructed, face not static (shortcuts off)
 // u^i, both transverse B~cc and the face-normal B~ are +0.0 on the whole tile: the static face flux applies
@@ -123,30 +136,33 @@ k_flux_tma(const __grid_constant__ Par P, const __grid_constant__ Fields f, int 
   const unsigned rowb = (unsigned)(nt * sizeof(double));
   __shared__ unsigned nzacc;
   if (t == 0) { mbar_init(&mbar, 1); nzacc = 0; }
+  const unsigned ld = slots_to_load<DIR>(P, f, m);                  // block-uniform: slots that are staged at all
   __syncthreads();
   if (use_tm) {
     // ---- one tensor copy per field: the box holds maxW (maxM) rows whether or not the tile is ragged
     if (t < 32) {                                                   // lanes 0..16 of warp 0: one field each
-      if (t == 0) mbar_arrive_expect_tx(&mbar, (unsigned)(7 * maxW + 10 * maxM) * rowb);
+      if (t == 0) mbar_arrive_expect_tx(&mbar, (unsigned)(__popc(ld) * maxW + 10 * maxM) * rowb);
       __syncwarp();
       const int K = DIR == 2 ? m * nt + d0 : m * nt + o;            // plane coordinate of tile row 0 ...
       if (t < 7) {
+        if ((ld >> t) & 1u) {
         const int cW1 = DIR == 0 ? d0 : (DIR == 1 ? d0 - 3 : o), cW2 = DIR == 2 ? K - 3 : K;
         tma_load_3d(sW + (size_t)t * slotW, &maps.w[t], 0, cW1, cW2, &mbar);
+        }
       } else if (t < 17) {
         const int cM1 = DIR == 0 ? d0 : (DIR == 1 ? d0 - 1 : o), cM2 = DIR == 2 ? K - 1 : K;
         tma_load_3d(sM + (size_t)(t - 7) * slotM, &maps.m[t - 7], 0, cM1, cM2, &mbar);
       }
     }
   } else {
-  if (t == 0) mbar_arrive_expect_tx(&mbar, (unsigned)(7 * nW + 10 * nM) * rowb);
+  if (t == 0) mbar_arrive_expect_tx(&mbar, (unsigned)(__popc(ld) * nW + 10 * nM) * rowb);
   // ---- one bulk copy per (field, row)
   const int ncW = 7 * nW, nc = ncW + 10 * nM;
   for (int c = t; c < nc; c += (int)blockDim.x) {
     if (c < ncW) {
       const int v = c / nW, r = c - v * nW;
       const int fld = v < 5 ? v : (v == 5 ? 5 + t1 : 5 + t2);
-      bulk_copy_g2s(sW + (size_t)v * slotW + r * nt, f.W[fld] + baseW + r * rs, rowb, &mbar);
+      if ((ld >> v) & 1u) bulk_copy_g2s(sW + (size_t)v * slotW + r * nt, f.W[fld] + baseW + r * rs, rowb, &mbar);
     } else {
       const int cc = c - ncW;
       const int q = cc / nM, r = cc - q * nM;
@@ -168,8 +184,8 @@ k_flux_tma(const __grid_constant__ Par P, const __grid_constant__ Fields f, int 
     Bfd = __ldg(f.Bf[DIR] + fi);
   }
   mbar_wait(&mbar, 0);
-  const unsigned nzm = ((RECON != 0 && (P.shortcuts & 1)) || (P.shortcuts & 4))
-                           ? tile_nonzero_mask(sW, slotW, nW * nt, &nzacc, (__double_as_longlong(Bfd) != 0LL) ? 0x80u : 0u)
+  const unsigned nzm = ((RECON != 0 && (P.shortcuts & 1)) || (P.shortcuts & 4) || ld != 0x7fu)
+                           ? tile_nonzero_mask(sW, slotW, nW * nt, &nzacc, (__double_as_longlong(Bfd) != 0LL) ? 0x80u : 0u, ld)
                            : ALWAYS_NZ;
   const bool stat = tile_is_static(P, nzm);          // block-uniform
   const unsigned rzm = (P.shortcuts & 1) ? nzm : ALWAYS_NZ;   // which slots are reconstructed
@@ -183,10 +199,10 @@ k_flux_tma(const __grid_constant__ Par P, const __grid_constant__ Fields f, int 
       // six stencil cells f-3 .. f+2: along i in one row (x) or one per shared row (y, z)
       const double* w = DIR == 0 ? sW + (size_t)v * slotW + a * nt + ii - 3 : sW + (size_t)v * slotW + a * nt + ii;
       const int s = DIR == 0 ? 1 : nt;
-      if (RECON == 0) {
+      if (!((rzm >> v) & 1u)) {
+        sL[v] = 0.0; sR[v] = 0.0;           // the field is +0.0 on the whole tile (or was not even staged)
+      } else if (RECON == 0) {
         sL[v] = w[2 * s]; sR[v] = w[3 * s];
-      } else if (!((rzm >> v) & 1u)) {
-        sL[v] = 0.0; sR[v] = 0.0;           // the field is +0.0 on the whole tile
       } else {
         const double q0 = w[0], q1 = w[s], q2 = w[2 * s], q3 = w[3 * s], q4 = w[4 * s], q5 = w[5 * s];
         double qm, qp;
@@ -278,28 +294,31 @@ k_flux_tma_cell(const __grid_constant__ Par P, const __grid_constant__ Fields f,
   const unsigned rowb = (unsigned)(nt * sizeof(double));
   __shared__ unsigned nzacc;
   if (t == 0) { mbar_init(&mbar, 1); nzacc = 0; }
+  const unsigned ld = slots_to_load<DIR>(P, f, m);                  // block-uniform: slots that are staged at all
   __syncthreads();
   if (use_tm) {
     if (t < 32) {                                                   // lanes 0..16 of warp 0: one field each
-      if (t == 0) mbar_arrive_expect_tx(&mbar, (unsigned)(7 * maxW + 10 * maxM) * rowb);
+      if (t == 0) mbar_arrive_expect_tx(&mbar, (unsigned)(__popc(ld) * maxW + 10 * maxM) * rowb);
       __syncwarp();
       const int K = DIR == 2 ? m * nt + d0 : m * nt + o;            // plane coordinate of tile row 0 ...
       if (t < 7) {
+        if ((ld >> t) & 1u) {
         const int cW1 = DIR == 0 ? d0 : (DIR == 1 ? d0 - 3 : o), cW2 = DIR == 2 ? K - 3 : K;
         tma_load_3d(sW + (size_t)t * slotW, &maps.w[t], 0, cW1, cW2, &mbar);
+        }
       } else if (t < 17) {
         const int cM1 = DIR == 0 ? d0 : (DIR == 1 ? d0 - 1 : o), cM2 = DIR == 2 ? K - 1 : K;
         tma_load_3d(sM + (size_t)(t - 7) * slotM, &maps.m[t - 7], 0, cM1, cM2, &mbar);
       }
     }
   } else {
-  if (t == 0) mbar_arrive_expect_tx(&mbar, (unsigned)(7 * nW + 10 * nM) * rowb);
+  if (t == 0) mbar_arrive_expect_tx(&mbar, (unsigned)(__popc(ld) * nW + 10 * nM) * rowb);
   const int ncW = 7 * nW, nc = ncW + 10 * nM;
   for (int c = t; c < nc; c += (int)blockDim.x) {
     if (c < ncW) {
       const int v = c / nW, r = c - v * nW;
       const int fld = v < 5 ? v : (v == 5 ? 5 + t1 : 5 + t2);
-      bulk_copy_g2s(sW + (size_t)v * slotW + r * nt, f.W[fld] + baseW + r * rs, rowb, &mbar);
+      if ((ld >> v) & 1u) bulk_copy_g2s(sW + (size_t)v * slotW + r * nt, f.W[fld] + baseW + r * rs, rowb, &mbar);
     } else {
       const int cc = c - ncW;
       const int q = cc / nM, r = cc - q * nM;
@@ -324,8 +343,8 @@ k_flux_tma_cell(const __grid_constant__ Par P, const __grid_constant__ Fields f,
     Bfd = __ldg(f.Bf[DIR] + fi);
   }
   mbar_wait(&mbar, 0);
-  const unsigned nzm = ((RECON != 0 && (P.shortcuts & 1)) || (P.shortcuts & 4))
-                           ? tile_nonzero_mask(sW, slotW, nW * nt, &nzacc, (__double_as_longlong(Bfd) != 0LL) ? 0x80u : 0u)
+  const unsigned nzm = ((RECON != 0 && (P.shortcuts & 1)) || (P.shortcuts & 4) || ld != 0x7fu)
+                           ? tile_nonzero_mask(sW, slotW, nW * nt, &nzacc, (__double_as_longlong(Bfd) != 0LL) ? 0x80u : 0u, ld)
                            : ALWAYS_NZ;
   const bool stat = tile_is_static(P, nzm);          // block-uniform
   const unsigned rzm = (P.shortcuts & 1) ? nzm : ALWAYS_NZ;   // which slots are reconstructed
@@ -337,8 +356,8 @@ k_flux_tma_cell(const __grid_constant__ Par P, const __grid_constant__ Fields f,
       const double* w = DIR == 0 ? sW + (size_t)v * slotW + a * nt + ii - 2 : sW + (size_t)v * slotW + a * nt + ii;
       const int s = DIR == 0 ? 1 : nt;
       double qp;
-      if (RECON == 0) { qm[v] = qp = w[2 * s]; }
-      else if (!((rzm >> v) & 1u)) { qm[v] = qp = 0.0; }     // the field is +0.0 on the whole tile
+      if (!((rzm >> v) & 1u)) { qm[v] = qp = 0.0; }          // the field is +0.0 on the whole tile (or was not staged)
+      else if (RECON == 0) { qm[v] = qp = w[2 * s]; }
       else recon<RECON>(w[0], w[s], w[2 * s], w[3 * s], w[4 * s], qm[v], qp);
       sQ[v * TMA_THREADS + t] = qp;
     }

@@ -154,6 +154,17 @@ __global__ void __launch_bounds__(128, AK_C2P_MINB) k_con2prim(const __grid_cons
     for (int v = 0; v < 5; ++v) f.U[v][c] = Ut[v];
   }
   if (f.status) f.status[c] = (unsigned char)st;
+  if (f.zflags) {
+    // which of this block's often-zero fields hold anything but +0.0: later kernels of the stage do not
+    // load a field whose bit stays clear.  A set bit is only ever added: the flag may say
+    // "non-zero" for a field that is zero (another thread's stale read), never the reverse.
+    unsigned nz = 0;
+#pragma unroll
+    for (int v = 1; v < 4; ++v) nz |= (unsigned)(__double_as_longlong(W5[v]) != 0LL) << v;
+#pragma unroll
+    for (int v = 0; v < 3; ++v) nz |= (unsigned)(__double_as_longlong(Bc[v]) != 0LL) << (5 + v);
+    if (nz != 0 && (__ldcg(f.zflags + m) & nz) != nz) atomicOr(f.zflags + m, nz);
+  }
   if (EMF) {
     const double u[3] = {W5[1], W5[2], W5[3]};
     double ul[3];
@@ -267,8 +278,9 @@ __global__ void __launch_bounds__(128, AK_FOFC_MINB) k_fofc_test(const __grid_co
   }
   Met3 g;
   load_met3(f, c, g);
+  const unsigned zf = (f.zflags && (P.shortcuts & 1)) ? f.zflags[m] : 0xffu;    // clear bit: the field is +0.0 in this block
 #pragma unroll
-  for (int v = 0; v < 3; ++v) Bc[v] = f.W[5 + v][c];
+  for (int v = 0; v < 3; ++v) Bc[v] = ((zf >> (5 + v)) & 1u) ? f.W[5 + v][c] : 0.0;
   const double Ds = Us[0], ts = Us[4];
   int st = c2p_cell<false, EOS>(P, g, Us, Bc, W5);
   // Eq. 12 asks whether D~*, tau~* lie in [min/M, M max] of the 27-cell neighbourhood.  The centre cell is one

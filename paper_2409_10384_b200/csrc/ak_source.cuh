@@ -37,8 +37,14 @@ __global__ void __launch_bounds__(128, AK_SRC_MINB) k_div_src(const __grid_const
   metric_inverse(g, det, sdet, gu);
   const double isd = 1.0 / sdet;
   const double rho = f.W[0][c], pr = f.W[4][c];
-  const double u[3] = {f.W[1][c], f.W[2][c], f.W[3][c]};
-  const double B[3] = {f.W[5][c] * isd, f.W[6][c] * isd, f.W[7][c] * isd};
+  const unsigned zf = (f.zflags && (P.shortcuts & 1)) ? f.zflags[m] : 0xffu;    // clear bit: the field is +0.0 in this block
+  double u[3], Bt[3];
+#pragma unroll
+  for (int v = 0; v < 3; ++v) {
+    u[v] = ((zf >> (1 + v)) & 1u) ? f.W[1 + v][c] : 0.0;
+    Bt[v] = ((zf >> (5 + v)) & 1u) ? f.W[5 + v][c] : 0.0;
+  }
+  const double B[3] = {Bt[0] * isd, Bt[1] * isd, Bt[2] * isd};
   double cons[5];
   prim2cons<EOS>(P, g, rho, u, pr, B, cons);
   double ul[3], Bl[3];
