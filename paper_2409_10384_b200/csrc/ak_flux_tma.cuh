@@ -110,7 +110,7 @@ __global__ void __launch_bounds__(TMA_THREADS, AK_TMA_MINB)
 k_flux_tma(const __grid_constant__ Par P, const __grid_constant__ Fields f, int NA,
            const __grid_constant__ TileMaps maps, int use_tm) {
   extern __shared__ __align__(128) double sm[];
-  __shared__ uint64_t mbar;
+  __shared__ uint64_t mbar, mbarM;      // primitive slabs / metric slabs: the metric lands while the states are reconstructed
   const int nt = P.nt, e = P.n + 2, t = threadIdx.x;
   constexpr int t1 = (DIR + 1) % 3, t2 = (DIR + 2) % 3;
   const int maxW = DIR == 0 ? NA : NA + 5, maxM = DIR == 0 ? NA : NA + 1;
@@ -135,13 +135,16 @@ k_flux_tma(const __grid_constant__ Par P, const __grid_constant__ Fields f, int 
   else { baseW = ix.cell(m, d0 - 3, o, 0); baseM = ix.cell(m, d0 - 1, o, 0); rs = (long long)nt * nt; }
   const unsigned rowb = (unsigned)(nt * sizeof(double));
   __shared__ unsigned nzacc;
-  if (t == 0) { mbar_init(&mbar, 1); nzacc = 0; }
+  if (t == 0) { mbar_init(&mbar, 1); mbar_init(&mbarM, 1); nzacc = 0; }
   const unsigned ld = slots_to_load<DIR>(P, f, m);                  // block-uniform: slots that are staged at all
   __syncthreads();
   if (use_tm) {
     // ---- one tensor copy per field: the box holds maxW (maxM) rows whether or not the tile is ragged
     if (t < 32) {                                                   // lanes 0..16 of warp 0: one field each
-      if (t == 0) mbar_arrive_expect_tx(&mbar, (unsigned)(__popc(ld) * maxW + 10 * maxM) * rowb);
+      if (t == 0) {
+        mbar_arrive_expect_tx(&mbar, (unsigned)(__popc(ld) * maxW) * rowb);
+        mbar_arrive_expect_tx(&mbarM, (unsigned)(10 * maxM) * rowb);
+      }
       __syncwarp();
       const int K = DIR == 2 ? m * nt + d0 : m * nt + o;            // plane coordinate of tile row 0 ...
       if (t < 7) {
@@ -151,11 +154,14 @@ k_flux_tma(const __grid_constant__ Par P, const __grid_constant__ Fields f, int 
         }
       } else if (t < 17) {
         const int cM1 = DIR == 0 ? d0 : (DIR == 1 ? d0 - 1 : o), cM2 = DIR == 2 ? K - 1 : K;
-        tma_load_3d(sM + (size_t)(t - 7) * slotM, &maps.m[t - 7], 0, cM1, cM2, &mbar);
+        tma_load_3d(sM + (size_t)(t - 7) * slotM, &maps.m[t - 7], 0, cM1, cM2, &mbarM);
       }
     }
   } else {
-  if (t == 0) mbar_arrive_expect_tx(&mbar, (unsigned)(__popc(ld) * nW + 10 * nM) * rowb);
+  if (t == 0) {
+    mbar_arrive_expect_tx(&mbar, (unsigned)(__popc(ld) * nW) * rowb);
+    mbar_arrive_expect_tx(&mbarM, (unsigned)(10 * nM) * rowb);
+  }
   // ---- one bulk copy per (field, row)
   const int ncW = 7 * nW, nc = ncW + 10 * nM;
   for (int c = t; c < nc; c += (int)blockDim.x) {
@@ -167,7 +173,7 @@ k_flux_tma(const __grid_constant__ Par P, const __grid_constant__ Fields f, int 
       const int cc = c - ncW;
       const int q = cc / nM, r = cc - q * nM;
       const int fld = q == 0 ? 6 : (q < 4 ? 6 + q : q - 4);   // alp, betx..betz, gxx..gzz
-      bulk_copy_g2s(sM + (size_t)q * slotM + r * nt, f.adm[fld] + baseM + r * rs, rowb, &mbar);
+      bulk_copy_g2s(sM + (size_t)q * slotM + r * nt, f.adm[fld] + baseM + r * rs, rowb, &mbarM);
     }
   }
   }
@@ -212,6 +218,9 @@ k_flux_tma(const __grid_constant__ Par P, const __grid_constant__ Fields f, int 
         sR[v] = qm;
       }
     }
+  }
+  mbar_wait(&mbarM, 0);
+  if (active) {
 #pragma unroll
     for (int q = 0; q < 10; ++q) {
       const double* g = DIR == 0 ? sM + (size_t)q * slotM + a * nt + ii - 1 : sM + (size_t)q * slotM + a * nt + ii;
@@ -269,7 +278,7 @@ __global__ void __launch_bounds__(TMA_THREADS, AK_TMAC_MINB)
 k_flux_tma_cell(const __grid_constant__ Par P, const __grid_constant__ Fields f, int NA,
                 const __grid_constant__ TileMaps maps, int use_tm) {
   extern __shared__ __align__(128) double sm[];
-  __shared__ uint64_t mbar;
+  __shared__ uint64_t mbar, mbarM;      // primitive slabs / metric slabs: the metric lands while the states are reconstructed
   const int nt = P.nt, e = P.n + 2, t = threadIdx.x;
   constexpr int t1 = (DIR + 1) % 3, t2 = (DIR + 2) % 3;
   const int maxW = DIR == 0 ? NA : NA + 5, maxM = DIR == 0 ? NA : NA + 1;
@@ -293,12 +302,15 @@ k_flux_tma_cell(const __grid_constant__ Par P, const __grid_constant__ Fields f,
   else { baseW = ix.cell(m, d0 - 3, o, 0); baseM = ix.cell(m, d0 - 1, o, 0); rs = (long long)nt * nt; }
   const unsigned rowb = (unsigned)(nt * sizeof(double));
   __shared__ unsigned nzacc;
-  if (t == 0) { mbar_init(&mbar, 1); nzacc = 0; }
+  if (t == 0) { mbar_init(&mbar, 1); mbar_init(&mbarM, 1); nzacc = 0; }
   const unsigned ld = slots_to_load<DIR>(P, f, m);                  // block-uniform: slots that are staged at all
   __syncthreads();
   if (use_tm) {
     if (t < 32) {                                                   // lanes 0..16 of warp 0: one field each
-      if (t == 0) mbar_arrive_expect_tx(&mbar, (unsigned)(__popc(ld) * maxW + 10 * maxM) * rowb);
+      if (t == 0) {
+        mbar_arrive_expect_tx(&mbar, (unsigned)(__popc(ld) * maxW) * rowb);
+        mbar_arrive_expect_tx(&mbarM, (unsigned)(10 * maxM) * rowb);
+      }
       __syncwarp();
       const int K = DIR == 2 ? m * nt + d0 : m * nt + o;            // plane coordinate of tile row 0 ...
       if (t < 7) {
@@ -308,11 +320,14 @@ k_flux_tma_cell(const __grid_constant__ Par P, const __grid_constant__ Fields f,
         }
       } else if (t < 17) {
         const int cM1 = DIR == 0 ? d0 : (DIR == 1 ? d0 - 1 : o), cM2 = DIR == 2 ? K - 1 : K;
-        tma_load_3d(sM + (size_t)(t - 7) * slotM, &maps.m[t - 7], 0, cM1, cM2, &mbar);
+        tma_load_3d(sM + (size_t)(t - 7) * slotM, &maps.m[t - 7], 0, cM1, cM2, &mbarM);
       }
     }
   } else {
-  if (t == 0) mbar_arrive_expect_tx(&mbar, (unsigned)(__popc(ld) * nW + 10 * nM) * rowb);
+  if (t == 0) {
+    mbar_arrive_expect_tx(&mbar, (unsigned)(__popc(ld) * nW) * rowb);
+    mbar_arrive_expect_tx(&mbarM, (unsigned)(10 * nM) * rowb);
+  }
   const int ncW = 7 * nW, nc = ncW + 10 * nM;
   for (int c = t; c < nc; c += (int)blockDim.x) {
     if (c < ncW) {
@@ -323,7 +338,7 @@ k_flux_tma_cell(const __grid_constant__ Par P, const __grid_constant__ Fields f,
       const int cc = c - ncW;
       const int q = cc / nM, r = cc - q * nM;
       const int fld = q == 0 ? 6 : (q < 4 ? 6 + q : q - 4);
-      bulk_copy_g2s(sM + (size_t)q * slotM + r * nt, f.adm[fld] + baseM + r * rs, rowb, &mbar);
+      bulk_copy_g2s(sM + (size_t)q * slotM + r * nt, f.adm[fld] + baseM + r * rs, rowb, &mbarM);
     }
   }
   }
@@ -368,6 +383,7 @@ k_flux_tma_cell(const __grid_constant__ Par P, const __grid_constant__ Fields f,
 #endif
   const int back = DIR == 0 ? 1 : nci;                 // thread of the lower cell
   double sL[7], mL[10], mR[10], Fo[7];
+  mbar_wait(&mbarM, 0);
   if (has_face) {
 #pragma unroll
     for (int v = 0; v < 7; ++v) sL[v] = sQ[v * TMA_THREADS + t - back];
