@@ -67,6 +67,7 @@ struct ak_ctx {
   int cap[8];                   // grid caps (blocks) per kernel class in the overlapped schedule, 0 = none
   int sweep_smem_pad;           // bytes: dynamic shared memory the sweeps ask for at least when overlapped
   unsigned int* zflags;         // [nmb] per-block zero-field flags written by k_con2prim (Fields::zflags)
+  int fuse_src;                 // 1: part (6) runs inside the FOFC-test kernel (+ k_src_fix), 0: k_div_src after the re-flux
   int tile_tm;                  // tile kernels: stage tiles with tensor-map box copies (1) or row by row (0)
   int pencil_wi;                // y/z sweeps: x-lanes per block of k_flux_pencil (0: tile kernels k_flux_tma)
   // FOFC stage blend (ak_set_fofc_blend)
@@ -488,7 +489,14 @@ int launch_fofc(ak_ctx* c, const Lane& L, double dt) {
     CK(cudaMemsetAsync(L.f.stats + S_FOFC_CELLS, 0, sizeof(unsigned long long) * 2, L.st));
     if (L.P.fofc) {
       const unsigned g = capped(ntest, 128, L.ov ? c->cap[KC_FOFC_TEST] : 0);
-      if ((long long)g * 128 < ntest) {
+      if (c->fuse_src && L.f.dU[0]) {
+        // part (6) fused into the test kernel (k_src_fix after the re-flux redoes the cells it touches)
+        if ((long long)g * 128 < ntest) {
+          if (L.P.eos) k_fofc_test<1, true, true><<<g, 128, 0, L.st>>>(L.P, L.f, dt);
+          else k_fofc_test<0, true, true><<<g, 128, 0, L.st>>>(L.P, L.f, dt);
+        } else if (L.P.eos) k_fofc_test<1, false, true><<<g, 128, 0, L.st>>>(L.P, L.f, dt);
+        else k_fofc_test<0, false, true><<<g, 128, 0, L.st>>>(L.P, L.f, dt);
+      } else if ((long long)g * 128 < ntest) {
         if (L.P.eos) k_fofc_test<1, true><<<g, 128, 0, L.st>>>(L.P, L.f, dt);
         else k_fofc_test<0, true><<<g, 128, 0, L.st>>>(L.P, L.f, dt);
       } else if (L.P.eos) k_fofc_test<1><<<g, 128, 0, L.st>>>(L.P, L.f, dt);
@@ -540,6 +548,17 @@ int launch_ct(ak_ctx* c, const Lane& L, bool have_cell_emf) {
 int launch_src(ak_ctx* c, const Lane& L) {
   Timer t(c, KC_SRC, L.st);
   const long long n = L.P.n;
+  if (c->fuse_src && L.P.fofc) {
+    // the fused FOFC-test kernel has written dU~/dt from the high-order fluxes: redo the cells with a re-fluxed face
+    const long long ntest = (n + 2) * (n + 2) * (n + 2) * L.P.nmb;
+    unsigned g = (unsigned)(ntest < 148LL * 8 * 128 ? nblk(ntest, 128) : 148 * 8);
+    if (L.ov && c->cap[KC_SRC] > 0 && g > (unsigned)c->cap[KC_SRC]) g = (unsigned)c->cap[KC_SRC];
+    if (L.P.eos) k_src_fix<1><<<g, 128, 0, L.st>>>(L.P, L.f);
+    else k_src_fix<0><<<g, 128, 0, L.st>>>(L.P, L.f);
+    CK(cudaGetLastError());
+    c->launches[KC_SRC] += 1;
+    return AK_OK;
+  }
   const unsigned g = capped(n * n * n * L.P.nmb, 128, L.ov ? c->cap[KC_SRC] : 0);
   if ((long long)g * 128 < n * n * n * L.P.nmb) {
     if (L.P.eos) k_div_src<1, true><<<g, 128, 0, L.st>>>(L.P, L.f);
@@ -640,6 +659,8 @@ int ak_create(const ak_params* p, const double* dx3, ak_ctx** out) {
     c->sweep_smem_pad = envi("AK_OV_SMEM_PAD", AK_OV_SMEM_PAD_DEFAULT);
     c->pencil_wi = envi("AK_PENCIL_WI", AK_PENCIL_WI_DEFAULT);
     c->tile_tm = envi("AK_TILE_TENSORMAP", 1);
+    // measured on C4 (DESIGN.md §6 item 21): fused 4.18 + fix 0.51 ms against 1.95 + 2.15 ms separately -> off
+    c->fuse_src = envi("AK_FUSE_SRC", 0);
   }
   Par& P = c->P;
   P.nmb = p->nmb; P.n = p->n; P.nt = p->n + 8; P.px = P.nt + 4; P.is = 4; P.ie = p->n + 3;

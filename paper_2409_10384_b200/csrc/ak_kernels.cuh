@@ -258,9 +258,18 @@ __device__ __forceinline__ double div_flux(const Fields& f, const Ix& ix, int v,
          (f.F[14 + v][fz + sz] - f.F[14 + v][fz]) * idx[2];
 }
 
+template <int EOS>
+__device__ __forceinline__ void div_src_cell(const Par& P, const Fields& f, int m, long long c, const double div[5]);   // ak_source.cuh
+
+#ifndef AK_FSRC_MINB
+#define AK_FSRC_MINB 4    // blocks/SM of the FOFC test fused with part (6)
+#endif
 // ---- K3: FOFC estimate and test (DMP Eq. 12) -------------------------------
-template <int EOS = 0, bool STRIDE = false>
-__global__ void __launch_bounds__(128, AK_FOFC_MINB) k_fofc_test(const __grid_constant__ Par P,
+// SRC: also part (6) for the interior cells, from the flux differences this kernel forms anyway (the high-order
+// fluxes; cells next to re-fluxed faces are redone by k_src_fix): the 15 flux fields are read once instead of
+// twice, and the memory-bound sources of one warp overlap the dependent chains of another's con2prim check.
+template <int EOS = 0, bool STRIDE = false, bool SRC = false>
+__global__ void __launch_bounds__(128, SRC ? AK_FSRC_MINB : AK_FOFC_MINB) k_fofc_test(const __grid_constant__ Par P,
                                                    const __grid_constant__ Fields f, double dt) {
   long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   do {
@@ -270,11 +279,17 @@ __global__ void __launch_bounds__(128, AK_FOFC_MINB) k_fofc_test(const __grid_co
   const long long c = ix.cell(m, k, j, i);
   const double idx[3] = {1.0 / f.dx[3 * m + 0], 1.0 / f.dx[3 * m + 1], 1.0 / f.dx[3 * m + 2]};
   double Us[5], Bc[3], W5[5];
+  {
+    double dv[5];
 #pragma unroll
-  for (int v = 0; v < 5; ++v) {
-    const double div = div_flux(f, ix, v, m, k, j, i, idx);
-    if (f.U0[0]) Us[v] = f.fa * f.U0[v][c] + f.fb * (f.U[v][c] - dt * div);
-    else Us[v] = f.U[v][c] - dt * div;
+    for (int v = 0; v < 5; ++v) dv[v] = div_flux(f, ix, v, m, k, j, i, idx);
+    if (SRC && i >= P.is && i <= P.ie && j >= P.is && j <= P.ie && k >= P.is && k <= P.ie)
+      div_src_cell<EOS>(P, f, m, c, dv);
+#pragma unroll
+    for (int v = 0; v < 5; ++v) {
+      if (f.U0[0]) Us[v] = f.fa * f.U0[v][c] + f.fb * (f.U[v][c] - dt * dv[v]);
+      else Us[v] = f.U[v][c] - dt * dv[v];
+    }
   }
   Met3 g;
   load_met3(f, c, g);

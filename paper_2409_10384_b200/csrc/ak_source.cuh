@@ -9,27 +9,17 @@ namespace ak {
 #ifndef AK_SRC_MINB
 #define AK_SRC_MINB 4
 #endif
-template <int EOS = 0, bool STRIDE = false>
-__global__ void __launch_bounds__(128, AK_SRC_MINB) k_div_src(const __grid_constant__ Par P,
-                                                 const __grid_constant__ Fields f) {
-  const int n = P.n;
-  const long long per = (long long)n * n * n;
-  long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  do {
-  if (idx >= per * P.nmb) return;
-  const int m = (int)(idx / per);
-  int r = (int)(idx - (long long)m * per);
-  const int i = r % n + P.is; r /= n;
-  const int j = r % n + P.is;
-  const int k = r / n + P.is;
-  const Ix ix{P.nt, P.px};
-  const long long c = ix.cell(m, k, j, i);
+// Part (6) for ONE interior cell c of block m, given the flux differences div[v] (div_flux) of the five hydro
+// variables: dU~/dt = -div + geometric sources (Eq. 9); also the matter epilogue.  Called by k_div_src (one
+// thread per interior cell), by the fused FOFC-test kernel (k_fofc_test<EOS, STRIDE, true>, which has the
+// same div in registers) and by k_src_fix (cells next to re-fluxed faces).
+template <int EOS>
+__device__ __forceinline__ void div_src_cell(const Par& P, const Fields& f, int m, long long c, const double div[5]) {
   const double dxm[3] = {f.dx[3 * m + 0], f.dx[3 * m + 1], f.dx[3 * m + 2]};
-  const double idx3[3] = {1.0 / dxm[0], 1.0 / dxm[1], 1.0 / dxm[2]};
   const double h2[3] = {0.5 / dxm[0], 0.5 / dxm[1], 0.5 / dxm[2]};
   double du[5];
 #pragma unroll
-  for (int v = 0; v < 5; ++v) du[v] = -div_flux(f, ix, v, m, k, j, i, idx3);
+  for (int v = 0; v < 5; ++v) du[v] = -div[v];
 
   Met3 g, gu;
   load_met3(f, c, g);
@@ -120,8 +110,61 @@ __global__ void __launch_bounds__(128, AK_SRC_MINB) k_div_src(const __grid_const
   du[4] = du[4] + sdet * (alp * KS - Sda);
 #pragma unroll
   for (int v = 0; v < 5; ++v) f.dU[v][c] = du[v];
+}
+
+template <int EOS = 0, bool STRIDE = false>
+__global__ void __launch_bounds__(128, AK_SRC_MINB) k_div_src(const __grid_constant__ Par P,
+                                                 const __grid_constant__ Fields f) {
+  const int n = P.n;
+  const long long per = (long long)n * n * n;
+  long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  do {
+  if (idx >= per * P.nmb) return;
+  const int m = (int)(idx / per);
+  int r = (int)(idx - (long long)m * per);
+  const int i = r % n + P.is; r /= n;
+  const int j = r % n + P.is;
+  const int k = r / n + P.is;
+  const Ix ix{P.nt, P.px};
+  const long long c = ix.cell(m, k, j, i);
+  const double idx3[3] = {1.0 / f.dx[3 * m + 0], 1.0 / f.dx[3 * m + 1], 1.0 / f.dx[3 * m + 2]};
+  double div[5];
+#pragma unroll
+  for (int v = 0; v < 5; ++v) div[v] = div_flux(f, ix, v, m, k, j, i, idx3);
+  div_src_cell<EOS>(P, f, m, c, div);
   idx += (long long)gridDim.x * blockDim.x;
   } while (STRIDE);
+}
+
+// Part (6) again for the interior cells that have a re-fluxed face: the flagged cells of the FOFC list and
+// their six face neighbours (a face is redone iff one of its two cells is flagged).  The fused FOFC-test
+// kernel wrote dU~/dt of every interior cell from the high-order fluxes; these cells are recomputed from the
+// final ones with the same per-cell function, so every value equals what k_div_src after the re-flux would
+// write.  A cell reached from two flagged neighbours is written twice with the same bits.
+template <int EOS = 0>
+__global__ void __launch_bounds__(128, AK_SRC_MINB) k_src_fix(const __grid_constant__ Par P,
+                                                              const __grid_constant__ Fields f) {
+  const unsigned cnt = f.count[3];
+  const Ix ix{P.nt, P.px};
+  const long long nt = P.nt;
+  for (unsigned long long e = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; e < 7ull * cnt;
+       e += (unsigned long long)gridDim.x * blockDim.x) {
+    const unsigned which = (unsigned)(e / cnt);                 // 0: the cell itself, 1..6: -x +x -y +y -z +z
+    long long c = (long long)f.list[e - (unsigned long long)which * cnt];
+    const long long st = which == 0 ? 0 : (which <= 2 ? 1 : (which <= 4 ? nt : nt * nt));
+    c += (which & 1u) ? -st : st;
+    const int i = (int)(c % nt);
+    const long long row = c / nt;
+    const int j = (int)(row % nt);
+    const long long mk = row / nt;
+    const int k = (int)(mk % nt), m = (int)(mk / nt);
+    if (i < P.is || i > P.ie || j < P.is || j > P.ie || k < P.is || k > P.ie) continue;     // interior cells only
+    const double idx3[3] = {1.0 / f.dx[3 * m + 0], 1.0 / f.dx[3 * m + 1], 1.0 / f.dx[3 * m + 2]};
+    double div[5];
+#pragma unroll
+    for (int v = 0; v < 5; ++v) div[v] = div_flux(f, ix, v, m, k, j, i, idx3);
+    div_src_cell<EOS>(P, f, m, c, div);
+  }
 }
 
 // ---- matter terms for a spacetime solver: E = tau + D, S_i, S_ij = T_ij, undensitised,

@@ -254,3 +254,27 @@ def test_exact_shortcuts_with_signed_zeros_and_partly_zero_fields():
         assert np.array_equal(x, y)
         assert np.array_equal(np.signbit(x), np.signbit(y))
     assert np.array_equal(ra["flag"], rb["flag"])
+
+
+def test_fused_fofc_test_and_sources_path_is_exact(monkeypatch):
+    """AK_FUSE_SRC=1 (opt-in; slower on C4, DESIGN.md §6 item 21): part (6) inside the FOFC-test kernel from the
+    high-order fluxes, then k_src_fix for the cells next to re-fluxed faces.  Must give the bits of the default
+    path (k_div_src after the re-flux), matter epilogue included, on blocks with many flags."""
+    import torch
+    from paper_2409_10384_b200 import ak
+    w = _noise_batch(5, 8, seed0=90)
+    out = []
+    for fuse in ("0", "1"):
+        monkeypatch.setenv("AK_FUSE_SRC", fuse)             # read by ak_create
+        with gpukit.GpuStage(copy.deepcopy(w), recon=2, dmp_M=1.1) as g:
+            M = [torch.full_like(g.W[0], float("nan")) for _ in range(10)]
+            ak.ak_rhs(g.ctx, g.U, g.Bf, g.W, 0, g.dt_fofc, g.dU, g.E, g.flag, g.status, matter=M)
+            torch.cuda.synchronize()
+            out.append((g.result(), [t.cpu().numpy() for t in M], g.stats()))
+    (ra, ma, sa), (rb, mb, sb) = out
+    assert np.count_nonzero(ra["flag"]) > 20 and sa == sb
+    for x, y in zip(ra["dU"] + ra["E"] + ra["W"], rb["dU"] + rb["E"] + rb["W"]):
+        assert np.array_equal(x, y)
+    for x, y in zip(ma, mb):
+        assert np.array_equal(x, y, equal_nan=True)
+    assert np.array_equal(ra["flag"], rb["flag"])
