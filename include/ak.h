@@ -156,6 +156,19 @@ int ak_rhs(ak_ctx*, const ak_cons* U, const ak_faceB* Bf, const ak_prim* W, int 
  * another).  nchunks is clamped to nmb. */
 int ak_set_overlap(ak_ctx*, int nchunks);
 
+/* CUDA-graph replay of the stage ("launches captured once in a CUDA graph per ctx"; D:§6.4).  With on != 0,
+ * ak_rhs in the serial schedule runs an argument set (every pointer, the parameters, w_is_valid, dt_fofc, the
+ * FOFC blend, the shortcut mask) plainly the first time it sees it, captures the same launch sequence into a
+ * CUDA graph the second time (on a context-owned stream: the caller's may be the legacy default stream, which
+ * cannot capture) and from then on replays it with one cudaGraphLaunch on the context's stream.  Up to four
+ * argument sets are kept (the stages of an SSP-RK3 step differ in their blend), least recently used evicted.
+ * Same kernels, same bits.  It pays where a stage is launch-bound (a few small MeshBlocks: D:§6.4 has the
+ * numbers), not on large batches.  Bypassed while ak_timing is enabled and under ak_set_overlap.  on == 0
+ * synchronises the context's stream and destroys the graphs.  ak_graph_replays: stages replayed from a graph
+ * since the last ak_set_graph (diagnostic; < 0 for a NULL context). */
+int ak_set_graph(ak_ctx*, int on);
+long long ak_graph_replays(const ak_ctx*);
+
 /* Exact data-dependent shortcuts (D:§6.3).  mask bit 0: a field of (u^x, u^y, u^z, B~cc^t1, B~cc^t2) that is
  * +0.0 on the whole tile a sweep block stages is not reconstructed (every scheme of P:133 returns +0.0 on
  * both sides of every face for it); bit 1: a cell with S~ = 0 and B~ = 0 exactly runs its con2prim root

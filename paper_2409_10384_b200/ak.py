@@ -25,7 +25,7 @@ EXPORTS = ("ak_create", "ak_set_metric", "ak_con2prim", "ak_rhs", "ak_emf", "ak_
            "ak_set_fofc_blend", "ak_fill_ghosts", "ak_stage_update", "ak_advance", "ak_set_neighbors",
            "ak_matter_sources", "ak_halo_slab_elems", "ak_halo_pack", "ak_halo_unpack",
            "ak_set_eos_hybrid", "ak_set_overlap", "ak_advance_hooked",
-           "ak_set_exact_shortcuts", "ak_con2prim_static")
+           "ak_set_exact_shortcuts", "ak_con2prim_static", "ak_set_graph", "ak_graph_replays")
 BC_PERIODIC, BC_OUTFLOW = 0, 1
 
 _dp = C.POINTER(C.c_double)
@@ -128,6 +128,9 @@ def lib():
         L.ak_set_neighbors.argtypes = [C.c_void_p, C.POINTER(C.c_int), C.c_int]
         L.ak_set_overlap.argtypes = [C.c_void_p, C.c_int]
         L.ak_set_exact_shortcuts.argtypes = [C.c_void_p, C.c_int]
+        L.ak_set_graph.argtypes = [C.c_void_p, C.c_int]
+        L.ak_graph_replays.argtypes = [C.c_void_p]
+        L.ak_graph_replays.restype = C.c_longlong
         L.ak_con2prim_static.argtypes = [C.POINTER(AkParams), C.POINTER(AkCons), C.POINTER(AkFaceB), C.POINTER(AkAdm),
                                          C.POINTER(AkPrim), C.c_void_p, C.POINTER(AkStats)]
         _lib = L
@@ -237,6 +240,15 @@ def ak_con2prim_static(params, U, Bf, adm, W, status=None, want_counts=False):
     if want_counts:
         return dict(n_c2p_fail=s.n_c2p_fail, n_cons_floor=s.n_cons_floor, n_prim_floor=s.n_prim_floor)
     return None
+
+
+def ak_set_graph(ctx, on):
+    """CUDA-graph replay of the serial stage (include/ak.h)."""
+    _chk(lib().ak_set_graph(ctx, int(on)), "ak_set_graph")
+
+
+def ak_graph_replays(ctx):
+    return int(lib().ak_graph_replays(ctx))
 
 
 def ak_set_exact_shortcuts(ctx, mask):

@@ -67,6 +67,12 @@ struct ak_ctx {
   int cap[8];                   // grid caps (blocks) per kernel class in the overlapped schedule, 0 = none
   int sweep_smem_pad;           // bytes: dynamic shared memory the sweeps ask for at least when overlapped
   unsigned int* zflags;         // [nmb] per-block zero-field flags written by k_con2prim (Fields::zflags)
+  // CUDA-graph replay of the serial stage (ak_set_graph): a few instantiated graphs keyed on the arguments
+  int graph_on;
+  cudaStream_t gstream;         // capture stream (the caller's may be the legacy default stream, which cannot capture)
+  struct GraphSlot { unsigned long long key; cudaGraphExec_t exec; unsigned long long age; } gslot[4];
+  unsigned long long gclock;
+  long long graph_replays;      // stages replayed from a graph since ak_set_graph (diagnostic)
   int fuse_src;                 // 1: part (6) runs inside the FOFC-test kernel (+ k_src_fix), 0: k_div_src after the re-flux
   int tile_tm;                  // tile kernels: stage tiles with tensor-map box copies (1) or row by row (0)
   int pencil_wi;                // y/z sweeps: x-lanes per block of k_flux_pencil (0: tile kernels k_flux_tma)
@@ -740,6 +746,8 @@ int ak_destroy(ak_ctx* c) {
     cudaFree(c->lane_mask[l][0]); cudaFree(c->lane_mask[l][1]);
   }
   if (c->lane_stats_h) cudaFreeHost(c->lane_stats_h);
+  for (auto& g : c->gslot) if (g.exec) cudaGraphExecDestroy(g.exec);
+  if (c->gstream) cudaStreamDestroy(c->gstream);
   if (c->ov_ev) {
     for (int q = 0; q < c->ov_nev; ++q) if (c->ov_ev[q]) cudaEventDestroy(c->ov_ev[q]);
     free(c->ov_ev);
@@ -814,6 +822,96 @@ int ak_con2prim(ak_ctx* c, const ak_cons* U, const ak_faceB* Bf, const ak_prim* 
   return launch_c2p(c, L, false);
 }
 
+}  // extern "C"
+
+namespace {
+// the serial schedule of one stage: the whole batch, kernel after kernel, on stream st
+int rhs_serial(ak_ctx* c, const Fields& f, int w_is_valid, double dt_fofc, cudaStream_t st) {
+  // counters of every chunk slot start from zero (a stage that skips part (1) reports no con2prim counts)
+  CK(cudaMemsetAsync(c->stats, 0, sizeof(unsigned long long) * S_NSTAT * MAXCH, st));
+  CK(cudaMemsetAsync(c->count, 0, sizeof(unsigned) * 4 * MAXCH, st));
+  int r;
+  const Lane L = {c->P, f, st, false};
+  if (!w_is_valid && (r = launch_c2p(c, L, true)) != AK_OK) return r;
+  if ((r = launch_flux<0>(c, L)) != AK_OK) return r;
+  if ((r = launch_flux<1>(c, L)) != AK_OK) return r;
+  if ((r = launch_flux<2>(c, L)) != AK_OK) return r;
+  if ((r = launch_fofc(c, L, dt_fofc)) != AK_OK) return r;
+  if ((r = launch_ct(c, L, !w_is_valid)) != AK_OK) return r;
+  return launch_src(c, L);
+}
+
+// FNV-1a over everything the launch sequence depends on: the parameters, every pointer, the blend, the flags
+unsigned long long rhs_key(const ak_ctx* c, const Fields& f, int w_is_valid, double dt_fofc) {
+  unsigned long long h = 1469598103934665603ull;
+  auto mix = [&](const void* p, size_t n) {
+    const unsigned char* b = (const unsigned char*)p;
+    for (size_t q = 0; q < n; ++q) { h ^= b[q]; h *= 1099511628211ull; }
+  };
+  mix(&c->P, sizeof(Par)); mix(&f, sizeof(Fields)); mix(&w_is_valid, sizeof(int)); mix(&dt_fofc, sizeof(double));
+  mix(&c->tile_tm, sizeof(int)); mix(&c->pencil_wi, sizeof(int)); mix(&c->fuse_src, sizeof(int));
+  return h | 1ull;               // 0 marks an empty slot
+}
+
+// Serial stage through the graph cache.  First sighting of an argument set: plain launches (this also raises
+// the shared-memory attributes, which must not happen inside a capture).  Second: the same launch code runs
+// under stream capture on the context's capture stream and is instantiated.  From then on: one cudaGraphLaunch
+// on the caller's stream.
+int rhs_graphed(ak_ctx* c, const Fields& f, int w_is_valid, double dt_fofc) {
+  const unsigned long long key = rhs_key(c, f, w_is_valid, dt_fofc);
+  ak_ctx::GraphSlot* s = nullptr;
+  for (auto& g : c->gslot) if (g.key == key) s = &g;
+  if (s && s->exec) {
+    s->age = ++c->gclock;
+    CK(cudaGraphLaunch(s->exec, c->stream));
+    c->graph_replays += 1;
+    return AK_OK;
+  }
+  if (!s) {                      // remember the key (evicting the least recently used slot), run it plainly
+    s = &c->gslot[0];
+    for (auto& g : c->gslot) if (g.age < s->age) s = &g;
+    if (s->exec) { cudaGraphExecDestroy(s->exec); s->exec = nullptr; }
+    s->key = key; s->age = ++c->gclock;
+    return rhs_serial(c, f, w_is_valid, dt_fofc, c->stream);
+  }
+  s->age = ++c->gclock;
+  cudaGraph_t graph = nullptr;
+  CK(cudaStreamBeginCapture(c->gstream, cudaStreamCaptureModeThreadLocal));
+  const int r = rhs_serial(c, f, w_is_valid, dt_fofc, c->gstream);
+  const cudaError_t e = cudaStreamEndCapture(c->gstream, &graph);
+  if (r != AK_OK || e != cudaSuccess || !graph) {
+    if (graph) cudaGraphDestroy(graph);
+    cudaGetLastError();
+    s->key = 0;                  // do not try this argument set again under capture
+    if (r != AK_OK) return r;
+    return rhs_serial(c, f, w_is_valid, dt_fofc, c->stream);
+  }
+  const cudaError_t ei = cudaGraphInstantiate(&s->exec, graph, 0);
+  cudaGraphDestroy(graph);
+  if (ei != cudaSuccess) { s->exec = nullptr; s->key = 0; cudaGetLastError(); return rhs_serial(c, f, w_is_valid, dt_fofc, c->stream); }
+  CK(cudaGraphLaunch(s->exec, c->stream));
+  c->graph_replays += 1;
+  return AK_OK;
+}
+}  // namespace
+
+extern "C" {
+
+int ak_set_graph(ak_ctx* c, int on) {
+  if (!c) return AK_EINVAL;
+  CK(cudaSetDevice(c->hp.device));
+  if (on && !c->gstream) CK(cudaStreamCreateWithFlags(&c->gstream, cudaStreamNonBlocking));
+  if (!on) {
+    CK(cudaStreamSynchronize(c->stream));
+    for (auto& g : c->gslot) { if (g.exec) cudaGraphExecDestroy(g.exec); g.exec = nullptr; g.key = 0; g.age = 0; }
+  }
+  c->graph_on = on != 0;
+  c->graph_replays = 0;
+  return AK_OK;
+}
+
+long long ak_graph_replays(const ak_ctx* c) { return c ? c->graph_replays : -1; }
+
 int ak_rhs(ak_ctx* c, const ak_cons* U, const ak_faceB* Bf, const ak_prim* W, int w_is_valid, double dt_fofc,
            const ak_rhs_out* out) {
   if (!c || !out) return AK_EINVAL;
@@ -838,23 +936,18 @@ int ak_rhs(ak_ctx* c, const ak_cons* U, const ak_faceB* Bf, const ak_prim* W, in
   }
   CK(cudaSetDevice(c->hp.device));
   c->stats_from_host = false;
-  // counters of every chunk slot start from zero (a stage that skips part (1) reports no con2prim counts)
-  CK(cudaMemsetAsync(c->stats, 0, sizeof(unsigned long long) * S_NSTAT * MAXCH, c->stream));
-  CK(cudaMemsetAsync(c->count, 0, sizeof(unsigned) * 4 * MAXCH, c->stream));
   int r;
   const int nch = c->ov_chunks < 2 ? 1 : (c->ov_chunks < c->P.nmb ? c->ov_chunks : c->P.nmb);
   if (nch < 2) {
-    // serial schedule: the whole batch, kernel after kernel, on the context's stream
-    const Lane L = {c->P, f, c->stream, false};
-    if (!w_is_valid && (r = launch_c2p(c, L, true)) != AK_OK) return r;
-    if ((r = launch_flux<0>(c, L)) != AK_OK) return r;
-    if ((r = launch_flux<1>(c, L)) != AK_OK) return r;
-    if ((r = launch_flux<2>(c, L)) != AK_OK) return r;
-    if ((r = launch_fofc(c, L, dt_fofc)) != AK_OK) return r;
-    c->have_flux = true;
-    if ((r = launch_ct(c, L, !w_is_valid)) != AK_OK) return r;
-    return launch_src(c, L);
+    // serial schedule; replayed from a CUDA graph when ak_set_graph is on (not while ak_timing brackets classes)
+    r = (c->graph_on && !c->timing) ? rhs_graphed(c, f, w_is_valid, dt_fofc)
+                                    : rhs_serial(c, f, w_is_valid, dt_fofc, c->stream);
+    if (r == AK_OK) c->have_flux = true;
+    return r;
   }
+  // counters of every chunk slot start from zero (a stage that skips part (1) reports no con2prim counts)
+  CK(cudaMemsetAsync(c->stats, 0, sizeof(unsigned long long) * S_NSTAT * MAXCH, c->stream));
+  CK(cudaMemsetAsync(c->count, 0, sizeof(unsigned) * 4 * MAXCH, c->stream));
   // overlapped schedule: MeshBlocks are independent, so the batch is cut into nch chunks.
   // Stream A runs part (1) of chunk i+1 and stream C parts (4)-(6) of chunk i-1 (memory- and latency-bound,
   // capped grids, high priority) while stream B runs the fp64-bound sweeps of chunk i.  Only events order

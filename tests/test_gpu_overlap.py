@@ -278,3 +278,57 @@ def test_fused_fofc_test_and_sources_path_is_exact(monkeypatch):
     for x, y in zip(ma, mb):
         assert np.array_equal(x, y, equal_nan=True)
     assert np.array_equal(ra["flag"], rb["flag"])
+
+
+def test_graph_replay_equals_plain_launches():
+    """ak_set_graph: the stage replayed from a CUDA graph gives the bits of the plain launches, call after call,
+    with the graph really in use (ak_graph_replays), through ak_rhs and through ak_advance (three blends per RK3
+    step -> three cached graphs), and a changed argument (another output buffer, w_is_valid) is noticed."""
+    import torch
+    from paper_2409_10384_b200 import ak
+    w = _noise_batch(3, 8, seed0=120)
+    over = dict(recon=2, dmp_M=1.1)
+    with gpukit.GpuStage(copy.deepcopy(w), **over) as a, gpukit.GpuStage(copy.deepcopy(w), **over) as b:
+        ak.ak_set_graph(b.ctx, 1)
+        for it in range(5):                    # plain, capture + replay, replay, replay, replay
+            a.rhs(); b.rhs()
+            ra, rb = a.result(), b.result()
+            for k in ("dU", "E", "W", "U"):
+                for x, y in zip(ra[k], rb[k]):
+                    assert np.array_equal(x, y), (it, k)
+            assert np.array_equal(ra["flag"], rb["flag"]) and np.array_equal(ra["status"], rb["status"])
+            assert a.stats() == b.stats()
+        assert ak.ak_graph_replays(b.ctx) == 4
+        assert np.count_nonzero(ra["flag"]) > 0
+        # another dU buffer: a new argument set, not a stale replay into the old buffer
+        old = [t.clone() for t in b.dU]
+        b.dU = [torch.zeros_like(t) for t in b.dU]            # (dU is written on interior cells only)
+        for t in old:
+            t.fill_(123.0)
+        b.rhs()
+        for x, y in zip(b.dU, a.dU):
+            assert torch.equal(x, y)
+        assert all(bool((t == 123.0).all()) for t in old)
+        a.rhs(w_is_valid=True); b.rhs(w_is_valid=True); b.rhs(w_is_valid=True); b.rhs(w_is_valid=True)
+        for x, y in zip(b.dU + b.E, a.dU + a.E):
+            assert torch.equal(x, y)
+        # timing on: graphs bypassed, still the same
+        ak.ak_timing(b.ctx, 1); b.rhs(w_is_valid=True); ak.ak_timing(b.ctx, 0)
+        for x, y in zip(b.dU + b.E, a.dU + a.E):
+            assert torch.equal(x, y)
+        ak.ak_set_graph(b.ctx, 0)
+        b.rhs(w_is_valid=True)
+        for x, y in zip(b.dU + b.E, a.dU + a.E):
+            assert torch.equal(x, y)
+    res = []
+    for on in (0, 1):
+        with gpukit.GpuStage(copy.deepcopy(w), **over) as g:
+            ak.ak_set_graph(g.ctx, on)
+            ak.ak_advance(g.ctx, 3, 4, 0.02 / 8, (0, 1, 0), g.U, g.Bf, g.W)
+            torch.cuda.synchronize()
+            res.append([t.cpu().numpy() for t in g.U + g.Bf + g.W])
+            if on:
+                assert ak.ak_graph_replays(g.ctx) >= 6          # 12 stages: 3 plain, then graphs
+    for x, y in zip(*res):
+        assert np.array_equal(x, y)
+    assert ak.lib().ak_set_graph(None, 1) == ak.AK_EINVAL
