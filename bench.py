@@ -369,9 +369,12 @@ def run_e2e(R, steps):
     hflag, hst = pin("cell", torch.uint8), pin("cell", torch.uint8)
     nbytes = lambda ts: int(sum(t.numel() * t.element_size() for t in ts))
     h2d = nbytes(hU + hB)
-    d2h = nbytes(hU + hdU + hE + [hflag, hst])
     call = lambda: ak.ak_rhs_host(R["ctx"], hU, hB, None, R["dt_fofc"], hdU, hE, hflag, hst)
     call()                                                   # warm-up: allocates staging
+    # device -> host per step: dU/dt, E and both masks whole, and of U~ the cells part (1) changed (status != 0:
+    # five doubles each, stored straight into the pinned arrays by the library instead of copying U~ back whole)
+    n_changed = int((hst != 0).sum())
+    d2h = nbytes(hdU + hE + [hflag, hst]) + 40 * n_changed
     ts = []
     for _ in range(steps):
         for h, h0 in zip(hU, hU0):
@@ -385,9 +388,9 @@ def run_e2e(R, steps):
         import torch.distributed as dist
         dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
     val = R["zones_total"] * steps / float(tmax.item())
-    # the host path must give what the device path gave
-    same = all(bool(torch.equal(h, d.cpu())) for h, d in zip(hdU, R["dU"]))
-    return dict(value=val, unit=UNIT, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h, steps=steps,
+    # the host path must give what the device path gave (dU/dt; and U~ with the floored cells written back)
+    same = all(bool(torch.equal(h, d.cpu())) for h, d in zip(hdU + hU, R["dU"] + R["U"]))
+    return dict(value=val, unit=UNIT, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h, u_cells_written_back=n_changed, steps=steps,
                 ms_per_step=1e3 * float(tmax.item()) / steps, matches_device_path=same)
 
 

@@ -203,6 +203,9 @@ int ak_get_flux(ak_ctx*, int dir, int comp, double* dst);
  * ak_set_metric (device pointers: the snapshot is frozen across stages).  Copies U and Bf
  * to context-owned device staging, runs parts (1)-(6), copies back U (floored cells), W,
  * dU, E and the two masks, and synchronises.  Staging is allocated on first use.
+ * U is written back only where part (1) changed it: when all five U arrays are pinned (cudaHostAlloc /
+ * cudaHostRegister) host memory, the pipelined path stores just the cells with a non-zero status straight into
+ * them instead of copying the fields back whole (the values are the same either way); pageable arrays are copied.
  * W == NULL (or all eight members NULL): the primitives are an intermediate of the stage and are not
  * copied back (3.1 of the 8.5 GB a C4 stage would otherwise return).  Batches of >= 16 blocks are
  * pipelined in chunks over two internal streams so that H2D, kernels and D2H overlap; the fluxes of such

@@ -1102,6 +1102,25 @@ int ak_kernel_ms(ak_ctx* c, double ms_out[8], long long launches_out[8]) {
 // Pipelined host path: the batch is cut into chunks of blocks that alternate between two lanes
 // (child contexts with their own streams), so that the H2D copy of one chunk, the kernels of
 // another and the D2H copy of a third overlap (PCIe is full duplex).
+// Sparse write-back of U~ for the host path: con2prim rewrites only the cells whose status is non-zero, so when
+// the caller's U~ arrays are pinned host memory the device can address, those cells alone are written there
+// (zero-copy stores) instead of copying every field back whole.
+__global__ void __launch_bounds__(256) k_writeback_floored(const unsigned char* __restrict__ status, long long ncell,
+                                                           const double* u0, const double* u1, const double* u2,
+                                                           const double* u3, const double* u4, double* h0, double* h1,
+                                                           double* h2, double* h3, double* h4) {
+  for (long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x; c < ncell; c += (long long)gridDim.x * blockDim.x) {
+    if (status[c] != 0) { h0[c] = u0[c]; h1[c] = u1[c]; h2[c] = u2[c]; h3[c] = u3[c]; h4[c] = u4[c]; }
+  }
+}
+// device-side address of a host buffer the GPU can write (pinned / registered memory), or nullptr
+static double* mapped_host(double* h) {
+  cudaPointerAttributes at;
+  if (cudaPointerGetAttributes(&at, h) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+  if (at.type != cudaMemoryTypeHost || !at.devicePointer) return nullptr;
+  return (double*)at.devicePointer;
+}
+
 static int rhs_host_pipelined(ak_ctx* c, int chunk, double* const hU[5], const double* const hB[3], double* const hW[8],
                               double dt_fofc, double* const hdU[5], double* const hE[3], unsigned char* hflag,
                               unsigned char* hstatus) {
@@ -1142,6 +1161,9 @@ static int rhs_host_pipelined(ak_ctx* c, int chunk, double* const hU[5], const d
     c->lane_chunk = chunk;
   }
   CK(cudaStreamSynchronize(c->stream));            // the metric and anything queued by the caller
+  double* mU[5];
+  bool sparse_u = true;                            // every U~ array pinned: floored cells are written back singly
+  for (int q = 0; q < 5; ++q) { mU[q] = mapped_host(hU[q]); sparse_u = sparse_u && mU[q] != nullptr; }
   for (int ch = 0; ch < nchunks; ++ch) {
     const int l = ch & 1;
     ak_ctx* k = c->lane[l];
@@ -1161,8 +1183,15 @@ static int rhs_host_pipelined(ak_ctx* c, int chunk, double* const hU[5], const d
     const ak_rhs_out dO = {b[16], b[17], b[18], b[19], b[20], b[21], b[22], b[23], c->lane_mask[l][0], c->lane_mask[l][1], nullptr};
     const int r = ak_rhs(k, &dU_, &dB_, &dW_, 0, dt_fofc, &dO);
     if (r != AK_OK) return r;
+    if (sparse_u) {
+      const long long o0 = m0 * per[0];
+      k_writeback_floored<<<148 * 4, 256, 0, st>>>(c->lane_mask[l][1], per[0] * chunk, b[0], b[1], b[2], b[3], b[4],
+                                                   mU[0] + o0, mU[1] + o0, mU[2] + o0, mU[3] + o0, mU[4] + o0);
+      CK(cudaGetLastError());
+    }
     for (int q = 0; q < 5; ++q) {
-      CK(cudaMemcpyAsync(hU[q] + m0 * per[0], b[q], sizeof(double) * per[0] * chunk, cudaMemcpyDeviceToHost, st));
+      if (!sparse_u)
+        CK(cudaMemcpyAsync(hU[q] + m0 * per[0], b[q], sizeof(double) * per[0] * chunk, cudaMemcpyDeviceToHost, st));
       CK(cudaMemcpyAsync(hdU[q] + m0 * per[0], b[16 + q], sizeof(double) * per[0] * chunk, cudaMemcpyDeviceToHost, st));
     }
     for (int q = 0; q < 8 && hW[0]; ++q)

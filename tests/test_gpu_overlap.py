@@ -332,3 +332,30 @@ def test_graph_replay_equals_plain_launches():
     for x, y in zip(*res):
         assert np.array_equal(x, y)
     assert ak.lib().ak_set_graph(None, 1) == ak.AK_EINVAL
+
+
+def test_host_entry_sparse_writeback_of_floored_cells_into_pinned_memory():
+    """ak_rhs_host, pipelined path (16 blocks), pinned U~ arrays: only the cells part (1) changed (status != 0)
+    are stored back, straight into the pinned arrays; with pageable arrays U~ is copied whole.  Both must leave
+    the host U~ equal to the device path's, floors present."""
+    import torch
+    from paper_2409_10384_b200 import ak
+    w = _noise_batch(16, 8, seed0=200, frac=0.05)
+    over = dict(rho_atm=3e-6, T_atm=0.6, f_thr=1.0)           # atmosphere above the low-density cells: floors fire
+    with gpukit.GpuStage(copy.deepcopy(w), **over) as a:
+        a.rhs()
+        ra = a.result()
+        assert np.count_nonzero(ra["status"]) > 50
+        assert any(not np.array_equal(u, r) for u, r in zip(w["U"], ra["U"]))
+        sh = a.sh
+        for pinned in (True, False):
+            mk = (lambda arr: torch.from_numpy(np.ascontiguousarray(arr)).pin_memory()) if pinned else \
+                 (lambda arr: torch.from_numpy(np.ascontiguousarray(arr).copy()))
+            hU = [mk(u) for u in w["U"]]; hB = [mk(b) for b in w["Bf"]]
+            hdU = [mk(np.zeros(sh["cell"])) for _ in range(5)]
+            hE = [mk(np.zeros(sh[k])) for k in ("ex", "ey", "ez")]
+            hflag = mk(np.zeros(sh["cell"], dtype=np.uint8)); hst = mk(np.zeros(sh["cell"], dtype=np.uint8))
+            ak.ak_rhs_host(a.ctx, hU, hB, None, w["dt_fofc"], hdU, hE, hflag, hst)
+            for x, y in zip(hdU + hE + hU, ra["dU"] + ra["E"] + ra["U"]):
+                assert np.array_equal(x.numpy(), y), pinned
+            assert np.array_equal(hflag.numpy(), ra["flag"]) and np.array_equal(hst.numpy(), ra["status"])
