@@ -14,9 +14,13 @@
  *   P:137-139 atmosphere, P:141-157 FOFC(+DMP, Eq. 12), P:161 con2prim.
  * No blocking, fusion or reordering: loops over blocks, cells, faces, edges.
  *
- * Pins (tests/test_oracle_*.py, -m "not gpu"): see DESIGN.md §5.  Policy choices
- * the paper leaves open (floor order R5, M_max R6, "requires a floor" R8, DMP
- * variables R13) are "parity unpinned" beyond oracle==GPU and are listed there.
+ * Pins (tests/test_oracle_*.py, -m "not gpu"): see DESIGN.md §5.  Round 2 added
+ * tests/test_oracle_pins_r2.py: WENO-Z weights against the literal formula in exact
+ * rationals, the CT upwind sense and weight locations, the face-state floor, and
+ * lambda+- with B != 0 against the numerical flux Jacobian - each seen to fail on
+ * one-line mutations of this code.  Policy choices the paper leaves open (floor
+ * order R5, M_max R6, "requires a floor" R8, DMP variables R13, root-finder path R2)
+ * are "parity unpinned" beyond oracle==GPU and are listed there.
  *
  * Data layout (the library boundary's, restated): a MeshBlock has n^3 interior
  * cells, ng=4 ghosts, nt=n+8 stored cells per direction; i fastest.
