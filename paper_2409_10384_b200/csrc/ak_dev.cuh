@@ -79,6 +79,14 @@ __device__ __forceinline__ void metric_inverse(const Met3& g, double& det, doubl
   u.zz = (g.xx * g.yy - g.xy * g.xy) * id;
   sdet = sqrt(det);
 }
+// determinant and its square root only: the same operations as in metric_inverse
+__device__ __forceinline__ void metric_det(const Met3& g, double& det, double& sdet) {
+  const double cxx = g.yy * g.zz - g.yz * g.yz;
+  const double cxy = g.xz * g.yz - g.xy * g.zz;
+  const double cxz = g.xy * g.yz - g.xz * g.yy;
+  det = g.xx * cxx + g.xy * cxy + g.xz * cxz;
+  sdet = sqrt(det);
+}
 // determinant and one diagonal element of the inverse only (face geometry, O5)
 template <int DIR>
 __device__ __forceinline__ void metric_det_gdd(const Met3& g, double& sdet, double& gdd) {
@@ -348,9 +356,13 @@ __device__ __forceinline__ int c2p_cell(const Par& P, const Met3& g, double Ut[5
                                         double W5[5]) {
   int status = 0;
   double det, sdet;
-  Met3 gu;
-  metric_inverse(g, det, sdet, gu);
+  metric_det(g, det, sdet);                   // the inverse metric is formed only where a cell needs it (below)
   const double isd = 1.0 / sdet;
+  // Static unmagnetised cell (exact shortcut, bit 1; ideal gas): S~_i = +0.0 and B~ = +-0.0.  Then B_i, B^2, r_i,
+  // r^i, r^2, (rB) are all zeros, and everything the solve leaves behind is known in closed form (see below).
+  const bool zero_SB = EOS == 0 && (P.shortcuts & 2) != 0 &&
+                       (__double_as_longlong(Ut[1]) | __double_as_longlong(Ut[2]) | __double_as_longlong(Ut[3])) == 0LL &&
+                       Bt[0] == 0.0 && Bt[1] == 0.0 && Bt[2] == 0.0;
   double D = Ut[0] * isd, tau = Ut[4] * isd;
   const double Sl[3] = {Ut[1] * isd, Ut[2] * isd, Ut[3] * isd};
   const double B[3] = {Bt[0] * isd, Bt[1] * isd, Bt[2] * isd};
@@ -361,9 +373,12 @@ __device__ __forceinline__ int c2p_cell(const Par& P, const Met3& g, double Ut[5
     status |= ST_FAIL;
     solve = false;
   }
-  double Bl[3];
-  lower(g, B, Bl);
-  const double B2 = dot3(Bl, B);
+  double B2 = 0.0;                            // B = +-0: B_i B^i is a zero, and no use below sees its sign
+  if (!zero_SB) {
+    double Bl[3];
+    lower(g, B, Bl);
+    B2 = dot3(Bl, B);
+  }
   // conserved floors: D floor -> magnetisation cap -> tau floor (reading R5)
   bool atmo = false;
   if (solve && D < P.thr) {
@@ -380,7 +395,33 @@ __device__ __forceinline__ int c2p_cell(const Par& P, const Met3& g, double Ut[5
     pr = eos_P_at_T<EOS>(P, D, P.T_atm);
     solve = false;
   }
+  if (solve && zero_SB) {
+    // tau floor: D eps_atm + 0.5 (+-0) = D eps_atm (non-zero).  Then q = tau/D > 0 and, for EVERY trial mu of the
+    // master function: x = 1/(1 + mu 0) = 1, rbar^2 = +0, qbar = q, v^2 = 0, W^ = 1/sqrt(1) = 1, eps^ = 1 (q - mu 0)
+    // + ddiv(0, 2) = q.  The state the root finder leaves behind does not depend on the root, so neither do rho =
+    // D 1, P = rho (Gamma - 1) q, u^i = W^ mu x (r^i + c B^i) = (+)(+0 + +-0) = +0 (S~_i = +0 makes r_i, r^i = +0).
+    // The bracket cannot fail: nu = (1 + a^)(1 + q) > 1, f(1) = 1 - 1/nu > 0 > f(0) = -1/nu; and the Illinois
+    // iteration on the linear f(mu) = mu - 1/nu repeats its secant point to ~3 ulp at once (|dmu| <= tol mu).
+    const double tau_atm = D * eos_eps_at_T<EOS>(P, D, P.T_atm);
+    if (tau < tau_atm) { tau = tau_atm; status |= ST_TAUFLOOR; }
+    const double iD = 1.0 / D;
+    const double q = tau * iD;
+    if (q > 0.0 && isfinite(q)) {
+      rho = D;
+      pr = eos_P<EOS>(P, rho, q);
+      if (!(isfinite(rho) && isfinite(pr))) {
+        status |= ST_FAIL;
+        rho = P.rho_atm; pr = P.P_atm;
+      }
+      solve = false;                          // done: on to the primitive floors
+    }
+  }
   if (solve) {
+    Met3 gu;
+    {
+      double det_, sdet_;
+      metric_inverse(g, det_, sdet_, gu);
+    }
     const double tau_atm = D * eos_eps_at_T<EOS>(P, D, P.T_atm) + 0.5 * B2;
     if (tau < tau_atm) { tau = tau_atm; status |= ST_TAUFLOOR; }
     const double iD = 1.0 / D;
@@ -406,7 +447,20 @@ __device__ __forceinline__ int c2p_cell(const Par& P, const Met3& g, double Ut[5
       if (mu_hi > 1.0) mu_hi = 1.0;
     }
     double mu = 0.0;
-    if (ok) {
+    // Static unmagnetised cell, ideal gas (exact shortcut, bit 1): with S = 0 and B = 0 exactly, r^2 = b^2 =
+    // (rb)^2 = 0 and, for EVERY trial mu, x = 1/(1 + mu 0) = 1, rbar^2 = +0, qbar = q - 0 - 0 = q, v^2 = 0, W^ =
+    // 1/sqrt(1) = 1, eps^ = 1 (q - mu 0) + ddiv(0, 2) = q: the state the root finder would leave behind does not
+    // depend on the root, so neither do rho = D 1, P = rho (Gamma - 1) q and u^i = W^ mu x (+-0) = +-0 (mu > 0
+    // enters through its sign only).  The bracket cannot fail: nu = (1 + a^)(1 + q) > 1 gives f(1) = 1 - 1/nu >
+    // 0 > f(0) = -1/nu, and the Illinois iteration on the linear f(mu) = mu - 1/nu reaches |dmu| <= tol mu within
+    // a few steps (the second secant point already repeats the first to ~3 ulp).  So: no master-function
+    // evaluation, no iteration.
+    const bool closed = EOS == 0 && (P.shortcuts & 2) && ok && s.r2 == 0.0 && s.bs2 == 0.0 && s.rb2 == 0.0 &&
+                        s.q > 0.0 && isfinite(s.q);
+    if (closed) {                             // zeros of other signs (S~_i = -0.0): the same closed form, r^i kept
+      s.x = 1.0; s.rbar2 = 0.0; s.qbar = s.q; s.vsq = 0.0; s.iW = 1.0; s.What = 1.0; s.eps = s.q;
+      mu = 1.0;
+    } else if (ok) {
       const double f_hi = s.f(mu_hi);
       // S = 0 and B = 0 exactly (static atmosphere, the bulk of a merger grid): every later evaluation is
       // mu - inv with the inv this one left behind (q > 0 keeps eps = qbar away from a signed zero)
