@@ -7,6 +7,7 @@
 #endif
 #include "ak_flux_tma.cuh"
 #include "ak_flux_pencil.cuh"
+#include "ak_flux_static.cuh"
 #include "ak_driver.cuh"
 
 #include <cmath>
@@ -67,6 +68,8 @@ struct ak_ctx {
   int cap[8];                   // grid caps (blocks) per kernel class in the overlapped schedule, 0 = none
   int sweep_smem_pad;           // bytes: dynamic shared memory the sweeps ask for at least when overlapped
   unsigned int* zflags;         // [nmb] per-block zero-field flags written by k_con2prim (Fields::zflags)
+  unsigned int* mlist;          // [2 nmb] static / general MeshBlocks (k_split_blocks), [2] their counts behind
+  int split_blocks;             // 1: static MeshBlocks take k_flux_static (serial schedule, part (1) in the same call)
   // CUDA-graph replay of the serial stage (ak_set_graph): a few instantiated graphs keyed on the arguments
   int graph_on;
   cudaStream_t gstream;         // capture stream (the caller's may be the legacy default stream, which cannot capture)
@@ -402,6 +405,70 @@ int launch_pencil(ak_ctx* c, const Lane& L) {
   return AK_OK;
 }
 
+// do the tile kernels apply to this batch (else launch_flux falls back to k_flux and knows no block lists)
+bool tile_kernels_apply(const ak_ctx* c, const Par& P) {
+  const int n = P.n, e = n + 2;
+  if (!AK_FLUX_TMA || n % 2 != 0 || c->pencil_wi > 0) return false;
+  for (int d = 0; d < 3; ++d) {
+    const int cellv = (AK_FLUX_CELL_MASK >> d) & 1;
+    const int nfi = cellv ? (d == 0 ? n + 4 : e) : (d == 0 ? n + 3 : e);
+    if (nfi * (cellv && d != 0 ? 2 : 1) > TMA_THREADS) return false;
+    const int nfd = d == 0 ? e : n + 3;
+    const int namax = TMA_THREADS / nfi - (cellv && d != 0 ? 1 : 0);
+    const int tiles = (nfd + namax - 1) / namax, NA = (nfd + tiles - 1) / tiles;
+    const int maxW = d == 0 ? NA : NA + 5, maxM = d == 0 ? NA : NA + 1;
+    if (sizeof(double) * ((size_t)7 * tile_slot(maxW, P.nt) + (size_t)10 * tile_slot(maxM, P.nt) + (cellv ? 7 * TMA_THREADS : 0)) >
+        200 * 1024)
+      return false;
+  }
+  return true;
+}
+
+template <int DIR, int RECON>
+int launch_flux_static_r(ak_ctx* c, const Lane& L, int NA, unsigned grid, int bd, size_t smem, const TileMaps& M) {
+  static int have0[64] = {0}, have1[64] = {0};
+  if (L.P.eos) {
+    auto kern = k_flux_static<DIR, RECON, 1>;
+    const int r = raise_smem_attr(kern, c->hp.device, smem, have1);
+    if (r != AK_OK) return r;
+    kern<<<grid, bd, smem, L.st>>>(L.P, L.f, NA, M);
+  } else {
+    auto kern = k_flux_static<DIR, RECON, 0>;
+    const int r = raise_smem_attr(kern, c->hp.device, smem, have0);
+    if (r != AK_OK) return r;
+    kern<<<grid, bd, smem, L.st>>>(L.P, L.f, NA, M);
+  }
+  return AK_OK;
+}
+
+template <int DIR>
+int launch_flux_static(ak_ctx* c, const Lane& L) {
+  const int n = L.P.n, nt = L.P.nt, e = n + 2;
+  const int nfi = DIR == 0 ? n + 3 : e, nfd = DIR == 0 ? e : n + 3;
+  const int namax = TMA_THREADS / nfi;
+  const int tiles = (nfd + namax - 1) / namax, NA = (nfd + tiles - 1) / tiles;
+  const int maxW = DIR == 0 ? NA : NA + 5, maxM = DIR == 0 ? NA : NA + 1;
+  const size_t smem = sizeof(double) * ((size_t)2 * tile_slot(maxW, nt) + (size_t)10 * tile_slot(maxM, nt));
+  TileMaps M;
+  const cuuint32_t unt = (cuuint32_t)nt;
+  const cuuint32_t bW[3] = {unt, DIR == 2 ? 1u : (cuuint32_t)maxW, DIR == 2 ? (cuuint32_t)maxW : 1u};
+  const cuuint32_t bM[3] = {unt, DIR == 2 ? 1u : (cuuint32_t)maxM, DIR == 2 ? (cuuint32_t)maxM : 1u};
+  if (!field_maps<DIR>(L.P, L.f, bW, bM, M)) return AK_ECUDA;
+  const unsigned grid = (unsigned)((long long)L.P.nmb * e * tiles);
+  const int bd = ((NA * nfi + 31) / 32) * 32;
+  int r;
+  switch (L.P.recon) {
+    case 0: r = launch_flux_static_r<DIR, 0>(c, L, NA, grid, bd, smem, M); break;
+    case 1: r = launch_flux_static_r<DIR, 1>(c, L, NA, grid, bd, smem, M); break;
+    case 3: r = launch_flux_static_r<DIR, 3>(c, L, NA, grid, bd, smem, M); break;
+    case 4: r = launch_flux_static_r<DIR, 4>(c, L, NA, grid, bd, smem, M); break;
+    default: r = launch_flux_static_r<DIR, 2>(c, L, NA, grid, bd, smem, M); break;
+  }
+  if (r != AK_OK) return r;
+  CK(cudaGetLastError());
+  return AK_OK;
+}
+
 template <int DIR>
 int launch_flux(ak_ctx* c, const Lane& L) {
   Timer t(c, KC_FX + DIR, L.st);
@@ -457,9 +524,15 @@ int launch_flux(ak_ctx* c, const Lane& L) {
       if (r != AK_OK) return r;
       CK(cudaGetLastError());
       c->launches[KC_FX + DIR] += 1;
+      if (L.f.mlist) {                         // the static MeshBlocks of k_split_blocks: the light kernel
+        r = launch_flux_static<DIR>(c, L);
+        if (r != AK_OK) return r;
+        c->launches[KC_FX + DIR] += 1;
+      }
       return AK_OK;
     }
   }
+  if (L.f.mlist) return AK_ESTATE;             // (lists are only handed out when the tile kernels apply)
   const long long nf = (long long)(n + 3) * (n + 2) * (n + 2) * L.P.nmb;
   const unsigned g = nblk(nf, 128);
   if (L.P.eos) {
@@ -667,6 +740,7 @@ int ak_create(const ak_params* p, const double* dx3, ak_ctx** out) {
     c->tile_tm = envi("AK_TILE_TENSORMAP", 1);
     // measured on C4 (DESIGN.md §6 item 21): fused 4.18 + fix 0.51 ms against 1.95 + 2.15 ms separately -> off
     c->fuse_src = envi("AK_FUSE_SRC", 0);
+    c->split_blocks = envi("AK_SPLIT_BLOCKS", 1);
   }
   Par& P = c->P;
   P.nmb = p->nmb; P.n = p->n; P.nt = p->n + 8; P.px = P.nt + 4; P.is = 4; P.ie = p->n + 3;
@@ -701,6 +775,7 @@ int ak_create(const ak_params* p, const double* dx3, ak_ctx** out) {
   if (e == cudaSuccess) e = cudaMalloc(&c->stats, sizeof(unsigned long long) * S_NSTAT * MAXCH);
   if (e == cudaSuccess) e = cudaMemsetAsync(c->count, 0, sizeof(unsigned) * 4 * MAXCH, c->stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(c->stats, 0, sizeof(unsigned long long) * S_NSTAT * MAXCH, c->stream);
+  if (e == cudaSuccess) e = cudaMalloc(&c->mlist, sizeof(unsigned) * (2 * nb + 2));
   if (e == cudaSuccess) e = cudaMalloc(&c->zflags, sizeof(unsigned) * nb);
   if (e == cudaSuccess) e = cudaMemsetAsync(c->zflags, 0xff, sizeof(unsigned) * nb, c->stream);
   if (e == cudaSuccess) e = cudaMalloc(&c->dx, sizeof(double) * 3 * nb);
@@ -754,7 +829,7 @@ int ak_destroy(ak_ctx* c) {
     for (int q = 0; q < 3; ++q)
       if (c->ovs[q] && !(q == 2 && c->ovs[2] == c->ovs[0])) cudaStreamDestroy(c->ovs[q]);
   }
-  cudaFree(c->flag_own); cudaFree(c->count); cudaFree(c->stats); cudaFree(c->dx); cudaFree(c->zflags);
+  cudaFree(c->flag_own); cudaFree(c->count); cudaFree(c->stats); cudaFree(c->dx); cudaFree(c->zflags); cudaFree(c->mlist);
   delete c;
   return AK_OK;
 }
@@ -833,9 +908,20 @@ int rhs_serial(ak_ctx* c, const Fields& f, int w_is_valid, double dt_fofc, cudaS
   int r;
   const Lane L = {c->P, f, st, false};
   if (!w_is_valid && (r = launch_c2p(c, L, true)) != AK_OK) return r;
-  if ((r = launch_flux<0>(c, L)) != AK_OK) return r;
-  if ((r = launch_flux<1>(c, L)) != AK_OK) return r;
-  if ((r = launch_flux<2>(c, L)) != AK_OK) return r;
+  // MeshBlocks that part (1) found static and unmagnetised as a whole go to the light sweep kernel
+  Fields fs = f;
+  if (!w_is_valid && c->split_blocks && (c->P.shortcuts & 5) == 5 && c->tile_tm && tmap_encoder() &&
+      tile_kernels_apply(c, c->P)) {
+    unsigned* cnt = c->mlist + 2 * (size_t)c->P.nmb;
+    CK(cudaMemsetAsync(cnt, 0, sizeof(unsigned) * 2, st));
+    k_split_blocks<<<nblk(c->P.nmb, 256), 256, 0, st>>>(c->P.nmb, c->zflags, c->mlist, cnt);
+    CK(cudaGetLastError());
+    fs.mlist = c->mlist; fs.mcount = cnt;
+  }
+  const Lane LS = {c->P, fs, st, false};
+  if ((r = launch_flux<0>(c, LS)) != AK_OK) return r;
+  if ((r = launch_flux<1>(c, LS)) != AK_OK) return r;
+  if ((r = launch_flux<2>(c, LS)) != AK_OK) return r;
   if ((r = launch_fofc(c, L, dt_fofc)) != AK_OK) return r;
   if ((r = launch_ct(c, L, !w_is_valid)) != AK_OK) return r;
   return launch_src(c, L);

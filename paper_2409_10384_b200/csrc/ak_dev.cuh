@@ -53,7 +53,10 @@ struct Fields {
   double fa, fb;                // U0[0] == nullptr: U* = U - dt div F (R9)
   double* M[10];                // matter terms E, S_i, S_ij written by K6 on interior cells (M[0] == nullptr: none)
   unsigned int* zflags;         // [nmb] bit q set: primitive field W[q] (q = 1..3 u^i, 5..7 B~cc^i) of that block holds
-                                // a value that is not +0.0 (written by k_con2prim, conservative); nullptr: unknown
+                                // a value that is not +0.0 (written by k_con2prim, conservative); bits 8..10: a face
+                                // value of B~f^x,y,z of that block is not +0.0; nullptr: unknown
+  const unsigned int* mlist;    // sweeps over MeshBlock lists (k_split_blocks): [0, nmb) static blocks, [nmb, 2 nmb)
+  const unsigned int* mcount;   // the others; mcount[0], mcount[1] their lengths; nullptr: every block, in order
 };
 
 enum { ST_DFLOOR = 1, ST_TAUFLOOR = 2, ST_MAGCAP = 4, ST_RHOFLOOR = 8, ST_TFLOOR = 16,

@@ -1,0 +1,115 @@
+// ak_flux_static.cuh — K2 for MeshBlocks that are static and unmagnetised as a whole (round 2).
+//
+// k_con2prim records per MeshBlock whether any u^i, any cell-centred B~ or any face B~ holds a value that
+// is not +0.0 (Fields::zflags).  A block where none does — static atmosphere without field, 72 % of C4's
+// blocks — needs of the 17 staged fields only rho, P and the ten metric fields, and of the Riemann solve only
+// static_side() (ak_flux.cuh: Eq. 8 with W = 1, v = 0, B = 0 substituted term by term, the same bits as
+// the general code on such data).  This kernel does just that: 12 tensor-map box copies per tile, 33 KB of
+// shared memory instead of 52 KB and no general side_state() in the register budget, so that 5-6 blocks are
+// resident on an SM instead of 3 and the tile-load latency — the top stall of the default-mode sweeps
+// (profiles/r2_final.md) — is covered.  k_split_blocks makes the two lists of MeshBlocks (static / general)
+// on the device; both sweep kernels are launched over the full grid and a block whose list entry does not
+// exist returns at once.
+//
+// Same tiles as k_flux_tma: x: NA rows of n+3 faces; y, z: NA face rows of n+2 lanes.  One thread per face.
+#pragma once
+#include "ak_flux_tma.cuh"
+
+namespace ak {
+
+#ifndef AK_STATIC_MINB
+#define AK_STATIC_MINB 4
+#endif
+
+// lists of MeshBlocks: mlist[0..count[0]) static, mlist[nmb + 0 .. nmb + count[1]) general
+__global__ void __launch_bounds__(256) k_split_blocks(int nmb, const unsigned* __restrict__ zflags,
+                                                      unsigned* __restrict__ mlist, unsigned* __restrict__ mcount) {
+  for (int m = blockIdx.x * blockDim.x + threadIdx.x; m < nmb; m += gridDim.x * blockDim.x) {
+    const int which = (zflags[m] & 0x7eeu) ? 1 : 0;      // u^i (1..3), B~cc (5..7), face B~ (8..10)
+    mlist[which * nmb + atomicAdd(mcount + which, 1u)] = (unsigned)m;
+  }
+}
+
+template <int DIR, int RECON, int EOS = 0>
+__global__ void __launch_bounds__(TMA_THREADS, AK_STATIC_MINB)
+k_flux_static(const __grid_constant__ Par P, const __grid_constant__ Fields f, int NA,
+              const __grid_constant__ TileMaps maps) {
+  extern __shared__ __align__(128) double sm[];
+  __shared__ uint64_t mbar, mbarM;
+  const int nt = P.nt, e = P.n + 2, t = threadIdx.x;
+  const int maxW = DIR == 0 ? NA : NA + 5, maxM = DIR == 0 ? NA : NA + 1;
+  const int slotW = tile_slot(maxW, nt), slotM = tile_slot(maxM, nt);
+  double* sW = sm;                             // [2][slotW]   rho, P
+  double* sM = sm + 2 * slotW;                 // [10][slotM]
+  const int nfd = DIR == 0 ? e : P.n + 3;
+  const int tiles = (nfd + NA - 1) / NA;
+  int bid = blockIdx.x;
+  const int td = bid % tiles; bid /= tiles;
+  const int o = bid % e + P.is - 1;
+  const int mm = bid / e;
+  if (mm >= (int)f.mcount[0]) return;          // fewer static blocks than the grid provides for (block-uniform)
+  const int m = (int)f.mlist[mm];
+  const int d0 = P.is - 1 + td * NA;
+  const int na = min(NA, P.is - 1 + nfd - d0);
+  const Ix ix{nt, P.px};
+  const unsigned rowb = (unsigned)(nt * sizeof(double));
+  if (t == 0) { mbar_init(&mbar, 1); mbar_init(&mbarM, 1); }
+  __syncthreads();
+  if (t < 32) {                                // lanes 0..11 of warp 0: one field each
+    if (t == 0) {
+      mbar_arrive_expect_tx(&mbar, (unsigned)(2 * maxW) * rowb);
+      mbar_arrive_expect_tx(&mbarM, (unsigned)(10 * maxM) * rowb);
+    }
+    __syncwarp();
+    const int K = DIR == 2 ? m * nt + d0 : m * nt + o;
+    if (t < 2) {
+      const int cW1 = DIR == 0 ? d0 : (DIR == 1 ? d0 - 3 : o), cW2 = DIR == 2 ? K - 3 : K;
+      tma_load_3d(sW + (size_t)t * slotW, &maps.w[t == 0 ? 0 : 4], 0, cW1, cW2, &mbar);
+    } else if (t < 12) {
+      const int cM1 = DIR == 0 ? d0 : (DIR == 1 ? d0 - 1 : o), cM2 = DIR == 2 ? K - 1 : K;
+      tma_load_3d(sM + (size_t)(t - 2) * slotM, &maps.m[t - 2], 0, cM1, cM2, &mbarM);
+    }
+  }
+  const int nfi = DIR == 0 ? P.n + 3 : e;
+  const int a = t / nfi, ii = t - a * nfi + P.is - 1;
+  if (a >= na) return;                         // no barrier below: threads without a face leave
+  long long fi;
+  if (DIR == 0) fi = ix.face(0, m, o, d0 + a, ii);
+  else if (DIR == 1) fi = ix.face(1, m, o, d0 + a, ii);
+  else fi = ix.face(2, m, d0 + a, o, ii);
+  mbar_wait(&mbar, 0);
+  double sL[7], sR[7];
+#pragma unroll
+  for (int v = 0; v < 7; ++v) { sL[v] = 0.0; sR[v] = 0.0; }
+#pragma unroll
+  for (int v2 = 0; v2 < 2; ++v2) {
+    const int v = v2 == 0 ? 0 : 4;
+    const double* w = DIR == 0 ? sW + (size_t)v2 * slotW + a * nt + ii - 3 : sW + (size_t)v2 * slotW + a * nt + ii;
+    const int s = DIR == 0 ? 1 : nt;
+    if (RECON == 0) {
+      sL[v] = w[2 * s]; sR[v] = w[3 * s];
+    } else {
+      const double q0 = w[0], q1 = w[s], q2 = w[2 * s], q3 = w[3 * s], q4 = w[4 * s], q5 = w[5 * s];
+      double qm, qp;
+      recon<RECON>(q0, q1, q2, q3, q4, qm, qp);
+      sL[v] = qp;
+      recon<RECON>(q1, q2, q3, q4, q5, qm, qp);
+      sR[v] = qm;
+    }
+  }
+  mbar_wait(&mbarM, 0);
+  double mL[10], mR[10], Fo[7];
+#pragma unroll
+  for (int q = 0; q < 10; ++q) {
+    const double* g = DIR == 0 ? sM + (size_t)q * slotM + a * nt + ii - 1 : sM + (size_t)q * slotM + a * nt + ii;
+    mL[q] = g[0];
+    mR[q] = g[DIR == 0 ? 1 : nt];
+  }
+  FaceGeo G;
+  face_geometry<DIR>(mL, mR, G);
+  face_flux_static<DIR, EOS>(P, P.riemann, G, sL, sR, Fo);
+#pragma unroll
+  for (int v = 0; v < 7; ++v) f.F[7 * DIR + v][fi] = Fo[v];
+}
+
+}  // namespace ak

@@ -123,7 +123,11 @@ k_flux_tma(const __grid_constant__ Par P, const __grid_constant__ Fields f, int 
   int bid = blockIdx.x;
   const int td = bid % tiles; bid /= tiles;
   const int o = bid % e + P.is - 1;            // the fixed transverse index (k for x,y; j for z)
-  const int m = bid / e;
+  int m = bid / e;
+  if (f.mlist) {                               // the general blocks of k_split_blocks (block-uniform exit)
+    if (m >= (int)f.mcount[1]) return;
+    m = (int)f.mlist[P.nmb + m];
+  }
   const int d0 = P.is - 1 + td * NA;           // first row (x) / first face along d (y,z)
   const int na = min(NA, P.is - 1 + nfd - d0); // rows / faces actually present in this tile
   const int nW = DIR == 0 ? na : na + 5, nM = DIR == 0 ? na : na + 1;
@@ -291,7 +295,11 @@ k_flux_tma_cell(const __grid_constant__ Par P, const __grid_constant__ Fields f,
   int bid = blockIdx.x;
   const int td = bid % tiles; bid /= tiles;
   const int o = bid % e + P.is - 1;
-  const int m = bid / e;
+  int m = bid / e;
+  if (f.mlist) {                               // the general blocks of k_split_blocks (block-uniform exit)
+    if (m >= (int)f.mcount[1]) return;
+    m = (int)f.mlist[P.nmb + m];
+  }
   const int d0 = P.is - 1 + td * NA;
   const int na = min(NA, P.is - 1 + nfd - d0);
   const int nW = DIR == 0 ? na : na + 5, nM = DIR == 0 ? na : na + 1;

@@ -115,9 +115,18 @@ __global__ void __launch_bounds__(128, AK_C2P_MINB) k_con2prim(const __grid_cons
   const long long fx = row * P.px + i;
   const long long fy = (mk * (nt + 1) + j) * nt + i;
   const long long fz = (((long long)m * (nt + 1) + k) * nt + j) * nt + i;
-  Bc[0] = 0.5 * (__ldg(f.Bf[0] + fx) + __ldg(f.Bf[0] + fx + 1));
-  Bc[1] = 0.5 * (__ldg(f.Bf[1] + fy) + __ldg(f.Bf[1] + fy + nt));
-  Bc[2] = 0.5 * (__ldg(f.Bf[2] + fz) + __ldg(f.Bf[2] + fz + (long long)nt * nt));
+  // every face of the block is the lower or the upper face of one of its cells: the OR of the bit patterns
+  // tells whether the block holds a face value that is not +0.0 (zflags bits 8..10)
+  unsigned fnz = 0;
+  {
+    const double a0 = __ldg(f.Bf[0] + fx), a1 = __ldg(f.Bf[0] + fx + 1);
+    const double b0 = __ldg(f.Bf[1] + fy), b1 = __ldg(f.Bf[1] + fy + nt);
+    const double c0 = __ldg(f.Bf[2] + fz), c1 = __ldg(f.Bf[2] + fz + (long long)nt * nt);
+    Bc[0] = 0.5 * (a0 + a1); Bc[1] = 0.5 * (b0 + b1); Bc[2] = 0.5 * (c0 + c1);
+    fnz = ((unsigned)((__double_as_longlong(a0) | __double_as_longlong(a1)) != 0LL) << 8) |
+          ((unsigned)((__double_as_longlong(b0) | __double_as_longlong(b1)) != 0LL) << 9) |
+          ((unsigned)((__double_as_longlong(c0) | __double_as_longlong(c1)) != 0LL) << 10);
+  }
 #if AK_C2P_PARK
   // The metric and B are needed again only after the root solve.  Parked in shared memory they
   // leave the registers for the solve; left to the compiler they are spilled to local memory,
@@ -158,7 +167,7 @@ __global__ void __launch_bounds__(128, AK_C2P_MINB) k_con2prim(const __grid_cons
     // which of this block's often-zero fields hold anything but +0.0: later kernels of the stage do not
     // load a field whose bit stays clear.  A set bit is only ever added: the flag may say
     // "non-zero" for a field that is zero (another thread's stale read), never the reverse.
-    unsigned nz = 0;
+    unsigned nz = fnz;
 #pragma unroll
     for (int v = 1; v < 4; ++v) nz |= (unsigned)(__double_as_longlong(W5[v]) != 0LL) << v;
 #pragma unroll
