@@ -740,7 +740,10 @@ int ak_create(const ak_params* p, const double* dx3, ak_ctx** out) {
     c->tile_tm = envi("AK_TILE_TENSORMAP", 1);
     // measured on C4 (DESIGN.md §6 item 21): fused 4.18 + fix 0.51 ms against 1.95 + 2.15 ms separately -> off
     c->fuse_src = envi("AK_FUSE_SRC", 0);
-    c->split_blocks = envi("AK_SPLIT_BLOCKS", 1);
+    // -1: automatic — only for batches of >= 2^23 stored cells: the split adds 4 launches, empty thread blocks and
+    // 51 tensor-map encodes per stage, which cost the small configs 3-14 % (C0 0.144 -> 0.165 ms, C3 1.53 -> 1.58)
+    // and gain C4 1 % (13.75 -> 13.59 ms)
+    c->split_blocks = envi("AK_SPLIT_BLOCKS", -1);
   }
   Par& P = c->P;
   P.nmb = p->nmb; P.n = p->n; P.nt = p->n + 8; P.px = P.nt + 4; P.is = 4; P.ie = p->n + 3;
@@ -910,12 +913,14 @@ int rhs_serial(ak_ctx* c, const Fields& f, int w_is_valid, double dt_fofc, cudaS
   if (!w_is_valid && (r = launch_c2p(c, L, true)) != AK_OK) return r;
   // MeshBlocks that part (1) found static and unmagnetised as a whole go to the light sweep kernel
   Fields fs = f;
-  if (!w_is_valid && c->split_blocks && (c->P.shortcuts & 5) == 5 && c->tile_tm && tmap_encoder() &&
+  const bool want_split = c->split_blocks > 0 || (c->split_blocks < 0 && c->sz.cell >= (1LL << 23));
+  if (!w_is_valid && want_split && (c->P.shortcuts & 5) == 5 && c->tile_tm && tmap_encoder() &&
       tile_kernels_apply(c, c->P)) {
     unsigned* cnt = c->mlist + 2 * (size_t)c->P.nmb;
     CK(cudaMemsetAsync(cnt, 0, sizeof(unsigned) * 2, st));
     k_split_blocks<<<nblk(c->P.nmb, 256), 256, 0, st>>>(c->P.nmb, c->zflags, c->mlist, cnt);
     CK(cudaGetLastError());
+    c->launches[KC_C2P] += 1;                  // counted with part (1), whose flags it sorts
     fs.mlist = c->mlist; fs.mcount = cnt;
   }
   const Lane LS = {c->P, fs, st, false};

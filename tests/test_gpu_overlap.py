@@ -359,3 +359,39 @@ def test_host_entry_sparse_writeback_of_floored_cells_into_pinned_memory():
             for x, y in zip(hdU + hE + hU, ra["dU"] + ra["E"] + ra["U"]):
                 assert np.array_equal(x.numpy(), y), pinned
             assert np.array_equal(hflag.numpy(), ra["flag"]) and np.array_equal(hst.numpy(), ra["status"])
+
+
+@pytest.mark.parametrize("name,blocks,over", [
+    ("C2", [0, 21, 22, 41, 42, 63], dict()),                 # static atmosphere blocks and blocks with moving stars
+    ("C1", [0, 7], dict(recon=4, riemann=0)),                # every block static (v = 0), but magnetised near the star
+    ("C4", [0, 1, 300, 301], dict(recon=0)),                 # donor cell through the light kernel
+])
+def test_static_block_sweep_kernel_is_exact(monkeypatch, name, blocks, over):
+    """AK_SPLIT_BLOCKS=1 (automatic only for batches of >= 2^23 stored cells, e.g. C4, where the full-batch parity
+    test covers it): MeshBlocks that con2prim found static and unmagnetised as a whole — u, B~cc and every face B~
+    +0.0 — take k_flux_static, the others the general tile kernels through the device-side block lists.  Same bits
+    as without the split and as the oracle, fluxes and the signs of their zeros included."""
+    from paper_2409_10384_b200 import ak
+    w = wl.make_blocks(name, blocks=blocks)
+    U_in = [u.copy() for u in w["U"]]
+    res = []
+    for split in ("0", "1"):
+        monkeypatch.setenv("AK_SPLIT_BLOCKS", split)         # read by ak_create
+        with gpukit.GpuStage(copy.deepcopy(w), **over) as g:
+            g.rhs()
+            res.append((g.result(), g.flux(), g.stats()))
+            g.rhs()                                          # a second call re-sorts the blocks: same result
+            again = g.result()
+            for x, y in zip(res[-1][0]["dU"] + res[-1][0]["E"], again["dU"] + again["E"]):
+                assert np.array_equal(x, y)
+    (r0, f0, s0), (r1, f1, s1) = res
+    for k in ("dU", "E", "W", "U"):
+        for x, y in zip(r0[k], r1[k]):
+            assert np.array_equal(x, y), k
+    assert np.array_equal(r0["flag"], r1["flag"]) and np.array_equal(r0["status"], r1["status"]) and s0 == s1
+    for x, y in zip(f0, f1):
+        assert np.array_equal(x, y) and np.array_equal(np.signbit(x), np.signbit(y))
+    p = dict(w["params"]); p.update(over)
+    o = orc.rhs(orc.make_params(**p), w["dx"], w["U"], w["Bf"], w["adm"], w["dt_fofc"], nthreads=8)
+    o["U"] = w["U"]
+    gpukit.assert_parity(r1, o, U_in, label=name + " split")
