@@ -365,6 +365,7 @@ def test_host_entry_sparse_writeback_of_floored_cells_into_pinned_memory():
     ("C2", [0, 21, 22, 41, 42, 63], dict()),                 # static atmosphere blocks and blocks with moving stars
     ("C1", [0, 7], dict(recon=4, riemann=0)),                # every block static (v = 0), but magnetised near the star
     ("C4", [0, 1, 300, 301], dict(recon=0)),                 # donor cell through the light kernel
+    ("C2", [0, 21, 63], dict(eos_hybrid=dict(K0=40.0, gammas=[2.0, 2.2], rho_breaks=[6.4e-4], gamma_th=2.0))),
 ])
 def test_static_block_sweep_kernel_is_exact(monkeypatch, name, blocks, over):
     """AK_SPLIT_BLOCKS=1 (automatic only for batches of >= 2^23 stored cells, e.g. C4, where the full-batch parity
@@ -391,6 +392,9 @@ def test_static_block_sweep_kernel_is_exact(monkeypatch, name, blocks, over):
     assert np.array_equal(r0["flag"], r1["flag"]) and np.array_equal(r0["status"], r1["status"]) and s0 == s1
     for x, y in zip(f0, f1):
         assert np.array_equal(x, y) and np.array_equal(np.signbit(x), np.signbit(y))
+    if "eos_hybrid" in over:
+        return      # rho^Gamma is pow() on the device and libm's in the oracle (rounding-level differences: hybrid
+                    # parity against the oracle is tests/test_gpu_eos.py's subject); split on = split off is the point here
     p = dict(w["params"]); p.update(over)
     o = orc.rhs(orc.make_params(**p), w["dx"], w["U"], w["Bf"], w["adm"], w["dt_fofc"], nthreads=8)
     o["U"] = w["U"]
