@@ -19,7 +19,7 @@ SO = os.path.join(HERE, "libak.so")
 SO_FMA = os.path.join(HERE, "libak_fma.so")
 SOURCES = ["ak_api.cu"]
 HEADERS = ["ak_dev.cuh", "ak_flux.cuh", "ak_kernels.cuh", "ak_source.cuh", "ak_flux_tma.cuh", "ak_flux_pencil.cuh",
-           "ak_driver.cuh"]
+           "ak_flux_static.cuh", "ak_driver.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "--fmad=false", "-O3", "-lineinfo",
               "-std=c++17", "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
 

@@ -444,7 +444,7 @@ int launch_flux_static_r(ak_ctx* c, const Lane& L, int NA, unsigned grid, int bd
 template <int DIR>
 int launch_flux_static(ak_ctx* c, const Lane& L) {
   const int n = L.P.n, nt = L.P.nt, e = n + 2;
-  const int nfi = DIR == 0 ? n + 3 : e, nfd = DIR == 0 ? e : n + 3;
+  const int nfi = DIR == 0 ? ((AK_STATIC_ONCE_MASK & 1) ? n + 4 : n + 3) : e, nfd = DIR == 0 ? e : n + 3;   // threads per tile row
   const int namax = TMA_THREADS / nfi;
   const int tiles = (nfd + namax - 1) / namax, NA = (nfd + tiles - 1) / tiles;
   const int maxW = DIR == 0 ? NA : NA + 5, maxM = DIR == 0 ? NA : NA + 1;

@@ -87,6 +87,14 @@ constexpr unsigned ALWAYS_NZ = 0xffu;   // every slot reconstructed, face not st
 // u^i, both transverse B~cc and the face-normal B~ are +0.0 on the whole tile: the static face flux applies
 __device__ __forceinline__ bool tile_is_static(const Par& P, unsigned nzm) { return (P.shortcuts & 4) && !(nzm & 0xeeu); }
 
+// both transverse B~cc and the face-normal B~ are +0.0 on the whole tile: side_state<.., NOB = true> applies
+__device__ __forceinline__ bool tile_has_no_B(const Par& P, unsigned nzm) {
+#ifdef AK_NO_NOB
+  return false;
+#else
+  return (P.shortcuts & 4) && !(nzm & 0xe0u);
+#endif
+}
 // Tensor maps of the 17 fields a sweep stages (host: ak_api.cu, cuTensorMapEncodeTiled).  Every cell field is
 // the rank-3 tensor (i: nt, j: nt, K = m nt + k) of doubles; the box is the whole tile of one field, so a
 // block issues 17 tensor copies (cp.async.bulk.tensor.3d, SASS UTMALDG) instead of one 1-D bulk copy per
@@ -251,8 +259,12 @@ k_flux_tma(const __grid_constant__ Par P, const __grid_constant__ Fields f, int 
 #pragma unroll
     for (int v = 0; v < 7; ++v) pR[v * (int)blockDim.x] = sR[v];
   }
-  face_flux_parked<DIR, EOS>(P, P.riemann, G, sL, sm + 14 * (int)blockDim.x + t, (int)blockDim.x, Bfd, Fo, sm + t,
-                             (int)blockDim.x);
+  if (tile_has_no_B(P, nzm))                         // block-uniform: moving but unmagnetised matter
+    face_flux_parked<DIR, EOS, true>(P, P.riemann, G, sL, sm + 14 * (int)blockDim.x + t, (int)blockDim.x, Bfd, Fo,
+                                     sm + t, (int)blockDim.x);
+  else
+    face_flux_parked<DIR, EOS>(P, P.riemann, G, sL, sm + 14 * (int)blockDim.x + t, (int)blockDim.x, Bfd, Fo, sm + t,
+                               (int)blockDim.x);
 #else
   face_flux<DIR, true, EOS>(P, P.riemann, mL, mR, sL, sR, Bfd, Fo);
 #endif
@@ -420,8 +432,12 @@ k_flux_tma_cell(const __grid_constant__ Par P, const __grid_constant__ Fields f,
 #pragma unroll
     for (int v = 0; v < 7; ++v) pR[v * (int)blockDim.x] = qm[v];
   }
-  face_flux_parked<DIR, EOS>(P, P.riemann, G, sL, sm + 14 * (int)blockDim.x + t, (int)blockDim.x, Bfd, Fo, sm + t,
-                             (int)blockDim.x);
+  if (tile_has_no_B(P, nzm))                         // block-uniform: moving but unmagnetised matter
+    face_flux_parked<DIR, EOS, true>(P, P.riemann, G, sL, sm + 14 * (int)blockDim.x + t, (int)blockDim.x, Bfd, Fo,
+                                     sm + t, (int)blockDim.x);
+  else
+    face_flux_parked<DIR, EOS>(P, P.riemann, G, sL, sm + 14 * (int)blockDim.x + t, (int)blockDim.x, Bfd, Fo, sm + t,
+                               (int)blockDim.x);
 #else
   face_flux<DIR, true, EOS>(P, P.riemann, mL, mR, sL, qm, Bfd, Fo);
 #endif

@@ -256,6 +256,42 @@ def test_exact_shortcuts_with_signed_zeros_and_partly_zero_fields():
     assert np.array_equal(ra["flag"], rb["flag"])
 
 
+@pytest.mark.parametrize("over", [dict(recon=2, dmp_M=1.1), dict(recon=1, riemann=0),
+                                  dict(recon=2, eos_hybrid=dict(K0=40.0, gammas=[2.0, 2.2], rho_breaks=[6.4e-4], gamma_th=2.0))])
+def test_unmagnetised_moving_tiles_take_the_no_B_side_state_exactly(over):
+    """side_state<.., NOB> (mask bit 2): tiles whose B components are all +0.0 while the matter moves.  Velocities
+    of both signs (so that (Bv) = 0 v_x + 0 v_y + 0 v_z comes out as +0 and as -0), a slab of u = -0.0, a slab at
+    rest, and one corner of the block magnetised so that the general side_state runs beside it.  Masks 0, 4 and 7
+    must agree bit for bit, signs of zeros in the fluxes included."""
+    from paper_2409_10384_b200 import ak
+    w = wl.make_test_noise_block(seed=17, n=8, frac=0.0)
+    outs = []
+    for mask in (0, 4, 7):
+        with gpukit.GpuStage(copy.deepcopy(w), **over) as g:
+            ak.ak_set_exact_shortcuts(g.ctx, mask)
+            g.con2prim()
+            import torch
+            sh = tuple(g.W[1].shape)
+            for v in (1, 2, 3):
+                u = 0.3 * (np.random.default_rng(40 + v).random(sh) - 0.5)
+                u[0, :, :4, :] = -np.abs(u[0, :, :4, :])        # every component negative: (Bv) = -0
+                u[0, :, 4:6, :] = -0.0
+                u[0, :, 6:8, :] = 0.0
+                g.W[v].copy_(torch.from_numpy(u))
+            for v in (5, 6, 7): g.W[v].zero_()
+            for b in g.Bf: b.zero_()
+            g.W[5][0, 12:, 12:, 12:] = 1e-3                      # a magnetised corner: B~cc^x only
+            g.rhs(w_is_valid=True)
+            outs.append((g.result(), g.flux()))
+    ra, fa = outs[0]
+    assert any(np.any(np.signbit(x) & (x == 0.0)) for x in fa), "no negative zero in any flux: the case does not bite"
+    for rb, fb in outs[1:]:
+        for x, y in zip(ra["dU"] + ra["E"] + fa, rb["dU"] + rb["E"] + fb):
+            assert np.array_equal(x, y)
+            assert np.array_equal(np.signbit(x), np.signbit(y))
+        assert np.array_equal(ra["flag"], rb["flag"])
+
+
 def test_fused_fofc_test_and_sources_path_is_exact(monkeypatch):
     """AK_FUSE_SRC=1 (opt-in; slower on C4, DESIGN.md §6 item 21): part (6) inside the FOFC-test kernel from the
     high-order fluxes, then k_src_fix for the cells next to re-fluxed faces.  Must give the bits of the default
