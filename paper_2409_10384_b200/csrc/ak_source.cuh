@@ -9,6 +9,23 @@ namespace ak {
 #ifndef AK_SRC_MINB
 #define AK_SRC_MINB 4
 #endif
+// k_div_src runs at 128 registers (16 warps per SM), and the compiler issues the loads of the metric, rho and P
+// only after the flux differences: an exposed DRAM latency per group.  Register-free prefetches of those
+// centre lines before the first load: div+sources 2.15 -> 1.94 ms on C4.  Measured and NOT done: the same for
+// K_ij (+16: no gain), for the y/z neighbours of the metric that the centred differences read (before the first
+// load: 2.08; after the centre loads, in flight during the stress-tensor arithmetic: 2.2-3.4 ms — they evict
+// the lines the other warps are waiting for), and the metric lines of k_fofc_test (2.01 -> 2.07 ms).
+// 0: off; 4 | 1: prefetch.global.L1; 4 | 2: prefetch.global.L2 (same time); +16: K_ij as well.
+#ifndef AK_SRC_PREFETCH
+#define AK_SRC_PREFETCH 5
+#endif
+__device__ __forceinline__ void src_prefetch(const void* p) {
+#if (AK_SRC_PREFETCH & 3) == 1
+  asm volatile("prefetch.global.L1 [%0];" ::"l"(p));
+#elif (AK_SRC_PREFETCH & 3) == 2
+  asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+#endif
+}
 // Part (6) for ONE interior cell c of block m, given the flux differences div[v] (div_flux) of the five hydro
 // variables: dU~/dt = -div + geometric sources (Eq. 9); also the matter epilogue.  Called by k_div_src (one
 // thread per interior cell), by the fused FOFC-test kernel (k_fofc_test<EOS, STRIDE, true>, which has the
@@ -127,6 +144,19 @@ __global__ void __launch_bounds__(128, AK_SRC_MINB) k_div_src(const __grid_const
   const int k = r / n + P.is;
   const Ix ix{P.nt, P.px};
   const long long c = ix.cell(m, k, j, i);
+#if AK_SRC_PREFETCH
+  {
+#if AK_SRC_PREFETCH & 16
+#pragma unroll
+    for (int q = 10; q < 16; ++q) src_prefetch(f.adm[q] + c);
+#endif
+#if AK_SRC_PREFETCH & 4
+#pragma unroll
+    for (int q = 0; q < 10; ++q) src_prefetch(f.adm[q] + c);
+    src_prefetch(f.W[0] + c); src_prefetch(f.W[4] + c);
+#endif
+  }
+#endif
   const double idx3[3] = {1.0 / f.dx[3 * m + 0], 1.0 / f.dx[3 * m + 1], 1.0 / f.dx[3 * m + 2]};
   double div[5];
 #pragma unroll
