@@ -68,8 +68,10 @@ struct ak_ctx {
   int cap[8];                   // grid caps (blocks) per kernel class in the overlapped schedule, 0 = none
   int sweep_smem_pad;           // bytes: dynamic shared memory the sweeps ask for at least when overlapped
   unsigned int* zflags;         // [nmb] per-block zero-field flags written by k_con2prim (Fields::zflags)
-  unsigned int* mlist;          // [2 nmb] static / general MeshBlocks (k_split_blocks), [2] their counts behind
-  int split_blocks;             // 1: static MeshBlocks take k_flux_static (serial schedule, part (1) in the same call)
+  unsigned char* rowflag;       // [nmb nt nt] per-row flags written by k_con2prim (Fields::rowflag)
+  unsigned int* tlist;          // [6 tcap] static / general tiles per direction (k_split_tiles), [6] their counts behind
+  unsigned int tcap;            // nmb (n+2) max_d tiles_d
+  int split_blocks;             // 1: static tiles take k_flux_static (serial schedule, part (1) in the same call)
   // CUDA-graph replay of the serial stage (ak_set_graph): a few instantiated graphs keyed on the arguments
   int graph_on;
   cudaStream_t gstream;         // capture stream (the caller's may be the legacy default stream, which cannot capture)
@@ -203,6 +205,7 @@ void chunk_fields(const ak_ctx* c, const Fields& f, int m0, int nb, int ci, Fiel
   for (int q = 0; q < 21; ++q) g.F[q] += fsz[q / 7];
   g.flag += cell;
   if (g.zflags) g.zflags += m0;
+  if (g.rowflag) g.rowflag += nt * nt * m0;
   if (g.status) g.status += cell;
   if (g.M[0]) for (int q = 0; q < 10; ++q) g.M[q] += cell;
   g.dx += 3LL * m0;
@@ -245,6 +248,7 @@ int launch_c2p(ak_ctx* c, const Lane& L, bool with_emf) {
   Timer t(c, KC_C2P, L.st);
   CK(cudaMemsetAsync(L.f.stats, 0, sizeof(unsigned long long) * 3, L.st));
   if (L.f.zflags) CK(cudaMemsetAsync(L.f.zflags, 0, sizeof(unsigned) * L.P.nmb, L.st));   // this pass sets the bits
+  if (L.f.rowflag) CK(cudaMemsetAsync(L.f.rowflag, 0, (size_t)L.P.nmb * L.P.nt * L.P.nt, L.st));
   const long long ncell = (long long)L.P.nmb * L.P.nt * L.P.nt * L.P.nt;
   const unsigned g = capped(ncell, 128, L.ov ? c->cap[KC_C2P] : 0);
   const bool stride = (long long)g * 128 < ncell;       // a capped grid needs the grid-stride form
@@ -406,6 +410,19 @@ int launch_pencil(ak_ctx* c, const Lane& L) {
 }
 
 // do the tile kernels apply to this batch (else launch_flux falls back to k_flux and knows no block lists)
+// the tiling of a sweep of direction d: NA rows (x) / face rows (y, z) per tile, `tiles` tiles along the tiled extent;
+// for the general kernel (face or cell variant) and for k_flux_static
+void sweep_tiling(int d, int n, bool for_static, int& NA, int& tiles) {
+  const int e = n + 2;
+  const int cellv = for_static ? 0 : ((AK_FLUX_CELL_MASK >> d) & 1);
+  const int nfi = for_static ? (d == 0 ? ((AK_STATIC_ONCE_MASK & 1) ? n + 4 : n + 3) : e)
+                             : (cellv ? (d == 0 ? n + 4 : e) : (d == 0 ? n + 3 : e));
+  const int nfd = d == 0 ? e : n + 3;
+  const int namax = TMA_THREADS / nfi - (cellv && d != 0 ? 1 : 0);
+  tiles = (nfd + namax - 1) / namax;
+  NA = (nfd + tiles - 1) / tiles;
+}
+
 bool tile_kernels_apply(const ak_ctx* c, const Par& P) {
   const int n = P.n, e = n + 2;
   if (!AK_FLUX_TMA || n % 2 != 0 || c->pencil_wi > 0) return false;
@@ -444,9 +461,9 @@ int launch_flux_static_r(ak_ctx* c, const Lane& L, int NA, unsigned grid, int bd
 template <int DIR>
 int launch_flux_static(ak_ctx* c, const Lane& L) {
   const int n = L.P.n, nt = L.P.nt, e = n + 2;
-  const int nfi = DIR == 0 ? ((AK_STATIC_ONCE_MASK & 1) ? n + 4 : n + 3) : e, nfd = DIR == 0 ? e : n + 3;   // threads per tile row
-  const int namax = TMA_THREADS / nfi;
-  const int tiles = (nfd + namax - 1) / namax, NA = (nfd + tiles - 1) / tiles;
+  const int nfi = DIR == 0 ? ((AK_STATIC_ONCE_MASK & 1) ? n + 4 : n + 3) : e;   // threads per tile row
+  int NA, tiles;
+  sweep_tiling(DIR, n, true, NA, tiles);
   const int maxW = DIR == 0 ? NA : NA + 5, maxM = DIR == 0 ? NA : NA + 1;
   const size_t smem = sizeof(double) * ((size_t)2 * tile_slot(maxW, nt) + (size_t)10 * tile_slot(maxM, nt));
   TileMaps M;
@@ -524,7 +541,7 @@ int launch_flux(ak_ctx* c, const Lane& L) {
       if (r != AK_OK) return r;
       CK(cudaGetLastError());
       c->launches[KC_FX + DIR] += 1;
-      if (L.f.mlist) {                         // the static MeshBlocks of k_split_blocks: the light kernel
+      if (L.f.tlist) {                         // the static tiles of k_split_tiles: the light kernel
         r = launch_flux_static<DIR>(c, L);
         if (r != AK_OK) return r;
         c->launches[KC_FX + DIR] += 1;
@@ -532,7 +549,7 @@ int launch_flux(ak_ctx* c, const Lane& L) {
       return AK_OK;
     }
   }
-  if (L.f.mlist) return AK_ESTATE;             // (lists are only handed out when the tile kernels apply)
+  if (L.f.tlist) return AK_ESTATE;             // (lists are only handed out when the tile kernels apply)
   const long long nf = (long long)(n + 3) * (n + 2) * (n + 2) * L.P.nmb;
   const unsigned g = nblk(nf, 128);
   if (L.P.eos) {
@@ -778,7 +795,17 @@ int ak_create(const ak_params* p, const double* dx3, ak_ctx** out) {
   if (e == cudaSuccess) e = cudaMalloc(&c->stats, sizeof(unsigned long long) * S_NSTAT * MAXCH);
   if (e == cudaSuccess) e = cudaMemsetAsync(c->count, 0, sizeof(unsigned) * 4 * MAXCH, c->stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(c->stats, 0, sizeof(unsigned long long) * S_NSTAT * MAXCH, c->stream);
-  if (e == cudaSuccess) e = cudaMalloc(&c->mlist, sizeof(unsigned) * (2 * nb + 2));
+  {
+    int tmax = 1;
+    for (int d = 0; d < 3; ++d) {
+      int NA, tiles;
+      sweep_tiling(d, p->n, false, NA, tiles);
+      if (tiles > tmax) tmax = tiles;
+    }
+    c->tcap = (unsigned)((size_t)nb * (p->n + 2) * tmax);
+  }
+  if (e == cudaSuccess) e = cudaMalloc(&c->tlist, sizeof(unsigned) * (6 * (size_t)c->tcap + 6));
+  if (e == cudaSuccess) e = cudaMalloc(&c->rowflag, (size_t)nb * c->P.nt * c->P.nt);
   if (e == cudaSuccess) e = cudaMalloc(&c->zflags, sizeof(unsigned) * nb);
   if (e == cudaSuccess) e = cudaMemsetAsync(c->zflags, 0xff, sizeof(unsigned) * nb, c->stream);
   if (e == cudaSuccess) e = cudaMalloc(&c->dx, sizeof(double) * 3 * nb);
@@ -832,7 +859,7 @@ int ak_destroy(ak_ctx* c) {
     for (int q = 0; q < 3; ++q)
       if (c->ovs[q] && !(q == 2 && c->ovs[2] == c->ovs[0])) cudaStreamDestroy(c->ovs[q]);
   }
-  cudaFree(c->flag_own); cudaFree(c->count); cudaFree(c->stats); cudaFree(c->dx); cudaFree(c->zflags); cudaFree(c->mlist);
+  cudaFree(c->flag_own); cudaFree(c->count); cudaFree(c->stats); cudaFree(c->dx); cudaFree(c->zflags); cudaFree(c->tlist); cudaFree(c->rowflag);
   delete c;
   return AK_OK;
 }
@@ -903,6 +930,21 @@ int ak_con2prim(ak_ctx* c, const ak_cons* U, const ak_faceB* Bf, const ak_prim* 
 }  // extern "C"
 
 namespace {
+// tile lists are made when part (1) runs in the same call, every exact shortcut is on, and both sweep kernels
+// tile each direction alike (they do for every n with the default build)
+bool split_wanted(ak_ctx* c, int w_is_valid) {
+  const bool want = c->split_blocks > 0 || (c->split_blocks < 0 && c->sz.cell >= (1LL << 23));
+  if (w_is_valid || !want || (c->P.shortcuts & 5) != 5 || !c->tile_tm || !tmap_encoder() || !tile_kernels_apply(c, c->P))
+    return false;
+  for (int d = 0; d < 3; ++d) {
+    int NAg, tg, NAs, ts;
+    sweep_tiling(d, c->P.n, false, NAg, tg);
+    sweep_tiling(d, c->P.n, true, NAs, ts);
+    if (NAg != NAs || tg != ts) return false;
+  }
+  return true;
+}
+
 // the serial schedule of one stage: the whole batch, kernel after kernel, on stream st
 int rhs_serial(ak_ctx* c, const Fields& f, int w_is_valid, double dt_fofc, cudaStream_t st) {
   // counters of every chunk slot start from zero (a stage that skips part (1) reports no con2prim counts)
@@ -911,17 +953,22 @@ int rhs_serial(ak_ctx* c, const Fields& f, int w_is_valid, double dt_fofc, cudaS
   int r;
   const Lane L = {c->P, f, st, false};
   if (!w_is_valid && (r = launch_c2p(c, L, true)) != AK_OK) return r;
-  // MeshBlocks that part (1) found static and unmagnetised as a whole go to the light sweep kernel
+  // tiles that part (1) found static and unmagnetised as a whole go to the light sweep kernel
   Fields fs = f;
-  const bool want_split = c->split_blocks > 0 || (c->split_blocks < 0 && c->sz.cell >= (1LL << 23));
-  if (!w_is_valid && want_split && (c->P.shortcuts & 5) == 5 && c->tile_tm && tmap_encoder() &&
-      tile_kernels_apply(c, c->P)) {
-    unsigned* cnt = c->mlist + 2 * (size_t)c->P.nmb;
-    CK(cudaMemsetAsync(cnt, 0, sizeof(unsigned) * 2, st));
-    k_split_blocks<<<nblk(c->P.nmb, 256), 256, 0, st>>>(c->P.nmb, c->zflags, c->mlist, cnt);
+  if (f.rowflag) {                             // (ak_rhs hands the row flags out only when split_wanted())
+    TileShapes sh;
+    int tmax = 0;
+    for (int d = 0; d < 3; ++d) {
+      sweep_tiling(d, c->P.n, false, sh.NA[d], sh.tiles[d]);
+      if (sh.tiles[d] > tmax) tmax = sh.tiles[d];
+    }
+    unsigned* cnt = c->tlist + 6 * (size_t)c->tcap;
+    CK(cudaMemsetAsync(cnt, 0, sizeof(unsigned) * 6, st));
+    const dim3 grid(nblk((long long)c->P.nmb * (c->P.n + 2) * tmax, 256), 3);
+    k_split_tiles<<<grid, 256, 0, st>>>(c->P, f.rowflag, sh, c->tlist, cnt, c->tcap);
     CK(cudaGetLastError());
     c->launches[KC_C2P] += 1;                  // counted with part (1), whose flags it sorts
-    fs.mlist = c->mlist; fs.mcount = cnt;
+    fs.tlist = c->tlist; fs.tcount = cnt; fs.tcap = c->tcap;
   }
   const Lane LS = {c->P, fs, st, false};
   if ((r = launch_flux<0>(c, LS)) != AK_OK) return r;
@@ -1020,6 +1067,7 @@ int ak_rhs(ak_ctx* c, const ak_cons* U, const ak_faceB* Bf, const ak_prim* W, in
   // per-block zero-field flags: part (1) of this call writes them, the later parts read them; primitives the
   // caller supplies (w_is_valid) come without
   f.zflags = w_is_valid ? nullptr : c->zflags;
+  f.rowflag = (c->ov_chunks <= 1 && split_wanted(c, w_is_valid)) ? c->rowflag : nullptr;
   if (out->matter) {
     const ak_matter* mo = out->matter;
     double* mp[10] = {mo->E, mo->Sx, mo->Sy, mo->Sz, mo->Sxx, mo->Sxy, mo->Sxz, mo->Syy, mo->Syz, mo->Szz};

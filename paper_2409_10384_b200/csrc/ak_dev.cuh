@@ -55,8 +55,11 @@ struct Fields {
   unsigned int* zflags;         // [nmb] bit q set: primitive field W[q] (q = 1..3 u^i, 5..7 B~cc^i) of that block holds
                                 // a value that is not +0.0 (written by k_con2prim, conservative); bits 8..10: a face
                                 // value of B~f^x,y,z of that block is not +0.0; nullptr: unknown
-  const unsigned int* mlist;    // sweeps over MeshBlock lists (k_split_blocks): [0, nmb) static blocks, [nmb, 2 nmb)
-  const unsigned int* mcount;   // the others; mcount[0], mcount[1] their lengths; nullptr: every block, in order
+  unsigned char* rowflag;       // [nmb][nt][nt] 1: row (m, k, j) holds a u^i or a face B~ that is not +0.0 (written by
+                                // k_con2prim, cleared before it); nullptr: not wanted
+  const unsigned int* tlist;    // sweeps over TILE lists (k_split_tiles): list 2 d + w of direction d (w = 0 static
+  const unsigned int* tcount;   // tiles, 1 the others) starts at tlist + (2 d + w) tcap and holds tcount[2 d + w] tile
+  unsigned int tcap;            // numbers (m e + o') tiles + td; nullptr: every tile, in order
 };
 
 enum { ST_DFLOOR = 1, ST_TAUFLOOR = 2, ST_MAGCAP = 4, ST_RHOFLOOR = 8, ST_TFLOOR = 16,

@@ -1,17 +1,17 @@
-// ak_flux_static.cuh — K2 for MeshBlocks that are static and unmagnetised as a whole (round 2).
+// ak_flux_static.cuh — K2 for tiles that are static and unmagnetised as a whole (round 2).
 //
-// k_con2prim records per MeshBlock whether any u^i, any cell-centred B~ or any face B~ holds a value that
-// is not +0.0 (Fields::zflags).  A block where none does — static atmosphere without field, 72 % of C4's
-// blocks — needs of the 17 staged fields only rho, P and the ten metric fields, and of the Riemann solve only
-// static_side() (ak_flux.cuh: Eq. 8 with W = 1, v = 0, B = 0 substituted term by term, the same bits as
-// the general code on such data).  This kernel does just that: 12 tensor-map box copies per tile, 33 KB of
-// shared memory instead of 52 KB and no general side_state() in the register budget, so that 5-6 blocks are
-// resident on an SM instead of 3 and the tile-load latency — the top stall of the default-mode sweeps
-// (profiles/r2_final.md) — is covered.  k_split_blocks makes the two lists of MeshBlocks (static / general)
-// on the device; both sweep kernels are launched over the full grid and a block whose list entry does not
-// exist returns at once.
+// k_con2prim records per ROW of cells whether any u^i or any face B~ of the row holds a value that is not +0.0
+// (Fields::rowflag).  A tile none of whose rows does — static atmosphere without field: 72 % of C4's MeshBlocks
+// and four tiles in five of the others — needs of the 17 staged fields only rho, P and the ten metric fields,
+// and of the Riemann solve only static_side() (ak_flux.cuh: Eq. 8 with W = 1, v = 0, B = 0 substituted term by
+// term, the same bits as the general code on such data).  This kernel does just that: 12 tensor-map box copies
+// per tile, 33 KB of shared memory instead of 52 KB and no general side_state() in the register budget, so that
+// 5 blocks are resident on an SM instead of 3 and the tile-load latency — the top stall of the default-mode
+// sweeps (profiles/r2_final.md) — is covered.  k_split_tiles makes, per direction, the two lists of tiles
+// (static / general) on the device; both sweep kernels are launched over the full grid and a block whose list
+// entry does not exist returns at once.
 //
-// Same tiles as k_flux_tma: x: NA rows of n+3 faces; y, z: NA face rows of n+2 lanes.  One thread per face.
+// Same tiles as k_flux_tma: x: NA rows of n+3 faces; y, z: NA face rows of n+2 lanes.
 #pragma once
 #include "ak_flux_tma.cuh"
 
@@ -24,12 +24,45 @@ namespace ak {
 #define AK_STATIC_ONCE_MASK 1   // bit d: the sweep of direction d reconstructs every cell once (below)
 #endif
 
-// lists of MeshBlocks: mlist[0..count[0]) static, mlist[nmb + 0 .. nmb + count[1]) general
-__global__ void __launch_bounds__(256) k_split_blocks(int nmb, const unsigned* __restrict__ zflags,
-                                                      unsigned* __restrict__ mlist, unsigned* __restrict__ mcount) {
-  for (int m = blockIdx.x * blockDim.x + threadIdx.x; m < nmb; m += gridDim.x * blockDim.x) {
-    const int which = (zflags[m] & 0x7eeu) ? 1 : 0;      // u^i (1..3), B~cc (5..7), face B~ (8..10)
-    mlist[which * nmb + atomicAdd(mcount + which, 1u)] = (unsigned)m;
+// Tile lists.  One thread per tile of one direction: the tile is static iff none of the rows of cells it stages
+// has its row flag set (conservative: the flags cover all three u^i and all face fields, the tile test of the
+// general kernel only what that direction uses; a static tile that lands in the general list is still
+// recognised there).  Appended warp by warp, so that the lists keep the order of the tiles in memory up to the
+// order in which warps arrive.  shape[d] = {NA, tiles} of direction d (the launcher's tiling).
+struct TileShapes { int NA[3], tiles[3]; };
+__global__ void __launch_bounds__(256) k_split_tiles(const __grid_constant__ Par P, const unsigned char* __restrict__ rowflag,
+                                                     const __grid_constant__ TileShapes sh, unsigned* __restrict__ tlist,
+                                                     unsigned* __restrict__ tcount, unsigned tcap) {
+  const int e = P.n + 2, nt = P.nt;
+  const int d = blockIdx.y;
+  const int tiles = sh.tiles[d], NA = sh.NA[d];
+  const long long ntile = (long long)P.nmb * e * tiles;
+  const long long tile = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  bool live = tile < ntile, any = false;
+  if (live) {
+    long long b = tile;
+    const int td = (int)(b % tiles); b /= tiles;
+    const int o = (int)(b % e) + P.is - 1;
+    const int m = (int)(b / e);
+    const int nfd = d == 0 ? e : P.n + 3;
+    const int d0 = P.is - 1 + td * NA;
+    const int na = min(NA, P.is - 1 + nfd - d0);
+    // rows of cells the tile stages: x: (k = o, j in [d0, d0+na)); y: (k = o, j in [d0-3, d0+na+2));
+    // z: (k in [d0-3, d0+na+2), j = o)
+    const int r0 = d == 0 ? d0 : d0 - 3, nr = d == 0 ? na : na + 5;
+    const unsigned char* rf = rowflag + (size_t)m * nt * nt;
+    for (int r = r0; r < r0 + nr; ++r) any |= (d == 2 ? rf[r * nt + o] : rf[o * nt + r]) != 0;
+  }
+#pragma unroll
+  for (int w = 0; w < 2; ++w) {
+    const bool mine = live && (any == (w == 1));
+    const unsigned bal = __ballot_sync(0xffffffffu, mine);
+    if (bal == 0) continue;
+    const int lane = threadIdx.x & 31, leader = __ffs(bal) - 1;
+    unsigned base = 0;
+    if (lane == leader) base = atomicAdd(tcount + 2 * d + w, (unsigned)__popc(bal));
+    base = __shfl_sync(0xffffffffu, base, leader);
+    if (mine) tlist[(size_t)(2 * d + w) * tcap + base + __popc(bal & ((1u << lane) - 1u))] = (unsigned)tile;
   }
 }
 
@@ -46,12 +79,11 @@ k_flux_static(const __grid_constant__ Par P, const __grid_constant__ Fields f, i
   double* sM = sm + 2 * slotW;                 // [10][slotM]
   const int nfd = DIR == 0 ? e : P.n + 3;
   const int tiles = (nfd + NA - 1) / NA;
-  int bid = blockIdx.x;
+  if (blockIdx.x >= f.tcount[2 * DIR]) return; // fewer static tiles than the grid provides for (block-uniform)
+  int bid = (int)f.tlist[(size_t)(2 * DIR) * f.tcap + blockIdx.x];
   const int td = bid % tiles; bid /= tiles;
   const int o = bid % e + P.is - 1;
-  const int mm = bid / e;
-  if (mm >= (int)f.mcount[0]) return;          // fewer static blocks than the grid provides for (block-uniform)
-  const int m = (int)f.mlist[mm];
+  const int m = bid / e;
   const int d0 = P.is - 1 + td * NA;
   const int na = min(NA, P.is - 1 + nfd - d0);
   const Ix ix{nt, P.px};

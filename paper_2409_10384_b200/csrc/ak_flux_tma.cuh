@@ -129,13 +129,13 @@ k_flux_tma(const __grid_constant__ Par P, const __grid_constant__ Fields f, int 
   const int nfd = DIR == 0 ? e : P.n + 3;      // extent that NA tiles: rows (x) or faces along d (y,z)
   const int tiles = (nfd + NA - 1) / NA;
   int bid = blockIdx.x;
+  if (f.tlist) {                               // the general tiles of k_split_tiles (block-uniform exit)
+    if (blockIdx.x >= f.tcount[2 * DIR + 1]) return;
+    bid = (int)f.tlist[(size_t)(2 * DIR + 1) * f.tcap + blockIdx.x];
+  }
   const int td = bid % tiles; bid /= tiles;
   const int o = bid % e + P.is - 1;            // the fixed transverse index (k for x,y; j for z)
-  int m = bid / e;
-  if (f.mlist) {                               // the general blocks of k_split_blocks (block-uniform exit)
-    if (m >= (int)f.mcount[1]) return;
-    m = (int)f.mlist[P.nmb + m];
-  }
+  const int m = bid / e;
   const int d0 = P.is - 1 + td * NA;           // first row (x) / first face along d (y,z)
   const int na = min(NA, P.is - 1 + nfd - d0); // rows / faces actually present in this tile
   const int nW = DIR == 0 ? na : na + 5, nM = DIR == 0 ? na : na + 1;
@@ -305,13 +305,13 @@ k_flux_tma_cell(const __grid_constant__ Par P, const __grid_constant__ Fields f,
   const int nfd = DIR == 0 ? e : P.n + 3;
   const int tiles = (nfd + NA - 1) / NA;
   int bid = blockIdx.x;
-  const int td = bid % tiles; bid /= tiles;
-  const int o = bid % e + P.is - 1;
-  int m = bid / e;
-  if (f.mlist) {                               // the general blocks of k_split_blocks (block-uniform exit)
-    if (m >= (int)f.mcount[1]) return;
-    m = (int)f.mlist[P.nmb + m];
+  if (f.tlist) {                               // the general tiles of k_split_tiles (block-uniform exit)
+    if (blockIdx.x >= f.tcount[2 * DIR + 1]) return;
+    bid = (int)f.tlist[(size_t)(2 * DIR + 1) * f.tcap + blockIdx.x];
   }
+  const int td = bid % tiles; bid /= tiles;
+  const int o = bid % e + P.is - 1;            // the fixed transverse index (k for x,y; j for z)
+  const int m = bid / e;
   const int d0 = P.is - 1 + td * NA;
   const int na = min(NA, P.is - 1 + nfd - d0);
   const int nW = DIR == 0 ? na : na + 5, nM = DIR == 0 ? na : na + 1;

@@ -173,6 +173,18 @@ __global__ void __launch_bounds__(128, AK_C2P_MINB) k_con2prim(const __grid_cons
 #pragma unroll
     for (int v = 0; v < 3; ++v) nz |= (unsigned)(__double_as_longlong(Bc[v]) != 0LL) << (5 + v);
     if (nz != 0 && (__ldcg(f.zflags + m) & nz) != nz) atomicOr(f.zflags + m, nz);
+    // the same per ROW of cells (m, k, j), for the tile lists of k_split_tiles: a row whose byte stays 0 has
+    // u^i = +0 and every face B~ of its cells = +0 (hence B~cc = +0).
+    if (f.rowflag) {                           // (one store per row segment of the warp, not one per cell)
+      const bool fl = (nz & 0x70eu) != 0;
+      const unsigned act = __activemask();
+      const unsigned bal = __ballot_sync(act, fl);
+      if (bal != 0) {
+        const int rw = (int)row;
+        const unsigned same = __match_any_sync(act, rw);
+        if (fl && (int)(threadIdx.x & 31) == __ffs(bal & same) - 1) f.rowflag[rw] = 1;
+      }
+    }
   }
   if (EMF) {
     const double u[3] = {W5[1], W5[2], W5[3]};

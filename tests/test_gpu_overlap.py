@@ -405,9 +405,9 @@ def test_host_entry_sparse_writeback_of_floored_cells_into_pinned_memory():
 ])
 def test_static_block_sweep_kernel_is_exact(monkeypatch, name, blocks, over):
     """AK_SPLIT_BLOCKS=1 (automatic only for batches of >= 2^23 stored cells, e.g. C4, where the full-batch parity
-    test covers it): MeshBlocks that con2prim found static and unmagnetised as a whole — u, B~cc and every face B~
-    +0.0 — take k_flux_static, the others the general tile kernels through the device-side block lists.  Same bits
-    as without the split and as the oracle, fluxes and the signs of their zeros included."""
+    test covers it): tiles none of whose staged rows con2prim found to hold a u^i or a face B~ other than +0.0 take
+    k_flux_static, the others the general tile kernels, through the device-side tile lists of k_split_tiles.  Same
+    bits as without the split and as the oracle, fluxes and the signs of their zeros included."""
     from paper_2409_10384_b200 import ak
     w = wl.make_blocks(name, blocks=blocks)
     U_in = [u.copy() for u in w["U"]]
@@ -435,3 +435,41 @@ def test_static_block_sweep_kernel_is_exact(monkeypatch, name, blocks, over):
     o = orc.rhs(orc.make_params(**p), w["dx"], w["U"], w["Bf"], w["adm"], w["dt_fofc"], nthreads=8)
     o["U"] = w["U"]
     gpukit.assert_parity(r1, o, U_in, label=name + " split")
+
+
+def test_tile_lists_cover_every_row_a_tile_stages(monkeypatch):
+    """k_split_tiles: a tile is static only if EVERY row of cells it stages is — the 5 halo rows of a y or z tile
+    included.  A static atmosphere block with single moving cells and single magnetised faces placed next to
+    tile boundaries (tiles of 7 face rows starting at index 3: 3, 10, 17, 24, 31, 38) and at random: a tile list
+    that forgot a halo row would hand a tile with non-zero data to the light kernel, which reads rho and P only.
+    Split on must give the bits of split off with the shortcuts off, signs of zero fluxes included."""
+    from paper_2409_10384_b200 import ak
+    w = wl.make_blocks("C2", blocks=[0, 63])
+    nt = 40
+    U = [u.reshape(2, nt, nt, nt) for u in w["U"]]
+    for q in (1, 2, 3): U[q][...] = 0.0                      # two blocks at rest, without field
+    for b in w["Bf"]: b[...] = 0.0
+    rng = np.random.default_rng(11)
+    cells = [(0, 19, 9, 20), (0, 16, 30, 5), (0, 3, 3, 3), (0, 36, 36, 36), (0, 12, 24, 38), (1, 22, 2, 1), (1, 38, 17, 20)]
+    # the outermost halo rows of a tile [d0, d0+7): d0-3 (7, 14, 21, 28) and d0+8 (11, 18, 25, 32), in j (y) and k (z)
+    cells += [(0, 20, 7, 20), (0, 21, 20, 10), (1, 5, 14, 30), (1, 28, 33, 7), (0, 25, 11, 11), (1, 18, 9, 9), (1, 6, 32, 2)]
+    cells += [(int(rng.integers(2)),) + tuple(int(x) for x in rng.integers(0, nt, 3)) for _ in range(6)]
+    for q, (m, k, j, i) in enumerate(cells):
+        U[1 + q % 3][m, k, j, i] = (1e-3 if q % 2 else -1e-3) * U[0][m, k, j, i]      # S~_a = +-1e-3 D~
+    bx = w["Bf"][0].reshape(2, nt, nt, -1); by = w["Bf"][1].reshape(2, nt, nt + 1, nt); bz = w["Bf"][2].reshape(2, nt + 1, nt, nt)
+    bx[1, 10, 10, 21] = 1e-6; by[0, 30, 17, 8] = -1e-6; bz[1, 24, 5, 33] = 1e-6; bz[0, 2, 38, 0] = -0.0
+    res = []
+    for split, mask in (("0", 0), ("1", 7)):
+        monkeypatch.setenv("AK_SPLIT_BLOCKS", split)
+        with gpukit.GpuStage(copy.deepcopy(w)) as g:
+            ak.ak_set_exact_shortcuts(g.ctx, mask)
+            g.rhs()
+            res.append((g.result(), g.flux(), g.stats()))
+    (r0, f0, s0), (r1, f1, s1) = res
+    assert any(np.any(x[0, 19, 9, 20] != 0.0) for x in r0["W"][1:4])        # the poked cell does move
+    for k in ("dU", "E", "W", "U"):
+        for x, y in zip(r0[k], r1[k]):
+            assert np.array_equal(x, y), k
+    assert np.array_equal(r0["flag"], r1["flag"]) and np.array_equal(r0["status"], r1["status"]) and s0 == s1
+    for x, y in zip(f0, f1):
+        assert np.array_equal(x, y) and np.array_equal(np.signbit(x), np.signbit(y))
