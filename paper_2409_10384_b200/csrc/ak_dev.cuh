@@ -246,10 +246,21 @@ struct C2P {
   // f(mu) = mu - inv with inv = 1/nu the same number at every evaluation: after one full evaluation
   // (which leaves inv and the trial state behind) the root finder runs on that one subtraction
   bool stat; double inv;
+  // unmagnetised cell (exact shortcut, bit 1): bs2 and rb2 are +0.0, r2 is finite and q > 0.  Then for every trial
+  // mu >= +0 (the root finder never leaves [0, mu_hi]): x = 1/(1 + mu 0) = 1; rbar2 = r2 1 1 + ((mu 1) 2)(+0) =
+  // r2 + 0 (the addition is kept: it turns a -0 into the +0 of the full expression); bs2 r2 - rb2 = +-0, so qbar
+  // = (q - 0) - (+-0) = q for q != 0.  One reciprocal and ~15 further operations per evaluation dropped.
+  bool nob;
   __device__ __forceinline__ void aux(double mu) {
-    x = 1.0 / (1.0 + mu * bs2);
-    rbar2 = r2 * x * x + mu * x * (1.0 + x) * rb2;
-    qbar = q - 0.5 * bs2 - 0.5 * mu * mu * x * x * (bs2 * r2 - rb2);
+    if (nob) {
+      x = 1.0;
+      rbar2 = r2 + 0.0;
+      qbar = q;
+    } else {
+      x = 1.0 / (1.0 + mu * bs2);
+      rbar2 = r2 * x * x + mu * x * (1.0 + x) * rb2;
+      qbar = q - 0.5 * bs2 - 0.5 * mu * mu * x * x * (bs2 * r2 - rb2);
+    }
     vsq = fmin(mu * mu * rbar2, v0sq);
     iW = sqrt(1.0 - vsq);
     What = 1.0 / iW;
@@ -445,6 +456,8 @@ __device__ __forceinline__ int c2p_cell(const Par& P, const Met3& g, double Ut[5
     s.v0sq = ddiv(s.r2, 1.0 + s.r2);
     s.gm1 = P.gm1;
     s.stat = false; s.inv = 0.0;
+    s.nob = (P.shortcuts & 2) != 0 && (__double_as_longlong(s.bs2) | __double_as_longlong(s.rb2)) == 0LL &&
+            isfinite(s.r2) && s.q > 0.0;
     bool ok = true;
     double mu_hi = 1.0;
     if (!(s.r2 < 1.0)) {
