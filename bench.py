@@ -668,8 +668,10 @@ def main():
     hbm_peak, peak_src = measured_peaks()
     rf, table, table_full, stage = roofline(R, hbm_peak, peak_src)
     shortcuts = dict(mask=7, what="reconstruction skipped for fields that are +0.0 on a whole staged tile; con2prim root "
-                     "find of cells with S~ = 0 and B~ = 0 on f(mu) = mu - const; static face flux on tiles with u = 0 and "
-                     "B = 0 (include/ak.h ak_set_exact_shortcuts)",
+                     "find of cells with S~ = 0 and B~ = 0 on f(mu) = mu - const, master function of cells with B = 0 "
+                     "without its B terms; static face flux on tiles with u = 0 and B = 0 (through a lighter kernel, "
+                     "tile lists made on the device), B = 0 side state on moving unmagnetised tiles "
+                     "(include/ak.h ak_set_exact_shortcuts)",
                      default_ms_per_step=round(R["ms_step"], 4), full_arithmetic_ms_per_step=round(R["full_ms"], 4),
                      full_arithmetic_value=R["zones_total"] / (R["full_ms"] * 1e-3),
                      outputs_bit_identical=R["full_same"],

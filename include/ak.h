@@ -172,10 +172,14 @@ long long ak_graph_replays(const ak_ctx*);
 /* Exact data-dependent shortcuts (D:§6.3).  mask bit 0: a field of (u^x, u^y, u^z, B~cc^t1, B~cc^t2) that is
  * +0.0 on the whole tile a sweep block stages is not reconstructed (every scheme of P:133 returns +0.0 on
  * both sides of every face for it); bit 1: a cell with S~ = 0 and B~ = 0 exactly runs its con2prim root
- * find on f(mu) = mu - const, which is what the master function then is; bit 2: a sweep block whose tile
+ * find on f(mu) = mu - const, which is what the master function then is, and a cell with B = 0 evaluates
+ * the master function with x = 1, rbar^2 = r^2, qbar = q; bit 2: a sweep block whose tile
  * holds u^i = +0.0 and every B~ component +0.0 evaluates the face flux of Eq. 8 with W = 1, v = 0, B = 0
  * substituted (no index lowering, no Lorentz factor, no Alfven speed: what side_state computes then, term
- * by term).  All three leave every output bit unchanged (the parity tests run with them on and off); what
+ * by term), and one whose tile holds moving matter but every B~ component +0.0 with B = 0 substituted.
+ * With all three on, batches of >= 2^23 stored cells also sort their sweep tiles on the device into a static
+ * and a general list and run the static ones through a lighter kernel (D:§6 item 29; AK_SPLIT_BLOCKS=0/1
+ * at ak_create forces that off / on).  All of it leaves every output bit unchanged (the parity tests run with them on and off); what
  * they change is the time on inputs with exact zeros — static atmosphere, unmagnetised regions: most of a
  * merger grid.  Default 7 (all; also settable by the environment variable AK_EXACT_SHORTCUTS at
  * ak_create); 0 times the full arithmetic. */

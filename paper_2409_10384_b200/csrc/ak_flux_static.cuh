@@ -27,8 +27,7 @@ namespace ak {
 // Tile lists.  One thread per tile of one direction: the tile is static iff none of the rows of cells it stages
 // has its row flag set (conservative: the flags cover all three u^i and all face fields, the tile test of the
 // general kernel only what that direction uses; a static tile that lands in the general list is still
-// recognised there).  Appended warp by warp, so that the lists keep the order of the tiles in memory up to the
-// order in which warps arrive.  shape[d] = {NA, tiles} of direction d (the launcher's tiling).
+// recognised there).  shape[d] = {NA, tiles} of direction d (the launcher's tiling).
 struct TileShapes { int NA[3], tiles[3]; };
 __global__ void __launch_bounds__(256) k_split_tiles(const __grid_constant__ Par P, const unsigned char* __restrict__ rowflag,
                                                      const __grid_constant__ TileShapes sh, unsigned* __restrict__ tlist,
@@ -53,16 +52,30 @@ __global__ void __launch_bounds__(256) k_split_tiles(const __grid_constant__ Par
     const unsigned char* rf = rowflag + (size_t)m * nt * nt;
     for (int r = r0; r < r0 + nr; ++r) any |= (d == 2 ? rf[r * nt + o] : rf[o * nt + r]) != 0;
   }
+  // append: one atomic per thread block and list, so that 256 consecutive tiles (~1.5 MeshBlocks' worth of one
+  // direction) stay consecutive in their list and run together -- neighbouring tiles share halo rows, L2 lines
+  // and DRAM pages (appending warp by warp left the lists in the order warps happened to arrive: L2 hit rate of
+  // the light kernel 38 -> 8 %)
+  __shared__ unsigned wcnt[2][8], wbase[2][8];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  unsigned bal[2];
 #pragma unroll
   for (int w = 0; w < 2; ++w) {
-    const bool mine = live && (any == (w == 1));
-    const unsigned bal = __ballot_sync(0xffffffffu, mine);
-    if (bal == 0) continue;
-    const int lane = threadIdx.x & 31, leader = __ffs(bal) - 1;
-    unsigned base = 0;
-    if (lane == leader) base = atomicAdd(tcount + 2 * d + w, (unsigned)__popc(bal));
-    base = __shfl_sync(0xffffffffu, base, leader);
-    if (mine) tlist[(size_t)(2 * d + w) * tcap + base + __popc(bal & ((1u << lane) - 1u))] = (unsigned)tile;
+    bal[w] = __ballot_sync(0xffffffffu, live && (any == (w == 1)));
+    if (lane == 0) wcnt[w][wid] = (unsigned)__popc(bal[w]);
+  }
+  __syncthreads();
+  if (threadIdx.x < 2) {
+    const int w = threadIdx.x;
+    unsigned tot = 0;
+    for (int q = 0; q < 8; ++q) { wbase[w][q] = tot; tot += wcnt[w][q]; }
+    const unsigned base = tot ? atomicAdd(tcount + 2 * d + w, tot) : 0u;
+    for (int q = 0; q < 8; ++q) wbase[w][q] += base;
+  }
+  __syncthreads();
+  if (live) {
+    const int w = any ? 1 : 0;
+    tlist[(size_t)(2 * d + w) * tcap + wbase[w][wid] + __popc(bal[w] & ((1u << lane) - 1u))] = (unsigned)tile;
   }
 }
 
