@@ -54,8 +54,7 @@ __global__ void __launch_bounds__(256) k_split_tiles(const __grid_constant__ Par
   }
   // append: one atomic per thread block and list, so that 256 consecutive tiles (~1.5 MeshBlocks' worth of one
   // direction) stay consecutive in their list and run together -- neighbouring tiles share halo rows, L2 lines
-  // and DRAM pages (appending warp by warp left the lists in the order warps happened to arrive: L2 hit rate of
-  // the light kernel 38 -> 8 %)
+  // and DRAM pages (appending warp by warp leaves the lists in the order warps happen to arrive: +0.03 ms per stage)
   __shared__ unsigned wcnt[2][8], wbase[2][8];
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   unsigned bal[2];
