@@ -9,7 +9,10 @@ namespace ak {
 
 // ------------------------------------------------------------------ O4: reconstruction
 // Five cell values qmm..qpp centred on cell i  ->  qm at its left face, qp at its right face.
-template <int KIND>
+// PLAIN: the two weighted means of WENO-Z by a plain division instead of ddiv() — the same quotient bit for bit
+// (ddiv only sidesteps the division's slow path for a ZERO dividend); for fields that are never zero (rho, P in
+// the light kernel) it saves the ~10 instructions of ddiv's test and selects per quotient.
+template <int KIND, bool PLAIN = false>
 __device__ __forceinline__ void recon(double qmm, double qm1, double q0, double qp1, double qpp,
                                       double& qm, double& qp) {
   if (KIND == 0) {            // donor cell
@@ -92,14 +95,14 @@ __device__ __forceinline__ void recon(double qmm, double qm1, double q0, double 
       const double p1 = (-qm1 + 5.0 * q0 + 2.0 * qp1) * c6;
       const double p2 = (2.0 * q0 + 5.0 * qp1 - qpp) * c6;
       const double w0 = 0.1 * t0, w1 = 0.6 * t1, w2 = 0.3 * t2;
-      qp = ddiv(w0 * p0 + w1 * p1 + w2 * p2, w0 + w1 + w2);
+      qp = PLAIN ? (w0 * p0 + w1 * p1 + w2 * p2) / (w0 + w1 + w2) : ddiv(w0 * p0 + w1 * p1 + w2 * p2, w0 + w1 + w2);
     }
     {  // mirror image
       const double p0 = (2.0 * qpp - 7.0 * qp1 + 11.0 * q0) * c6;
       const double p1 = (-qp1 + 5.0 * q0 + 2.0 * qm1) * c6;
       const double p2 = (2.0 * q0 + 5.0 * qm1 - qmm) * c6;
       const double w0 = 0.1 * t2, w1 = 0.6 * t1, w2 = 0.3 * t0;
-      qm = ddiv(w0 * p0 + w1 * p1 + w2 * p2, w0 + w1 + w2);
+      qm = PLAIN ? (w0 * p0 + w1 * p1 + w2 * p2) / (w0 + w1 + w2) : ddiv(w0 * p0 + w1 * p1 + w2 * p2, w0 + w1 + w2);
     }
   }
 }

@@ -20,6 +20,9 @@ namespace ak {
 #ifndef AK_STATIC_MINB
 #define AK_STATIC_MINB 4
 #endif
+#ifndef AK_STATIC_PLAIN_DIV
+#define AK_STATIC_PLAIN_DIV 1   // rho and P are never zero: WENO-Z's quotients by plain division (see recon<>)
+#endif
 #ifndef AK_STATIC_ONCE_MASK
 #define AK_STATIC_ONCE_MASK 1   // bit d: the sweep of direction d reconstructs every cell once (below)
 #endif
@@ -150,19 +153,19 @@ k_flux_static(const __grid_constant__ Par P, const __grid_constant__ Fields f, i
       } else if (!ONCE) {
         const double q0 = w[0], q1 = w[s], q2 = w[2 * s], q3 = w[3 * s], q4 = w[4 * s], q5 = w[5 * s];
         double qm, qp;
-        recon<RECON>(q0, q1, q2, q3, q4, qm, qp);
+        recon<RECON, AK_STATIC_PLAIN_DIV != 0>(q0, q1, q2, q3, q4, qm, qp);
         sL[v] = qp;
-        recon<RECON>(q1, q2, q3, q4, q5, qm, qp);
+        recon<RECON, AK_STATIC_PLAIN_DIV != 0>(q1, q2, q3, q4, q5, qm, qp);
         sR[v] = qm;
       } else {
         const double q1 = w[s], q2 = w[2 * s], q3 = w[3 * s], q4 = w[4 * s], q5 = w[5 * s];
         double qm, qp;
-        recon<RECON>(q1, q2, q3, q4, q5, qm, qp);
+        recon<RECON, AK_STATIC_PLAIN_DIV != 0>(q1, q2, q3, q4, q5, qm, qp);
         sR[v] = qm;
         xch[v2][t] = qp;
         if (DIR != 0 && a == 0) {
           double qm0;
-          recon<RECON>(w[0], q1, q2, q3, q4, qm0, qp);
+          recon<RECON, AK_STATIC_PLAIN_DIV != 0>(w[0], q1, q2, q3, q4, qm0, qp);
           sL[v] = qp;
         }
       }
