@@ -71,6 +71,7 @@ struct ak_ctx {
   unsigned char* rowflag;       // [nmb nt nt] per-row flags written by k_con2prim (Fields::rowflag)
   unsigned int* tlist;          // [6 tcap] static / general tiles per direction (k_split_tiles), [6] their counts behind
   unsigned int tcap;            // nmb (n+2) max_d tiles_d
+  int ct_fused;                 // 1: the three CT components in one launch (k_ct_all)
   int split_blocks;             // 1: static tiles take k_flux_static (serial schedule, part (1) in the same call)
   // CUDA-graph replay of the serial stage (ak_set_graph): a few instantiated graphs keyed on the arguments
   int graph_on;
@@ -631,6 +632,9 @@ int launch_ct(ak_ctx* c, const Lane& L, bool have_cell_emf) {
     k_ct<0, true><<<g, 128, 0, L.st>>>(L.P, L.f);
     k_ct<1, true><<<g, 128, 0, L.st>>>(L.P, L.f);
     k_ct<2, true><<<g, 128, 0, L.st>>>(L.P, L.f);
+  } else if (c->ct_fused) {
+    k_ct_all<<<nblk((n + 1) * (n + 1) * (n + 1) * L.P.nmb, 128), 128, 0, L.st>>>(L.P, L.f);
+    c->launches[KC_CT] -= 2;
   } else {
     k_ct<0><<<g, 128, 0, L.st>>>(L.P, L.f);
     k_ct<1><<<g, 128, 0, L.st>>>(L.P, L.f);
@@ -761,6 +765,7 @@ int ak_create(const ak_params* p, const double* dx3, ak_ctx** out) {
     // 51 tensor-map encodes per stage, which cost the small configs 3-14 % (C0 0.144 -> 0.165 ms, C3 1.53 -> 1.58)
     // and gain C4 1 % (13.75 -> 13.59 ms)
     c->split_blocks = envi("AK_SPLIT_BLOCKS", -1);
+    c->ct_fused = envi("AK_CT_FUSED", 1);
   }
   Par& P = c->P;
   P.nmb = p->nmb; P.n = p->n; P.nt = p->n + 8; P.px = P.nt + 4; P.is = 4; P.ie = p->n + 3;

@@ -437,23 +437,9 @@ __global__ void __launch_bounds__(128) k_cell_emf(const __grid_constant__ Par P,
 
 // ---- K5: corner EMFs, component C3 (Gardiner & Stone 2005; DESIGN.md §3 O8) ------------------
 // a, b cyclic after C3.  Edge (ia, ib, ic): ia, ib in [is, ie+1], ic in [is, ie].
-template <int C3, bool STRIDE = false>
-__global__ void __launch_bounds__(128) k_ct(const __grid_constant__ Par P,
-                                            const __grid_constant__ Fields f) {
+template <int C3>
+__device__ __forceinline__ void ct_edge(const Par& P, const Fields& f, const Ix& ix, int m, const int p3[3]) {
   constexpr int a = (C3 + 1) % 3, b = (C3 + 2) % 3;
-  const int n = P.n;
-  const int ei = n + (C3 == 0 ? 0 : 1), ej = n + (C3 == 1 ? 0 : 1), ek = n + (C3 == 2 ? 0 : 1);
-  const long long per = (long long)ei * ej * ek;
-  long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  do {
-  if (idx >= per * P.nmb) return;
-  const int m = (int)(idx / per);
-  int r = (int)(idx - (long long)m * per);
-  int p3[3];
-  p3[0] = r % ei + P.is; r /= ei;
-  p3[1] = r % ej + P.is;
-  p3[2] = r / ej + P.is;
-  const Ix ix{P.nt, P.px};
   // offsets of one step along a and b, in cells and in the a-face / b-face layouts
   const long long cst[3] = {1, P.nt, (long long)P.nt * P.nt};
   const long long c0 = ix.cell(m, p3[2], p3[1], p3[0]);
@@ -485,8 +471,47 @@ __global__ void __launch_bounds__(128) k_ct(const __grid_constant__ Par P,
   const double dap = w2p * (Eaf_0m - Ec_mm) + (1.0 - w2p) * (Eaf_00 - Ec_m0);
   const double e = 0.25 * (Eaf_00 + Eaf_0m + Ebf_00 + Ebf_m0) + 0.25 * ((dbp - dbm) + (dap - dam));
   f.E[C3][ix.edge(C3, m, p3[2], p3[1], p3[0])] = e;
+}
+
+template <int C3, bool STRIDE = false>
+__global__ void __launch_bounds__(128) k_ct(const __grid_constant__ Par P,
+                                            const __grid_constant__ Fields f) {
+  const int n = P.n;
+  const int ei = n + (C3 == 0 ? 0 : 1), ej = n + (C3 == 1 ? 0 : 1), ek = n + (C3 == 2 ? 0 : 1);
+  const long long per = (long long)ei * ej * ek;
+  long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  do {
+  if (idx >= per * P.nmb) return;
+  const int m = (int)(idx / per);
+  int r = (int)(idx - (long long)m * per);
+  int p3[3];
+  p3[0] = r % ei + P.is; r /= ei;
+  p3[1] = r % ej + P.is;
+  p3[2] = r / ej + P.is;
+  const Ix ix{P.nt, P.px};
+  ct_edge<C3>(P, f, ix, m, p3);
   idx += (long long)gridDim.x * blockDim.x;
   } while (STRIDE);
+}
+
+// All three components in one launch: one thread per corner point (i, j, k) in [is, ie+1]^3, which owns the edges
+// that start there (E_x if i <= ie, E_y if j <= ie, E_z if k <= ie).  Each mass-flux field is needed by two
+// components and each face EMF field by one; in one kernel the second use hits L1/L2 instead of DRAM.
+__global__ void __launch_bounds__(128) k_ct_all(const __grid_constant__ Par P, const __grid_constant__ Fields f) {
+  const int n1 = P.n + 1;
+  const long long per = (long long)n1 * n1 * n1;
+  const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= per * P.nmb) return;
+  const int m = (int)(idx / per);
+  int r = (int)(idx - (long long)m * per);
+  int p3[3];
+  p3[0] = r % n1 + P.is; r /= n1;
+  p3[1] = r % n1 + P.is;
+  p3[2] = r / n1 + P.is;
+  const Ix ix{P.nt, P.px};
+  if (p3[0] <= P.ie) ct_edge<0>(P, f, ix, m, p3);
+  if (p3[1] <= P.ie) ct_edge<1>(P, f, ix, m, p3);
+  if (p3[2] <= P.ie) ct_edge<2>(P, f, ix, m, p3);
 }
 
 }  // namespace ak
