@@ -58,7 +58,7 @@ FP64_PIPE_PEAK_TINST = 148 * 4 * 16 * 1.965e9 * 1e-12
 # pass (profiles/r2_final.md: the pass the roofline object is taken from), keyed by (blocks, kernel class);
 # other sizes: null.
 NCU_TRAFFIC_BYTES = {(768, "con2prim"): 12.23e9, (768, "flux_x"): 7.72e9, (768, "flux_y"): 8.12e9,
-                     (768, "flux_z"): 8.19e9, (768, "fofc_test"): 9.00e9, (768, "div_src"): 11.38e9}
+                     (768, "flux_z"): 8.19e9, (768, "fofc_test"): 9.00e9, (768, "div_src"): 11.37e9}
 
 
 def kernel_units(nmb, n):
