@@ -420,6 +420,7 @@ void sweep_tiling(int d, int n, bool for_static, int& NA, int& tiles) {
                              : (cellv ? (d == 0 ? n + 4 : e) : (d == 0 ? n + 3 : e));
   const int nfd = d == 0 ? e : n + 3;
   const int namax = TMA_THREADS / nfi - (cellv && d != 0 ? 1 : 0);
+  if (namax < 1) { NA = 1; tiles = nfd; return; }     // a row does not fit a block: the tile kernels do not apply
   tiles = (nfd + namax - 1) / namax;
   NA = (nfd + tiles - 1) / tiles;
 }

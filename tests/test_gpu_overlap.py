@@ -473,3 +473,14 @@ def test_tile_lists_cover_every_row_a_tile_stages(monkeypatch):
     assert np.array_equal(r0["flag"], r1["flag"]) and np.array_equal(r0["status"], r1["status"]) and s0 == s1
     for x, y in zip(f0, f1):
         assert np.array_equal(x, y) and np.array_equal(np.signbit(x), np.signbit(y))
+
+
+def test_create_with_rows_longer_than_a_sweep_block():
+    """n + 4 > 256 threads: the tile kernels (and with them the tile lists) do not apply; ak_create must size its
+    list scratch without dividing by a tile height of zero, and the context must come up and go away cleanly."""
+    from paper_2409_10384_b200 import ak
+    w = wl.make_blocks("C0")
+    p = dict(w["params"]); p.update(nmb=1, n=254)
+    par = ak.make_params(device=0, stream=0, **p)
+    ctx = ak.ak_create(par, np.ones((1, 3)) * 0.01)
+    ak.ak_destroy(ctx)
