@@ -15,6 +15,19 @@
 
 namespace ak {
 
+// Stores of data that no later kernel of the stage finds in L2 anyway (the batch is two hundred times the L2):
+// st.global.cs (evict-first) keeps the lines that ARE re-read — halo rows of neighbouring tiles — resident longer.
+// AK_STREAM_ST bits: 1 light sweep kernel, 2 general sweep kernels, 4 con2prim, 8 div+sources.  Measured on C4
+// (same-box A/B, stage): 0: 12.25-12.32 ms, 1: 12.24, 3: 12.23, 12: 12.22, 15: 12.19.
+#ifndef AK_STREAM_ST
+#define AK_STREAM_ST 15
+#endif
+template <int BIT>
+__device__ __forceinline__ void st_out(double* p, double v) {
+  if (AK_STREAM_ST & BIT) __stcs(p, v); else *p = v;
+}
+
+
 // ------------------------------------------------------------------ parameters / fields
 struct Par {
   int nmb, n, nt, px, is, ie;   // is = 4, ie = n + 3

@@ -191,7 +191,7 @@ k_flux_static(const __grid_constant__ Par P, const __grid_constant__ Fields f, i
   face_geometry<DIR>(mL, mR, G);
   face_flux_static<DIR, EOS>(P, P.riemann, G, sL, sR, Fo);
 #pragma unroll
-  for (int v = 0; v < 7; ++v) f.F[7 * DIR + v][fi] = Fo[v];
+  for (int v = 0; v < 7; ++v) st_out<1>(f.F[7 * DIR + v] + fi, Fo[v]);
 }
 
 }  // namespace ak

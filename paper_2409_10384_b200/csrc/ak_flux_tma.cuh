@@ -249,7 +249,7 @@ k_flux_tma(const __grid_constant__ Par P, const __grid_constant__ Fields f, int 
     if (!active) return;
     face_flux_static<DIR, EOS>(P, P.riemann, G, sL, sR, Fo);
 #pragma unroll
-    for (int v = 0; v < 7; ++v) f.F[7 * DIR + v][fi] = Fo[v];
+    for (int v = 0; v < 7; ++v) st_out<2>(f.F[7 * DIR + v] + fi, Fo[v]);
     return;
   }
   __syncthreads();
@@ -269,7 +269,7 @@ k_flux_tma(const __grid_constant__ Par P, const __grid_constant__ Fields f, int 
   face_flux<DIR, true, EOS>(P, P.riemann, mL, mR, sL, sR, Bfd, Fo);
 #endif
 #pragma unroll
-  for (int v = 0; v < 7; ++v) f.F[7 * DIR + v][fi] = Fo[v];
+  for (int v = 0; v < 7; ++v) st_out<2>(f.F[7 * DIR + v] + fi, Fo[v]);
 }
 
 // ---- reconstruct-once variant -------------------------------------------------------------------
@@ -422,7 +422,7 @@ k_flux_tma_cell(const __grid_constant__ Par P, const __grid_constant__ Fields f,
     if (!has_face) return;
     face_flux_static<DIR, EOS>(P, P.riemann, G, sL, qm, Fo);
 #pragma unroll
-    for (int v = 0; v < 7; ++v) f.F[7 * DIR + v][fi] = Fo[v];
+    for (int v = 0; v < 7; ++v) st_out<2>(f.F[7 * DIR + v] + fi, Fo[v]);
     return;
   }
   __syncthreads();
@@ -442,7 +442,7 @@ k_flux_tma_cell(const __grid_constant__ Par P, const __grid_constant__ Fields f,
   face_flux<DIR, true, EOS>(P, P.riemann, mL, mR, sL, qm, Bfd, Fo);
 #endif
 #pragma unroll
-  for (int v = 0; v < 7; ++v) f.F[7 * DIR + v][fi] = Fo[v];
+  for (int v = 0; v < 7; ++v) st_out<2>(f.F[7 * DIR + v] + fi, Fo[v]);
 }
 
 }  // namespace ak

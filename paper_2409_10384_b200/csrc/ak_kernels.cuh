@@ -155,9 +155,9 @@ __global__ void __launch_bounds__(128, AK_C2P_MINB) k_con2prim(const __grid_cons
   const int st = c2p_cell<true, EOS>(P, g, Ut, Bc, W5);
 #endif
 #pragma unroll
-  for (int v = 0; v < 5; ++v) f.W[v][c] = W5[v];
+  for (int v = 0; v < 5; ++v) st_out<4>(f.W[v] + c, W5[v]);
 #pragma unroll
-  for (int v = 0; v < 3; ++v) f.W[5 + v][c] = Bc[v];
+  for (int v = 0; v < 3; ++v) st_out<4>(f.W[5 + v] + c, Bc[v]);
   if (st != 0) {
 #pragma unroll
     for (int v = 0; v < 5; ++v) f.U[v][c] = Ut[v];
@@ -195,9 +195,9 @@ __global__ void __launch_bounds__(128, AK_C2P_MINB) k_con2prim(const __grid_cons
     const double alp = __ldg(f.adm[6] + c), ialp = 1.0 / alp;
     const double vh[3] = {u[0] * iW - __ldg(f.adm[7] + c) * ialp, u[1] * iW - __ldg(f.adm[8] + c) * ialp,
                           u[2] * iW - __ldg(f.adm[9] + c) * ialp};
-    f.Ecc[0][c] = -(alp * (vh[1] * Bc[2] - vh[2] * Bc[1]));
-    f.Ecc[1][c] = -(alp * (vh[2] * Bc[0] - vh[0] * Bc[2]));
-    f.Ecc[2][c] = -(alp * (vh[0] * Bc[1] - vh[1] * Bc[0]));
+    st_out<4>(f.Ecc[0] + c, -(alp * (vh[1] * Bc[2] - vh[2] * Bc[1])));
+    st_out<4>(f.Ecc[1] + c, -(alp * (vh[2] * Bc[0] - vh[0] * Bc[2])));
+    st_out<4>(f.Ecc[2] + c, -(alp * (vh[0] * Bc[1] - vh[1] * Bc[0])));
   }
   warp_count(f.stats + S_C2P_FAIL, (st & ST_FAIL) != 0);
   warp_count(f.stats + S_CONS_FLOOR, (st & (ST_DFLOOR | ST_TAUFLOOR | ST_MAGCAP)) != 0);

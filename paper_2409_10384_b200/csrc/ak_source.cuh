@@ -126,7 +126,7 @@ __device__ __forceinline__ void div_src_cell(const Par& P, const Fields& f, int 
   const double Sda = Su[0] * dalp[0] + Su[1] * dalp[1] + Su[2] * dalp[2];
   du[4] = du[4] + sdet * (alp * KS - Sda);
 #pragma unroll
-  for (int v = 0; v < 5; ++v) f.dU[v][c] = du[v];
+  for (int v = 0; v < 5; ++v) st_out<8>(f.dU[v] + c, du[v]);
 }
 
 template <int EOS = 0, bool STRIDE = false>
