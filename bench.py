@@ -57,8 +57,8 @@ FP64_PIPE_PEAK_TINST = 148 * 4 * 16 * 1.965e9 * 1e-12
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu capture of the full-arithmetic
 # pass (profiles/r2_final.md: the pass the roofline object is taken from), keyed by (blocks, kernel class);
 # other sizes: null.
-NCU_TRAFFIC_BYTES = {(768, "con2prim"): 12.23e9, (768, "flux_x"): 7.72e9, (768, "flux_y"): 8.12e9,
-                     (768, "flux_z"): 8.19e9, (768, "fofc_test"): 9.00e9, (768, "div_src"): 11.37e9}
+NCU_TRAFFIC_BYTES = {(768, "con2prim"): 11.83e9, (768, "flux_x"): 7.71e9, (768, "flux_y"): 8.11e9,
+                     (768, "flux_z"): 8.18e9, (768, "fofc_test"): 9.03e9, (768, "div_src"): 11.37e9}
 
 
 def kernel_units(nmb, n):
